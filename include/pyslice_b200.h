@@ -1,0 +1,181 @@
+/* pyslice_b200.h — C ABI of the B200-native TACAW hot path (arxiv 2602.10064, "PySlice").
+ *
+ * What the library computes (citations are lines of the paper text, PAPER.md, with the
+ * section / equation they fall in; readings A1..A22 are listed in DESIGN.md §3):
+ *
+ *   PAPER.md:81  (§2.2 "Atomic Scattering Potentials")
+ *        f(q) = sum_i a_i/(q^2+b_i) + sum_i c_i exp(-d_i q^2)
+ *        V_s(k) = sum_{j in slice s} f_Zj(|k|) exp(-2 pi i k.r_j),  inverse FFT -> V_s(r)
+ *   PAPER.md:79  (§2.2 "Multislice")
+ *        t(r) = exp(i sigma V(r)),  P(k) = exp(-i pi lambda dz |k|^2),
+ *        psi_exit = P_{N-1} t_N ... P_1 t_2 P_0 t_1 psi_probe
+ *   PAPER.md:89  (§2.2 data containers)  exit waves indexed (probe, time, kx, ky): k-space
+ *   PAPER.md:73  (§2.1 "TACAW")
+ *        psi~(k,w) = F_t[ psi(k,t) - <psi(k,t)>_t ],   I(k,w) = |psi~(k,w)|^2
+ *   PAPER.md:89, 394, 397, 422  dispersion(), spectral_diffraction(), spectrum_image()
+ *   PAPER.md:289-301 (Suppl. Eq. 4-6)  dk = 1/L, df = 1/(N dt), f_max = 1/(2 dt)
+ *
+ * Conventions
+ *   - Every pointer named d_* is DEVICE memory owned by the caller (e.g. a torch tensor);
+ *     every other pointer is HOST memory, read during the call and never retained.
+ *   - All hot-path calls are asynchronous on the stream given to ps_create(); the library
+ *     never synchronises the device on the hot path and never frees caller memory.
+ *   - Scratch memory the library needs is allocated by the ctx itself (cudaMalloc, grown
+ *     on demand, freed by ps_destroy) unless the caller installs a workspace with
+ *     ps_set_workspace().
+ *   - Every failure is a negative ps_status plus a message from ps_last_error(); nothing
+ *     aborts or throws across this boundary.  There is no CPU fallback of any kind.
+ *   - Grids: nx, ny powers of two in [32, 2048]; cells orthorhombic (Angstrom).
+ *     k = m/L (no 2 pi), FFT index order 0..N/2-1,-N/2..-1, forward transform
+ *     exp(-2 pi i ...), as numpy (A1).
+ *   - Band limit (A10): A(k) = [kx^2+ky^2 <= kc^2], kc = (2/3) min(nx/(2Lx), ny/(2Ly)),
+ *     applied in every propagator, to V(k) and to the probe.
+ *   - Results are deterministic for fixed inputs (no floating-point atomics anywhere).
+ *   - One ctx per host thread.
+ */
+#ifndef PYSLICE_B200_H
+#define PYSLICE_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define PS_API __attribute__((visibility("default")))
+#else
+#define PS_API
+#endif
+
+typedef struct ps_ctx ps_ctx;   /* opaque: owns its tables, plans and the scratch it allocated */
+
+typedef enum {
+    PS_OK = 0,
+    PS_EINVAL = -1,        /* bad argument (null pointer, size <= 0, bin out of range, ...)   */
+    PS_EUNSUPPORTED = -2,  /* non power-of-two grid, grid out of range, Z without coefficients,
+                              n_frames not a power of two in ps_tacaw, ...                     */
+    PS_EWORKSPACE = -3,    /* installed workspace too small / scratch allocation failed       */
+    PS_ECUDA = -4,         /* a CUDA runtime call or kernel launch failed                      */
+    PS_ESTATE = -5         /* call order violated (geometry / form factors not set, ...)       */
+} ps_status;
+
+/* exit-wave layouts accepted by ps_multislice / ps_tacaw */
+#define PS_LAYOUT_DENSE 0  /* complex64 [P][F][ny][nx], k-space, FFT index order (A13)        */
+
+/* ---------------------------------------------------------------- life cycle */
+
+/* Create a context bound to CUDA device `device` and to `cuda_stream` (a cudaStream_t; NULL =
+ * the legacy default stream).  Fails with PS_ECUDA when no usable device exists. */
+PS_API ps_status ps_create(ps_ctx** out, int device, void* cuda_stream);
+PS_API void ps_destroy(ps_ctx* ctx);
+/* Message of the last failure on this ctx (valid until the next call on it); "" if none.
+ * With ctx == NULL returns the message of the last failed ps_create of this thread. */
+PS_API const char* ps_last_error(const ps_ctx* ctx);
+/* Library version string, e.g. "pyslice_b200 0.1 (sm_100a)". */
+PS_API const char* ps_version(void);
+
+/* ---------------------------------------------------------------- host-side setup (not timed) */
+
+/* Form-factor coefficients, general (n_lorentz, n_gauss) form (A5):
+ *   f_Z(q) = sum_{i<n_lorentz} a_i/(q^2+b_i) + sum_{i<n_gauss} c_i exp(-d_i q^2),  q = |k| in 1/A.
+ * coef is host [n_elem][2*n_lorentz+2*n_gauss], row layout a.., b.., c.., d..
+ * (a: 1/A, b: 1/A^2, c: A, d: A^2).  Z lists the atomic number of each row.  Copied. */
+PS_API ps_status ps_set_form_factors(ps_ctx* ctx, int n_elem, const int32_t* Z, int n_lorentz, int n_gauss,
+                              const double* coef);
+
+/* Cell (orthorhombic, Angstrom), grid and slicing (A7):
+ * n_slices = max(1, round(Lz/slice_dz)), dz_eff = Lz/n_slices; slices are half-open
+ * [s dz, (s+1) dz), z wrapped periodically, beam along +z (A8).  Builds the aperture tables. */
+PS_API ps_status ps_set_geometry(ps_ctx* ctx, const double cell[3], int nx, int ny, double slice_dz);
+/* n_k_aperture = number of grid points with A(k) = 1.  Any out pointer may be NULL. */
+PS_API ps_status ps_get_geometry(const ps_ctx* ctx, int* n_slices, double* dz_eff, int* n_k_aperture);
+
+/* Scratch needed by ps_build_slices on `n_frames_chunk` frames at a time (the only call that
+ * needs scratch).  ps_set_workspace installs caller-owned device memory (d_ws == NULL removes
+ * it and returns the ctx to self-allocation).  ps_build_slices processes frames in chunks that
+ * fit whatever scratch is available. */
+PS_API size_t    ps_workspace_bytes(const ps_ctx* ctx, int n_frames_chunk, int n_atoms);
+PS_API ps_status ps_set_workspace(ps_ctx* ctx, void* d_ws, size_t bytes);
+
+/* Tuning knob: number of waves whose slice loop runs back to back (so that the chunk of waves
+ * stays resident in the 126 MB L2 between the two FFT passes of a slice).  0 = library default. */
+PS_API ps_status ps_set_wave_chunk(ps_ctx* ctx, int n_waves);
+
+/* ---------------------------------------------------------------- hot path */
+
+/* a0+a2+a3: projected potentials of every slice of every frame.
+ *   d_pos        float32 [n_frames][n_atoms][3] Cartesian positions, Angstrom
+ *   d_Z          int32   [n_atoms] atomic numbers (every value must have coefficients)
+ *   d_V          float32 [n_frames][n_slices][ny][nx], V*Angstrom               (written)
+ *   d_slice_idx  int32   [n_frames][n_atoms] slice of every atom, or NULL       (written)
+ * Fixed-point ingest: u = pos/L - floor(pos/L) (float64), U = floor(u 2^32) clamped,
+ * slice = (U_z * n_slices) >> 32 — bit-exact against the oracle. */
+PS_API ps_status ps_build_slices(ps_ctx* ctx, const float* d_pos, const int32_t* d_Z, int n_frames, int n_atoms,
+                          float* d_V, int32_t* d_slice_idx);
+
+/* a4: incident waves (PAPER.md:378-380 plane wave; 404-419 focused probe; A12, A18).
+ *   semi_angle_mrad == 0 and is_tilt == 0 : plane wave psi0 = 1 (xy ignored, may be NULL)
+ *   is_tilt != 0 : xy_or_tilt[i] = integer reciprocal-grid point (m_t, n_t):
+ *                  psi0 = exp(2 pi i (m_t x/Lx + n_t y/Ly))
+ *   else         : probe at xy_or_tilt[i] = (x0, y0) Angstrom:
+ *                  Psi0(k) = [lambda|k| <= alpha] A(k) exp(-2 pi i k.r0), psi0 = ifft2(Psi0),
+ *                  scaled so that sum_r |psi0|^2 = nx ny.
+ *   d_psi0  complex64 [n][ny][nx], real space                                   (written) */
+PS_API ps_status ps_make_incident(ps_ctx* ctx, double kV, double semi_angle_mrad, int n, const double* xy_or_tilt,
+                           int is_tilt, void* d_psi0);
+
+/* a5+a6: multislice for every (probe, frame) pair:
+ *   for s = 0..S-1: psi <- psi exp(i sigma V_s); psi <- ifft2(P A fft2(psi));
+ *   exit = fft2(psi)/sqrt(nx ny)   (k-space, unitary, A9, A13)
+ *   d_psi0  complex64 [n_probes][ny][nx]
+ *   d_V     float32   [n_frames][n_slices][ny][nx]
+ *   d_exit  complex64 [n_probes][n_frames][ny][nx]                              (written)
+ * The wave is propagated in place inside d_exit (no other wave storage). */
+PS_API ps_status ps_multislice(ps_ctx* ctx, double kV, const void* d_psi0, int n_probes, const float* d_V,
+                        int n_frames, void* d_exit, int exit_layout);
+
+/* a7: TACAW transform (A14): for every probe and k,
+ *   Psi~_n = sum_j (Psi_j - <Psi>_t) exp(-2 pi i n j / F),  I = |Psi~_n|^2,  f_n = n/(F dt).
+ *   bins: host list of n_bins signed FFT bins n (taken mod F), or NULL for all F bins in FFT
+ *   order (then n_bins must equal n_frames).  n_frames must be a power of two in [32, 4096].
+ *   d_I  float32 [n_probes][n_bins][ny][nx]                                      (written)
+ * dt_fs only defines the frequency axis (f_n in THz = n/(F dt_fs 1e-3)); it does not enter I. */
+PS_API ps_status ps_tacaw(ps_ctx* ctx, const void* d_exit, int exit_layout, int n_probes, int n_frames, double dt_fs,
+                   int n_bins, const int32_t* bins, float* d_I);
+
+/* Streaming variant for frames x grid > HBM (BASELINE config 4): per-bin DFT accumulation over
+ * frame chunks.  acc[p][b][k] += sum_j Psi_j e^{-2 pi i n_b j/F}; slot n_bins holds sum_j Psi_j
+ * (the mean term).  finish: I = |acc_b - [n_b mod F == 0] * F * mean|^2 (exact for integer bins).
+ *   d_acc  complex64 [n_probes][n_bins+1][ny][nx], zeroed by begin; any n_frames_total >= 1. */
+PS_API ps_status ps_tacaw_begin(ps_ctx* ctx, int n_probes, int n_frames_total, double dt_fs, int n_bins,
+                         const int32_t* bins, void* d_acc);
+/* d_exit_chunk complex64 [n_probes][n_frames_chunk][ny][nx] = frames frame0.. of every probe. */
+PS_API ps_status ps_tacaw_add(ps_ctx* ctx, const void* d_exit_chunk, int frame0, int n_frames_chunk);
+PS_API ps_status ps_tacaw_finish(ps_ctx* ctx, float* d_I /* float32 [n_probes][n_bins][ny][nx] */);
+
+/* a8: reductions over d_I = float32 [P][n_bins][ny][nx] (A15-A17).
+ * ps_sdp: spectral diffraction pattern, sum over probes and bins bin_lo..bin_hi inclusive
+ *         (positions in the bin list) -> d_out float32 [ny][nx]. */
+PS_API ps_status ps_sdp(ps_ctx* ctx, const float* d_I, int P, int n_bins, int bin_lo, int bin_hi, float* d_out);
+/* ps_spectrum_image: d_out[p][b] = sum over k with k_in <= |k| < k_out (1/A; k_out <= 0 means
+ * no outer limit) of I[p][b][k] -> float32 [P][n_bins]. */
+PS_API ps_status ps_spectrum_image(ps_ctx* ctx, const float* d_I, int P, int n_bins, double k_in, double k_out,
+                            float* d_out);
+/* ps_dispersion: nearest grid pixel of each path point, ix = floor(kx Lx + 0.5) mod nx (A17);
+ * d_pix int32 [n_path] = iy*nx+ix (bit-exact), d_out[b][i] = sum_p I[p][b][pix_i]. */
+PS_API ps_status ps_dispersion(ps_ctx* ctx, const float* d_I, int P, int n_bins, int n_path, const double* kx,
+                        const double* ky, int32_t* d_pix, float* d_out);
+/* ps_qbin: radial histogram, bin = floor(sqrt(kx^2+ky^2)/dq), dropped (-1) if >= n_q;
+ * d_qidx int32 [ny][nx] (bit-exact), d_out[b][q] = sum_p sum_{k in q} I[p][b][k]. */
+PS_API ps_status ps_qbin(ps_ctx* ctx, const float* d_I, int P, int n_bins, double dq, int n_q, int32_t* d_qidx,
+                  float* d_out);
+
+/* Number of kernels this ctx has launched so far (bench.py's `gpu_launches`). */
+PS_API long long ps_launch_count(const ps_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PYSLICE_B200_H */

@@ -1,0 +1,117 @@
+// common.cuh — context object and host helpers shared by the translation units of libpyslice_b200.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string>
+#include <vector>
+
+#include "../../include/pyslice_b200.h"
+
+namespace psb {
+
+constexpr int kColTile = 16;        // columns per tile of the column passes / activity granularity
+constexpr int kMaxGrid = 2048;
+constexpr int kMinGrid = 32;
+constexpr int kNumSM = 148;         // B200
+
+struct DeviceBuf {                  // library-owned device allocation, grown on demand
+    void* p = nullptr;
+    size_t bytes = 0;
+};
+
+struct KvTables {                   // tables that depend on the accelerating voltage
+    double kV = -1.0;
+    double lambda = 0.0, sigma = 0.0;
+    float2* d_px_mid = nullptr;     // [nx]  exp(-i pi lambda dz kx^2) / (nx ny)   (inverse-FFT norm folded in)
+    float2* d_px_last = nullptr;    // [nx]  exp(-i pi lambda dz kx^2) / sqrt(nx ny)
+    float2* d_py = nullptr;         // [ny]  exp(-i pi lambda dz ky^2)
+};
+
+struct TacawStream {                // state of ps_tacaw_begin/add/finish
+    bool active = false;
+    int n_probes = 0, n_frames_total = 0, n_bins = 0, frames_seen = 0;
+    void* d_acc = nullptr;
+    int32_t* d_bins = nullptr;      // [n_bins] bins mod F (library-owned)
+    std::vector<int32_t> bins;
+};
+
+}  // namespace psb
+
+struct ps_ctx {
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    std::string err;
+    long long launches = 0;
+
+    // geometry
+    bool have_geom = false;
+    double cell[3] = {0, 0, 0};
+    int nx = 0, ny = 0, n_slices = 0;
+    double dz_eff = 0.0, kc = 0.0;
+    int n_k_aperture = 0;
+    int mcut = 0, ncut = 0;                 // largest |m|, |n| inside the aperture
+    std::vector<int32_t> h_nmax;            // [nx] per column m (FFT order): max |n| with A=1, -1 if none
+    int32_t* d_nmax = nullptr;
+    std::vector<int32_t> h_tiles;           // active column tiles (kColTile columns) in the aperture
+    int32_t* d_tiles = nullptr;
+    uint8_t* d_tile_active = nullptr;       // [nx/kColTile]
+    int n_tiles_active = 0;
+    int wave_chunk = 0;
+
+    // form factors
+    bool have_ff = false;
+    int n_elem = 0, n_lorentz = 0, n_gauss = 0;
+    std::vector<int32_t> ffZ;
+    std::vector<double> ffcoef;
+    float* d_ftab = nullptr;                // [n_elem][ncut+1][2 mcut+1]  C/(LxLy) f_Z(|k|) A(k)
+    int32_t* d_elem_of_Z = nullptr;         // [128] element row of atomic number Z, -1 if absent
+    bool ftab_valid = false;
+
+    psb::KvTables kv;
+
+    // scratch
+    psb::DeviceBuf scratch;                 // library-owned
+    void* user_ws = nullptr;
+    size_t user_ws_bytes = 0;
+
+    psb::TacawStream ts;
+    psb::DeviceBuf misc;                    // small per-call tables (bin slots, path pixels)
+};
+
+namespace psb {
+
+inline ps_status fail(ps_ctx* c, ps_status s, const std::string& msg) {
+    if (c) c->err = msg;
+    return s;
+}
+
+#define PSB_CUDA(ctx, expr)                                                                         \
+    do {                                                                                            \
+        cudaError_t _e = (expr);                                                                    \
+        if (_e != cudaSuccess)                                                                      \
+            return psb::fail((ctx), PS_ECUDA, std::string(#expr) + ": " + cudaGetErrorString(_e)); \
+    } while (0)
+
+#define PSB_LAUNCH_CHECK(ctx, name)                                                                 \
+    do {                                                                                            \
+        cudaError_t _e = cudaGetLastError();                                                        \
+        if (_e != cudaSuccess)                                                                      \
+            return psb::fail((ctx), PS_ECUDA, std::string("launch ") + name + ": " + cudaGetErrorString(_e)); \
+        (ctx)->launches++;                                                                          \
+    } while (0)
+
+inline bool is_pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
+inline int signed_index(int i, int n) { return i < (n + 1) / 2 ? i : i - n; }
+
+ps_status ensure_buf(ps_ctx* c, DeviceBuf& b, size_t bytes);
+ps_status ensure_kv(ps_ctx* c, double kV);
+ps_status ensure_ftab(ps_ctx* c);
+
+// physical constants (CODATA values; DESIGN.md §3 "Constants")
+constexpr double kHC_keVA = 12.398419843;
+constexpr double kM0C2_keV = 510.99895;
+constexpr double kBohr_A = 0.529177211;
+constexpr double kE2_VA = 14.3996455;
+
+}  // namespace psb

@@ -1,0 +1,232 @@
+// fft_core.cuh — in-register / shared-memory radix FFT building blocks for sm_100a.
+//
+// One transform of length N (a power of two, 32 <= N <= 4096) is carried by T = N/16 threads,
+// each holding 16 complex values in registers in the "canonical" layout
+//      v[e] = x[t + e*T],   t = thread index inside the transform, e = 0..15.
+// The transform is a mixed-radix Stockham autosort FFT with at most three stages
+//      N = 16 * R2 * R3,   R2 = min(16, N/16),  R3 = N/(16*R2)
+// (stage s reads x[j + r*N/R], multiplies by W_{Ns*R}^{(j mod Ns) r}, does an R-point DFT and
+// writes y[(j/Ns)*Ns*R + (j mod Ns) + r*Ns]).  Both the input of the first stage and the output
+// of the last stage are canonical, so a pointwise product between two transforms (transmission
+// function, propagator) needs no data movement, and only the (#stages-1) exchanges between
+// stages go through shared memory.  Stage twiddles depend only on t, so each thread computes
+// them once (sincospif on exactly reduced integer phases) and keeps them in registers while it
+// loops over rows / columns / batches.
+//
+// Only the forward transform exp(-2 pi i nk/N) is coded; the inverse (unnormalised) is obtained
+// by swapping real and imaginary parts on the way in and out (free register renaming).
+//
+// Implements the transforms of PAPER.md:79 (fft2/ifft2 of the slice loop), PAPER.md:81 (inverse
+// FFT of V(k)) and PAPER.md:73 (time-axis transform); numpy sign convention (A1).
+#pragma once
+#include <cuda_runtime.h>
+
+namespace psb {
+
+__device__ __forceinline__ float2 cmul(const float2 a, const float2 b) {
+    return make_float2(fmaf(a.x, b.x, -a.y * b.y), fmaf(a.x, b.y, a.y * b.x));
+}
+__device__ __forceinline__ float2 cswap(const float2 a) { return make_float2(a.y, a.x); }
+
+// ---------------------------------------------------------------- small DFTs (forward, natural order)
+__device__ __forceinline__ void dft2(float2& a, float2& b) {
+    const float2 t = a;
+    a = make_float2(t.x + b.x, t.y + b.y);
+    b = make_float2(t.x - b.x, t.y - b.y);
+}
+// X0=a+b+c+d, X1=a-ib-c+id, X2=a-b+c-d, X3=a+ib-c-id   (W4 = -i)
+__device__ __forceinline__ void dft4(float2& a, float2& b, float2& c, float2& d) {
+    const float2 s0 = make_float2(a.x + c.x, a.y + c.y);
+    const float2 s1 = make_float2(a.x - c.x, a.y - c.y);
+    const float2 s2 = make_float2(b.x + d.x, b.y + d.y);
+    const float2 s3 = make_float2(b.x - d.x, b.y - d.y);
+    a = make_float2(s0.x + s2.x, s0.y + s2.y);
+    c = make_float2(s0.x - s2.x, s0.y - s2.y);
+    b = make_float2(s1.x + s3.y, s1.y - s3.x);
+    d = make_float2(s1.x - s3.y, s1.y + s3.x);
+}
+
+template <int R> struct Dft;
+template <> struct Dft<2> {
+    static __device__ __forceinline__ void run(float2 (&w)[2]) { dft2(w[0], w[1]); }
+};
+template <> struct Dft<4> {
+    static __device__ __forceinline__ void run(float2 (&w)[4]) { dft4(w[0], w[1], w[2], w[3]); }
+};
+template <> struct Dft<8> {
+    // n = 2 n1 + n2, k = k1 + 4 k2
+    static __device__ __forceinline__ void run(float2 (&w)[8]) {
+        constexpr float h = 0.70710678118654752440f;
+        dft4(w[0], w[2], w[4], w[6]);
+        dft4(w[1], w[3], w[5], w[7]);
+        // y[1][k1] *= W8^k1
+        w[3] = make_float2((w[3].x + w[3].y) * h, (w[3].y - w[3].x) * h);       // (1-i)/sqrt2
+        w[5] = make_float2(w[5].y, -w[5].x);                                    // -i
+        w[7] = make_float2((w[7].y - w[7].x) * h, -(w[7].x + w[7].y) * h);      // (-1-i)/sqrt2
+        dft2(w[0], w[1]); dft2(w[2], w[3]); dft2(w[4], w[5]); dft2(w[6], w[7]);
+        // now w = {X0,X4,X1,X5,X2,X6,X3,X7}
+        const float2 x4 = w[1], x1 = w[2], x5 = w[3], x2 = w[4], x6 = w[5], x3 = w[6];
+        w[1] = x1; w[2] = x2; w[3] = x3; w[4] = x4; w[5] = x5; w[6] = x6;
+    }
+};
+template <> struct Dft<16> {
+    // n = 4 n1 + n2, k = k1 + 4 k2
+    static __device__ __forceinline__ void run(float2 (&w)[16]) {
+        constexpr float c1 = 0.92387953251128675613f, s1 = 0.38268343236508977173f;
+        constexpr float h = 0.70710678118654752440f;
+        dft4(w[0], w[4], w[8], w[12]);      // y[0][k1] at w[4 k1 + 0]
+        dft4(w[1], w[5], w[9], w[13]);
+        dft4(w[2], w[6], w[10], w[14]);
+        dft4(w[3], w[7], w[11], w[15]);
+        // w[4 k1 + n2] *= W16^(n2 k1)
+        w[5] = cmul(w[5], make_float2(c1, -s1));                                    // W^1
+        w[6] = make_float2((w[6].x + w[6].y) * h, (w[6].y - w[6].x) * h);           // W^2
+        w[7] = cmul(w[7], make_float2(s1, -c1));                                    // W^3
+        w[9] = make_float2((w[9].x + w[9].y) * h, (w[9].y - w[9].x) * h);           // W^2
+        w[10] = make_float2(w[10].y, -w[10].x);                                     // W^4 = -i
+        w[11] = make_float2((w[11].y - w[11].x) * h, -(w[11].x + w[11].y) * h);     // W^6
+        w[13] = cmul(w[13], make_float2(s1, -c1));                                  // W^3
+        w[14] = make_float2((w[14].y - w[14].x) * h, -(w[14].x + w[14].y) * h);     // W^6
+        w[15] = cmul(w[15], make_float2(-c1, s1));                                  // W^9
+        dft4(w[0], w[1], w[2], w[3]);       // X[k1 + 4 k2] at w[4 k1 + k2]
+        dft4(w[4], w[5], w[6], w[7]);
+        dft4(w[8], w[9], w[10], w[11]);
+        dft4(w[12], w[13], w[14], w[15]);
+        // transpose 4x4 to natural order
+        float2 t;
+        t = w[1]; w[1] = w[4]; w[4] = t;
+        t = w[2]; w[2] = w[8]; w[8] = t;
+        t = w[3]; w[3] = w[12]; w[12] = t;
+        t = w[6]; w[6] = w[9]; w[9] = t;
+        t = w[7]; w[7] = w[13]; w[13] = t;
+        t = w[11]; w[11] = w[14]; w[14] = t;
+    }
+};
+
+// ---------------------------------------------------------------- plan
+template <int N> struct Plan {
+    static_assert(N >= 32 && N <= 4096 && (N & (N - 1)) == 0, "N must be a power of two in [32, 4096]");
+    static constexpr int T = N / 16;                          // threads per transform
+    static constexpr int R2 = (N / 16 >= 16) ? 16 : N / 16;   // second-stage radix
+    static constexpr int R3 = N / (16 * R2);                  // third-stage radix (1 = none)
+    static constexpr int B2 = 16 / R2;                        // butterflies per thread, stage 2
+    static constexpr int B3 = (R3 > 1) ? 16 / R3 : 1;
+    static constexpr int NTW2 = B2 * (R2 - 1);
+};
+
+// exp(-2 pi i num/den), num reduced mod den exactly in integers first
+__device__ __forceinline__ float2 root_of_unity(int num, int den) {
+    num &= (den - 1);                                          // den is a power of two
+    float s, c;
+    sincospif(2.0f * (float)num / (float)den, &s, &c);         // num/den exact in fp32 (den <= 4096)
+    return make_float2(c, -s);
+}
+
+template <int N> struct Twiddles {
+    using P = Plan<N>;
+    float2 w2[P::NTW2];                 // stage 2: W_{16 R2}^{(j mod 16) r}, r = 1..R2-1, per butterfly
+    float2 w3[P::B3];                   // stage 3: base W_N^{(j mod 16 R2)} per butterfly
+    __device__ __forceinline__ void init(const int t) {
+#pragma unroll
+        for (int b = 0; b < P::B2; ++b) {
+            const int q = (t + b * P::T) & 15;
+#pragma unroll
+            for (int r = 1; r < P::R2; ++r) w2[b * (P::R2 - 1) + r - 1] = root_of_unity(q * r, 16 * P::R2);
+        }
+        if (P::R3 > 1) {
+#pragma unroll
+            for (int b = 0; b < P::B3; ++b) {
+                const int q = (t + b * P::T) & (16 * P::R2 - 1);
+                w3[b] = root_of_unity(q, N);
+            }
+        } else {
+            w3[0] = make_float2(1.f, 0.f);
+        }
+    }
+};
+
+// ---------------------------------------------------------------- exchange policies
+// A policy gives the shared-memory slot of logical element idx of *this thread's* transform and
+// the barrier covering all threads of that transform.
+struct RowSlots {            // one transform per contiguous padded line; pad 1 per 16 (conflict-free)
+    float2* line;
+    __device__ __forceinline__ float2& at(const int idx) const { return line[idx + (idx >> 4)]; }
+};
+template <int C> struct ColSlots {   // C transforms interleaved (lane = column), no padding needed
+    float2* base;                    // already offset by the column index c
+    __device__ __forceinline__ float2& at(const int idx) const { return base[idx * C]; }
+};
+struct BlockSync { static __device__ __forceinline__ void sync() { __syncthreads(); } };
+struct WarpSync  { static __device__ __forceinline__ void sync() { __syncwarp(); } };
+
+template <int N> struct RowLine { static constexpr int LEN = N + N / 16; };      // padded line length (float2)
+
+// ---------------------------------------------------------------- the transform
+template <int N, class Slots, class Sync>
+__device__ __forceinline__ void fft_forward(float2 (&v)[16], const int t, const Twiddles<N>& tw, const Slots& sm) {
+    using P = Plan<N>;
+    constexpr int T = P::T;
+    // stage 1: radix 16, Ns = 1, no twiddle
+    Dft<16>::run(v);
+    Sync::sync();                                             // earlier readers of the buffer are done
+#pragma unroll
+    for (int r = 0; r < 16; ++r) sm.at(16 * t + r) = v[r];
+    Sync::sync();
+#pragma unroll
+    for (int e = 0; e < 16; ++e) v[e] = sm.at(t + e * T);
+    // stage 2: radix R2, Ns = 16
+    constexpr int R2 = P::R2, B2 = P::B2;
+#pragma unroll
+    for (int b = 0; b < B2; ++b) {
+        float2 w[R2];
+#pragma unroll
+        for (int r = 0; r < R2; ++r) w[r] = v[b + r * B2];
+#pragma unroll
+        for (int r = 1; r < R2; ++r) w[r] = cmul(w[r], tw.w2[b * (R2 - 1) + r - 1]);
+        Dft<R2>::run(w);
+#pragma unroll
+        for (int r = 0; r < R2; ++r) v[b + r * B2] = w[r];
+    }
+    if constexpr (P::R3 > 1) {
+        constexpr int R3 = P::R3, B3 = P::B3;
+        Sync::sync();
+#pragma unroll
+        for (int b = 0; b < B2; ++b) {
+            const int j = t + b * T;
+            const int j0 = (j >> 4) * (16 * R2) + (j & 15);
+#pragma unroll
+            for (int r = 0; r < R2; ++r) sm.at(j0 + 16 * r) = v[b + r * B2];
+        }
+        Sync::sync();
+#pragma unroll
+        for (int e = 0; e < 16; ++e) v[e] = sm.at(t + e * T);
+        // stage 3: radix R3, Ns = 16 R2, twiddle base^r
+#pragma unroll
+        for (int b = 0; b < B3; ++b) {
+            float2 w[R3];
+#pragma unroll
+            for (int r = 0; r < R3; ++r) w[r] = v[b + r * B3];
+            float2 p[R3];                                     // p[r] = base^r (balanced products)
+            p[1] = tw.w3[b];
+#pragma unroll
+            for (int r = 2; r < R3; ++r) p[r] = cmul(p[r / 2], p[r - r / 2]);
+#pragma unroll
+            for (int r = 1; r < R3; ++r) w[r] = cmul(w[r], p[r]);
+            Dft<R3>::run(w);
+#pragma unroll
+            for (int r = 0; r < R3; ++r) v[b + r * B3] = w[r];
+        }
+    }
+}
+
+// unnormalised inverse: swap, forward, swap
+template <int N, class Slots, class Sync>
+__device__ __forceinline__ void fft_inverse(float2 (&v)[16], const int t, const Twiddles<N>& tw, const Slots& sm) {
+#pragma unroll
+    for (int e = 0; e < 16; ++e) v[e] = cswap(v[e]);
+    fft_forward<N, Slots, Sync>(v, t, tw, sm);
+#pragma unroll
+    for (int e = 0; e < 16; ++e) v[e] = cswap(v[e]);
+}
+
+}  // namespace psb

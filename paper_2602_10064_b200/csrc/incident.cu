@@ -1,0 +1,255 @@
+// incident.cu — ps_make_incident: incident waves in real space (PAPER.md:378-380 plane wave, "aperture=0";
+// PAPER.md:404-419 focused probe, 30 mrad example; readings A12, A18 of DESIGN.md §3).
+//   plane:  psi0 = 1
+//   tilt:   psi0 = exp(2 pi i (m_t x/Lx + n_t y/Ly)) on a reciprocal-grid point
+//   probe:  Psi0(k) = [lambda |k| <= alpha] A(k) exp(-2 pi i k.r0),  psi0 = ifft2(Psi0) scaled to sum|psi0|^2 = nx ny
+// The probe's k-space fill is generated inside the column pass (no k-space array is stored).
+#include <math.h>
+#include <type_traits>
+
+#include "common.cuh"
+#include "fft_core.cuh"
+
+namespace psb {
+
+__global__ void k_fill_plane_tilt(float2* __restrict__ psi, const int nx, const int ny, const int n,
+                                  const int32_t* __restrict__ tilts /* [n][2] or null */) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long total = (long long)n * nx * ny;
+    if (i >= total) return;
+    if (!tilts) { psi[i] = make_float2(1.f, 0.f); return; }
+    const int ix = (int)(i % nx), iy = (int)((i / nx) % ny), p = (int)(i / ((long long)nx * ny));
+    const int mt = tilts[2 * p], nt = tilts[2 * p + 1];
+    const int a = (int)(((long long)mt * ix) % nx + nx) % nx, b = (int)(((long long)nt * iy) % ny + ny) % ny;
+    float s, c;
+    sincospif(2.0f * ((float)a / (float)nx + (float)b / (float)ny), &s, &c);
+    psi[i] = make_float2(c, s);
+}
+
+template <int NY> struct PColCfg {
+    static constexpr int T = Plan<NY>::T;
+    static constexpr int C = (NY <= 512) ? 16 : ((NY == 1024) ? 8 : 4);
+    static constexpr int THREADS = C * T;
+    static constexpr size_t SMEM = (size_t)NY * C * sizeof(float2);
+};
+
+// column pass of the probe: generate Psi0(kx, :) and inverse-transform along y -> mixed layout
+template <int NY>
+__global__ void __launch_bounds__(PColCfg<NY>::THREADS)
+k_probe_col(float2* __restrict__ psi, const int nx, const int32_t* __restrict__ tiles, const int n_tiles,
+            const int32_t* __restrict__ pmax /* [nx] per-column limit of |n| inside probe aperture and band limit */,
+            const uint32_t* __restrict__ U0 /* [n][2] fixed-point probe positions */, const float scale,
+            const int n_items) {
+    using Cfg = PColCfg<NY>;
+    constexpr int T = Cfg::T, C = Cfg::C, SUB = kColTile / C;
+    extern __shared__ float2 smem[];
+    const int c = threadIdx.x % C, t = threadIdx.x / C;
+    ColSlots<C> slots{smem + c};
+    Twiddles<NY> tw;
+    tw.init(t);
+    const int per_wave = n_tiles * SUB;
+    for (int item = blockIdx.x; item < n_items; item += gridDim.x) {
+        const int p = item / per_wave, rem = item % per_wave;
+        const int kx = tiles[rem / SUB] * kColTile + (rem % SUB) * C + c;
+        const int m = kx < nx / 2 ? kx : kx - nx;
+        const int nm = pmax[kx];
+        const uint32_t ux = U0[2 * p], uy = U0[2 * p + 1];
+        float2 v[16];
+#pragma unroll
+        for (int e = 0; e < 16; ++e) {
+            const int iy = t + e * T;
+            const int n = iy < NY / 2 ? iy : iy - NY;
+            float2 z = make_float2(0.f, 0.f);
+            if (abs(n) <= nm) {
+                const uint32_t ph = (uint32_t)m * ux + (uint32_t)n * uy;
+                float s, cc;
+                sincospif((float)(ph >> 8) * (2.0f / 16777216.0f), &s, &cc);
+                z = make_float2(cc * scale, -s * scale);
+            }
+            v[e] = z;
+        }
+        fft_inverse<NY, ColSlots<C>, BlockSync>(v, t, tw, slots);
+        float2* dst = psi + (size_t)p * NY * nx + kx;
+#pragma unroll
+        for (int e = 0; e < 16; ++e) dst[(size_t)(t + e * T) * nx] = v[e];
+    }
+}
+
+template <int NX> struct PRowCfg {
+    static constexpr int T = Plan<NX>::T;
+    static constexpr int THREADS = 256;
+    static constexpr int RPB = THREADS / T;
+    static constexpr size_t SMEM = (size_t)RPB * RowLine<NX>::LEN * sizeof(float2);
+    using Sync = typename std::conditional<(T <= 32), WarpSync, BlockSync>::type;
+};
+
+// in-place inverse row transform of the mixed array (only active column tiles hold data)
+template <int NX>
+__global__ void __launch_bounds__(PRowCfg<NX>::THREADS)
+k_row_ifft(float2* __restrict__ psi, const uint8_t* __restrict__ tile_active, const long long n_rows,
+           const int n_items) {
+    using Cfg = PRowCfg<NX>;
+    constexpr int T = Cfg::T;
+    extern __shared__ float2 smem[];
+    const int t = threadIdx.x % T, r = threadIdx.x / T;
+    RowSlots slots{smem + (size_t)r * RowLine<NX>::LEN};
+    Twiddles<NX> tw;
+    tw.init(t);
+    unsigned amask = 0;
+#pragma unroll
+    for (int e = 0; e < 16; ++e) amask |= (tile_active[(t + e * T) / kColTile] ? 1u : 0u) << e;
+    for (int item = blockIdx.x; item < n_items; item += gridDim.x) {
+        const long long rho = (long long)item * Cfg::RPB + r;
+        const bool valid = rho < n_rows;
+        float2* row = psi + (size_t)(valid ? rho : 0) * NX;
+        float2 v[16];
+#pragma unroll
+        for (int e = 0; e < 16; ++e)
+            v[e] = (valid && ((amask >> e) & 1u)) ? row[t + e * T] : make_float2(0.f, 0.f);
+        fft_inverse<NX, RowSlots, typename Cfg::Sync>(v, t, tw, slots);
+        if (valid) {
+#pragma unroll
+            for (int e = 0; e < 16; ++e) row[t + e * T] = v[e];
+        }
+    }
+}
+
+template <class K>
+static int blocks_cap_i(K kernel, int threads, size_t smem) {
+    int per_sm = 1, dev = 0, n_sm = kNumSM;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, smem) != cudaSuccess || per_sm < 1)
+        per_sm = 1;
+    return n_sm * per_sm;
+}
+
+template <int NY>
+static cudaError_t launch_probe_col(ps_ctx* c, float2* psi, const int32_t* pmax, const uint32_t* U0, float scale, int n) {
+    using Cfg = PColCfg<NY>;
+    auto kern = k_probe_col<NY>;
+    static int cap = 0;
+    if (!cap) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
+        if (e != cudaSuccess) return e;
+        cap = blocks_cap_i(kern, Cfg::THREADS, Cfg::SMEM);
+    }
+    const int n_items = n * c->n_tiles_active * (kColTile / Cfg::C);
+    kern<<<n_items < cap ? n_items : cap, Cfg::THREADS, Cfg::SMEM, c->stream>>>(psi, c->nx, c->d_tiles, c->n_tiles_active,
+                                                                               pmax, U0, scale, n_items);
+    return cudaGetLastError();
+}
+
+template <int NX>
+static cudaError_t launch_row_ifft(ps_ctx* c, float2* psi, int n) {
+    using Cfg = PRowCfg<NX>;
+    auto kern = k_row_ifft<NX>;
+    static int cap = 0;
+    if (!cap) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
+        if (e != cudaSuccess) return e;
+        cap = blocks_cap_i(kern, Cfg::THREADS, Cfg::SMEM);
+    }
+    const long long n_rows = (long long)n * c->ny;
+    const int n_items = (int)((n_rows + Cfg::RPB - 1) / Cfg::RPB);
+    kern<<<n_items < cap ? n_items : cap, Cfg::THREADS, Cfg::SMEM, c->stream>>>(psi, c->d_tile_active, n_rows, n_items);
+    return cudaGetLastError();
+}
+
+#define PSB_DISPATCH_N(n, CALL)                                                    \
+    switch (n) {                                                                   \
+        case 32: { constexpr int N_ = 32; CALL; } break;                           \
+        case 64: { constexpr int N_ = 64; CALL; } break;                           \
+        case 128: { constexpr int N_ = 128; CALL; } break;                         \
+        case 256: { constexpr int N_ = 256; CALL; } break;                         \
+        case 512: { constexpr int N_ = 512; CALL; } break;                         \
+        case 1024: { constexpr int N_ = 1024; CALL; } break;                       \
+        case 2048: { constexpr int N_ = 2048; CALL; } break;                       \
+        default: break;                                                            \
+    }
+
+static uint32_t host_fixed(double pos, double L) {
+    const double q = pos / L;
+    const double u = q - floor(q);
+    double U = floor(u * 4294967296.0);
+    if (U > 4294967295.0) U = 4294967295.0;
+    return (uint32_t)U;
+}
+
+}  // namespace psb
+
+using namespace psb;
+
+extern "C" ps_status ps_make_incident(ps_ctx* c, double kV, double semi_angle_mrad, int n, const double* xy_or_tilt,
+                                      int is_tilt, void* d_psi0) {
+    if (!c) return PS_EINVAL;
+    if (!c->have_geom) return fail(c, PS_ESTATE, "ps_make_incident: ps_set_geometry has not been called");
+    if (!d_psi0 || n < 1 || !(kV > 0.0) || semi_angle_mrad < 0.0)
+        return fail(c, PS_EINVAL, "ps_make_incident: null pointer, non-positive count/voltage or negative angle");
+    const int nx = c->nx, ny = c->ny;
+    float2* psi = (float2*)d_psi0;
+    const long long total = (long long)n * nx * ny;
+    const bool probe = !is_tilt && semi_angle_mrad > 0.0;
+    if ((is_tilt || probe) && !xy_or_tilt) return fail(c, PS_EINVAL, "ps_make_incident: xy_or_tilt is NULL");
+
+    if (!probe) {
+        int32_t* d_t = nullptr;
+        if (is_tilt) {
+            std::vector<int32_t> h(2 * (size_t)n);
+            for (int i = 0; i < 2 * n; ++i) {
+                const double v = xy_or_tilt[i];
+                if (v != floor(v) || fabs(v) > 1e6) return fail(c, PS_EINVAL, "ps_make_incident: tilt indices must be integers");
+                h[i] = (int32_t)v;
+            }
+            ps_status st = ensure_buf(c, c->misc, 4096 + h.size() * 4);
+            if (st != PS_OK) return st;
+            d_t = (int32_t*)((char*)c->misc.p + 4096);
+            PSB_CUDA(c, cudaMemcpyAsync(d_t, h.data(), h.size() * 4, cudaMemcpyHostToDevice, c->stream));
+            PSB_CUDA(c, cudaStreamSynchronize(c->stream));                   // h is a stack-lifetime buffer
+        }
+        k_fill_plane_tilt<<<(unsigned)((total + 255) / 256), 256, 0, c->stream>>>(psi, nx, ny, n, d_t);
+        PSB_LAUNCH_CHECK(c, "k_fill_plane_tilt");
+        return PS_OK;
+    }
+
+    // focused probe: per-column limits of the probe aperture (float64, same predicate as the definition)
+    const double lam = kHC_keVA / sqrt(kV * (2.0 * kM0C2_keV + kV));
+    const double alpha = semi_angle_mrad * 1.0e-3;
+    std::vector<int32_t> pmax(nx, -1);
+    long long n_ap = 0;
+    for (int ix = 0; ix < nx; ++ix) {
+        const double kx = signed_index(ix, nx) / c->cell[0];
+        int best = -1;
+        for (int nn = 0; nn <= c->h_nmax[ix]; ++nn) {
+            const double ky = nn / c->cell[1];
+            const double k2 = kx * kx + ky * ky;
+            if (lam * sqrt(k2) <= alpha) best = nn; else break;
+        }
+        pmax[ix] = best;
+        if (best >= 0) n_ap += 2 * best + 1;
+    }
+    if (n_ap == 0) return fail(c, PS_EINVAL, "ps_make_incident: probe aperture holds no grid point");
+    std::vector<uint32_t> U0(2 * (size_t)n);
+    for (int i = 0; i < n; ++i) {
+        U0[2 * i] = host_fixed(xy_or_tilt[2 * i], c->cell[0]);
+        U0[2 * i + 1] = host_fixed(xy_or_tilt[2 * i + 1], c->cell[1]);
+    }
+    const size_t need = 4096 + (size_t)nx * 4 + 256 + U0.size() * 4;
+    ps_status st = ensure_buf(c, c->misc, need);
+    if (st != PS_OK) return st;
+    int32_t* d_pmax = (int32_t*)((char*)c->misc.p + 4096);
+    uint32_t* d_U0 = (uint32_t*)((char*)c->misc.p + 4096 + (((size_t)nx * 4 + 255) & ~(size_t)255));
+    PSB_CUDA(c, cudaMemcpyAsync(d_pmax, pmax.data(), (size_t)nx * 4, cudaMemcpyHostToDevice, c->stream));
+    PSB_CUDA(c, cudaMemcpyAsync(d_U0, U0.data(), U0.size() * 4, cudaMemcpyHostToDevice, c->stream));
+    PSB_CUDA(c, cudaStreamSynchronize(c->stream));
+    const float scale = (float)(1.0 / sqrt((double)n_ap));
+    cudaError_t e = cudaErrorInvalidValue;
+    PSB_DISPATCH_N(ny, (e = launch_probe_col<N_>(c, psi, d_pmax, d_U0, scale, n)));
+    if (e != cudaSuccess) return fail(c, PS_ECUDA, std::string("k_probe_col: ") + cudaGetErrorString(e));
+    c->launches++;
+    e = cudaErrorInvalidValue;
+    PSB_DISPATCH_N(nx, (e = launch_row_ifft<N_>(c, psi, n)));
+    if (e != cudaSuccess) return fail(c, PS_ECUDA, std::string("k_row_ifft: ") + cudaGetErrorString(e));
+    c->launches++;
+    return PS_OK;
+}

@@ -1,0 +1,496 @@
+// potential.cu — ps_build_slices: projected potential of every slice of every frame (§2.2):
+//     V_s(k) = sum_{j in slice s} f_Zj(|k|) exp(-2 pi i k.r_j),   V_s(r) = inverse FFT of V_s(k)
+// with f(q) = sum a_i/(q^2+b_i) + sum c_i exp(-d_i q^2) tabulated per element on the band-limited
+// half plane (A2, A5, A10).  Pipeline per chunk of frames:
+//   k_bin      float32 positions -> 2^-32 fixed-point fractions, slice index, (slice, element) key   (a0)
+//   k_sort     stable counting sort of each frame's atoms by key (one warp per frame, deterministic)
+//   k_vk       structure factor x form factor on the in-aperture half plane, direct separable sum    (a2)
+//   k_v_col    Hermitian completion + two slices packed as re/im + inverse column FFT                (a3)
+//   k_v_row    inverse row FFT, unpack -> V[f][s][ny][nx] float32 (V*Angstrom)
+// Phases are formed as (m * U) mod 2^32 in integer arithmetic, so their error does not grow with |m|.
+#include <type_traits>
+
+#include "common.cuh"
+#include "fft_core.cuh"
+
+namespace psb {
+
+// ------------------------------------------------------------------------------------ a0: ingest
+__global__ void k_check_Z(const int32_t* __restrict__ Z, const int n_atoms, const int32_t* __restrict__ elem_of_Z,
+                          int* __restrict__ flag) {
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= n_atoms) return;
+    const int z = Z[j];
+    if (z < 1 || z > 127 || elem_of_Z[z] < 0) atomicExch(flag, z == 0 ? -1 : z);
+}
+
+__device__ __forceinline__ uint32_t to_fixed(const float pos, const double L) {
+    const double q = __ddiv_rn((double)pos, L);
+    const double u = __dsub_rn(q, floor(q));
+    double U = floor(__dmul_rn(u, 4294967296.0));
+    if (U > 4294967295.0) U = 4294967295.0;
+    return (uint32_t)U;
+}
+
+__global__ void k_bin(const float* __restrict__ pos, const int32_t* __restrict__ Z,
+                      const int32_t* __restrict__ elem_of_Z, const long long n_total, const int n_atoms,
+                      const double Lx, const double Ly, const double Lz, const int n_slices, const int n_elem,
+                      uint32_t* __restrict__ Ux, uint32_t* __restrict__ Uy, int32_t* __restrict__ key,
+                      int32_t* __restrict__ slice_idx) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_total) return;
+    const int j = (int)(i % n_atoms);
+    const float x = pos[3 * i], y = pos[3 * i + 1], z = pos[3 * i + 2];
+    Ux[i] = to_fixed(x, Lx);
+    Uy[i] = to_fixed(y, Ly);
+    const uint32_t Uz = to_fixed(z, Lz);
+    const int s = (int)(((unsigned long long)Uz * (unsigned long long)n_slices) >> 32);
+    const int zz = Z[j];
+    const int e = (zz >= 1 && zz <= 127) ? elem_of_Z[zz] : -1;
+    key[i] = (e >= 0) ? s * n_elem + e : -1;
+    if (slice_idx) slice_idx[i] = s;
+}
+
+// one warp per frame: histogram, exclusive scan, stable placement
+__global__ void __launch_bounds__(32)
+k_sort(const uint32_t* __restrict__ Ux, const uint32_t* __restrict__ Uy, const int32_t* __restrict__ key,
+       const int n_atoms, const int n_bins, uint32_t* __restrict__ sUx, uint32_t* __restrict__ sUy,
+       int32_t* __restrict__ offsets) {
+    extern __shared__ int cursor[];                       // [n_bins + 1]
+    const int f = blockIdx.x, lane = threadIdx.x;
+    const size_t base = (size_t)f * n_atoms;
+    for (int b = lane; b <= n_bins; b += 32) cursor[b] = 0;
+    __syncwarp();
+    for (int j = lane; j < n_atoms; j += 32) {
+        const int k = key[base + j];
+        if (k >= 0) atomicAdd(&cursor[k], 1);
+    }
+    __syncwarp();
+    int carry = 0;                                        // exclusive scan, 32 bins at a time
+    for (int b0 = 0; b0 <= n_bins; b0 += 32) {
+        const int b = b0 + lane;
+        const int cnt = (b < n_bins) ? cursor[b] : 0;
+        int incl = cnt;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const int o = __shfl_up_sync(0xffffffffu, incl, d);
+            if (lane >= d) incl += o;
+        }
+        const int excl = carry + incl - cnt;
+        if (b <= n_bins) {
+            cursor[b] = excl;
+            offsets[(size_t)f * (n_bins + 1) + b] = excl;
+        }
+        carry += __shfl_sync(0xffffffffu, incl, 31);
+    }
+    __syncwarp();
+    for (int j0 = 0; j0 < n_atoms; j0 += 32) {
+        const int j = j0 + lane;
+        const int k = (j < n_atoms) ? key[base + j] : -1;
+        const unsigned grp = __match_any_sync(0xffffffffu, k);
+        const int rank = __popc(grp & ((1u << lane) - 1u));
+        int dst = -1;
+        if (k >= 0) dst = cursor[k] + rank;
+        __syncwarp();
+        if (k >= 0 && rank == __popc(grp) - 1) cursor[k] += __popc(grp);
+        __syncwarp();
+        if (dst >= 0) {
+            sUx[base + dst] = Ux[base + j];
+            sUy[base + dst] = Uy[base + j];
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------ a2: V(k) assembly
+constexpr int VK_TM = 64, VK_TN = 32, VK_CH = 32, VK_THREADS = 128;
+
+__device__ __forceinline__ float2 phase_factor(const int m, const uint32_t U) {
+    // exp(-2 pi i m u), u = U/2^32: fraction (m*U mod 2^32) exactly, then 24 bits into fp32
+    const uint32_t ph = (uint32_t)m * U;
+    float s, c;
+    sincospif((float)(ph >> 8) * (2.0f / 16777216.0f), &s, &c);
+    return make_float2(c, -s);
+}
+
+__global__ void __launch_bounds__(VK_THREADS)
+k_vk(const uint32_t* __restrict__ sUx, const uint32_t* __restrict__ sUy, const int32_t* __restrict__ offsets,
+     const float* __restrict__ ftab, const int32_t* __restrict__ nmax, float2* __restrict__ Vk, const int n_atoms,
+     const int n_slices, const int n_elem, const int mcut, const int ncut, const int nx, const int tiles_m) {
+    __shared__ __align__(16) float2 ex[VK_CH][VK_TM];
+    __shared__ __align__(16) float2 ey[VK_CH][VK_TN];
+    const int f = blockIdx.z, s = blockIdx.y;
+    const int tmx = blockIdx.x % tiles_m, tny = blockIdx.x / tiles_m;
+    const int m0 = -mcut + tmx * VK_TM, n0 = tny * VK_TN;
+    const int mw = 2 * mcut + 1, nh = ncut + 1;
+    const int n_bins = n_slices * n_elem;
+    const int32_t* off = offsets + (size_t)f * (n_bins + 1) + (size_t)s * n_elem;
+    if (off[n_elem] == off[0]) return;                                     // empty slice: Vk left unwritten
+    const int tx = threadIdx.x % 16, ty = threadIdx.x / 16;
+    const size_t abase = (size_t)f * n_atoms;
+    float2* out = Vk + ((size_t)f * n_slices + s) * nh * mw;
+
+    // is any point of this tile inside the aperture?
+    int inside = 0;
+    if (threadIdx.x < VK_TM) {
+        const int m = m0 + threadIdx.x;
+        if (m <= mcut) inside = nmax[m < 0 ? m + nx : m] >= n0;
+    }
+    inside = __syncthreads_or(inside);
+    float2 tot[4][4];
+#pragma unroll
+    for (int a = 0; a < 4; ++a)
+#pragma unroll
+        for (int b = 0; b < 4; ++b) tot[a][b] = make_float2(0.f, 0.f);
+
+    if (inside) {
+        for (int e = 0; e < n_elem; ++e) {
+            const int jb = off[e], je = off[e + 1];
+            if (jb == je) continue;
+            float2 acc[4][4];
+#pragma unroll
+            for (int a = 0; a < 4; ++a)
+#pragma unroll
+                for (int b = 0; b < 4; ++b) acc[a][b] = make_float2(0.f, 0.f);
+            for (int j0 = jb; j0 < je; j0 += VK_CH) {
+                const int cnt = min(VK_CH, je - j0);
+                __syncthreads();
+                for (int i = threadIdx.x; i < cnt * VK_TM; i += VK_THREADS) {
+                    const int jj = i / VK_TM, a = i % VK_TM;
+                    ex[jj][a] = phase_factor(m0 + a, sUx[abase + j0 + jj]);
+                }
+                for (int i = threadIdx.x; i < cnt * VK_TN; i += VK_THREADS) {
+                    const int jj = i / VK_TN, b = i % VK_TN;
+                    ey[jj][b] = phase_factor(n0 + b, sUy[abase + j0 + jj]);
+                }
+                __syncthreads();
+                for (int jj = 0; jj < cnt; ++jj) {
+                    float2 xa[4], yb[4];
+                    const float4 x01 = *reinterpret_cast<const float4*>(&ex[jj][tx * 4]);
+                    const float4 x23 = *reinterpret_cast<const float4*>(&ex[jj][tx * 4 + 2]);
+                    const float4 y01 = *reinterpret_cast<const float4*>(&ey[jj][ty * 4]);
+                    const float4 y23 = *reinterpret_cast<const float4*>(&ey[jj][ty * 4 + 2]);
+                    xa[0] = make_float2(x01.x, x01.y); xa[1] = make_float2(x01.z, x01.w);
+                    xa[2] = make_float2(x23.x, x23.y); xa[3] = make_float2(x23.z, x23.w);
+                    yb[0] = make_float2(y01.x, y01.y); yb[1] = make_float2(y01.z, y01.w);
+                    yb[2] = make_float2(y23.x, y23.y); yb[3] = make_float2(y23.z, y23.w);
+#pragma unroll
+                    for (int a = 0; a < 4; ++a)
+#pragma unroll
+                        for (int b = 0; b < 4; ++b) {
+                            acc[a][b].x = fmaf(xa[a].x, yb[b].x, acc[a][b].x);
+                            acc[a][b].x = fmaf(-xa[a].y, yb[b].y, acc[a][b].x);
+                            acc[a][b].y = fmaf(xa[a].x, yb[b].y, acc[a][b].y);
+                            acc[a][b].y = fmaf(xa[a].y, yb[b].x, acc[a][b].y);
+                        }
+                }
+            }
+            const float* ft = ftab + (size_t)e * nh * mw;
+#pragma unroll
+            for (int a = 0; a < 4; ++a)
+#pragma unroll
+                for (int b = 0; b < 4; ++b) {
+                    const int m = m0 + tx * 4 + a, n = n0 + ty * 4 + b;
+                    if (m <= mcut && n <= ncut) {
+                        const float fv = __ldg(ft + (size_t)n * mw + (m + mcut));
+                        tot[a][b].x = fmaf(fv, acc[a][b].x, tot[a][b].x);
+                        tot[a][b].y = fmaf(fv, acc[a][b].y, tot[a][b].y);
+                    }
+                }
+        }
+    }
+#pragma unroll
+    for (int a = 0; a < 4; ++a)
+#pragma unroll
+        for (int b = 0; b < 4; ++b) {
+            const int m = m0 + tx * 4 + a, n = n0 + ty * 4 + b;
+            if (m <= mcut && n <= ncut) out[(size_t)n * mw + (m + mcut)] = tot[a][b];
+        }
+}
+
+// ------------------------------------------------------------------------------------ a3: inverse FFT of slice pairs
+template <int NY> struct VColCfg {
+    static constexpr int T = Plan<NY>::T;
+    static constexpr int C = (NY <= 512) ? 16 : ((NY == 1024) ? 8 : 4);
+    static constexpr int THREADS = C * T;
+    static constexpr size_t SMEM = (size_t)NY * C * sizeof(float2);
+};
+
+// reads the half-plane box of Va (slice 2*pr) and Vb (slice 2*pr+1), forms z = Va + i Vb on the full
+// plane by Hermitian symmetry, inverse-transforms along y, writes the mixed array Zm[f][pr][y][kx].
+template <int NY>
+__global__ void __launch_bounds__(VColCfg<NY>::THREADS)
+k_v_col(const float2* __restrict__ Vk, const int32_t* __restrict__ offsets, float2* __restrict__ Zm, const int nx,
+        const int32_t* __restrict__ tiles, const int n_tiles, const int32_t* __restrict__ nmax, const int n_slices,
+        const int n_elem, const int mcut, const int ncut, const int n_pairs, const int n_items) {
+    using Cfg = VColCfg<NY>;
+    constexpr int T = Cfg::T, C = Cfg::C, SUB = kColTile / C;
+    extern __shared__ float2 smem[];
+    const int c = threadIdx.x % C, t = threadIdx.x / C;
+    ColSlots<C> slots{smem + c};
+    Twiddles<NY> tw;
+    tw.init(t);
+    const int per_pair = n_tiles * SUB;
+    const int mw = 2 * mcut + 1, nh = ncut + 1, n_bins = n_slices * n_elem;
+
+    for (int item = blockIdx.x; item < n_items; item += gridDim.x) {
+        const int fp = item / per_pair, rem = item % per_pair;
+        const int f = fp / n_pairs, pr = fp % n_pairs;
+        const int sa = 2 * pr, sb = 2 * pr + 1;
+        const int32_t* off = offsets + (size_t)f * (n_bins + 1);
+        const bool has_a = off[(sa + 1) * n_elem] > off[sa * n_elem];
+        const bool has_b = (sb < n_slices) && off[(sb + 1) * n_elem] > off[sb * n_elem];
+        if (!has_a && !has_b) continue;                                    // block-uniform
+        const int kx = tiles[rem / SUB] * kColTile + (rem % SUB) * C + c;
+        const int m = kx < nx / 2 ? kx : kx - nx;
+        const int nm = nmax[kx];
+        const float2* Va = Vk + ((size_t)f * n_slices + sa) * nh * mw;
+        const float2* Vb = Vk + ((size_t)f * n_slices + sb) * nh * mw;
+        float2 v[16];
+#pragma unroll
+        for (int e = 0; e < 16; ++e) {
+            const int iy = t + e * T;
+            const int n = iy < NY / 2 ? iy : iy - NY;
+            float2 z = make_float2(0.f, 0.f);
+            if (abs(n) <= nm) {
+                const bool direct = (n > 0) || (n == 0 && m >= 0);
+                const size_t idx = direct ? (size_t)n * mw + (m + mcut) : (size_t)(-n) * mw + (mcut - m);
+                const float2 a = has_a ? __ldg(Va + idx) : make_float2(0.f, 0.f);
+                const float2 b = has_b ? __ldg(Vb + idx) : make_float2(0.f, 0.f);
+                z = direct ? make_float2(a.x - b.y, a.y + b.x) : make_float2(a.x + b.y, b.x - a.y);
+            }
+            v[e] = z;
+        }
+        fft_inverse<NY, ColSlots<C>, BlockSync>(v, t, tw, slots);
+        float2* dst = Zm + ((size_t)fp * NY) * nx + kx;
+#pragma unroll
+        for (int e = 0; e < 16; ++e) dst[(size_t)(t + e * T) * nx] = v[e];
+    }
+}
+
+template <int NX> struct VRowCfg {
+    static constexpr int T = Plan<NX>::T;
+    static constexpr int THREADS = 256;
+    static constexpr int RPB = THREADS / T;
+    static constexpr size_t SMEM = (size_t)RPB * RowLine<NX>::LEN * sizeof(float2);
+    using Sync = typename std::conditional<(T <= 32), WarpSync, BlockSync>::type;
+};
+
+template <int NX>
+__global__ void __launch_bounds__(VRowCfg<NX>::THREADS)
+k_v_row(const float2* __restrict__ Zm, const int32_t* __restrict__ offsets, float* __restrict__ V,
+        const uint8_t* __restrict__ tile_active, const int ny, const int n_slices, const int n_elem,
+        const int n_pairs, const long long n_rows, const int n_items) {
+    using Cfg = VRowCfg<NX>;
+    constexpr int T = Cfg::T;
+    extern __shared__ float2 smem[];
+    const int t = threadIdx.x % T, r = threadIdx.x / T;
+    RowSlots slots{smem + (size_t)r * RowLine<NX>::LEN};
+    Twiddles<NX> tw;
+    tw.init(t);
+    unsigned amask = 0;
+#pragma unroll
+    for (int e = 0; e < 16; ++e) amask |= (tile_active[(t + e * T) / kColTile] ? 1u : 0u) << e;
+    const int n_bins = n_slices * n_elem;
+
+    for (int item = blockIdx.x; item < n_items; item += gridDim.x) {
+        const long long rho = (long long)item * Cfg::RPB + r;
+        const bool valid = rho < n_rows;
+        int y = 0, fp = 0;
+        if (valid) { fp = (int)(rho / ny); y = (int)(rho % ny); }
+        const int f = fp / n_pairs, pr = fp % n_pairs;
+        const int sa = 2 * pr, sb = 2 * pr + 1;
+        const int32_t* off = offsets + (size_t)f * (n_bins + 1);
+        const bool has_a = valid && off[(sa + 1) * n_elem] > off[sa * n_elem];
+        const bool has_b = valid && (sb < n_slices) && off[(sb + 1) * n_elem] > off[sb * n_elem];
+        const bool any = has_a || has_b;
+        const float2* src = Zm + ((size_t)fp * ny + y) * NX;
+        float2 v[16];
+#pragma unroll
+        for (int e = 0; e < 16; ++e)
+            v[e] = (any && ((amask >> e) & 1u)) ? src[t + e * T] : make_float2(0.f, 0.f);
+        fft_inverse<NX, RowSlots, typename Cfg::Sync>(v, t, tw, slots);
+        if (valid) {
+            float* va = V + (((size_t)f * n_slices + sa) * ny + y) * NX;
+#pragma unroll
+            for (int e = 0; e < 16; ++e) va[t + e * T] = v[e].x;
+            if (sb < n_slices) {
+                float* vb = V + (((size_t)f * n_slices + sb) * ny + y) * NX;
+#pragma unroll
+                for (int e = 0; e < 16; ++e) vb[t + e * T] = v[e].y;
+            }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------ host side
+struct ScratchLayout {
+    size_t ux, uy, key, sux, suy, off, vk, zm, total;
+};
+static inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+static ScratchLayout scratch_layout(const ps_ctx* c, int nfc, int n_atoms) {
+    ScratchLayout L;
+    const size_t na = (size_t)nfc * n_atoms;
+    const int n_pairs = (c->n_slices + 1) / 2;
+    size_t o = 0;
+    L.ux = o; o += align256(na * 4);
+    L.uy = o; o += align256(na * 4);
+    L.key = o; o += align256(na * 4);
+    L.sux = o; o += align256(na * 4);
+    L.suy = o; o += align256(na * 4);
+    L.off = o; o += align256((size_t)nfc * ((size_t)c->n_slices * c->n_elem + 1) * 4);
+    L.vk = o; o += align256((size_t)nfc * c->n_slices * (c->ncut + 1) * (2 * c->mcut + 1) * sizeof(float2));
+    L.zm = o; o += align256((size_t)nfc * n_pairs * c->nx * c->ny * sizeof(float2));
+    L.total = o + 256;
+    return L;
+}
+
+template <class K>
+static int blocks_cap(K kernel, int threads, size_t smem) {
+    int per_sm = 1, dev = 0, n_sm = kNumSM;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, smem) != cudaSuccess || per_sm < 1)
+        per_sm = 1;
+    return n_sm * per_sm;
+}
+
+template <int NY>
+static cudaError_t launch_v_col(ps_ctx* c, const float2* Vk, const int32_t* off, float2* Zm, int nfc) {
+    using Cfg = VColCfg<NY>;
+    auto kern = k_v_col<NY>;
+    static int cap = 0;
+    if (!cap) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
+        if (e != cudaSuccess) return e;
+        cap = blocks_cap(kern, Cfg::THREADS, Cfg::SMEM);
+    }
+    const int n_pairs = (c->n_slices + 1) / 2;
+    const long long n_items = (long long)nfc * n_pairs * c->n_tiles_active * (kColTile / Cfg::C);
+    const int grid = (int)(n_items < cap ? n_items : cap);
+    kern<<<grid, Cfg::THREADS, Cfg::SMEM, c->stream>>>(Vk, off, Zm, c->nx, c->d_tiles, c->n_tiles_active, c->d_nmax,
+                                                      c->n_slices, c->n_elem, c->mcut, c->ncut, n_pairs, (int)n_items);
+    return cudaGetLastError();
+}
+
+template <int NX>
+static cudaError_t launch_v_row(ps_ctx* c, const float2* Zm, const int32_t* off, float* V, int nfc) {
+    using Cfg = VRowCfg<NX>;
+    auto kern = k_v_row<NX>;
+    static int cap = 0;
+    if (!cap) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
+        if (e != cudaSuccess) return e;
+        cap = blocks_cap(kern, Cfg::THREADS, Cfg::SMEM);
+    }
+    const int n_pairs = (c->n_slices + 1) / 2;
+    const long long n_rows = (long long)nfc * n_pairs * c->ny;
+    const long long n_items = (n_rows + Cfg::RPB - 1) / Cfg::RPB;
+    const int grid = (int)(n_items < cap ? n_items : cap);
+    kern<<<grid, Cfg::THREADS, Cfg::SMEM, c->stream>>>(Zm, off, V, c->d_tile_active, c->ny, c->n_slices, c->n_elem,
+                                                      n_pairs, n_rows, (int)n_items);
+    return cudaGetLastError();
+}
+
+#define PSB_DISPATCH_N(n, CALL)                                                    \
+    switch (n) {                                                                   \
+        case 32: { constexpr int N_ = 32; CALL; } break;                           \
+        case 64: { constexpr int N_ = 64; CALL; } break;                           \
+        case 128: { constexpr int N_ = 128; CALL; } break;                         \
+        case 256: { constexpr int N_ = 256; CALL; } break;                         \
+        case 512: { constexpr int N_ = 512; CALL; } break;                         \
+        case 1024: { constexpr int N_ = 1024; CALL; } break;                       \
+        case 2048: { constexpr int N_ = 2048; CALL; } break;                       \
+        default: break;                                                            \
+    }
+
+}  // namespace psb
+
+using namespace psb;
+
+extern "C" size_t ps_workspace_bytes(const ps_ctx* c, int n_frames_chunk, int n_atoms) {
+    if (!c || !c->have_geom || !c->have_ff || n_frames_chunk < 1 || n_atoms < 1) return 0;
+    return scratch_layout(c, n_frames_chunk, n_atoms).total;
+}
+
+extern "C" ps_status ps_build_slices(ps_ctx* c, const float* d_pos, const int32_t* d_Z, int n_frames, int n_atoms,
+                                     float* d_V, int32_t* d_slice_idx) {
+    if (!c) return PS_EINVAL;
+    if (!c->have_geom || !c->have_ff)
+        return fail(c, PS_ESTATE, "ps_build_slices: ps_set_geometry and ps_set_form_factors must be called first");
+    if (!d_pos || !d_Z || !d_V || n_frames < 1 || n_atoms < 1)
+        return fail(c, PS_EINVAL, "ps_build_slices: null pointer or non-positive size");
+    ps_status st = ensure_ftab(c);
+    if (st != PS_OK) return st;
+    const long long n_bins = (long long)c->n_slices * c->n_elem;
+    if ((n_bins + 1) * 4 > 200 * 1024)
+        return fail(c, PS_EUNSUPPORTED, "ps_build_slices: n_slices * n_elements too large for the sort kernel");
+
+    // validate Z (one 4-byte read-back before any work is queued; the rest of the call is asynchronous)
+    if ((st = ensure_buf(c, c->misc, 4096)) != PS_OK) return st;
+    int* d_flag = (int*)c->misc.p;
+    PSB_CUDA(c, cudaMemsetAsync(d_flag, 0, sizeof(int), c->stream));
+    k_check_Z<<<(n_atoms + 255) / 256, 256, 0, c->stream>>>(d_Z, n_atoms, c->d_elem_of_Z, d_flag);
+    PSB_LAUNCH_CHECK(c, "k_check_Z");
+    int h_flag = 0;
+    PSB_CUDA(c, cudaMemcpyAsync(&h_flag, d_flag, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    PSB_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (h_flag != 0)
+        return fail(c, PS_EUNSUPPORTED, "ps_build_slices: atomic number " + std::to_string(h_flag) +
+                                            " has no form-factor coefficients");
+
+    // scratch: installed workspace or library-owned buffer; frames are processed in chunks that fit
+    const size_t per_frame = scratch_layout(c, 1, n_atoms).total;
+    size_t avail = c->user_ws ? c->user_ws_bytes : (size_t)768 * 1024 * 1024;
+    int nfc = (int)(avail / per_frame);
+    if (nfc < 1) {
+        if (c->user_ws) return fail(c, PS_EWORKSPACE, "ps_build_slices: workspace smaller than one frame needs (" +
+                                                          std::to_string(per_frame) + " bytes)");
+        nfc = 1;
+    }
+    if (nfc > n_frames) nfc = n_frames;
+    ScratchLayout L = scratch_layout(c, nfc, n_atoms);
+    while (c->user_ws && L.total > c->user_ws_bytes && nfc > 1) L = scratch_layout(c, --nfc, n_atoms);
+    char* ws = (char*)c->user_ws;
+    if (!ws) {
+        if ((st = ensure_buf(c, c->scratch, L.total)) != PS_OK) return st;
+        ws = (char*)c->scratch.p;
+    } else if (L.total > c->user_ws_bytes) {
+        return fail(c, PS_EWORKSPACE, "ps_build_slices: workspace too small");
+    }
+    uint32_t *Ux = (uint32_t*)(ws + L.ux), *Uy = (uint32_t*)(ws + L.uy);
+    uint32_t *sUx = (uint32_t*)(ws + L.sux), *sUy = (uint32_t*)(ws + L.suy);
+    int32_t *key = (int32_t*)(ws + L.key), *off = (int32_t*)(ws + L.off);
+    float2 *Vk = (float2*)(ws + L.vk), *Zm = (float2*)(ws + L.zm);
+
+    const int tiles_m = (2 * c->mcut + 1 + VK_TM - 1) / VK_TM, tiles_n = (c->ncut + 1 + VK_TN - 1) / VK_TN;
+    const size_t img = (size_t)c->nx * c->ny;
+    static bool sort_attr = false;
+    if (!sort_attr) {
+        PSB_CUDA(c, cudaFuncSetAttribute(k_sort, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+        sort_attr = true;
+    }
+
+    for (int f0 = 0; f0 < n_frames; f0 += nfc) {
+        const int nf = (n_frames - f0 < nfc) ? n_frames - f0 : nfc;
+        const long long n_total = (long long)nf * n_atoms;
+        k_bin<<<(unsigned)((n_total + 255) / 256), 256, 0, c->stream>>>(
+            d_pos + (size_t)f0 * n_atoms * 3, d_Z, c->d_elem_of_Z, n_total, n_atoms, c->cell[0], c->cell[1], c->cell[2],
+            c->n_slices, c->n_elem, Ux, Uy, key, d_slice_idx ? d_slice_idx + (size_t)f0 * n_atoms : nullptr);
+        PSB_LAUNCH_CHECK(c, "k_bin");
+        k_sort<<<nf, 32, (size_t)(n_bins + 1) * sizeof(int), c->stream>>>(Ux, Uy, key, n_atoms, (int)n_bins, sUx, sUy, off);
+        PSB_LAUNCH_CHECK(c, "k_sort");
+        k_vk<<<dim3(tiles_m * tiles_n, c->n_slices, nf), VK_THREADS, 0, c->stream>>>(
+            sUx, sUy, off, c->d_ftab, c->d_nmax, Vk, n_atoms, c->n_slices, c->n_elem, c->mcut, c->ncut, c->nx, tiles_m);
+        PSB_LAUNCH_CHECK(c, "k_vk");
+        cudaError_t e = cudaErrorInvalidValue;
+        PSB_DISPATCH_N(c->ny, (e = launch_v_col<N_>(c, Vk, off, Zm, nf)));
+        if (e != cudaSuccess) return fail(c, PS_ECUDA, std::string("k_v_col: ") + cudaGetErrorString(e));
+        c->launches++;
+        e = cudaErrorInvalidValue;
+        PSB_DISPATCH_N(c->nx, (e = launch_v_row<N_>(c, Zm, off, d_V + (size_t)f0 * c->n_slices * img, nf)));
+        if (e != cudaSuccess) return fail(c, PS_ECUDA, std::string("k_v_row: ") + cudaGetErrorString(e));
+        c->launches++;
+    }
+    return PS_OK;
+}

@@ -1,0 +1,236 @@
+// reduce.cu — reductions over I[P][n_bins][ny][nx] (PAPER.md:89 TACAWData methods; PAPER.md:394 dispersion,
+// 397 spectral_diffraction, 422 spectrum_image, 107 frequency bands; readings A15-A17 of DESIGN.md §3).
+// All sums run in a fixed order (no floating-point atomics): results are bit-reproducible.
+// Index work (detector membership, nearest path pixel, radial q bin) is done in float64 with explicitly
+// rounded operations (no FMA contraction) so that it is bit-exact against the float64 definition.
+#include <math.h>
+
+#include "common.cuh"
+
+namespace psb {
+
+__device__ __forceinline__ double k_abs(const int ix, const int iy, const int nx, const int ny, const double Lx,
+                                        const double Ly) {
+    const int m = ix < (nx + 1) / 2 ? ix : ix - nx, n = iy < (ny + 1) / 2 ? iy : iy - ny;
+    const double kx = __ddiv_rn((double)m, Lx), ky = __ddiv_rn((double)n, Ly);
+    return __dsqrt_rn(__dadd_rn(__dmul_rn(kx, kx), __dmul_rn(ky, ky)));
+}
+
+__device__ __forceinline__ float block_sum(float v, float* sh) {   // fixed-order tree; result valid in thread 0
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) v += __shfl_down_sync(0xffffffffu, v, d);
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    if (lane == 0) sh[w] = v;
+    __syncthreads();
+    if (w == 0) {
+        v = (lane < (blockDim.x + 31) / 32) ? sh[lane] : 0.f;
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) v += __shfl_down_sync(0xffffffffu, v, d);
+    }
+    __syncthreads();
+    return v;
+}
+
+// ---------------------------------------------------------------- spectral diffraction pattern
+__global__ void k_sdp(const float* __restrict__ I, float* __restrict__ out, const int P, const int n_bins,
+                      const int lo, const int hi, const size_t npix) {
+    const size_t pix = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (pix >= npix) return;
+    float s = 0.f;
+    for (int p = 0; p < P; ++p)
+        for (int b = lo; b <= hi; ++b) s += I[((size_t)p * n_bins + b) * npix + pix];
+    out[pix] = s;
+}
+
+// ---------------------------------------------------------------- spectrum image
+__global__ void k_detector_mask(uint8_t* __restrict__ mask, const int nx, const int ny, const double Lx, const double Ly,
+                                const double k_in, const double k_out, const int has_out) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= (size_t)nx * ny) return;
+    const double k = k_abs((int)(i % nx), (int)(i / nx), nx, ny, Lx, Ly);
+    mask[i] = (k >= k_in && (!has_out || k < k_out)) ? 1 : 0;
+}
+
+__global__ void __launch_bounds__(256)
+k_spectrum_image(const float* __restrict__ I, const uint8_t* __restrict__ mask, float* __restrict__ out,
+                 const size_t npix) {
+    __shared__ float sh[32];
+    const float* src = I + (size_t)blockIdx.x * npix;        // blockIdx.x = p * n_bins + b
+    float s = 0.f;
+    for (size_t i = threadIdx.x; i < npix; i += blockDim.x)
+        if (mask[i]) s += src[i];
+    s = block_sum(s, sh);
+    if (threadIdx.x == 0) out[blockIdx.x] = s;
+}
+
+// ---------------------------------------------------------------- dispersion
+__global__ void k_path_pixels(const double* __restrict__ kx, const double* __restrict__ ky, int32_t* __restrict__ pix,
+                              const int n_path, const int nx, const int ny, const double Lx, const double Ly) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_path) return;
+    const long long ax = (long long)floor(__dadd_rn(__dmul_rn(kx[i], Lx), 0.5));
+    const long long ay = (long long)floor(__dadd_rn(__dmul_rn(ky[i], Ly), 0.5));
+    const int ix = (int)(((ax % nx) + nx) % nx), iy = (int)(((ay % ny) + ny) % ny);
+    pix[i] = iy * nx + ix;
+}
+
+__global__ void k_dispersion(const float* __restrict__ I, const int32_t* __restrict__ pix, float* __restrict__ out,
+                             const int P, const int n_bins, const int n_path, const size_t npix) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_bins * n_path) return;
+    const int b = i / n_path, j = i % n_path;
+    float s = 0.f;
+    for (int p = 0; p < P; ++p) s += I[((size_t)p * n_bins + b) * npix + pix[j]];
+    out[i] = s;
+}
+
+// ---------------------------------------------------------------- radial q bins
+__global__ void k_qidx(int32_t* __restrict__ qidx, const int nx, const int ny, const double Lx, const double Ly,
+                       const double dq, const int n_q) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= (size_t)nx * ny) return;
+    const double k = k_abs((int)(i % nx), (int)(i / nx), nx, ny, Lx, Ly);
+    const double b = floor(__ddiv_rn(k, dq));
+    qidx[i] = (b >= (double)n_q) ? -1 : (int32_t)b;
+}
+
+// one warp: histogram + exclusive scan + stable placement of pixel indices by q bin (deterministic order)
+__global__ void __launch_bounds__(32)
+k_order_by_bin(const int32_t* __restrict__ qidx, const int npix, const int n_q, int32_t* __restrict__ cursor /*[n_q+1]*/,
+               int32_t* __restrict__ offsets /*[n_q+1]*/, int32_t* __restrict__ order /*[npix]*/) {
+    const int lane = threadIdx.x;
+    for (int b = lane; b <= n_q; b += 32) cursor[b] = 0;
+    __syncwarp();
+    for (int j = lane; j < npix; j += 32) {
+        const int k = qidx[j];
+        if (k >= 0) atomicAdd(&cursor[k], 1);
+    }
+    __syncwarp();
+    int carry = 0;
+    for (int b0 = 0; b0 <= n_q; b0 += 32) {
+        const int b = b0 + lane;
+        const int cnt = (b < n_q) ? cursor[b] : 0;
+        int incl = cnt;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const int o = __shfl_up_sync(0xffffffffu, incl, d);
+            if (lane >= d) incl += o;
+        }
+        const int excl = carry + incl - cnt;
+        __syncwarp();
+        if (b <= n_q) { cursor[b] = excl; offsets[b] = excl; }
+        carry += __shfl_sync(0xffffffffu, incl, 31);
+    }
+    __syncwarp();
+    for (int j0 = 0; j0 < npix; j0 += 32) {
+        const int j = j0 + lane;
+        const int k = (j < npix) ? qidx[j] : -1;
+        const unsigned grp = __match_any_sync(0xffffffffu, k);
+        const int rank = __popc(grp & ((1u << lane) - 1u));
+        int dst = -1;
+        if (k >= 0) dst = cursor[k] + rank;
+        __syncwarp();
+        if (k >= 0 && rank == __popc(grp) - 1) cursor[k] += __popc(grp);
+        __syncwarp();
+        if (dst >= 0) order[dst] = j;
+    }
+}
+
+// one warp per (bin b, q): ordered segment sum
+__global__ void __launch_bounds__(128)
+k_qbin_sum(const float* __restrict__ I, const int32_t* __restrict__ offsets, const int32_t* __restrict__ order,
+           float* __restrict__ out, const int P, const int n_bins, const int n_q, const size_t npix) {
+    const int wid = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    if (wid >= n_bins * n_q) return;
+    const int b = wid / n_q, q = wid % n_q;
+    const int j0 = offsets[q], j1 = offsets[q + 1];
+    float s = 0.f;
+    for (int j = j0 + lane; j < j1; j += 32) {
+        const int pix = order[j];
+        for (int p = 0; p < P; ++p) s += I[((size_t)p * n_bins + b) * npix + pix];
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) s += __shfl_down_sync(0xffffffffu, s, d);
+    if (lane == 0) out[wid] = s;
+}
+
+}  // namespace psb
+
+using namespace psb;
+
+static ps_status check_I(ps_ctx* c, const char* who, const float* d_I, int P, int n_bins, const void* d_out) {
+    if (!c->have_geom) return fail(c, PS_ESTATE, std::string(who) + ": ps_set_geometry has not been called");
+    if (!d_I || !d_out || P < 1 || n_bins < 1) return fail(c, PS_EINVAL, std::string(who) + ": null pointer or non-positive size");
+    return PS_OK;
+}
+
+extern "C" ps_status ps_sdp(ps_ctx* c, const float* d_I, int P, int n_bins, int bin_lo, int bin_hi, float* d_out) {
+    if (!c) return PS_EINVAL;
+    ps_status st = check_I(c, "ps_sdp", d_I, P, n_bins, d_out);
+    if (st != PS_OK) return st;
+    if (bin_lo < 0 || bin_hi >= n_bins || bin_lo > bin_hi) return fail(c, PS_EINVAL, "ps_sdp: bin range outside [0, n_bins)");
+    const size_t npix = (size_t)c->nx * c->ny;
+    k_sdp<<<(unsigned)((npix + 255) / 256), 256, 0, c->stream>>>(d_I, d_out, P, n_bins, bin_lo, bin_hi, npix);
+    PSB_LAUNCH_CHECK(c, "k_sdp");
+    return PS_OK;
+}
+
+extern "C" ps_status ps_spectrum_image(ps_ctx* c, const float* d_I, int P, int n_bins, double k_in, double k_out,
+                                       float* d_out) {
+    if (!c) return PS_EINVAL;
+    ps_status st = check_I(c, "ps_spectrum_image", d_I, P, n_bins, d_out);
+    if (st != PS_OK) return st;
+    if (k_in < 0.0) return fail(c, PS_EINVAL, "ps_spectrum_image: k_in must be >= 0");
+    const size_t npix = (size_t)c->nx * c->ny;
+    if ((st = ensure_buf(c, c->misc, 4096 + npix)) != PS_OK) return st;
+    uint8_t* d_mask = (uint8_t*)c->misc.p + 4096;
+    k_detector_mask<<<(unsigned)((npix + 255) / 256), 256, 0, c->stream>>>(d_mask, c->nx, c->ny, c->cell[0], c->cell[1], k_in,
+                                                                           k_out, k_out > 0.0 ? 1 : 0);
+    PSB_LAUNCH_CHECK(c, "k_detector_mask");
+    k_spectrum_image<<<P * n_bins, 256, 0, c->stream>>>(d_I, d_mask, d_out, npix);
+    PSB_LAUNCH_CHECK(c, "k_spectrum_image");
+    return PS_OK;
+}
+
+extern "C" ps_status ps_dispersion(ps_ctx* c, const float* d_I, int P, int n_bins, int n_path, const double* kx,
+                                   const double* ky, int32_t* d_pix, float* d_out) {
+    if (!c) return PS_EINVAL;
+    ps_status st = check_I(c, "ps_dispersion", d_I, P, n_bins, d_out);
+    if (st != PS_OK) return st;
+    if (!kx || !ky || !d_pix || n_path < 1) return fail(c, PS_EINVAL, "ps_dispersion: null pointer or empty path");
+    const size_t need = 4096 + 2 * (size_t)n_path * sizeof(double);
+    if ((st = ensure_buf(c, c->misc, need)) != PS_OK) return st;
+    double* d_k = (double*)((char*)c->misc.p + 4096);
+    PSB_CUDA(c, cudaMemcpyAsync(d_k, kx, (size_t)n_path * 8, cudaMemcpyHostToDevice, c->stream));
+    PSB_CUDA(c, cudaMemcpyAsync(d_k + n_path, ky, (size_t)n_path * 8, cudaMemcpyHostToDevice, c->stream));
+    PSB_CUDA(c, cudaStreamSynchronize(c->stream));               // caller's host arrays are not retained
+    k_path_pixels<<<(n_path + 127) / 128, 128, 0, c->stream>>>(d_k, d_k + n_path, d_pix, n_path, c->nx, c->ny, c->cell[0],
+                                                               c->cell[1]);
+    PSB_LAUNCH_CHECK(c, "k_path_pixels");
+    const int total = n_bins * n_path;
+    k_dispersion<<<(total + 127) / 128, 128, 0, c->stream>>>(d_I, d_pix, d_out, P, n_bins, n_path, (size_t)c->nx * c->ny);
+    PSB_LAUNCH_CHECK(c, "k_dispersion");
+    return PS_OK;
+}
+
+extern "C" ps_status ps_qbin(ps_ctx* c, const float* d_I, int P, int n_bins, double dq, int n_q, int32_t* d_qidx,
+                             float* d_out) {
+    if (!c) return PS_EINVAL;
+    ps_status st = check_I(c, "ps_qbin", d_I, P, n_bins, d_out);
+    if (st != PS_OK) return st;
+    if (!d_qidx || !(dq > 0.0) || n_q < 1) return fail(c, PS_EINVAL, "ps_qbin: null pointer, dq <= 0 or n_q < 1");
+    const size_t npix = (size_t)c->nx * c->ny;
+    const size_t need = 4096 + (2 * ((size_t)n_q + 1) + npix) * 4 + 512;
+    if ((st = ensure_buf(c, c->misc, need)) != PS_OK) return st;
+    int32_t* d_cursor = (int32_t*)((char*)c->misc.p + 4096);
+    int32_t* d_off = d_cursor + (n_q + 1);
+    int32_t* d_order = d_off + (n_q + 1);
+    k_qidx<<<(unsigned)((npix + 255) / 256), 256, 0, c->stream>>>(d_qidx, c->nx, c->ny, c->cell[0], c->cell[1], dq, n_q);
+    PSB_LAUNCH_CHECK(c, "k_qidx");
+    k_order_by_bin<<<1, 32, 0, c->stream>>>(d_qidx, (int)npix, n_q, d_cursor, d_off, d_order);
+    PSB_LAUNCH_CHECK(c, "k_order_by_bin");
+    const long long warps = (long long)n_bins * n_q;
+    k_qbin_sum<<<(unsigned)((warps * 32 + 127) / 128), 128, 0, c->stream>>>(d_I, d_off, d_order, d_out, P, n_bins, n_q, npix);
+    PSB_LAUNCH_CHECK(c, "k_qbin_sum");
+    return PS_OK;
+}

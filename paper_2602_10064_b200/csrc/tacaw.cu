@@ -1,0 +1,258 @@
+// tacaw.cu — the TACAW transform (§2.1; Suppl. Eq. 5-6 at PAPER.md:295-301):
+//     Psi~(k, w_n) = sum_j ( Psi(k, t_j) - <Psi(k, t)>_t ) exp(-2 pi i n j / F),   I(k, w_n) = |Psi~|^2
+// Path A (ps_tacaw): one batched length-F FFT along the time axis per (probe, k) with the |.|^2 epilogue,
+//   reading the exit-wave stack [P][F][ny][nx] once; a block owns C adjacent k-pixels x all F frames, so
+//   every global access is a C*8-byte contiguous segment.  Pixels outside the band limit are exactly zero
+//   in every frame (ps_multislice wrote them as zeros) and are not read: their I is written as 0.
+//   The mean is removed by (i) subtracting the first frame's value before the transform, which strips
+//   the large elastic (Bragg) part so that fp32 rounding of it cannot leak into other bins, and
+//   (ii) zeroing bin 0 afterwards — identical to subtracting <Psi>_t for exact FFT bins (A14).
+// Path B (ps_tacaw_begin/add/finish): streaming per-bin DFT accumulation for stacks that do not fit HBM.
+#include "common.cuh"
+#include "fft_core.cuh"
+
+namespace psb {
+
+template <int NF> struct TacawCfg {
+    static constexpr int T = Plan<NF>::T;
+    static constexpr int C = (NF <= 512) ? 16 : ((NF == 1024) ? 8 : 4);
+    static constexpr int THREADS = C * T;
+    static constexpr size_t SMEM = (size_t)NF * C * sizeof(float2);
+};
+
+template <int NF>
+__global__ void __launch_bounds__(TacawCfg<NF>::THREADS)
+k_tacaw_fft(const float2* __restrict__ exitw, float* __restrict__ I, const int32_t* __restrict__ slot_of_bin,
+            const int n_out, const int nx, const int ny, const int32_t* __restrict__ nmax, const int n_items) {
+    using Cfg = TacawCfg<NF>;
+    constexpr int T = Cfg::T, C = Cfg::C;
+    extern __shared__ float2 smem[];
+    const int c = threadIdx.x % C, t = threadIdx.x / C;
+    ColSlots<C> slots{smem + c};
+    Twiddles<NF> tw;
+    tw.init(t);
+    const size_t npix = (size_t)nx * ny;
+    const int groups_per_row = nx / C, groups_per_probe = groups_per_row * ny;
+    int slot[16];
+#pragma unroll
+    for (int e = 0; e < 16; ++e) slot[e] = slot_of_bin[t + e * T];
+
+    for (int item = blockIdx.x; item < n_items; item += gridDim.x) {
+        const int p = item / groups_per_probe, g = item % groups_per_probe;
+        const int iy = g / groups_per_row, ix0 = (g % groups_per_row) * C;
+        const int ay = iy < ny / 2 ? iy : ny - iy;
+        const size_t pix = (size_t)iy * nx + ix0 + c;
+        float* out = I + (size_t)p * n_out * npix + pix;
+        const bool mine = ay <= nmax[ix0 + c];
+        if (!__syncthreads_or(mine)) {                       // whole group outside the band limit
+#pragma unroll
+            for (int e = 0; e < 16; ++e)
+                if (slot[e] >= 0) out[(size_t)slot[e] * npix] = 0.f;
+            continue;
+        }
+        const float2* src = exitw + (size_t)p * NF * npix + pix;
+        const float2 ref = __ldg(src);                       // frame 0 (A14: mean removal, see header)
+        float2 v[16];
+#pragma unroll
+        for (int e = 0; e < 16; ++e) {
+            const float2 x = src[(size_t)(t + e * T) * npix];
+            v[e] = make_float2(x.x - ref.x, x.y - ref.y);
+        }
+        fft_forward<NF, ColSlots<C>, BlockSync>(v, t, tw, slots);
+#pragma unroll
+        for (int e = 0; e < 16; ++e) {
+            if (slot[e] >= 0) {
+                const bool dc = (t + e * T) == 0;
+                out[(size_t)slot[e] * npix] = dc ? 0.f : fmaf(v[e].x, v[e].x, v[e].y * v[e].y);
+            }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------ path B: streaming DFT
+constexpr int SB_PIX = 128, SB_BINS = 16, SB_FR = 64;
+
+// acc[p][b][pix] += sum_{j in chunk} Psi[p][j][pix] * exp(-2 pi i n_b (frame0+j) / F)
+__global__ void __launch_bounds__(SB_PIX)
+k_tacaw_accum(const float2* __restrict__ chunk, float2* __restrict__ acc, const int32_t* __restrict__ bins,
+              const int n_bins, const int n_frames_total, const int frame0, const int n_frames_chunk,
+              const size_t npix, const int nx, const int ny, const int32_t* __restrict__ nmax) {
+    __shared__ float2 w[SB_FR][SB_BINS];
+    const size_t pix = (size_t)blockIdx.x * SB_PIX + threadIdx.x;
+    const int p = blockIdx.z, b0 = blockIdx.y * SB_BINS;
+    const int iy = (int)(pix / nx), ix = (int)(pix % nx);
+    const int ay = iy < ny / 2 ? iy : ny - iy;
+    const bool mine = pix < npix && ay <= nmax[ix];
+    if (!__syncthreads_or(mine)) return;                    // accumulators stay zero there
+    float2 a[SB_BINS];
+#pragma unroll
+    for (int b = 0; b < SB_BINS; ++b) a[b] = make_float2(0.f, 0.f);
+    const float2* src = chunk + (size_t)p * n_frames_chunk * npix + pix;
+    for (int j0 = 0; j0 < n_frames_chunk; j0 += SB_FR) {
+        const int cnt = min(SB_FR, n_frames_chunk - j0);
+        __syncthreads();
+        for (int i = threadIdx.x; i < cnt * SB_BINS; i += SB_PIX) {
+            const int jj = i / SB_BINS, b = i % SB_BINS;
+            float2 tw = make_float2(0.f, 0.f);
+            if (b0 + b <= n_bins) {                          // slot n_bins: plain sum (twiddle 1)
+                const long long n = (b0 + b < n_bins) ? bins[b0 + b] : 0;
+                const long long ph = (n * (long long)(frame0 + j0 + jj)) % n_frames_total;   // bins already in [0,F)
+                double s, cc;
+                sincospi(2.0 * (double)ph / (double)n_frames_total, &s, &cc);
+                tw = make_float2((float)cc, (float)(-s));
+            }
+            w[jj][b] = tw;
+        }
+        __syncthreads();
+        if (mine) {
+            for (int jj = 0; jj < cnt; ++jj) {
+                const float2 x = src[(size_t)(j0 + jj) * npix];
+#pragma unroll
+                for (int b = 0; b < SB_BINS; ++b) {
+                    const float2 ww = w[jj][b];
+                    a[b].x = fmaf(x.x, ww.x, a[b].x); a[b].x = fmaf(-x.y, ww.y, a[b].x);
+                    a[b].y = fmaf(x.x, ww.y, a[b].y); a[b].y = fmaf(x.y, ww.x, a[b].y);
+                }
+            }
+        }
+    }
+    if (mine) {
+#pragma unroll
+        for (int b = 0; b < SB_BINS; ++b)
+            if (b0 + b <= n_bins) {
+                float2* d = acc + ((size_t)p * (n_bins + 1) + b0 + b) * npix + pix;
+                const float2 o = *d;
+                *d = make_float2(o.x + a[b].x, o.y + a[b].y);
+            }
+    }
+}
+
+__global__ void k_tacaw_finish(const float2* __restrict__ acc, float* __restrict__ I, const int32_t* __restrict__ bins,
+                               const int n_bins, const size_t npix, const long long total) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= total) return;
+    const size_t pix = (size_t)(i % npix);
+    const int b = (int)((i / npix) % n_bins), p = (int)(i / (npix * n_bins));
+    const float2 a = acc[((size_t)p * (n_bins + 1) + b) * npix + pix];
+    I[i] = (bins[b] == 0) ? 0.f : fmaf(a.x, a.x, a.y * a.y);      // bin 0: sum_j (Psi_j - mean) = 0 exactly
+}
+
+template <int NF>
+static cudaError_t launch_tacaw(ps_ctx* c, const float2* exitw, float* I, const int32_t* slot, int n_out, int P) {
+    using Cfg = TacawCfg<NF>;
+    auto kern = k_tacaw_fft<NF>;
+    static int cap = 0;
+    if (!cap) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
+        if (e != cudaSuccess) return e;
+        int per_sm = 1, dev = 0, n_sm = kNumSM;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, Cfg::THREADS, Cfg::SMEM) != cudaSuccess || per_sm < 1)
+            per_sm = 1;
+        cap = n_sm * per_sm;
+    }
+    const long long n_items = (long long)P * c->ny * (c->nx / Cfg::C);
+    if (n_items > 0x7fffffffLL) return cudaErrorInvalidValue;
+    kern<<<(int)(n_items < cap ? n_items : cap), Cfg::THREADS, Cfg::SMEM, c->stream>>>(exitw, I, slot, n_out, c->nx, c->ny,
+                                                                                      c->d_nmax, (int)n_items);
+    return cudaGetLastError();
+}
+
+}  // namespace psb
+
+using namespace psb;
+
+extern "C" ps_status ps_tacaw(ps_ctx* c, const void* d_exit, int exit_layout, int n_probes, int n_frames, double dt_fs,
+                              int n_bins, const int32_t* bins, float* d_I) {
+    if (!c) return PS_EINVAL;
+    if (!c->have_geom) return fail(c, PS_ESTATE, "ps_tacaw: ps_set_geometry has not been called");
+    if (!d_exit || !d_I || n_probes < 1 || n_frames < 1 || n_bins < 1 || !(dt_fs > 0.0))
+        return fail(c, PS_EINVAL, "ps_tacaw: null pointer or non-positive size / dt");
+    if (exit_layout != PS_LAYOUT_DENSE) return fail(c, PS_EUNSUPPORTED, "ps_tacaw: unknown exit layout");
+    if (!is_pow2(n_frames) || n_frames < 32 || n_frames > 4096)
+        return fail(c, PS_EUNSUPPORTED, "ps_tacaw: n_frames must be a power of two in [32, 4096] (use ps_tacaw_begin/add/finish otherwise)");
+    if (!bins && n_bins != n_frames) return fail(c, PS_EINVAL, "ps_tacaw: bins == NULL requires n_bins == n_frames");
+    std::vector<int32_t> slot(n_frames, -1);
+    for (int b = 0; b < n_bins; ++b) {
+        long long n = bins ? bins[b] : b;
+        n %= n_frames; if (n < 0) n += n_frames;
+        if (slot[n] >= 0) return fail(c, PS_EINVAL, "ps_tacaw: duplicate bin in list");
+        slot[n] = b;
+    }
+    ps_status st = ensure_buf(c, c->misc, 4096 + (size_t)n_frames * 4);
+    if (st != PS_OK) return st;
+    int32_t* d_slot = (int32_t*)((char*)c->misc.p + 4096);
+    PSB_CUDA(c, cudaMemcpyAsync(d_slot, slot.data(), (size_t)n_frames * 4, cudaMemcpyHostToDevice, c->stream));
+    PSB_CUDA(c, cudaStreamSynchronize(c->stream));           // `slot` dies at return; 16 KB at most
+    cudaError_t e = cudaErrorInvalidValue;
+    switch (n_frames) {
+        case 32: e = launch_tacaw<32>(c, (const float2*)d_exit, d_I, d_slot, n_bins, n_probes); break;
+        case 64: e = launch_tacaw<64>(c, (const float2*)d_exit, d_I, d_slot, n_bins, n_probes); break;
+        case 128: e = launch_tacaw<128>(c, (const float2*)d_exit, d_I, d_slot, n_bins, n_probes); break;
+        case 256: e = launch_tacaw<256>(c, (const float2*)d_exit, d_I, d_slot, n_bins, n_probes); break;
+        case 512: e = launch_tacaw<512>(c, (const float2*)d_exit, d_I, d_slot, n_bins, n_probes); break;
+        case 1024: e = launch_tacaw<1024>(c, (const float2*)d_exit, d_I, d_slot, n_bins, n_probes); break;
+        case 2048: e = launch_tacaw<2048>(c, (const float2*)d_exit, d_I, d_slot, n_bins, n_probes); break;
+        case 4096: e = launch_tacaw<4096>(c, (const float2*)d_exit, d_I, d_slot, n_bins, n_probes); break;
+        default: break;
+    }
+    if (e != cudaSuccess) return fail(c, PS_ECUDA, std::string("k_tacaw_fft: ") + cudaGetErrorString(e));
+    c->launches++;
+    return PS_OK;
+}
+
+extern "C" ps_status ps_tacaw_begin(ps_ctx* c, int n_probes, int n_frames_total, double dt_fs, int n_bins,
+                                    const int32_t* bins, void* d_acc) {
+    if (!c) return PS_EINVAL;
+    if (!c->have_geom) return fail(c, PS_ESTATE, "ps_tacaw_begin: ps_set_geometry has not been called");
+    if (!d_acc || !bins || n_probes < 1 || n_frames_total < 1 || n_bins < 1 || !(dt_fs > 0.0))
+        return fail(c, PS_EINVAL, "ps_tacaw_begin: null pointer or non-positive size / dt");
+    TacawStream& ts = c->ts;
+    ts.bins.resize(n_bins);
+    for (int b = 0; b < n_bins; ++b) {
+        long long n = bins[b] % n_frames_total; if (n < 0) n += n_frames_total;
+        ts.bins[b] = (int32_t)n;
+    }
+    PSB_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (ts.d_bins) { cudaFree(ts.d_bins); ts.d_bins = nullptr; }
+    PSB_CUDA(c, cudaMalloc((void**)&ts.d_bins, (size_t)n_bins * 4));
+    PSB_CUDA(c, cudaMemcpy(ts.d_bins, ts.bins.data(), (size_t)n_bins * 4, cudaMemcpyHostToDevice));
+    const size_t bytes = (size_t)n_probes * (n_bins + 1) * c->nx * c->ny * sizeof(float2);
+    PSB_CUDA(c, cudaMemsetAsync(d_acc, 0, bytes, c->stream));
+    ts.active = true; ts.n_probes = n_probes; ts.n_frames_total = n_frames_total; ts.n_bins = n_bins;
+    ts.frames_seen = 0; ts.d_acc = d_acc;
+    return PS_OK;
+}
+
+extern "C" ps_status ps_tacaw_add(ps_ctx* c, const void* d_exit_chunk, int frame0, int n_frames_chunk) {
+    if (!c) return PS_EINVAL;
+    TacawStream& ts = c->ts;
+    if (!ts.active) return fail(c, PS_ESTATE, "ps_tacaw_add: ps_tacaw_begin has not been called");
+    if (!d_exit_chunk || frame0 < 0 || n_frames_chunk < 1 || frame0 + n_frames_chunk > ts.n_frames_total)
+        return fail(c, PS_EINVAL, "ps_tacaw_add: null pointer or frame range outside [0, n_frames_total)");
+    const size_t npix = (size_t)c->nx * c->ny;
+    dim3 grid((unsigned)((npix + SB_PIX - 1) / SB_PIX), (unsigned)((ts.n_bins + 1 + SB_BINS - 1) / SB_BINS), ts.n_probes);
+    k_tacaw_accum<<<grid, SB_PIX, 0, c->stream>>>((const float2*)d_exit_chunk, (float2*)ts.d_acc, ts.d_bins, ts.n_bins,
+                                                 ts.n_frames_total, frame0, n_frames_chunk, npix, c->nx, c->ny, c->d_nmax);
+    PSB_LAUNCH_CHECK(c, "k_tacaw_accum");
+    ts.frames_seen += n_frames_chunk;
+    return PS_OK;
+}
+
+extern "C" ps_status ps_tacaw_finish(ps_ctx* c, float* d_I) {
+    if (!c) return PS_EINVAL;
+    TacawStream& ts = c->ts;
+    if (!ts.active) return fail(c, PS_ESTATE, "ps_tacaw_finish: ps_tacaw_begin has not been called");
+    if (!d_I) return fail(c, PS_EINVAL, "ps_tacaw_finish: d_I is NULL");
+    if (ts.frames_seen != ts.n_frames_total)
+        return fail(c, PS_ESTATE, "ps_tacaw_finish: " + std::to_string(ts.frames_seen) + " of " +
+                                      std::to_string(ts.n_frames_total) + " frames were added");
+    const size_t npix = (size_t)c->nx * c->ny;
+    const long long total = (long long)ts.n_probes * ts.n_bins * npix;
+    k_tacaw_finish<<<(unsigned)((total + 255) / 256), 256, 0, c->stream>>>((const float2*)ts.d_acc, d_I, ts.d_bins, ts.n_bins,
+                                                                           npix, total);
+    PSB_LAUNCH_CHECK(c, "k_tacaw_finish");
+    ts.active = false;
+    return PS_OK;
+}

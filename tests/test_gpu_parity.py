@@ -1,0 +1,253 @@
+"""GPU parity tests: the CUDA path (through the C ABI) against the float64 oracle, element by element,
+on the same seeded inputs.  Run on the B200 box with `-m gpu`.
+
+Tolerances (BASELINE.json north_star): rel-L2 <= 1e-4 on exit waves, <= 1e-3 on
+|Psi(k,w)|^2, integers (slice binning, path pixels, q-bin indices, detector membership) bit-exact.
+Stage tolerances derived in DESIGN.md §7: V 2e-5, incident waves 1e-5, reductions 1e-5.
+"""
+import numpy as np
+import pytest
+
+from oracle import tacaw_oracle as O
+from workloads import make_workload
+
+from gpu_common import gpu_incident, make_ctx, oracle_incident, oracle_potential, rel_l2
+
+pytestmark = pytest.mark.gpu
+
+TOL_EXIT = 1e-4
+TOL_I = 1e-3
+TOL_V = 2e-5
+TOL_PSI0 = 1e-5
+TOL_RED = 1e-5
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device")
+    return torch
+
+
+def _t(torch, a, dtype=None):
+    return torch.as_tensor(np.ascontiguousarray(a), dtype=dtype).cuda()
+
+
+MINIS = ["c1_si_128", "c2_hbn_256", "c3_si_probe_512", "c4_interface_1024", "c5_al_sweep"]
+
+
+# ----------------------------------------------------------------------------- a0 + a2 + a3
+@pytest.mark.parametrize("name", MINIS)
+def test_build_slices_matches_oracle(torch, name):
+    import paper_2602_10064_b200 as ps
+    w = make_workload(name, mini=True)
+    ctx = make_ctx(w)
+    frames = [0, w.n_frames - 1]
+    pos = w.positions()[frames]
+    V, sidx = ps.ps_build_slices(ctx, _t(torch, pos), _t(torch, w.Z), want_slice_idx=True)
+    V = V.cpu().numpy(); sidx = sidx.cpu().numpy()
+    for i in range(len(frames)):
+        Vo, so = oracle_potential(w, pos[i])
+        assert np.array_equal(sidx[i], so), "slice binning must be bit-exact"
+        assert rel_l2(V[i], Vo) < TOL_V
+
+
+def test_build_slices_ragged_and_wrapped(torch):
+    """atom count not a multiple of anything, positions outside the cell (periodic wrap), odd slice count,
+    non-square grid."""
+    import paper_2602_10064_b200 as ps
+    w = make_workload("c4_interface_1024", mini=True)
+    w.nx, w.ny, w.n_slices = 64, 128, 5
+    keep = np.arange(w.n_atoms)[: w.n_atoms - 13]
+    w.Z = w.Z[keep]; w.R0 = w.R0[keep]; w.mode_amp = w.mode_amp[:, keep]
+    ctx = make_ctx(w)
+    pos = w.positions(0, 3)
+    pos[1] += np.array([3 * w.cell[0], -2 * w.cell[1], 5 * w.cell[2]], dtype=np.float32)
+    pos[2, ::7, 2] = 0.0                                       # atoms exactly on the cell boundary
+    V, sidx = ps.ps_build_slices(ctx, _t(torch, pos), _t(torch, w.Z), want_slice_idx=True)
+    V = V.cpu().numpy(); sidx = sidx.cpu().numpy()
+    for i in range(3):
+        Vo, so = oracle_potential(w, pos[i])
+        assert np.array_equal(sidx[i], so)
+        assert rel_l2(V[i], Vo) < TOL_V
+
+
+def test_build_slices_rejects_unknown_Z(torch):
+    import paper_2602_10064_b200 as ps
+    w = make_workload("c1_si_128", mini=True)
+    ctx = make_ctx(w)
+    Z = w.Z.copy(); Z[3] = 79
+    with pytest.raises(ps.PSError) as ei:
+        ps.ps_build_slices(ctx, _t(torch, w.positions(0, 1)), _t(torch, Z))
+    assert ei.value.status == -2
+
+
+# ----------------------------------------------------------------------------- a4
+@pytest.mark.parametrize("name", ["c3_si_probe_512", "c5_al_sweep", "c1_si_128"])
+def test_incident_matches_oracle(torch, name):
+    w = make_workload(name, mini=True)
+    ctx = make_ctx(w)
+    g = gpu_incident(ctx, w).cpu().numpy()
+    o = np.stack(oracle_incident(w))
+    assert g.shape == o.shape
+    assert rel_l2(g, o) < TOL_PSI0
+
+
+# ----------------------------------------------------------------------------- a5 + a6
+@pytest.mark.parametrize("name", MINIS)
+def test_multislice_matches_oracle_on_oracle_potential(torch, name):
+    """Isolates the slice loop: both sides consume the same float32 potentials and incident waves."""
+    import paper_2602_10064_b200 as ps
+    w = make_workload(name, mini=True)
+    ctx = make_ctx(w)
+    frames = [0, 1, w.n_frames - 1]
+    pos = w.positions()[frames]
+    V32 = np.stack([oracle_potential(w, p)[0] for p in pos]).astype(np.float32)
+    psi0 = np.stack(oracle_incident(w)).astype(np.complex64)
+    ex = ps.ps_multislice(ctx, w.kV, _t(torch, psi0), _t(torch, V32)).cpu().numpy()
+    for p in range(psi0.shape[0]):
+        for i in range(len(frames)):
+            eo = O.multislice(psi0[p].astype(np.complex128), V32[i].astype(np.float64), w.cell, w.kV)
+            assert rel_l2(ex[p, i], eo) < TOL_EXIT
+
+
+@pytest.mark.parametrize("nx,ny", [(32, 32), (64, 32), (128, 256), (512, 64), (1024, 32), (32, 2048), (2048, 32)])
+def test_multislice_grid_sizes(torch, nx, ny):
+    """Every FFT length the library instantiates, on a random smooth potential, non-square cells included."""
+    import paper_2602_10064_b200 as ps
+    rng = np.random.default_rng(nx * 7 + ny)
+    w = make_workload("c1_si_128", mini=True)
+    w.nx, w.ny, w.n_slices = nx, ny, 3
+    w.cell = np.array([nx * 0.11, ny * 0.13, 6.0])
+    ctx = make_ctx(w)
+    F = 2
+    Vk = (rng.normal(size=(F, 3, ny, nx)) + 1j * rng.normal(size=(F, 3, ny, nx)))
+    ky = np.fft.fftfreq(ny)[:, None]; kx = np.fft.fftfreq(nx)[None, :]
+    V32 = (400.0 * np.real(np.fft.ifft2(Vk * np.exp(-200.0 * (kx ** 2 + ky ** 2)))) * np.sqrt(nx * ny)).astype(np.float32)
+    psi0 = O.tilted_plane_wave(nx, ny, 1, -1).astype(np.complex64)[None]
+    ex = ps.ps_multislice(ctx, 80.0, _t(torch, psi0), _t(torch, V32)).cpu().numpy()
+    for i in range(F):
+        eo = O.multislice(psi0[0].astype(np.complex128), V32[i].astype(np.float64), w.cell, 80.0)
+        assert rel_l2(ex[0, i], eo) < TOL_EXIT
+
+
+def test_multislice_free_space_plane_wave_is_exact(torch):
+    """P5: V = 0 leaves the plane wave untouched: exit = sqrt(nx ny) at k = 0, zero elsewhere."""
+    import paper_2602_10064_b200 as ps
+    w = make_workload("c2_hbn_256", mini=True)
+    ctx = make_ctx(w)
+    V = torch.zeros((2, w.n_slices, w.ny, w.nx), dtype=torch.float32, device="cuda")
+    ex = ps.ps_multislice(ctx, w.kV, gpu_incident(ctx, w), V).cpu().numpy()
+    want = np.zeros((w.ny, w.nx), complex); want[0, 0] = np.sqrt(w.nx * w.ny)
+    for i in range(2):
+        assert np.abs(ex[0, i] - want).max() < 1e-4 * np.sqrt(w.nx * w.ny)
+
+
+def test_multislice_chunking_is_invisible(torch):
+    import paper_2602_10064_b200 as ps
+    w = make_workload("c3_si_probe_512", mini=True)
+    ctx = make_ctx(w)
+    pos = w.positions(0, 5)
+    V = ps.ps_build_slices(ctx, _t(torch, pos), _t(torch, w.Z))
+    psi0 = gpu_incident(ctx, w)
+    a = ps.ps_multislice(ctx, w.kV, psi0, V).clone()
+    for chunk in (1, 3, 7):
+        ctx.set_wave_chunk(chunk)
+        b = ps.ps_multislice(ctx, w.kV, psi0, V)
+        assert torch.equal(a, b)
+
+
+# ----------------------------------------------------------------------------- a7
+@pytest.mark.parametrize("F", [32, 64, 128, 256, 512, 1024, 2048, 4096])
+def test_tacaw_fft_lengths(torch, F):
+    import paper_2602_10064_b200 as ps
+    rng = np.random.default_rng(F)
+    w = make_workload("c1_si_128", mini=True)
+    w.nx, w.ny = 32, 32
+    ctx = make_ctx(w)
+    A = O.aperture_mask(w.cell, 32, 32)
+    x = (rng.normal(size=(2, F, 32, 32)) + 1j * rng.normal(size=(2, F, 32, 32))) * 0.05 + (3.0 - 2.0j)
+    x = (x * A).astype(np.complex64)
+    bins = np.array([0, 1, -1, 5, F // 2 - 1, -(F // 2), 7 - F], dtype=np.int32)
+    Ig = ps.ps_tacaw(ctx, _t(torch, x), 2.0, bins).cpu().numpy()
+    Iall = ps.ps_tacaw(ctx, _t(torch, x), 2.0).cpu().numpy()
+    for p in range(2):
+        Io = O.tacaw_intensity(x[p].astype(np.complex128))
+        assert rel_l2(Iall[p], Io) < TOL_I
+        assert rel_l2(Ig[p], Io[bins % F]) < TOL_I
+        assert np.all(Iall[p][0] == 0.0)                       # mean removed exactly
+
+
+def test_tacaw_streaming_matches_fft_path(torch):
+    import paper_2602_10064_b200 as ps
+    from paper_2602_10064_b200.binding import TacawStream
+    rng = np.random.default_rng(5)
+    w = make_workload("c1_si_128", mini=True)
+    ctx = make_ctx(w)
+    F, P = 96, 2                                               # not a power of two: streaming path only
+    A = O.aperture_mask(w.cell, w.nx, w.ny)
+    x = ((rng.normal(size=(P, F, w.ny, w.nx)) + 1j * rng.normal(size=(P, F, w.ny, w.nx))) * 0.1 + 1.5) * A
+    x = x.astype(np.complex64)
+    bins = np.arange(-3, 20, dtype=np.int32)
+    ts = TacawStream(ctx, P, F, 2.0, bins)
+    xg = _t(torch, x)
+    for f0, f1 in ((0, 40), (40, 41), (41, 96)):
+        ts.add(xg[:, f0:f1].contiguous(), f0)
+    Ig = ts.finish().cpu().numpy()
+    for p in range(P):
+        Io = O.tacaw_intensity(x[p].astype(np.complex128), bins)
+        assert rel_l2(Ig[p], Io) < TOL_I
+
+
+# ----------------------------------------------------------------------------- end to end + a8
+@pytest.mark.parametrize("name", MINIS)
+def test_end_to_end_mini(torch, name):
+    """positions -> I(k, w) on the mini twin of every config, all frames, against the oracle's run_path."""
+    import paper_2602_10064_b200 as ps
+    from workloads import form_factor_coefficients
+    w = make_workload(name, mini=True)
+    ctx = make_ctx(w)
+    pos = w.positions()
+    V = ps.ps_build_slices(ctx, _t(torch, pos), _t(torch, w.Z))
+    ex = ps.ps_multislice(ctx, w.kV, gpu_incident(ctx, w), V)
+    Ig = ps.ps_tacaw(ctx, ex, w.dt_fs, w.bins)
+    nl, ng, coef = form_factor_coefficients(w.elements, w.ff_kind)
+    Io, exo = O.run_path(pos, np.searchsorted(w.elements, w.Z), coef, nl, ng, w.cell, w.nx, w.ny, w.n_slices, w.kV,
+                         oracle_incident(w), w.bins)
+    assert rel_l2(ex.cpu().numpy(), exo) < TOL_EXIT
+    assert rel_l2(Ig.cpu().numpy(), Io) < TOL_I
+
+    # reductions on the GPU's own I against the oracle's definitions applied to the same array
+    I64 = Ig.cpu().numpy().astype(np.float64)
+    nb = I64.shape[1]
+    lo, hi = 1, min(4, nb - 1)
+    assert rel_l2(ps.ps_sdp(ctx, Ig, lo, hi).cpu().numpy(), O.sdp(I64, lo, hi)) < TOL_RED
+    kc = O.k_cut(w.cell, w.nx, w.ny)
+    si = ps.ps_spectrum_image(ctx, Ig, 0.2 * kc, 0.7 * kc).cpu().numpy()
+    assert rel_l2(si, O.spectrum_image(I64, w.cell, 0.2 * kc, 0.7 * kc)) < TOL_RED
+    si_all = ps.ps_spectrum_image(ctx, Ig).cpu().numpy()
+    assert rel_l2(si_all, I64.sum(axis=(2, 3))) < TOL_RED
+    kxp = np.linspace(-0.4 * kc, 0.9 * kc, 37); kyp = np.linspace(0.3 * kc, -0.5 * kc, 37)
+    dg, pix = ps.ps_dispersion(ctx, Ig, kxp, kyp)
+    do, pixo = O.dispersion(I64, w.cell, kxp, kyp)
+    assert np.array_equal(pix.cpu().numpy(), pixo), "path pixels must be bit-exact"
+    assert rel_l2(dg.cpu().numpy(), do) < TOL_RED
+    dq, nq = kc / 13.0, 11
+    qg, qidx = ps.ps_qbin(ctx, Ig, dq, nq)
+    qo, qidxo = O.qbin(I64, w.cell, dq, nq)
+    assert np.array_equal(qidx.cpu().numpy(), qidxo), "q-bin indices must be bit-exact"
+    assert rel_l2(qg.cpu().numpy(), qo) < TOL_RED
+
+
+def test_results_are_deterministic(torch):
+    import paper_2602_10064_b200 as ps
+    w = make_workload("c2_hbn_256", mini=True)
+    ctx = make_ctx(w)
+    pos = _t(torch, w.positions()); Z = _t(torch, w.Z)
+    outs = []
+    for _ in range(2):
+        V = ps.ps_build_slices(ctx, pos, Z)
+        ex = ps.ps_multislice(ctx, w.kV, gpu_incident(ctx, w), V)
+        outs.append(ps.ps_tacaw(ctx, ex, w.dt_fs, w.bins).clone())
+    assert torch.equal(outs[0], outs[1])
