@@ -1,0 +1,350 @@
+#!/usr/bin/env python
+"""bench.py — one JSON line for the TACAW hot path on B200 (contract: task prompt / DESIGN.md §8).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload NAME]
+
+A "step" is one pass of the whole hot path over one synthetic trajectory of the workload
+(BASELINE.json configs[1] by default: hBN-like monolayer, 256x256, 10 slices, 512 frames):
+    ps_build_slices -> ps_make_incident -> ps_multislice -> ps_tacaw -> ps_sdp / ps_spectrum_image /
+    ps_dispersion / ps_qbin.
+`value` = nx*ny*n_slices*frames*probes / step time, in Gpx*slice/s, inputs resident in HBM;
+`e2e` = the same with host buffers (pinned positions in, I(k,w) cube + reductions out) inside the timed
+region.  `roofline` is for the dominant kernel family of the step (per-launch CUDA events recorded by the
+library's ps_profile_* on its own stream, in a second pass of the same K steps); `cpu_baseline` is the
+float64 oracle timed on this box's host cores on a bounded sample of the same workload.
+With N > 1 (torchrun) every rank processes an independent trajectory (averaging over
+independent trajectories) and the I(k,w) cubes are summed with one NCCL all-reduce: weak scaling.
+`--impl reference` times the oracle (the only reference there is: the paper ships no code).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from workloads import form_factor_coefficients, make_workload  # noqa: E402
+
+METRIC = "multislice Gpx*slice/s over frames x probes (whole TACAW hot path per step)"
+UNIT = "Gpx*slice/s"
+# algorithmic bytes per pixel*slice of the slice step (pruned figure):
+#   row pass 4 (V) + 16 * f_col, column pass 16 * f_col, f_col = 2/3 of the columns inside the band limit
+ROW_BYTES = 4.0 + 16.0 * (2.0 / 3.0)
+COL_BYTES = 16.0 * (2.0 / 3.0)
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index: int, period_s: float = 0.02):
+        super().__init__(daemon=True)
+        self.index, self.period, self.stop_flag = index, period_s, threading.Event()
+        self.sm, self.reasons, self.max_mhz, self.ok = [], set(), None, False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+        except Exception:
+            self.ok = False
+
+    def run(self):
+        if not self.ok:
+            return
+        nv = self.nv
+        names = {"hw_slowdown": 0x8, "sw_power_cap": 0x4, "hw_thermal_slowdown": 0x40, "sw_thermal_slowdown": 0x20,
+                 "hw_power_brake": 0x80, "sync_boost": 0x10, "applications_clocks": 0x2}
+        while not self.stop_flag.is_set():
+            try:
+                self.sm.append(int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                try:
+                    r = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                except Exception:
+                    r = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def result(self):
+        self.stop_flag.set()
+        if not self.ok or not self.sm:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["nvml unavailable"]}
+        return {"sm_mhz": float(np.median(self.sm)), "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.sm)}
+
+
+def physical_gpu_index(local_rank: int) -> int:
+    vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+    if vis:
+        try:
+            return int(vis.split(",")[local_rank])
+        except Exception:
+            return local_rank
+    return local_rank
+
+
+# --------------------------------------------------------------------------------------------- oracle arm
+def oracle_sample(w, budget_s: float = 20.0):
+    """Times the float64 oracle (as it stands) on the first n frames of the workload; n is chosen from
+    a one-frame calibration so that the sample costs about `budget_s` seconds of CPU work."""
+    from oracle import tacaw_oracle as O
+    nl, ng, coef = form_factor_coefficients(w.elements, w.ff_kind)
+    elem = np.searchsorted(w.elements, w.Z)
+    if w.beam == "plane":
+        psi0 = [O.plane_wave(w.nx, w.ny)]
+    elif w.beam == "tilt":
+        psi0 = [O.tilted_plane_wave(w.nx, w.ny, int(m), int(n)) for m, n in w.tilts]
+    else:
+        psi0 = [O.probe_wave(w.cell, w.nx, w.ny, w.kV, w.semi_angle_mrad, x, y) for x, y in w.probe_xy]
+    psi0 = psi0[:1]                                             # one probe / tilt is enough for a rate
+    pos = w.positions(0, min(w.n_frames, 64))
+
+    def run(n):
+        t0 = time.perf_counter()
+        O.run_path(pos[:n], elem, coef, nl, ng, w.cell, w.nx, w.ny, w.n_slices, w.kV, psi0, None, frames=range(n))
+        return time.perf_counter() - t0
+
+    t1 = run(1)
+    n = int(max(2, min(pos.shape[0], budget_s / max(t1, 1e-3))))
+    t = run(n)
+    units = float(w.nx) * w.ny * w.n_slices * n * len(psi0)
+    return {"value": units / t / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle",
+            "sample": f"{n} of {w.n_frames} frames x {len(psi0)} probe(s), positions -> |Psi(k,w)|^2 "
+                      f"(float64 NumPy oracle, {t:.1f} s)"}, t, units
+
+
+def run_reference(args, w, rank):
+    if rank != 0:
+        return
+    t_all, u_all = 0.0, 0.0
+    cb = None
+    for _ in range(args.warmup if args.warmup < 2 else 1):
+        oracle_sample(w, budget_s=2.0)
+    for _ in range(max(1, args.steps)):
+        cb, t, u = oracle_sample(w, budget_s=max(2.0, 60.0 / max(1, args.steps)))
+        t_all += t; u_all += u
+    val = u_all / t_all / 1e9
+    cb["value"] = val
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * t_all / max(1, args.steps), "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": w.name, "note": "float64 NumPy oracle on host cores; each step is a bounded sample"},
+        "cpu_baseline": cb,
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+# --------------------------------------------------------------------------------------------- our arm
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="c2_hbn_256")
+    ap.add_argument("--frames", type=int, default=None, help="override the number of frames (parity/debug only)")
+    ap.add_argument("--wave-chunk", type=int, default=0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    w = make_workload(args.workload, n_frames=args.frames)
+
+    if args.impl == "reference":
+        run_reference(args, w, rank)
+        return
+
+    import torch
+    import torch.distributed as dist
+    import paper_2602_10064_b200 as ps
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    dev = torch.device("cuda", local_rank)
+
+    # ---- inputs: an independent seeded trajectory per rank (rank 0 = the workload's own seed)
+    if rank > 0:
+        w.seed += 7919 * rank
+        w.mode_phi = np.random.default_rng(w.seed).uniform(0, 2 * np.pi, w.mode_phi.shape[0])
+    pos_h = torch.from_numpy(w.positions()).pin_memory()
+    Z_h = torch.from_numpy(w.Z.copy())
+    F, P, S, nx, ny = w.n_frames, w.n_probes, w.n_slices, w.nx, w.ny
+    bins = w.bins if w.bins is not None else None
+    nb = F if bins is None else len(bins)
+
+    ctx = ps.Context(local_rank)
+    nl, ng, coef = form_factor_coefficients(w.elements, w.ff_kind)
+    ctx.set_form_factors(w.elements, nl, ng, coef)
+    ctx.set_geometry(w.cell, nx, ny, w.slice_dz)
+    if args.wave_chunk:
+        ctx.set_wave_chunk(args.wave_chunk)
+
+    pos_d = pos_h.to(dev)
+    Z_d = Z_h.to(dev)
+    V = torch.empty((F, S, ny, nx), dtype=torch.float32, device=dev)
+    psi0 = torch.empty((P, ny, nx), dtype=torch.complex64, device=dev)
+    exitw = torch.empty((P, F, ny, nx), dtype=torch.complex64, device=dev)
+    I = torch.empty((P, nb, ny, nx), dtype=torch.float32, device=dev)
+    sdp = torch.empty((ny, nx), dtype=torch.float32, device=dev)
+    simg = torch.empty((P, nb), dtype=torch.float32, device=dev)
+    n_path, n_q = 100, 64
+    kc = (2.0 / 3.0) * min(nx / (2 * w.cell[0]), ny / (2 * w.cell[1]))
+    kx_path = np.linspace(0.0, 0.9 * kc, n_path); ky_path = np.zeros(n_path)
+    disp = torch.empty((nb, n_path), dtype=torch.float32, device=dev)
+    qb = torch.empty((nb, n_q), dtype=torch.float32, device=dev)
+    I_h = torch.empty(I.shape, dtype=torch.float32).pin_memory()
+    red_h = [torch.empty(t.shape, dtype=torch.float32).pin_memory() for t in (sdp, simg, disp, qb)]
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)      # > 126 MB L2
+
+    if w.beam == "probe":
+        inc = dict(semi_angle_mrad=w.semi_angle_mrad, xy_or_tilt=w.probe_xy)
+    elif w.beam == "tilt":
+        inc = dict(semi_angle_mrad=0.0, xy_or_tilt=w.tilts.astype(np.float64), is_tilt=True)
+    else:
+        inc = dict(n=1)
+
+    def step(pos_dev):
+        ps.ps_build_slices(ctx, pos_dev, Z_d, d_V=V)
+        ps.ps_make_incident(ctx, w.kV, d_psi0=psi0, **inc)
+        ps.ps_multislice(ctx, w.kV, psi0, V, d_exit=exitw)
+        ps.ps_tacaw(ctx, exitw, w.dt_fs, bins, d_I=I)
+        if world > 1:
+            dist.all_reduce(I)                                   # trajectory averaging (sum)
+        ps.ps_sdp(ctx, I, 1, min(8, nb - 1), d_out=sdp)
+        ps.ps_spectrum_image(ctx, I, 0.0, 0.0, d_out=simg)
+        ps.ps_dispersion(ctx, I, kx_path, ky_path, d_out=disp)
+        ps.ps_qbin(ctx, I, kc / n_q, n_q, d_out=qb)
+
+    def step_e2e():
+        pos_dev = pos_h.to(dev, non_blocking=True)
+        step(pos_dev)
+        I_h.copy_(I, non_blocking=True)
+        for h, d in zip(red_h, (sdp, simg, disp, qb)):
+            h.copy_(d, non_blocking=True)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(fn, K, profile=False):
+        """K steps, each bracketed by its own event pair, L2 flushed (outside the pairs) between steps."""
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
+        barrier()
+        for a, b in evs:
+            flush.zero_()
+            a.record()
+            fn()
+            b.record()
+        barrier()
+        ms = sum(a.elapsed_time(b) for a, b in evs)
+        if world > 1:
+            t = torch.tensor([ms], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t.item())
+        return ms
+
+    for _ in range(max(3, args.warmup)):
+        step(pos_d)
+    barrier()
+
+    K = max(1, args.steps)
+    sampler = ClockSampler(physical_gpu_index(local_rank))
+    sampler.start()
+    l0 = ctx.launches
+    ms_total = timed(lambda: step(pos_d), K)
+    launches = ctx.launches - l0
+    clocks = sampler.result()
+
+    units_rank = float(nx) * ny * S * F * P
+    value = units_rank * world * K / (ms_total * 1e-3) / 1e9
+
+    # ---- end to end through the public API with host buffers
+    step_e2e(); barrier()
+    ms_e2e = timed(step_e2e, K)
+    e2e_value = units_rank * world * K / (ms_e2e * 1e-3) / 1e9
+    h2d = pos_h.numel() * 4
+    d2h = I_h.numel() * 4 + sum(h.numel() * 4 for h in red_h)
+
+    # ---- per-kernel device time (library-side CUDA events on its stream), same K steps
+    ctx.profile_read(reset=True)
+    ctx.profile_enable(True)
+    ms_prof_total = timed(lambda: step(pos_d), K)
+    prof = ctx.profile_read(reset=True)
+    ctx.profile_enable(False)
+
+    peak, peak_src = measured_peaks()
+    px_slices_per_step = units_rank
+    kern = {k: v for k, v in prof.items() if v[1] > 0}
+    dom = max(("k_row_transmit", "k_col_propagate"), key=lambda k: kern.get(k, (0.0, 0))[0])
+    dom_ms, dom_n = kern[dom]
+    alg_bytes_launch = (ROW_BYTES if dom == "k_row_transmit" else COL_BYTES) * px_slices_per_step * K / dom_n
+    achieved = alg_bytes_launch / (dom_ms / dom_n * 1e-3) / 1e9
+    ms_pair = kern["k_row_transmit"][0] + kern["k_col_propagate"][0]
+    pair_gbs = (ROW_BYTES + COL_BYTES) * px_slices_per_step * K / (ms_pair * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                "bytes_per_launch": alg_bytes_launch, "avg_launch_ms": dom_ms / dom_n,
+                "slice_step_pair": {"achieved": pair_gbs, "frac": pair_gbs / peak,
+                                    "gpx_slice_s": px_slices_per_step * K / (ms_pair * 1e-3) / 1e9},
+                "kernel_ms_per_step": {k: v[0] / K for k, v in kern.items()},
+                "profiled_ms_per_step": ms_prof_total / K}
+    if "k_tacaw_fft" in kern:
+        tb = (8.0 * F + 4.0 * nb) * ctx.n_k_aperture * P + 4.0 * nb * (nx * ny - ctx.n_k_aperture) * P
+        tms = kern["k_tacaw_fft"][0] / kern["k_tacaw_fft"][1]
+        roofline["tacaw"] = {"achieved": tb / (tms * 1e-3) / 1e9, "frac": tb / (tms * 1e-3) / 1e9 / peak,
+                             "bytes_per_launch": tb, "avg_launch_ms": tms}
+
+    cpu_baseline = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cpu_baseline, _, _ = oracle_sample(make_workload(args.workload, n_frames=args.frames))
+
+    if rank == 0:
+        print(json.dumps({
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": max(3, args.warmup),
+            "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "complex64 (f32)", "data": "synthetic",
+            "config": {"workload": w.name, "grid": [nx, ny], "n_slices": S, "frames": F, "probes": P,
+                       "atoms": int(w.n_atoms), "kV": w.kV, "omega_bins": nb,
+                       "l2": "256 MiB buffer written between timed steps (L2 flush); per-step CUDA events",
+                       "parallelism": f"independent trajectory per GPU x{world}, one all-reduce of I(k,w)"},
+            "tacaw_end_to_end_s": ms_total / K * 1e-3,
+            "clocks": clocks,
+            "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": ms_e2e / K, "h2d_bytes_per_step": h2d,
+                    "d2h_bytes_per_step": d2h},
+            "gpu_launches": int(launches),
+            "roofline": roofline,
+            "cpu_baseline": cpu_baseline}))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -172,6 +172,16 @@ PS_API ps_status ps_dispersion(ps_ctx* ctx, const float* d_I, int P, int n_bins,
 PS_API ps_status ps_qbin(ps_ctx* ctx, const float* d_I, int P, int n_bins, double dq, int n_q, int32_t* d_qidx,
                   float* d_out);
 
+/* Optional per-kernel timing.  While enabled, every launch group of the hot path is bracketed by a CUDA
+ * event pair on the ctx stream.  ps_profile_read synchronises the stream, folds the pending pairs into
+ * per-kernel totals and returns them: names[i] (static strings), ms[i] (summed device time) and
+ * launches[i] for i < *n_kernels (arrays of at least 16 entries; any may be NULL); reset != 0 clears
+ * the totals afterwards.  Kernel slots: k_bin, k_sort, k_vk, k_v_col, k_v_row, k_incident,
+ * k_row_transmit, k_col_propagate, k_tacaw_fft, k_tacaw_accum, k_tacaw_finish, k_reduce. */
+PS_API ps_status ps_profile_enable(ps_ctx* ctx, int on);
+PS_API ps_status ps_profile_read(ps_ctx* ctx, int reset, int* n_kernels, const char** names, double* ms,
+                                 long long* launches);
+
 /* Number of kernels this ctx has launched so far (bench.py's `gpu_launches`). */
 PS_API long long ps_launch_count(const ps_ctx* ctx);
 

@@ -42,6 +42,8 @@ _PROTOTYPES = {
     "ps_dispersion": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
     "ps_qbin": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_double, C.c_int, C.c_void_p, C.c_void_p]),
     "ps_launch_count": (C.c_longlong, [C.c_void_p]),
+    "ps_profile_enable": (C.c_int, [C.c_void_p, C.c_int]),
+    "ps_profile_read": (C.c_int, [C.c_void_p, C.c_int, C.POINTER(C.c_int), C.c_void_p, C.c_void_p, C.c_void_p]),
 }
 
 
@@ -134,6 +136,18 @@ class Context:
     @property
     def launches(self) -> int:
         return int(self._lib.ps_launch_count(self._h))
+
+    def profile_enable(self, on: bool = True):
+        self._check(self._lib.ps_profile_enable(self._h, int(bool(on))))
+
+    def profile_read(self, reset: bool = True) -> dict:
+        """{kernel name: (summed device ms, launch groups)} from the per-launch CUDA events."""
+        n = C.c_int()
+        names = (C.c_char_p * 16)()
+        ms = (C.c_double * 16)()
+        cnt = (C.c_longlong * 16)()
+        self._check(self._lib.ps_profile_read(self._h, int(bool(reset)), C.byref(n), names, ms, cnt))
+        return {names[i].decode(): (float(ms[i]), int(cnt[i])) for i in range(n.value)}
 
     def version(self) -> str:
         return self._lib.ps_version().decode()

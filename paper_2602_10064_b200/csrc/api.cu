@@ -145,6 +145,8 @@ extern "C" void ps_destroy(ps_ctx* c) {
     cudaFree(c->d_ftab); cudaFree(c->d_elem_of_Z);
     cudaFree(c->kv.d_px_mid); cudaFree(c->kv.d_px_last); cudaFree(c->kv.d_py);
     cudaFree(c->scratch.p); cudaFree(c->misc.p); cudaFree(c->ts.d_bins);
+    for (auto& r : c->prof_pending) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
+    for (auto e : c->prof_pool) cudaEventDestroy(e);
     delete c;
 }
 
@@ -245,5 +247,33 @@ extern "C" ps_status ps_set_workspace(ps_ctx* c, void* d_ws, size_t bytes) {
     if (((uintptr_t)d_ws & 255u) != 0) return fail(c, PS_EINVAL, "ps_set_workspace: pointer must be 256-byte aligned");
     c->user_ws = d_ws;
     c->user_ws_bytes = d_ws ? bytes : 0;
+    return PS_OK;
+}
+
+extern "C" ps_status ps_profile_enable(ps_ctx* c, int on) {
+    if (!c) return PS_EINVAL;
+    c->prof_on = on != 0;
+    return PS_OK;
+}
+
+extern "C" ps_status ps_profile_read(ps_ctx* c, int reset, int* n_kernels, const char** names, double* ms,
+                                     long long* launches) {
+    if (!c) return PS_EINVAL;
+    if (!c->prof_pending.empty()) {
+        PSB_CUDA(c, cudaStreamSynchronize(c->stream));
+        for (auto& r : c->prof_pending) {
+            float t = 0.f;
+            if (cudaEventElapsedTime(&t, r.a, r.b) == cudaSuccess) { c->prof_ms[r.id] += t; c->prof_n[r.id]++; }
+            c->prof_pool.push_back(r.a); c->prof_pool.push_back(r.b);
+        }
+        c->prof_pending.clear();
+    }
+    if (n_kernels) *n_kernels = K_COUNT;
+    for (int i = 0; i < K_COUNT; ++i) {
+        if (names) names[i] = kKernelNames[i];
+        if (ms) ms[i] = c->prof_ms[i];
+        if (launches) launches[i] = c->prof_n[i];
+        if (reset) { c->prof_ms[i] = 0.0; c->prof_n[i] = 0; }
+    }
     return PS_OK;
 }

@@ -28,6 +28,16 @@ struct KvTables {                   // tables that depend on the accelerating vo
     float2* d_py = nullptr;         // [ny]  exp(-i pi lambda dz ky^2)
 };
 
+enum KernelId {                      // per-kernel timing slots (ps_profile_*)
+    K_BIN = 0, K_SORT, K_VK, K_V_COL, K_V_ROW, K_INCIDENT, K_ROW_TRANSMIT, K_COL_PROPAGATE, K_TACAW_FFT,
+    K_TACAW_ACCUM, K_TACAW_FINISH, K_REDUCE, K_COUNT
+};
+static const char* const kKernelNames[K_COUNT] = {
+    "k_bin", "k_sort", "k_vk", "k_v_col", "k_v_row", "k_incident", "k_row_transmit", "k_col_propagate",
+    "k_tacaw_fft", "k_tacaw_accum", "k_tacaw_finish", "k_reduce"};
+
+struct ProfRec { cudaEvent_t a, b; int id; };
+
 struct TacawStream {                // state of ps_tacaw_begin/add/finish
     bool active = false;
     int n_probes = 0, n_frames_total = 0, n_bins = 0, frames_seen = 0;
@@ -77,6 +87,13 @@ struct ps_ctx {
 
     psb::TacawStream ts;
     psb::DeviceBuf misc;                    // small per-call tables (bin slots, path pixels)
+
+    // optional per-launch timing (CUDA events on the ctx stream)
+    bool prof_on = false;
+    std::vector<psb::ProfRec> prof_pending;
+    std::vector<cudaEvent_t> prof_pool;
+    double prof_ms[psb::K_COUNT] = {0};
+    long long prof_n[psb::K_COUNT] = {0};
 };
 
 namespace psb {
@@ -100,6 +117,24 @@ inline ps_status fail(ps_ctx* c, ps_status s, const std::string& msg) {
             return psb::fail((ctx), PS_ECUDA, std::string("launch ") + name + ": " + cudaGetErrorString(_e)); \
         (ctx)->launches++;                                                                          \
     } while (0)
+
+// records an event pair around the launches made while it is alive (only when profiling is enabled)
+struct ProfScope {
+    ps_ctx* c; int id; cudaEvent_t a = nullptr, b = nullptr;
+    ProfScope(ps_ctx* ctx, int kid) : c(ctx), id(kid) {
+        if (!c->prof_on) return;
+        for (cudaEvent_t* e : {&a, &b}) {
+            if (!c->prof_pool.empty()) { *e = c->prof_pool.back(); c->prof_pool.pop_back(); }
+            else if (cudaEventCreate(e) != cudaSuccess) { *e = nullptr; }
+        }
+        if (a && b) cudaEventRecord(a, c->stream);
+    }
+    ~ProfScope() {
+        if (!c->prof_on || !a || !b) return;
+        cudaEventRecord(b, c->stream);
+        c->prof_pending.push_back({a, b, id});
+    }
+};
 
 inline bool is_pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
 inline int signed_index(int i, int n) { return i < (n + 1) / 2 ? i : i - n; }

@@ -187,6 +187,7 @@ extern "C" ps_status ps_make_incident(ps_ctx* c, double kV, double semi_angle_mr
     if (!d_psi0 || n < 1 || !(kV > 0.0) || semi_angle_mrad < 0.0)
         return fail(c, PS_EINVAL, "ps_make_incident: null pointer, non-positive count/voltage or negative angle");
     const int nx = c->nx, ny = c->ny;
+    ProfScope ps_(c, K_INCIDENT);
     float2* psi = (float2*)d_psi0;
     const long long total = (long long)n * nx * ny;
     const bool probe = !is_tilt && semi_angle_mrad > 0.0;

@@ -245,13 +245,19 @@ extern "C" ps_status ps_multislice(ps_ctx* c, double kV, const void* d_psi0, int
             cm.F = n_frames;
             for (int s = 0; s < S; ++s) {
                 cudaError_t e = cudaErrorInvalidValue;
+                {
+                ProfScope ps_(c, K_ROW_TRANSMIT);
                 if (s == 0) { PSB_DISPATCH_N(c->nx, (e = launch_row<N_, true>(c, W, psi0, d_V, cm, s, sigma))); }
                 else        { PSB_DISPATCH_N(c->nx, (e = launch_row<N_, false>(c, W, psi0, d_V, cm, s, sigma))); }
+                }
                 if (e != cudaSuccess) return fail(c, PS_ECUDA, std::string("k_row_transmit: ") + cudaGetErrorString(e));
                 c->launches++;
                 e = cudaErrorInvalidValue;
+                {
+                ProfScope ps_(c, K_COL_PROPAGATE);
                 if (s == S - 1) { PSB_DISPATCH_N(c->ny, (e = launch_col<N_, true>(c, W, cm))); }
                 else            { PSB_DISPATCH_N(c->ny, (e = launch_col<N_, false>(c, W, cm))); }
+                }
                 if (e != cudaSuccess) return fail(c, PS_ECUDA, std::string("k_col_propagate: ") + cudaGetErrorString(e));
                 c->launches++;
             }

@@ -449,6 +449,7 @@ extern "C" ps_status ps_build_slices(ps_ctx* c, const float* d_pos, const int32_
         nfc = 1;
     }
     if (nfc > n_frames) nfc = n_frames;
+    if (nfc > 65535) nfc = 65535;                                          // grid.z limit of k_vk
     ScratchLayout L = scratch_layout(c, nfc, n_atoms);
     while (c->user_ws && L.total > c->user_ws_bytes && nfc > 1) L = scratch_layout(c, --nfc, n_atoms);
     char* ws = (char*)c->user_ws;
@@ -474,21 +475,29 @@ extern "C" ps_status ps_build_slices(ps_ctx* c, const float* d_pos, const int32_
     for (int f0 = 0; f0 < n_frames; f0 += nfc) {
         const int nf = (n_frames - f0 < nfc) ? n_frames - f0 : nfc;
         const long long n_total = (long long)nf * n_atoms;
+        { ProfScope ps_(c, K_BIN);
         k_bin<<<(unsigned)((n_total + 255) / 256), 256, 0, c->stream>>>(
             d_pos + (size_t)f0 * n_atoms * 3, d_Z, c->d_elem_of_Z, n_total, n_atoms, c->cell[0], c->cell[1], c->cell[2],
             c->n_slices, c->n_elem, Ux, Uy, key, d_slice_idx ? d_slice_idx + (size_t)f0 * n_atoms : nullptr);
+        }
         PSB_LAUNCH_CHECK(c, "k_bin");
+        { ProfScope ps_(c, K_SORT);
         k_sort<<<nf, 32, (size_t)(n_bins + 1) * sizeof(int), c->stream>>>(Ux, Uy, key, n_atoms, (int)n_bins, sUx, sUy, off);
+        }
         PSB_LAUNCH_CHECK(c, "k_sort");
+        { ProfScope ps_(c, K_VK);
         k_vk<<<dim3(tiles_m * tiles_n, c->n_slices, nf), VK_THREADS, 0, c->stream>>>(
             sUx, sUy, off, c->d_ftab, c->d_nmax, Vk, n_atoms, c->n_slices, c->n_elem, c->mcut, c->ncut, c->nx, tiles_m);
+        }
         PSB_LAUNCH_CHECK(c, "k_vk");
         cudaError_t e = cudaErrorInvalidValue;
-        PSB_DISPATCH_N(c->ny, (e = launch_v_col<N_>(c, Vk, off, Zm, nf)));
+        { ProfScope ps_(c, K_V_COL);
+        PSB_DISPATCH_N(c->ny, (e = launch_v_col<N_>(c, Vk, off, Zm, nf))); }
         if (e != cudaSuccess) return fail(c, PS_ECUDA, std::string("k_v_col: ") + cudaGetErrorString(e));
         c->launches++;
         e = cudaErrorInvalidValue;
-        PSB_DISPATCH_N(c->nx, (e = launch_v_row<N_>(c, Zm, off, d_V + (size_t)f0 * c->n_slices * img, nf)));
+        { ProfScope ps_(c, K_V_ROW);
+        PSB_DISPATCH_N(c->nx, (e = launch_v_row<N_>(c, Zm, off, d_V + (size_t)f0 * c->n_slices * img, nf))); }
         if (e != cudaSuccess) return fail(c, PS_ECUDA, std::string("k_v_row: ") + cudaGetErrorString(e));
         c->launches++;
     }

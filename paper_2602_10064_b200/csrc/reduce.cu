@@ -168,6 +168,7 @@ extern "C" ps_status ps_sdp(ps_ctx* c, const float* d_I, int P, int n_bins, int 
     if (!c) return PS_EINVAL;
     ps_status st = check_I(c, "ps_sdp", d_I, P, n_bins, d_out);
     if (st != PS_OK) return st;
+    ProfScope ps_(c, K_REDUCE);
     if (bin_lo < 0 || bin_hi >= n_bins || bin_lo > bin_hi) return fail(c, PS_EINVAL, "ps_sdp: bin range outside [0, n_bins)");
     const size_t npix = (size_t)c->nx * c->ny;
     k_sdp<<<(unsigned)((npix + 255) / 256), 256, 0, c->stream>>>(d_I, d_out, P, n_bins, bin_lo, bin_hi, npix);
@@ -180,6 +181,7 @@ extern "C" ps_status ps_spectrum_image(ps_ctx* c, const float* d_I, int P, int n
     if (!c) return PS_EINVAL;
     ps_status st = check_I(c, "ps_spectrum_image", d_I, P, n_bins, d_out);
     if (st != PS_OK) return st;
+    ProfScope ps_(c, K_REDUCE);
     if (k_in < 0.0) return fail(c, PS_EINVAL, "ps_spectrum_image: k_in must be >= 0");
     const size_t npix = (size_t)c->nx * c->ny;
     if ((st = ensure_buf(c, c->misc, 4096 + npix)) != PS_OK) return st;
@@ -197,6 +199,7 @@ extern "C" ps_status ps_dispersion(ps_ctx* c, const float* d_I, int P, int n_bin
     if (!c) return PS_EINVAL;
     ps_status st = check_I(c, "ps_dispersion", d_I, P, n_bins, d_out);
     if (st != PS_OK) return st;
+    ProfScope ps_(c, K_REDUCE);
     if (!kx || !ky || !d_pix || n_path < 1) return fail(c, PS_EINVAL, "ps_dispersion: null pointer or empty path");
     const size_t need = 4096 + 2 * (size_t)n_path * sizeof(double);
     if ((st = ensure_buf(c, c->misc, need)) != PS_OK) return st;
@@ -218,6 +221,7 @@ extern "C" ps_status ps_qbin(ps_ctx* c, const float* d_I, int P, int n_bins, dou
     if (!c) return PS_EINVAL;
     ps_status st = check_I(c, "ps_qbin", d_I, P, n_bins, d_out);
     if (st != PS_OK) return st;
+    ProfScope ps_(c, K_REDUCE);
     if (!d_qidx || !(dq > 0.0) || n_q < 1) return fail(c, PS_EINVAL, "ps_qbin: null pointer, dq <= 0 or n_q < 1");
     const size_t npix = (size_t)c->nx * c->ny;
     const size_t need = 4096 + (2 * ((size_t)n_q + 1) + npix) * 4 + 512;

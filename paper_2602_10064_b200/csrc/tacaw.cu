@@ -186,6 +186,7 @@ extern "C" ps_status ps_tacaw(ps_ctx* c, const void* d_exit, int exit_layout, in
     PSB_CUDA(c, cudaMemcpyAsync(d_slot, slot.data(), (size_t)n_frames * 4, cudaMemcpyHostToDevice, c->stream));
     PSB_CUDA(c, cudaStreamSynchronize(c->stream));           // `slot` dies at return; 16 KB at most
     cudaError_t e = cudaErrorInvalidValue;
+    ProfScope ps_(c, K_TACAW_FFT);
     switch (n_frames) {
         case 32: e = launch_tacaw<32>(c, (const float2*)d_exit, d_I, d_slot, n_bins, n_probes); break;
         case 64: e = launch_tacaw<64>(c, (const float2*)d_exit, d_I, d_slot, n_bins, n_probes); break;
@@ -233,6 +234,7 @@ extern "C" ps_status ps_tacaw_add(ps_ctx* c, const void* d_exit_chunk, int frame
         return fail(c, PS_EINVAL, "ps_tacaw_add: null pointer or frame range outside [0, n_frames_total)");
     const size_t npix = (size_t)c->nx * c->ny;
     dim3 grid((unsigned)((npix + SB_PIX - 1) / SB_PIX), (unsigned)((ts.n_bins + 1 + SB_BINS - 1) / SB_BINS), ts.n_probes);
+    ProfScope ps_(c, K_TACAW_ACCUM);
     k_tacaw_accum<<<grid, SB_PIX, 0, c->stream>>>((const float2*)d_exit_chunk, (float2*)ts.d_acc, ts.d_bins, ts.n_bins,
                                                  ts.n_frames_total, frame0, n_frames_chunk, npix, c->nx, c->ny, c->d_nmax);
     PSB_LAUNCH_CHECK(c, "k_tacaw_accum");
@@ -250,6 +252,7 @@ extern "C" ps_status ps_tacaw_finish(ps_ctx* c, float* d_I) {
                                       std::to_string(ts.n_frames_total) + " frames were added");
     const size_t npix = (size_t)c->nx * c->ny;
     const long long total = (long long)ts.n_probes * ts.n_bins * npix;
+    ProfScope ps_(c, K_TACAW_FINISH);
     k_tacaw_finish<<<(unsigned)((total + 255) / 256), 256, 0, c->stream>>>((const float2*)ts.d_acc, d_I, ts.d_bins, ts.n_bins,
                                                                            npix, total);
     PSB_LAUNCH_CHECK(c, "k_tacaw_finish");

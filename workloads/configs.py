@@ -170,7 +170,7 @@ def make_workload(name: str, *, mini: bool = False, n_frames: int | None = None,
         # 8 modes A=0.05/sqrt(8) + white noise 0.01, 5-Gaussian form factors.
         a, reps, F, g, S = 5.431, (3, 3, 3), 64, 128, 12
         if mini:
-            reps, F, g, S = (2, 2, 1), 16, 64, 4
+            reps, F, g, S = (2, 2, 1), 32, 64, 4
         F = n_frames or F; g = grid or g
         rng = np.random.default_rng(1001)
         R, Z = _tile(_DIAMOND, [14] * 8, np.array([a, a, a]), reps)
