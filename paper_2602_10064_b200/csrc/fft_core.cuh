@@ -28,6 +28,16 @@ __device__ __forceinline__ float2 cmul(const float2 a, const float2 b) {
 }
 __device__ __forceinline__ float2 cswap(const float2 a) { return make_float2(a.y, a.x); }
 
+// exp(i x) for |x| up to a few thousand radians: two-constant Cody-Waite reduction to [-pi, pi]
+// (exact for the quotients that occur), then the SFU sine / cosine (abs. error 2^-21.4 there).
+// Error budget: DESIGN.md section 7.
+__device__ __forceinline__ float2 cis_fast(const float x) {
+    const float k = rintf(x * 0.15915494309189535f);
+    float r = fmaf(-k, 6.28125f, x);                       // 2 pi = 6.28125 + 1.9353071795864769e-3
+    r = fmaf(-k, 1.9353071795864769e-3f, r);
+    return make_float2(__cosf(r), __sinf(r));
+}
+
 // ---------------------------------------------------------------- small DFTs (forward, natural order)
 __device__ __forceinline__ void dft2(float2& a, float2& b) {
     const float2 t = a;

@@ -23,6 +23,7 @@ template <int NX> struct RowCfg {
     static constexpr int T = Plan<NX>::T;
     static constexpr int THREADS = (T > 256) ? T : 256;
     static constexpr int RPB = THREADS / T;                               // rows per block
+    static constexpr int MIN_BLOCKS = (THREADS <= 256) ? 2 : 1;           // cap registers at 128
     static constexpr size_t SMEM = (size_t)RPB * RowLine<NX>::LEN * sizeof(float2);
     using Sync = typename std::conditional<(T <= 32), WarpSync, BlockSync>::type;
 };
@@ -32,7 +33,7 @@ struct ChunkMap {           // chunk of waves: probes [p0,p0+np) x frames [f0,f0
 };
 
 template <int NX, bool FIRST>
-__global__ void __launch_bounds__(RowCfg<NX>::THREADS)
+__global__ void __launch_bounds__(RowCfg<NX>::THREADS, RowCfg<NX>::MIN_BLOCKS)
 k_row_transmit(float2* __restrict__ W, const float2* __restrict__ psi0, const float* __restrict__ V,
                const uint8_t* __restrict__ tile_active, const ChunkMap cm, const int ny, const int n_slices,
                const int slice, const float sigma, const int n_items) {
@@ -60,6 +61,12 @@ k_row_transmit(float2* __restrict__ W, const float2* __restrict__ psi0, const fl
         }
         float2* wrow = W + (((size_t)p * cm.F + f) * ny + y) * NX;
         float2 v[16];
+        float sv[16];                                    // sigma * V of this row, fetched with the wave
+        {
+            const float* vrow = V + (((size_t)f * n_slices + slice) * ny + y) * NX;
+#pragma unroll
+            for (int e = 0; e < 16; ++e) sv[e] = valid ? __ldg(vrow + t + e * T) : 0.f;
+        }
         if (FIRST) {
             const float2* src = psi0 + ((size_t)p * ny + y) * NX;
 #pragma unroll
@@ -70,15 +77,8 @@ k_row_transmit(float2* __restrict__ W, const float2* __restrict__ psi0, const fl
                 v[e] = (valid && ((amask >> e) & 1u)) ? wrow[t + e * T] : make_float2(0.f, 0.f);
             fft_inverse<NX, RowSlots, typename Cfg::Sync>(v, t, tw, slots);
         }
-        if (valid) {
-            const float* vrow = V + (((size_t)f * n_slices + slice) * ny + y) * NX;
 #pragma unroll
-            for (int e = 0; e < 16; ++e) {
-                float s, c;
-                sincosf(sigma * __ldg(vrow + t + e * T), &s, &c);
-                v[e] = cmul(v[e], make_float2(c, s));
-            }
-        }
+        for (int e = 0; e < 16; ++e) v[e] = cmul(v[e], cis_fast(sigma * sv[e]));
         fft_forward<NX, RowSlots, typename Cfg::Sync>(v, t, tw, slots);
         if (valid) {
 #pragma unroll
@@ -232,6 +232,10 @@ extern "C" ps_status ps_multislice(ps_ctx* c, double kV, const void* d_psi0, int
     const int np = n_probes < chunk ? n_probes : chunk;
     int nf = chunk / np;
     if (nf < 1) nf = 1;
+    if (nf < n_frames) {                                     // equal-sized frame chunks (no short tail chunk)
+        const int n_chunks = (n_frames + nf - 1) / nf;
+        nf = (n_frames + n_chunks - 1) / n_chunks;
+    }
     float2* W = (float2*)d_exit;
     const float2* psi0 = (const float2*)d_psi0;
     const float sigma = (float)c->kv.sigma;
