@@ -144,7 +144,7 @@ extern "C" void ps_destroy(ps_ctx* c) {
     cudaFree(c->d_nmax); cudaFree(c->d_tiles); cudaFree(c->d_tile_active);
     cudaFree(c->d_ftab); cudaFree(c->d_elem_of_Z);
     cudaFree(c->kv.d_px_mid); cudaFree(c->kv.d_px_last); cudaFree(c->kv.d_py);
-    cudaFree(c->scratch.p); cudaFree(c->misc.p); cudaFree(c->ts.d_bins);
+    cudaFree(c->scratch.p); cudaFree(c->misc.p); cudaFree(c->qorder.p); cudaFree(c->ts.d_bins);
     for (auto& r : c->prof_pending) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
     for (auto e : c->prof_pool) cudaEventDestroy(e);
     delete c;
@@ -221,6 +221,7 @@ extern "C" ps_status ps_set_geometry(ps_ctx* c, const double cell[3], int nx, in
     if ((s = upload(c, &c->d_tile_active, act)) != PS_OK) return s;
     c->kv.kV = -1.0;
     c->ftab_valid = false;
+    c->qorder_valid = false;
     c->have_geom = true;
     return PS_OK;
 }

@@ -87,6 +87,10 @@ struct ps_ctx {
 
     psb::TacawStream ts;
     psb::DeviceBuf misc;                    // small per-call tables (bin slots, path pixels)
+    psb::DeviceBuf qorder;                  // ps_qbin: cursor, offsets and pixel order by q bin (cached)
+    bool qorder_valid = false;
+    double qorder_dq = 0.0;
+    int qorder_nq = 0;
 
     // optional per-launch timing (CUDA events on the ctx stream)
     bool prof_on = false;

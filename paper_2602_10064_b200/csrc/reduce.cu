@@ -51,14 +51,22 @@ __global__ void k_detector_mask(uint8_t* __restrict__ mask, const int nx, const 
     mask[i] = (k >= k_in && (!has_out || k < k_out)) ? 1 : 0;
 }
 
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(1024)
 k_spectrum_image(const float* __restrict__ I, const uint8_t* __restrict__ mask, float* __restrict__ out,
                  const size_t npix) {
     __shared__ float sh[32];
-    const float* src = I + (size_t)blockIdx.x * npix;        // blockIdx.x = p * n_bins + b
+    const float4* src = reinterpret_cast<const float4*>(I + (size_t)blockIdx.x * npix);   // blockIdx.x = p * n_bins + b
+    const uchar4* m4 = reinterpret_cast<const uchar4*>(mask);
     float s = 0.f;
-    for (size_t i = threadIdx.x; i < npix; i += blockDim.x)
-        if (mask[i]) s += src[i];
+    for (size_t i = threadIdx.x; i < npix / 4; i += blockDim.x) {      // npix is a multiple of 1024
+        const float4 x = src[i];
+        const uchar4 m = m4[i];
+        float q = m.x ? x.x : 0.f;                                     // fixed order inside the quad
+        q += m.y ? x.y : 0.f;
+        q += m.z ? x.z : 0.f;
+        q += m.w ? x.w : 0.f;
+        s += q;
+    }
     s = block_sum(s, sh);
     if (threadIdx.x == 0) out[blockIdx.x] = s;
 }
@@ -189,7 +197,7 @@ extern "C" ps_status ps_spectrum_image(ps_ctx* c, const float* d_I, int P, int n
     k_detector_mask<<<(unsigned)((npix + 255) / 256), 256, 0, c->stream>>>(d_mask, c->nx, c->ny, c->cell[0], c->cell[1], k_in,
                                                                            k_out, k_out > 0.0 ? 1 : 0);
     PSB_LAUNCH_CHECK(c, "k_detector_mask");
-    k_spectrum_image<<<P * n_bins, 256, 0, c->stream>>>(d_I, d_mask, d_out, npix);
+    k_spectrum_image<<<P * n_bins, 1024, 0, c->stream>>>(d_I, d_mask, d_out, npix);
     PSB_LAUNCH_CHECK(c, "k_spectrum_image");
     return PS_OK;
 }
@@ -224,15 +232,20 @@ extern "C" ps_status ps_qbin(ps_ctx* c, const float* d_I, int P, int n_bins, dou
     ProfScope ps_(c, K_REDUCE);
     if (!d_qidx || !(dq > 0.0) || n_q < 1) return fail(c, PS_EINVAL, "ps_qbin: null pointer, dq <= 0 or n_q < 1");
     const size_t npix = (size_t)c->nx * c->ny;
-    const size_t need = 4096 + (2 * ((size_t)n_q + 1) + npix) * 4 + 512;
-    if ((st = ensure_buf(c, c->misc, need)) != PS_OK) return st;
-    int32_t* d_cursor = (int32_t*)((char*)c->misc.p + 4096);
+    // pixel order by q bin depends only on (geometry, dq, n_q): built once and kept in the ctx
+    const size_t need = (2 * ((size_t)n_q + 1) + npix) * 4 + 512;
+    const bool cached = c->qorder_valid && c->qorder_dq == dq && c->qorder_nq == n_q && c->qorder.bytes >= need;
+    if (!cached && (st = ensure_buf(c, c->qorder, need)) != PS_OK) return st;
+    int32_t* d_cursor = (int32_t*)c->qorder.p;
     int32_t* d_off = d_cursor + (n_q + 1);
     int32_t* d_order = d_off + (n_q + 1);
     k_qidx<<<(unsigned)((npix + 255) / 256), 256, 0, c->stream>>>(d_qidx, c->nx, c->ny, c->cell[0], c->cell[1], dq, n_q);
     PSB_LAUNCH_CHECK(c, "k_qidx");
-    k_order_by_bin<<<1, 32, 0, c->stream>>>(d_qidx, (int)npix, n_q, d_cursor, d_off, d_order);
-    PSB_LAUNCH_CHECK(c, "k_order_by_bin");
+    if (!cached) {
+        k_order_by_bin<<<1, 32, 0, c->stream>>>(d_qidx, (int)npix, n_q, d_cursor, d_off, d_order);
+        PSB_LAUNCH_CHECK(c, "k_order_by_bin");
+        c->qorder_valid = true; c->qorder_dq = dq; c->qorder_nq = n_q;
+    }
     const long long warps = (long long)n_bins * n_q;
     k_qbin_sum<<<(unsigned)((warps * 32 + 127) / 128), 128, 0, c->stream>>>(d_I, d_off, d_order, d_out, P, n_bins, n_q, npix);
     PSB_LAUNCH_CHECK(c, "k_qbin_sum");
