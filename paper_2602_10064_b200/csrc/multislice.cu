@@ -14,6 +14,7 @@
 // The propagation is done in place inside the caller's exit-wave array.
 #include "common.cuh"
 #include "fft_core.cuh"
+#include "tma.cuh"
 #include <type_traits>
 
 namespace psb {
@@ -89,57 +90,123 @@ k_row_transmit(float2* __restrict__ W, const float2* __restrict__ psi0, const fl
 }
 
 // ------------------------------------------------------------------------------------ column pass
+// A block owns C adjacent k-columns x all NY rows of one wave per item.  The tile travels
+// global -> shared -> global through the TMA engine (2-D tensor map over the wave array viewed as
+// float32 [P*F*ny][2 nx]); the ring of NS shared-memory stages is, in turn, TMA destination, FFT
+// exchange buffer and TMA store source, so the load of item i+1 and the store of item i-1 overlap the
+// transforms of item i and no register is spent on staging.
 template <int NY> struct ColCfg {
     static constexpr int T = Plan<NY>::T;
-    static constexpr int C = (NY <= 512) ? 16 : 8;                        // columns per block
+    static constexpr int C = (NY <= 256) ? 16 : ((NY <= 1024) ? 8 : 4);   // columns per block
     static constexpr int THREADS = C * T;
-    static constexpr size_t SMEM = ((size_t)NY * C + NY) * sizeof(float2);
+    static constexpr int NS = 3;                                          // pipeline stages
+    static constexpr int BOX_R = (NY < 256) ? NY : 256;                   // TMA box rows (<= 256)
+    static constexpr int NBOX = NY / BOX_R;
+    static constexpr int MIN_BLOCKS = (THREADS <= 256) ? 2 : 1;
+    static constexpr uint32_t STAGE_BYTES = (uint32_t)NY * C * sizeof(float2);
+    static constexpr size_t SMEM = (size_t)NS * STAGE_BYTES + (size_t)NY * sizeof(float2) + NS * sizeof(uint64_t) + 128;
 };
 
 template <int NY, bool LAST>
-__global__ void __launch_bounds__(ColCfg<NY>::THREADS)
-k_col_propagate(float2* __restrict__ W, const int nx, const int32_t* __restrict__ tiles, const int n_tiles,
-                const uint8_t* __restrict__ tile_active, const int32_t* __restrict__ nmax,
-                const float2* __restrict__ px, const float2* __restrict__ py, const ChunkMap cm,
-                const int n_items) {
+__global__ void __launch_bounds__(ColCfg<NY>::THREADS, ColCfg<NY>::MIN_BLOCKS)
+k_col_propagate(const __grid_constant__ CUtensorMap wmap, const int tiles_lo, const int tile_gap, const int n_tiles,
+                const int32_t* __restrict__ nmax, const float2* __restrict__ px, const float2* __restrict__ py,
+                const ChunkMap cm, const int n_items) {
     using Cfg = ColCfg<NY>;
-    constexpr int T = Cfg::T, C = Cfg::C, SUB = kColTile / C;
-    extern __shared__ float2 smem[];
-    float2* py_s = smem + (size_t)NY * C;
+    constexpr int T = Cfg::T, C = Cfg::C, SUB = kColTile / C, NS = Cfg::NS, PF = NS - 2;   // prefetch distance
+    extern __shared__ __align__(1024) float2 smem_col[];      // no static shared memory: the window starts aligned
+    float2* stage0 = smem_col;
+    float2* py_s = smem_col + (size_t)NS * NY * C;
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem_col + (size_t)NS * NY * C + NY);
     const int c = threadIdx.x % C, t = threadIdx.x / C;
-    ColSlots<C> slots{smem + c};
+    const int per_wave = n_tiles * SUB;
+
+    auto issue_load = [&](const int item, const int s) {      // one thread: arm the barrier, launch the boxes
+        const int l = item / per_wave, rem = item % per_wave;
+        const int tj = rem / SUB;                             // active tiles: [0, tiles_lo) and [tiles_lo + gap, ..)
+        const int kx0 = (tj < tiles_lo ? tj : tj + tile_gap) * kColTile + (rem % SUB) * C;
+        const int p = cm.p0 + l % cm.np, f = cm.f0 + l / cm.np;
+        const int row0 = (p * cm.F + f) * NY;
+        tma::mbar_arrive_expect_tx(&full[s], Cfg::STAGE_BYTES);
+#pragma unroll
+        for (int b = 0; b < Cfg::NBOX; ++b)
+            tma::tensor_load_2d(stage0 + (size_t)s * NY * C + (size_t)b * Cfg::BOX_R * C, &wmap, 2 * kx0,
+                                row0 + b * Cfg::BOX_R, &full[s]);
+    };
+
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int s = 0; s < NS; ++s) tma::mbar_init(&full[s], 1);
+        tma::fence_mbar_init();
+    }
     for (int i = threadIdx.x; i < NY; i += Cfg::THREADS) py_s[i] = py[i];
     Twiddles<NY> tw;
     tw.init(t);
     __syncthreads();
-    const int per_wave = n_tiles * SUB;
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int k = 0; k < PF; ++k)
+            if (blockIdx.x + k * gridDim.x < n_items) issue_load(blockIdx.x + k * gridDim.x, k);
+    }
 
-    for (int item = blockIdx.x; item < n_items; item += gridDim.x) {
-        const int l = item / per_wave, rem = item % per_wave;
-        const int tile = LAST ? rem / SUB : tiles[rem / SUB];
-        const int kx = tile * kColTile + (rem % SUB) * C + c;
-        const int p = cm.p0 + l % cm.np, f = cm.f0 + l / cm.np;
-        float2* wcol = W + ((size_t)p * cm.F + f) * NY * nx + kx;
-        float2 v[16];
-        if (LAST && !tile_active[tile]) {                 // block-uniform: column tile outside the band limit
-#pragma unroll
-            for (int e = 0; e < 16; ++e) wcol[(size_t)(t + e * T) * nx] = make_float2(0.f, 0.f);
-            continue;
+    int it = 0;
+    for (int item = blockIdx.x; item < n_items; item += gridDim.x, ++it) {
+        const int s = it % NS;
+        if (threadIdx.x == 0) {
+            const int nxt = item + PF * gridDim.x;
+            if (nxt < n_items) {
+                tma::bulk_wait_read<1>();                     // stage (it+PF)%NS was stored NS-PF = 2 items ago: drained
+                issue_load(nxt, (it + PF) % NS);
+            }
         }
-#pragma unroll
-        for (int e = 0; e < 16; ++e) v[e] = wcol[(size_t)(t + e * T) * nx];
-        fft_forward<NY, ColSlots<C>, BlockSync>(v, t, tw, slots);
+        const int l = item / per_wave, rem = item % per_wave;
+        const int tj = rem / SUB;
+        const int kx0 = (tj < tiles_lo ? tj : tj + tile_gap) * kColTile + (rem % SUB) * C;
+        const int kx = kx0 + c;
         const int nm = nmax[kx];
         const float2 pxv = px[kx];
+        float2* st = stage0 + (size_t)s * NY * C;
+        ColSlots<C> slots{st + c};
+        tma::mbar_wait(&full[s], (it / NS) & 1);
+        float2 v[16];
+#pragma unroll
+        for (int e = 0; e < 16; ++e) v[e] = slots.at(t + e * T);
+        fft_forward<NY, ColSlots<C>, BlockSync>(v, t, tw, slots);
 #pragma unroll
         for (int e = 0; e < 16; ++e) {
             const int iy = t + e * T;
-            const int n = iy < NY / 2 ? iy : NY - iy;     // |signed index|
+            const int n = iy < NY / 2 ? iy : NY - iy;         // |signed index|
             v[e] = (n <= nm) ? cmul(v[e], cmul(pxv, py_s[iy])) : make_float2(0.f, 0.f);
         }
         if (!LAST) fft_inverse<NY, ColSlots<C>, BlockSync>(v, t, tw, slots);
+        __syncthreads();                                      // exchange reads of this stage are done
 #pragma unroll
-        for (int e = 0; e < 16; ++e) wcol[(size_t)(t + e * T) * nx] = v[e];
+        for (int e = 0; e < 16; ++e) slots.at(t + e * T) = v[e];
+        tma::fence_proxy_async();
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            const int p = cm.p0 + l % cm.np, f = cm.f0 + l / cm.np;
+            const int row0 = (p * cm.F + f) * NY;
+#pragma unroll
+            for (int b = 0; b < Cfg::NBOX; ++b)
+                tma::tensor_store_2d(&wmap, 2 * kx0, row0 + b * Cfg::BOX_R, st + (size_t)b * Cfg::BOX_R * C);
+            tma::bulk_commit();
+        }
+    }
+    if (threadIdx.x == 0) tma::bulk_wait_all<0>();
+}
+
+// last slice: column tiles outside the band limit of the k-space exit wave are exact zeros
+__global__ void k_zero_cols(float2* __restrict__ W, const int nx, const int ny, const int col_lo, const int col_hi,
+                            const ChunkMap cm) {
+    const int width = col_hi - col_lo;
+    const long long total = (long long)cm.np * cm.nf * ny * width;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x) {
+        const int x = (int)(i % width);
+        const long long row = i / width;
+        const int y = (int)(row % ny), l = (int)(row / ny);
+        const int p = cm.p0 + l % cm.np, f = cm.f0 + l / cm.np;
+        W[(((size_t)p * cm.F + f) * ny + y) * nx + col_lo + x] = make_float2(0.f, 0.f);
     }
 }
 
@@ -178,7 +245,7 @@ static cudaError_t launch_row(ps_ctx* c, float2* W, const float2* psi0, const fl
 }
 
 template <int NY, bool LAST>
-static cudaError_t launch_col(ps_ctx* c, float2* W, const ChunkMap& cm) {
+static cudaError_t launch_col(ps_ctx* c, const CUtensorMap& wmap, const ChunkMap& cm, int zero_lo, int zero_hi) {
     using Cfg = ColCfg<NY>;
     auto kern = k_col_propagate<NY, LAST>;
     static bool attr_done = false;
@@ -189,12 +256,18 @@ static cudaError_t launch_col(ps_ctx* c, float2* W, const ChunkMap& cm) {
         per_sm_grid = persistent_grid(kern, Cfg::THREADS, Cfg::SMEM, 1 << 30);
         attr_done = true;
     }
-    const int n_tiles = LAST ? c->nx / kColTile : c->n_tiles_active;
+    const int n_tiles = c->n_tiles_active;
     const int n_items = cm.np * cm.nf * n_tiles * (kColTile / Cfg::C);
     const int grid = n_items < per_sm_grid ? n_items : per_sm_grid;
-    kern<<<grid, Cfg::THREADS, Cfg::SMEM, c->stream>>>(W, c->nx, c->d_tiles, n_tiles, c->d_tile_active, c->d_nmax,
+    kern<<<grid, Cfg::THREADS, Cfg::SMEM, c->stream>>>(wmap, zero_lo / kColTile, (zero_hi - zero_lo) / kColTile, n_tiles, c->d_nmax,
                                                       LAST ? c->kv.d_px_last : c->kv.d_px_mid, c->kv.d_py, cm, n_items);
     return cudaGetLastError();
+}
+
+template <int NY>
+static bool make_wave_map(CUtensorMap* map, void* W, int nx, long long rows) {
+    using Cfg = ColCfg<NY>;
+    return tma::make_map_2d_f32(map, W, 2ull * nx, (uint64_t)rows, 2 * Cfg::C, Cfg::BOX_R);
 }
 
 #define PSB_DISPATCH_N(n, CALL)                                                    \
@@ -241,6 +314,26 @@ extern "C" ps_status ps_multislice(ps_ctx* c, double kV, const void* d_psi0, int
     const float sigma = (float)c->kv.sigma;
     const int S = c->n_slices;
 
+    // TMA view of the wave array: float32 [P*F*ny][2 nx]; box = C columns x up to 256 rows
+    const long long wave_rows = (long long)n_probes * n_frames * c->ny;
+    if (wave_rows > 0x7fffffffLL) return fail(c, PS_EUNSUPPORTED, "ps_multislice: n_probes*n_frames*ny exceeds 2^31");
+    CUtensorMap wmap;
+    bool map_ok = false;
+    PSB_DISPATCH_N(c->ny, (map_ok = make_wave_map<N_>(&wmap, d_exit, c->nx, wave_rows)));
+    if (!map_ok) return fail(c, PS_ECUDA, "ps_multislice: cuTensorMapEncodeTiled failed (exit-wave array must be 16-byte aligned)");
+    // contiguous range of columns outside the band limit (zero in the k-space exit wave)
+    int zero_lo = 0, zero_hi = 0;
+    {
+        const int nt = c->nx / kColTile;
+        std::vector<char> act(nt, 0);
+        for (int tI : c->h_tiles) act[tI] = 1;
+        int a = 0;
+        while (a < nt && act[a]) ++a;
+        int b = nt;
+        while (b > a && act[b - 1]) --b;
+        zero_lo = a * kColTile; zero_hi = b * kColTile;
+    }
+
     for (int p0 = 0; p0 < n_probes; p0 += np) {
         for (int f0 = 0; f0 < n_frames; f0 += nf) {
             ChunkMap cm;
@@ -259,8 +352,17 @@ extern "C" ps_status ps_multislice(ps_ctx* c, double kV, const void* d_psi0, int
                 e = cudaErrorInvalidValue;
                 {
                 ProfScope ps_(c, K_COL_PROPAGATE);
-                if (s == S - 1) { PSB_DISPATCH_N(c->ny, (e = launch_col<N_, true>(c, W, cm))); }
-                else            { PSB_DISPATCH_N(c->ny, (e = launch_col<N_, false>(c, W, cm))); }
+                if (s == S - 1) {
+                    if (zero_hi > zero_lo) {
+                        const long long tot = (long long)cm.np * cm.nf * c->ny * (zero_hi - zero_lo);
+                        const int zb = (int)((tot + 255) / 256 < 148 * 16 ? (tot + 255) / 256 : 148 * 16);
+                        k_zero_cols<<<zb, 256, 0, c->stream>>>(W, c->nx, c->ny, zero_lo, zero_hi, cm);
+                        c->launches++;
+                    }
+                    PSB_DISPATCH_N(c->ny, (e = launch_col<N_, true>(c, wmap, cm, zero_lo, zero_hi)));
+                } else {
+                    PSB_DISPATCH_N(c->ny, (e = launch_col<N_, false>(c, wmap, cm, zero_lo, zero_hi)));
+                }
                 }
                 if (e != cudaSuccess) return fail(c, PS_ECUDA, std::string("k_col_propagate: ") + cudaGetErrorString(e));
                 c->launches++;

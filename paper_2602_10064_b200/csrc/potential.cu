@@ -125,7 +125,9 @@ k_vk(const uint32_t* __restrict__ sUx, const uint32_t* __restrict__ sUy, const i
     const int n_bins = n_slices * n_elem;
     const int32_t* off = offsets + (size_t)f * (n_bins + 1) + (size_t)s * n_elem;
     if (off[n_elem] == off[0]) return;                                     // empty slice: Vk left unwritten
-    const int tx = threadIdx.x % 16, ty = threadIdx.x / 16;
+    // warp w owns the 32 x 16 sub-tile (m: 32 * (w & 1), n: 16 * (w >> 1)); lane -> 4 x 4 register tile
+    const int lane = threadIdx.x & 31, wrp = threadIdx.x >> 5;
+    const int tx = (lane & 7) + 8 * (wrp & 1), ty = (lane >> 3) + 4 * (wrp >> 1);
     const size_t abase = (size_t)f * n_atoms;
     float2* out = Vk + ((size_t)f * n_slices + s) * nh * mw;
 
@@ -136,6 +138,13 @@ k_vk(const uint32_t* __restrict__ sUx, const uint32_t* __restrict__ sUy, const i
         if (m <= mcut) inside = nmax[m < 0 ? m + nx : m] >= n0;
     }
     inside = __syncthreads_or(inside);
+    // warp-uniform: does this warp's 32 x 16 sub-tile touch the aperture?  (A(k) = 0 there otherwise)
+    bool warp_in = false;
+    {
+        const int m = m0 + 32 * (wrp & 1) + lane, nlo = n0 + 16 * (wrp >> 1);
+        const bool hit = (m <= mcut) && (nmax[m < 0 ? m + nx : m] >= nlo);
+        warp_in = __any_sync(0xffffffffu, hit);
+    }
     float2 tot[4][4];
 #pragma unroll
     for (int a = 0; a < 4; ++a)
@@ -163,6 +172,7 @@ k_vk(const uint32_t* __restrict__ sUx, const uint32_t* __restrict__ sUy, const i
                     ey[jj][b] = phase_factor(n0 + b, sUy[abase + j0 + jj]);
                 }
                 __syncthreads();
+                if (warp_in)
                 for (int jj = 0; jj < cnt; ++jj) {
                     float2 xa[4], yb[4];
                     const float4 x01 = *reinterpret_cast<const float4*>(&ex[jj][tx * 4]);
