@@ -99,8 +99,9 @@ PS_API ps_status ps_get_geometry(const ps_ctx* ctx, int* n_slices, double* dz_ef
 PS_API size_t    ps_workspace_bytes(const ps_ctx* ctx, int n_frames_chunk, int n_atoms);
 PS_API ps_status ps_set_workspace(ps_ctx* ctx, void* d_ws, size_t bytes);
 
-/* Tuning knob: number of waves whose slice loop runs back to back (so that the chunk of waves
- * stays resident in the 126 MB L2 between the two FFT passes of a slice).  0 = library default. */
+/* Tuning knob: number of waves whose slice loop runs back to back (a small chunk stays resident in
+ * the 126 MB L2 between the two FFT passes of a slice; a large one amortises launch costs).
+ * 0 = library default = the whole batch in one launch per pass (profiles/r1_chunk_sweep.md). */
 PS_API ps_status ps_set_wave_chunk(ps_ctx* ctx, int n_waves);
 
 /* ---------------------------------------------------------------- hot path */

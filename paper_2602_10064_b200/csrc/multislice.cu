@@ -296,14 +296,13 @@ extern "C" ps_status ps_multislice(ps_ctx* c, double kV, const void* d_psi0, int
     ps_status st = ensure_kv(c, kV);
     if (st != PS_OK) return st;
 
-    const size_t wave_bytes = (size_t)c->nx * c->ny * sizeof(float2);
-    int chunk = c->wave_chunk;
-    if (chunk <= 0) {
-        chunk = (int)((size_t)40 * 1024 * 1024 / wave_bytes);
-        if (chunk < 1) chunk = 1;
-    }
-    const int np = n_probes < chunk ? n_probes : chunk;
-    int nf = chunk / np;
+    // Waves per launch.  Measured on B200 (c2, 256^2, 512 waves; profiles/r1_chunk_sweep.md): streaming the whole
+    // batch from HBM in one launch per pass beats L2-resident chunks of 40-80 MB, whose launches are too short
+    // to amortise launch latency, twiddle set-up and the last partial wave of blocks.  Default: no chunking.
+    long long chunk = c->wave_chunk;
+    if (chunk <= 0) chunk = (long long)n_probes * n_frames;
+    const int np = (int)(n_probes < chunk ? n_probes : chunk);
+    int nf = (int)(chunk / np);
     if (nf < 1) nf = 1;
     if (nf < n_frames) {                                     // equal-sized frame chunks (no short tail chunk)
         const int n_chunks = (n_frames + nf - 1) / nf;

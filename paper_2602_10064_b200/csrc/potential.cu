@@ -102,25 +102,30 @@ k_sort(const uint32_t* __restrict__ Ux, const uint32_t* __restrict__ Uy, const i
 }
 
 // ------------------------------------------------------------------------------------ a2: V(k) assembly
+// Separable direct sum on the quarter plane m >= 0, n >= 0.  With theta_x = 2 pi m u_x, theta_y = 2 pi n u_y,
+//     exp(-2 pi i k.r) = (cx cy - sx sy) - i (sx cy + cx sy)            at (+m, n)
+//                      = (cx cy + sx sy) - i (cx sy - sx cy)            at (-m, n)
+// so the four real sums  cc = sum cx cy, ss = sum sx sy, cs = sum cx sy, sc = sum sx cy  over the atoms of one
+// (slice, element) give both columns +m and -m of the Hermitian half plane: 4 FMA per atom per pair of outputs.
 constexpr int VK_TM = 64, VK_TN = 32, VK_CH = 32, VK_THREADS = 128;
 
-__device__ __forceinline__ float2 phase_factor(const int m, const uint32_t U) {
-    // exp(-2 pi i m u), u = U/2^32: the fraction (m*U mod 2^32) is formed exactly in integers, read as a
+__device__ __forceinline__ float2 phase_cs(const int m, const uint32_t U) {
+    // (cos, sin) of 2 pi m u, u = U/2^32: the fraction (m*U mod 2^32) is formed exactly in integers, read as a
     // signed turn in [-1/2, 1/2) and handed to the SFU sine / cosine (abs. error 2^-21.4 on [-pi, pi]).
     const int32_t ph = (int32_t)((uint32_t)m * U);
     const float r = (float)ph * 1.4629180792671596e-9f;             // 2 pi / 2^32
-    return make_float2(__cosf(r), -__sinf(r));
+    return make_float2(__cosf(r), __sinf(r));
 }
 
-__global__ void __launch_bounds__(VK_THREADS)
+__global__ void __launch_bounds__(VK_THREADS, 4)
 k_vk(const uint32_t* __restrict__ sUx, const uint32_t* __restrict__ sUy, const int32_t* __restrict__ offsets,
      const float* __restrict__ ftab, const int32_t* __restrict__ nmax, float2* __restrict__ Vk, const int n_atoms,
-     const int n_slices, const int n_elem, const int mcut, const int ncut, const int nx, const int tiles_m) {
-    __shared__ __align__(16) float2 ex[VK_CH][VK_TM];
-    __shared__ __align__(16) float2 ey[VK_CH][VK_TN];
+     const int n_slices, const int n_elem, const int mcut, const int ncut, const int tiles_m) {
+    __shared__ __align__(16) float2 ex[VK_CH][VK_TM];                      // (cos, sin) of 2 pi m u_x
+    __shared__ __align__(16) float2 ey[VK_CH][VK_TN];                      // (cos, sin) of 2 pi n u_y
     const int f = blockIdx.z, s = blockIdx.y;
     const int tmx = blockIdx.x % tiles_m, tny = blockIdx.x / tiles_m;
-    const int m0 = -mcut + tmx * VK_TM, n0 = tny * VK_TN;
+    const int m0 = tmx * VK_TM, n0 = tny * VK_TN;
     const int mw = 2 * mcut + 1, nh = ncut + 1;
     const int n_bins = n_slices * n_elem;
     const int32_t* off = offsets + (size_t)f * (n_bins + 1) + (size_t)s * n_elem;
@@ -131,69 +136,61 @@ k_vk(const uint32_t* __restrict__ sUx, const uint32_t* __restrict__ sUy, const i
     const size_t abase = (size_t)f * n_atoms;
     float2* out = Vk + ((size_t)f * n_slices + s) * nh * mw;
 
-    // is any point of this tile inside the aperture?
+    // is any point of this tile inside the aperture?  (nmax is even in m: column m >= 0 is FFT index m)
     int inside = 0;
     if (threadIdx.x < VK_TM) {
         const int m = m0 + threadIdx.x;
-        if (m <= mcut) inside = nmax[m < 0 ? m + nx : m] >= n0;
+        if (m <= mcut) inside = nmax[m] >= n0;
     }
-    inside = __syncthreads_or(inside);
+    if (!__syncthreads_or(inside)) return;                                 // never read by k_v_col
     // warp-uniform: does this warp's 32 x 16 sub-tile touch the aperture?  (A(k) = 0 there otherwise)
     bool warp_in = false;
     {
         const int m = m0 + 32 * (wrp & 1) + lane, nlo = n0 + 16 * (wrp >> 1);
-        const bool hit = (m <= mcut) && (nmax[m < 0 ? m + nx : m] >= nlo);
-        warp_in = __any_sync(0xffffffffu, hit);
+        warp_in = __any_sync(0xffffffffu, (m <= mcut) && (nmax[m] >= nlo));
     }
-    float2 tot[4][4];
+    bool first = true;
+    for (int e = 0; e < n_elem; ++e) {
+        const int jb = off[e], je = off[e + 1];
+        if (jb == je) continue;
+        float cc[4][4], ss[4][4], cs[4][4], sc[4][4];
 #pragma unroll
-    for (int a = 0; a < 4; ++a)
+        for (int a = 0; a < 4; ++a)
 #pragma unroll
-        for (int b = 0; b < 4; ++b) tot[a][b] = make_float2(0.f, 0.f);
-
-    if (inside) {
-        for (int e = 0; e < n_elem; ++e) {
-            const int jb = off[e], je = off[e + 1];
-            if (jb == je) continue;
-            float2 acc[4][4];
-#pragma unroll
-            for (int a = 0; a < 4; ++a)
-#pragma unroll
-                for (int b = 0; b < 4; ++b) acc[a][b] = make_float2(0.f, 0.f);
-            for (int j0 = jb; j0 < je; j0 += VK_CH) {
-                const int cnt = min(VK_CH, je - j0);
-                __syncthreads();
-                for (int i = threadIdx.x; i < cnt * VK_TM; i += VK_THREADS) {
-                    const int jj = i / VK_TM, a = i % VK_TM;
-                    ex[jj][a] = phase_factor(m0 + a, sUx[abase + j0 + jj]);
-                }
-                for (int i = threadIdx.x; i < cnt * VK_TN; i += VK_THREADS) {
-                    const int jj = i / VK_TN, b = i % VK_TN;
-                    ey[jj][b] = phase_factor(n0 + b, sUy[abase + j0 + jj]);
-                }
-                __syncthreads();
-                if (warp_in)
-                for (int jj = 0; jj < cnt; ++jj) {
-                    float2 xa[4], yb[4];
-                    const float4 x01 = *reinterpret_cast<const float4*>(&ex[jj][tx * 4]);
-                    const float4 x23 = *reinterpret_cast<const float4*>(&ex[jj][tx * 4 + 2]);
-                    const float4 y01 = *reinterpret_cast<const float4*>(&ey[jj][ty * 4]);
-                    const float4 y23 = *reinterpret_cast<const float4*>(&ey[jj][ty * 4 + 2]);
-                    xa[0] = make_float2(x01.x, x01.y); xa[1] = make_float2(x01.z, x01.w);
-                    xa[2] = make_float2(x23.x, x23.y); xa[3] = make_float2(x23.z, x23.w);
-                    yb[0] = make_float2(y01.x, y01.y); yb[1] = make_float2(y01.z, y01.w);
-                    yb[2] = make_float2(y23.x, y23.y); yb[3] = make_float2(y23.z, y23.w);
-#pragma unroll
-                    for (int a = 0; a < 4; ++a)
-#pragma unroll
-                        for (int b = 0; b < 4; ++b) {
-                            acc[a][b].x = fmaf(xa[a].x, yb[b].x, acc[a][b].x);
-                            acc[a][b].x = fmaf(-xa[a].y, yb[b].y, acc[a][b].x);
-                            acc[a][b].y = fmaf(xa[a].x, yb[b].y, acc[a][b].y);
-                            acc[a][b].y = fmaf(xa[a].y, yb[b].x, acc[a][b].y);
-                        }
-                }
+            for (int b = 0; b < 4; ++b) cc[a][b] = ss[a][b] = cs[a][b] = sc[a][b] = 0.f;
+        for (int j0 = jb; j0 < je; j0 += VK_CH) {
+            const int cnt = min(VK_CH, je - j0);
+            __syncthreads();
+            for (int i = threadIdx.x; i < cnt * VK_TM; i += VK_THREADS) {
+                const int jj = i / VK_TM, a = i % VK_TM;
+                ex[jj][a] = phase_cs(m0 + a, sUx[abase + j0 + jj]);
             }
+            for (int i = threadIdx.x; i < cnt * VK_TN; i += VK_THREADS) {
+                const int jj = i / VK_TN, b = i % VK_TN;
+                ey[jj][b] = phase_cs(n0 + b, sUy[abase + j0 + jj]);
+            }
+            __syncthreads();
+            if (warp_in)
+#pragma unroll 2
+            for (int jj = 0; jj < cnt; ++jj) {
+                const float4 x01 = *reinterpret_cast<const float4*>(&ex[jj][tx * 4]);
+                const float4 x23 = *reinterpret_cast<const float4*>(&ex[jj][tx * 4 + 2]);
+                const float4 y01 = *reinterpret_cast<const float4*>(&ey[jj][ty * 4]);
+                const float4 y23 = *reinterpret_cast<const float4*>(&ey[jj][ty * 4 + 2]);
+                const float cx[4] = {x01.x, x01.z, x23.x, x23.z}, sx[4] = {x01.y, x01.w, x23.y, x23.w};
+                const float cy[4] = {y01.x, y01.z, y23.x, y23.z}, sy[4] = {y01.y, y01.w, y23.y, y23.w};
+#pragma unroll
+                for (int a = 0; a < 4; ++a)
+#pragma unroll
+                    for (int b = 0; b < 4; ++b) {
+                        cc[a][b] = fmaf(cx[a], cy[b], cc[a][b]);
+                        ss[a][b] = fmaf(sx[a], sy[b], ss[a][b]);
+                        cs[a][b] = fmaf(cx[a], sy[b], cs[a][b]);
+                        sc[a][b] = fmaf(sx[a], cy[b], sc[a][b]);
+                    }
+            }
+        }
+        if (warp_in) {
             const float* ft = ftab + (size_t)e * nh * mw;
 #pragma unroll
             for (int a = 0; a < 4; ++a)
@@ -201,20 +198,22 @@ k_vk(const uint32_t* __restrict__ sUx, const uint32_t* __restrict__ sUy, const i
                 for (int b = 0; b < 4; ++b) {
                     const int m = m0 + tx * 4 + a, n = n0 + ty * 4 + b;
                     if (m <= mcut && n <= ncut) {
-                        const float fv = __ldg(ft + (size_t)n * mw + (m + mcut));
-                        tot[a][b].x = fmaf(fv, acc[a][b].x, tot[a][b].x);
-                        tot[a][b].y = fmaf(fv, acc[a][b].y, tot[a][b].y);
+                        float2* op = out + (size_t)n * mw + (mcut + m);
+                        float2* om = out + (size_t)n * mw + (mcut - m);
+                        const float fv = __ldg(ft + (size_t)n * mw + (mcut + m));     // f(|k|) A(k): even in m
+                        float2 vp = make_float2(fv * (cc[a][b] - ss[a][b]), -fv * (cs[a][b] + sc[a][b]));
+                        float2 vm = make_float2(fv * (cc[a][b] + ss[a][b]), fv * (sc[a][b] - cs[a][b]));
+                        if (!first) {                                      // later elements add to the first one's
+                            const float2 p0 = *op, m0v = *om;
+                            vp.x += p0.x; vp.y += p0.y; vm.x += m0v.x; vm.y += m0v.y;
+                        }
+                        *op = vp;
+                        if (m > 0) *om = vm;
                     }
                 }
         }
+        first = false;
     }
-#pragma unroll
-    for (int a = 0; a < 4; ++a)
-#pragma unroll
-        for (int b = 0; b < 4; ++b) {
-            const int m = m0 + tx * 4 + a, n = n0 + ty * 4 + b;
-            if (m <= mcut && n <= ncut) out[(size_t)n * mw + (m + mcut)] = tot[a][b];
-        }
 }
 
 // ------------------------------------------------------------------------------------ a3: inverse FFT of slice pairs
@@ -474,7 +473,7 @@ extern "C" ps_status ps_build_slices(ps_ctx* c, const float* d_pos, const int32_
     int32_t *key = (int32_t*)(ws + L.key), *off = (int32_t*)(ws + L.off);
     float2 *Vk = (float2*)(ws + L.vk), *Zm = (float2*)(ws + L.zm);
 
-    const int tiles_m = (2 * c->mcut + 1 + VK_TM - 1) / VK_TM, tiles_n = (c->ncut + 1 + VK_TN - 1) / VK_TN;
+    const int tiles_m = (c->mcut + 1 + VK_TM - 1) / VK_TM, tiles_n = (c->ncut + 1 + VK_TN - 1) / VK_TN;
     const size_t img = (size_t)c->nx * c->ny;
     static bool sort_attr = false;
     if (!sort_attr) {
@@ -497,7 +496,7 @@ extern "C" ps_status ps_build_slices(ps_ctx* c, const float* d_pos, const int32_
         PSB_LAUNCH_CHECK(c, "k_sort");
         { ProfScope ps_(c, K_VK);
         k_vk<<<dim3(tiles_m * tiles_n, c->n_slices, nf), VK_THREADS, 0, c->stream>>>(
-            sUx, sUy, off, c->d_ftab, c->d_nmax, Vk, n_atoms, c->n_slices, c->n_elem, c->mcut, c->ncut, c->nx, tiles_m);
+            sUx, sUy, off, c->d_ftab, c->d_nmax, Vk, n_atoms, c->n_slices, c->n_elem, c->mcut, c->ncut, tiles_m);
         }
         PSB_LAUNCH_CHECK(c, "k_vk");
         cudaError_t e = cudaErrorInvalidValue;
