@@ -122,14 +122,16 @@ def form_factor(q2: np.ndarray, coef: np.ndarray, n_lorentz: int, n_gauss: int) 
 # ----------------------------------------------------------------------------- a2+a3: projected potential
 def projected_potential(pos32_frame: np.ndarray, elem_of_atom: np.ndarray, coef: np.ndarray,
                         n_lorentz: int, n_gauss: int, cell, nx: int, ny: int, n_slices: int,
-                        band_limit: bool = True, atom_chunk: int = 64):
+                        band_limit: bool = True, atom_chunk: int = 64, slices=None):
     """V[s][ny][nx] in V*Angstrom for one frame, and the int32 slice index of every atom.
 
     SURVEY §8(c) steps 3-4 / PAPER.md:81:
       V_s(k) = A(k) sum_{j in s} f_Zj(|k|) exp(-2 pi i (kx x_j + ky y_j)),
       V_s(r) = (C/(Lx Ly)) Nx Ny real(ifft2(V_s(k)))      (A1, A2; numpy ifft2 carries 1/(NxNy)).
     x_j, y_j are the fixed-point-quantised positions U/2^32 * L.  `elem_of_atom[j]` indexes rows of
-    `coef`.  `band_limit=False` drops A(k) (only used by pins that need the un-truncated sum)."""
+    `coef`.  `band_limit=False` drops A(k) (only used by pins that need the un-truncated sum).
+    `slices` (an iterable of slice numbers) restricts the work to those slices, the others stay zero: the
+    full-size parity tests sample slices this way (same arithmetic, fewer of them)."""
     L = np.asarray(cell, dtype=np.float64)
     U = fixed_point(pos32_frame, L)
     s_idx = slice_index(U[:, 2], n_slices)
@@ -143,7 +145,7 @@ def projected_potential(pos32_frame: np.ndarray, elem_of_atom: np.ndarray, coef:
     n_elem = coef.shape[0]
     f_tab = np.stack([form_factor(q2, coef[e], n_lorentz, n_gauss) for e in range(n_elem)])   # [nE][nk]
     V = np.zeros((n_slices, ny, nx), dtype=np.float64)
-    for s in range(n_slices):
+    for s in (range(n_slices) if slices is None else slices):
         Vk_a = np.zeros(kxa.shape[0], dtype=np.complex128)
         for e in range(n_elem):
             sel = np.nonzero((s_idx == s) & (elem_of_atom == e))[0]

@@ -21,10 +21,10 @@ def make_ctx(w, device=0):
     return ctx
 
 
-def oracle_potential(w, pos32_frame):
+def oracle_potential(w, pos32_frame, slices=None):
     nl, ng, coef = form_factor_coefficients(w.elements, w.ff_kind)
     elem = np.searchsorted(w.elements, w.Z)
-    return O.projected_potential(pos32_frame, elem, coef, nl, ng, w.cell, w.nx, w.ny, w.n_slices)
+    return O.projected_potential(pos32_frame, elem, coef, nl, ng, w.cell, w.nx, w.ny, w.n_slices, slices=slices)
 
 
 def oracle_incident(w):

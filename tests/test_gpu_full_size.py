@@ -1,0 +1,167 @@
+"""GPU parity at BASELINE.json's full grid / slice / atom sizes, in the launch configuration bench.py times
+(library-default chunking, whole batches per launch), on SAMPLED outputs the float64 oracle can compute one by one
+(SURVEY.md §8(d) "Parity sampling"):
+
+  * integers (slice binning) on every atom of the sampled frames: bit-exact;
+  * V on sampled slices of sampled frames against the oracle's potential from positions;
+  * exit waves of sampled (frame, probe) pairs against the oracle's slice loop run on the same float32 potentials
+    (the CUDA potentials, which the previous bullet ties to the oracle);
+  * I(k, w) on a seeded sample of k-pixels over all frames against the oracle's time transform of the same
+    exit-wave columns; out-of-band pixels exactly zero;
+  * properties that hold at any size: norm inside the band limit (pin P8), path-B == path-A.
+
+Frame counts are cut where the full count would not fit the test budget (the oracle needs ~1 s per 256^2 frame,
+~50 s per 512^2 x 80-slice frame); grid, slices, atoms, probes-per-launch and bins are the configs' own.
+"""
+import numpy as np
+import pytest
+
+from oracle import tacaw_oracle as O
+from workloads import make_workload
+
+from gpu_common import gpu_incident, make_ctx, oracle_incident, oracle_potential, rel_l2
+
+pytestmark = pytest.mark.gpu
+
+TOL_EXIT = 1e-4
+TOL_I = 1e-3
+TOL_V = 2e-5
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device")
+    return torch
+
+
+def _t(torch, a):
+    return torch.as_tensor(np.ascontiguousarray(a)).cuda()
+
+
+def _check_tacaw_sample(torch, ps, ctx, w, ex, I, bins, n_sample, seed):
+    """I[p][b][pix] against the oracle transform of the CUDA exit waves at sampled in-band pixels; zeros elsewhere."""
+    A = O.aperture_mask(w.cell, w.nx, w.ny)
+    iy, ix = np.nonzero(A)
+    rng = np.random.default_rng(seed)
+    sel = rng.choice(iy.size, size=min(n_sample, iy.size), replace=False)
+    sy, sx = torch.as_tensor(iy[sel]).cuda(), torch.as_tensor(ix[sel]).cuda()
+    P, F = ex.shape[0], ex.shape[1]
+    for p in range(P):
+        cols = ex[p][:, sy, sx].cpu().numpy().astype(np.complex128)          # [F][n_sample]
+        Io = O.tacaw_intensity(cols, bins)
+        Ig = I[p][:, sy, sx].cpu().numpy()
+        assert rel_l2(Ig, Io) < TOL_I
+    out = torch.as_tensor(~A).cuda()
+    assert float(I[:, :, out].abs().max()) == 0.0, "I outside the band limit must be exactly zero"
+
+
+def _check_norm(torch, ex, w):
+    """P8: exp(i sigma V) is unitary and P A only removes intensity: sum_k |Psi|^2 <= nx ny, and close to it."""
+    n = (ex.real.double() ** 2 + ex.imag.double() ** 2).sum(dim=(-2, -1)) / (w.nx * w.ny)
+    assert float(n.max()) <= 1.0 + 1e-5
+    assert float(n.min()) > 0.5
+
+
+def test_c2_full_bench_configuration(torch):
+    """Config 2 exactly as bench.py runs it: 1152 atoms, 256^2, 10 slices, all 512 frames, bins 0..49."""
+    import paper_2602_10064_b200 as ps
+    w = make_workload("c2_hbn_256")
+    ctx = make_ctx(w)
+    pos = w.positions()
+    V, sidx = ps.ps_build_slices(ctx, _t(torch, pos), _t(torch, w.Z), want_slice_idx=True)
+    ex = ps.ps_multislice(ctx, w.kV, gpu_incident(ctx, w), V)
+    I = ps.ps_tacaw(ctx, ex, w.dt_fs, w.bins)
+    psi0 = oracle_incident(w)[0]
+    for f in (0, 257, w.n_frames - 1):
+        Vo, so = oracle_potential(w, pos[f])
+        assert np.array_equal(sidx[f].cpu().numpy(), so), "slice binning must be bit-exact"
+        assert rel_l2(V[f].cpu().numpy(), Vo) < TOL_V
+        eo = O.multislice(psi0, Vo, w.cell, w.kV)                              # positions -> exit wave, all oracle
+        assert rel_l2(ex[0, f].cpu().numpy(), eo) < TOL_EXIT
+    # binning of every atom of every frame
+    so_all = O.slice_index(O.fixed_point(pos.reshape(-1, 3), w.cell)[:, 2], w.n_slices).reshape(pos.shape[:2])
+    assert np.array_equal(sidx.cpu().numpy(), so_all)
+    _check_norm(torch, ex, w)
+    _check_tacaw_sample(torch, ps, ctx, w, ex, I, w.bins, 4096, 21)
+
+
+def test_c3_full_grid_probe_chunk(torch):
+    """Config 3 geometry (10 240 atoms, 512^2, 80 slices, 30 mrad probes), 32 frames x one 16-probe scan row."""
+    import paper_2602_10064_b200 as ps
+    F = 32
+    w = make_workload("c3_si_probe_512", n_frames=F)
+    w.probe_xy = w.probe_xy[:16]
+    ctx = make_ctx(w)
+    pos = w.positions()
+    V, sidx = ps.ps_build_slices(ctx, _t(torch, pos), _t(torch, w.Z), want_slice_idx=True)
+    psi0 = gpu_incident(ctx, w)
+    ex = ps.ps_multislice(ctx, w.kV, psi0, V)
+    I = ps.ps_tacaw(ctx, ex, w.dt_fs)
+    f = 17
+    Vo, so = oracle_potential(w, pos[f], slices=(0, 41, 79))
+    assert np.array_equal(sidx[f].cpu().numpy(), so)
+    Vg = V[f].cpu().numpy()
+    for s in (0, 41, 79):
+        assert rel_l2(Vg[s], Vo[s]) < TOL_V
+    po = oracle_incident(w)
+    for p, fr in ((0, 0), (15, f)):
+        eo = O.multislice(po[p], V[fr].cpu().numpy().astype(np.float64), w.cell, w.kV)
+        assert rel_l2(ex[p, fr].cpu().numpy(), eo) < TOL_EXIT
+    _check_norm(torch, ex, w)
+    _check_tacaw_sample(torch, ps, ctx, w, ex, I, None, 1024, 31)
+
+
+def test_c4_full_grid_streaming_bins(torch):
+    """Config 4 geometry (48 600 atoms, 1024^2, 120 slices, 200 kV), 32 frames; path B (streaming per-bin DFT, two
+    chunks) against the oracle and against path A."""
+    import paper_2602_10064_b200 as ps
+    from paper_2602_10064_b200.binding import TacawStream
+    F = 32
+    w = make_workload("c4_interface_1024", n_frames=F)
+    ctx = make_ctx(w)
+    pos = w.positions()
+    V, sidx = ps.ps_build_slices(ctx, _t(torch, pos), _t(torch, w.Z), want_slice_idx=True)
+    ex = ps.ps_multislice(ctx, w.kV, gpu_incident(ctx, w), V)
+    f = 5
+    Vo, so = oracle_potential(w, pos[f], slices=(3, 118))
+    assert np.array_equal(sidx[f].cpu().numpy(), so)
+    for s in (3, 118):
+        assert rel_l2(V[f, s].cpu().numpy(), Vo[s]) < TOL_V
+    eo = O.multislice(oracle_incident(w)[0], V[f].cpu().numpy().astype(np.float64), w.cell, w.kV)
+    assert rel_l2(ex[0, f].cpu().numpy(), eo) < TOL_EXIT
+    del V
+    bins = np.arange(-8, 16, dtype=np.int32)
+    ts = TacawStream(ctx, 1, F, w.dt_fs, bins)
+    ts.add(ex[:, :20].contiguous(), 0)
+    ts.add(ex[:, 20:].contiguous(), 20)
+    IB = ts.finish()
+    IA = ps.ps_tacaw(ctx, ex, w.dt_fs, bins)
+    _check_norm(torch, ex, w)
+    _check_tacaw_sample(torch, ps, ctx, w, ex, IB, bins, 2048, 41)
+    _check_tacaw_sample(torch, ps, ctx, w, ex, IA, bins, 2048, 42)
+    assert rel_l2(IB.cpu().numpy(), IA.cpu().numpy()) < TOL_I
+
+
+@pytest.mark.parametrize("grid", [1024, 2048])
+def test_c5_large_grids_tilts(torch, grid):
+    """Config 5 geometry (40 960 atoms, 80 slices, 8 tilts) at its two largest grids (8 frames at 1024^2, 2 at
+    2048^2): the longest FFTs the library instantiates, on potentials built from atoms."""
+    import paper_2602_10064_b200 as ps
+    F = 32
+    w = make_workload("c5_al_sweep", n_frames=F, grid=grid)
+    ctx = make_ctx(w)
+    nf = 8 if grid == 1024 else 2                                             # frames through the slice loop
+    pos = w.positions(0, nf)
+    V, sidx = ps.ps_build_slices(ctx, _t(torch, pos), _t(torch, w.Z), want_slice_idx=True)
+    ex = ps.ps_multislice(ctx, w.kV, gpu_incident(ctx, w), V)
+    f = nf - 1
+    Vo, so = oracle_potential(w, pos[f], slices=(40,))
+    assert np.array_equal(sidx[f].cpu().numpy(), so)
+    assert rel_l2(V[f, 40].cpu().numpy(), Vo[40]) < TOL_V
+    po = oracle_incident(w)
+    p = 7 if grid == 1024 else 3
+    eo = O.multislice(po[p], V[f].cpu().numpy().astype(np.float64), w.cell, w.kV)
+    assert rel_l2(ex[p, f].cpu().numpy(), eo) < TOL_EXIT
+    _check_norm(torch, ex, w)
