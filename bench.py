@@ -165,6 +165,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="c2_hbn_256")
     ap.add_argument("--frames", type=int, default=None, help="override the number of frames (parity/debug only)")
+    ap.add_argument("--grid", type=int, default=None, help="override the grid size (config 5 sweeps 256..2048)")
+    ap.add_argument("--probes-side", type=int, default=None, help="override probes per scan side / number of tilts")
     ap.add_argument("--wave-chunk", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
@@ -172,7 +174,7 @@ def main():
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
-    w = make_workload(args.workload, n_frames=args.frames)
+    w = make_workload(args.workload, n_frames=args.frames, grid=args.grid, n_probes_side=args.probes_side)
 
     if args.impl == "reference":
         run_reference(args, w, rank)
@@ -324,7 +326,8 @@ def main():
 
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        cpu_baseline, _, _ = oracle_sample(make_workload(args.workload, n_frames=args.frames))
+        cpu_baseline, _, _ = oracle_sample(make_workload(args.workload, n_frames=args.frames, grid=args.grid,
+                                                           n_probes_side=args.probes_side))
 
     if rank == 0:
         print(json.dumps({

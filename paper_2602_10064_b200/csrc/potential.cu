@@ -51,42 +51,61 @@ __global__ void k_bin(const float* __restrict__ pos, const int32_t* __restrict__
     if (slice_idx) slice_idx[i] = s;
 }
 
-// one warp per frame: histogram, exclusive scan, stable placement
-__global__ void __launch_bounds__(32)
+// One block per frame, W warps: warp w owns the contiguous atom segment [w*seg, (w+1)*seg).  Per-warp histograms,
+// a (bin-major, warp-minor) exclusive scan, then every warp places its own segment in order: a stable counting
+// sort, so the order of atoms inside a (slice, element) bin — and with it every float sum downstream — is fixed.
+__global__ void __launch_bounds__(1024)
 k_sort(const uint32_t* __restrict__ Ux, const uint32_t* __restrict__ Uy, const int32_t* __restrict__ key,
        const int n_atoms, const int n_bins, uint32_t* __restrict__ sUx, uint32_t* __restrict__ sUy,
        int32_t* __restrict__ offsets) {
-    extern __shared__ int cursor[];                       // [n_bins + 1]
-    const int f = blockIdx.x, lane = threadIdx.x;
+    extern __shared__ int sm_sort[];                      // [W][n_bins] cursors, then [n_bins + 1] bin starts
+    const int f = blockIdx.x, lane = threadIdx.x & 31, w = threadIdx.x >> 5, W = blockDim.x >> 5;
+    int* cursor = sm_sort + (size_t)w * n_bins;
+    int* start = sm_sort + (size_t)W * n_bins;
     const size_t base = (size_t)f * n_atoms;
-    for (int b = lane; b <= n_bins; b += 32) cursor[b] = 0;
-    __syncwarp();
-    for (int j = lane; j < n_atoms; j += 32) {
+    const int seg = (n_atoms + W - 1) / W;
+    const int j_lo = min(w * seg, n_atoms), j_hi = min(j_lo + seg, n_atoms);
+    for (int i = threadIdx.x; i < W * n_bins; i += blockDim.x) sm_sort[i] = 0;
+    __syncthreads();
+    for (int j = j_lo + lane; j < j_hi; j += 32) {
         const int k = key[base + j];
         if (k >= 0) atomicAdd(&cursor[k], 1);
     }
-    __syncwarp();
-    int carry = 0;                                        // exclusive scan, 32 bins at a time
-    for (int b0 = 0; b0 <= n_bins; b0 += 32) {
-        const int b = b0 + lane;
-        const int cnt = (b < n_bins) ? cursor[b] : 0;
-        int incl = cnt;
-#pragma unroll
-        for (int d = 1; d < 32; d <<= 1) {
-            const int o = __shfl_up_sync(0xffffffffu, incl, d);
-            if (lane >= d) incl += o;
+    __syncthreads();
+    for (int b = threadIdx.x; b < n_bins; b += blockDim.x) {      // per bin: prefix over warps, total
+        int run = 0;
+        for (int ww = 0; ww < W; ++ww) {
+            const int t = sm_sort[(size_t)ww * n_bins + b];
+            sm_sort[(size_t)ww * n_bins + b] = run;
+            run += t;
         }
-        const int excl = carry + incl - cnt;
-        if (b <= n_bins) {
-            cursor[b] = excl;
-            offsets[(size_t)f * (n_bins + 1) + b] = excl;
-        }
-        carry += __shfl_sync(0xffffffffu, incl, 31);
+        start[b] = run;
     }
+    __syncthreads();
+    if (w == 0) {                                         // exclusive scan of the bin totals, 32 bins at a time
+        int carry = 0;
+        for (int b0 = 0; b0 <= n_bins; b0 += 32) {
+            const int b = b0 + lane;
+            const int cnt = (b < n_bins) ? start[b] : 0;
+            int incl = cnt;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const int o = __shfl_up_sync(0xffffffffu, incl, d);
+                if (lane >= d) incl += o;
+            }
+            if (b <= n_bins) {
+                start[b] = carry + incl - cnt;
+                offsets[(size_t)f * (n_bins + 1) + b] = carry + incl - cnt;
+            }
+            carry += __shfl_sync(0xffffffffu, incl, 31);
+        }
+    }
+    __syncthreads();
+    for (int b = lane; b < n_bins; b += 32) cursor[b] += start[b];
     __syncwarp();
-    for (int j0 = 0; j0 < n_atoms; j0 += 32) {
+    for (int j0 = j_lo; j0 < j_hi; j0 += 32) {
         const int j = j0 + lane;
-        const int k = (j < n_atoms) ? key[base + j] : -1;
+        const int k = (j < j_hi) ? key[base + j] : -1;
         const unsigned grp = __match_any_sync(0xffffffffu, k);
         const int rank = __popc(grp & ((1u << lane) - 1u));
         int dst = -1;
@@ -432,7 +451,7 @@ extern "C" ps_status ps_build_slices(ps_ctx* c, const float* d_pos, const int32_
     ps_status st = ensure_ftab(c);
     if (st != PS_OK) return st;
     const long long n_bins = (long long)c->n_slices * c->n_elem;
-    if ((n_bins + 1) * 4 > 200 * 1024)
+    if ((2 * n_bins + 2) * 4 > 200 * 1024)
         return fail(c, PS_EUNSUPPORTED, "ps_build_slices: n_slices * n_elements too large for the sort kernel");
 
     // validate Z (one 4-byte read-back before any work is queued; the rest of the call is asynchronous)
@@ -491,7 +510,15 @@ extern "C" ps_status ps_build_slices(ps_ctx* c, const float* d_pos, const int32_
         }
         PSB_LAUNCH_CHECK(c, "k_bin");
         { ProfScope ps_(c, K_SORT);
-        k_sort<<<nf, 32, (size_t)(n_bins + 1) * sizeof(int), c->stream>>>(Ux, Uy, key, n_atoms, (int)n_bins, sUx, sUy, off);
+        {
+            // as many warps as the 200 KB of cursors allow, at most 32, at least one per 64 atoms
+            int W = (int)((size_t)200 * 1024 / sizeof(int) / (size_t)(n_bins + 1)) - 1;
+            if (W > 32) W = 32;
+            if (W > (n_atoms + 63) / 64) W = (n_atoms + 63) / 64;
+            if (W < 1) W = 1;
+            const size_t smem = ((size_t)W * n_bins + n_bins + 1) * sizeof(int);
+            k_sort<<<nf, 32 * W, smem, c->stream>>>(Ux, Uy, key, n_atoms, (int)n_bins, sUx, sUy, off);
+        }
         }
         PSB_LAUNCH_CHECK(c, "k_sort");
         { ProfScope ps_(c, K_VK);
