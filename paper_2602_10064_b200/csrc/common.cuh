@@ -86,6 +86,9 @@ struct ps_ctx {
     size_t user_ws_bytes = 0;
 
     psb::TacawStream ts;
+    psb::DeviceBuf tacaw_groups;            // ps_tacaw: pixel-group lists [active..., inactive...] (first pixel of each)
+    int tacaw_groups_C = 0;                 // group width the lists were built for (0 = not built)
+    int tacaw_n_active = 0, tacaw_n_inactive = 0;
     psb::DeviceBuf misc;                    // small per-call tables (bin slots, path pixels)
     psb::DeviceBuf qorder;                  // ps_qbin: cursor, offsets and pixel order by q bin (cached)
     bool qorder_valid = false;

@@ -10,6 +10,7 @@
 // Path B (ps_tacaw_begin/add/finish): streaming per-bin DFT accumulation for stacks that do not fit HBM.
 #include "common.cuh"
 #include "fft_core.cuh"
+#include "tma.cuh"
 
 namespace psb {
 
@@ -66,6 +67,112 @@ k_tacaw_fft(const float2* __restrict__ exitw, float* __restrict__ I, const int32
                 out[(size_t)slot[e] * npix] = dc ? 0.f : fmaf(v[e].x, v[e].x, v[e].y * v[e].y);
             }
         }
+    }
+}
+
+// ------------------------------------------------------------------------------------ path A, TMA-staged
+// Same transform, fed by the copy engine: the exit-wave stack is viewed as a 2-D float32 tensor
+// [P*F rows][2*nx*ny floats]; one item = C adjacent in-band pixels x all F frames = NBOX boxes of (2C floats x
+// <=256 rows) landing in one shared-memory stage, which then serves as the FFT exchange buffer.  A ring of NS stages
+// keeps the loads of the next items in flight while the current one is transformed, so one 512-thread block per SM
+// streams from HBM without exposing the load latency.  Only groups with at least one in-band pixel are visited (list
+// built once per geometry); the other pixels of I are zero-filled by k_tacaw_zero.
+template <int NF> struct TacawTmaCfg {
+    static constexpr int T = Plan<NF>::T;
+    static constexpr int C = (NF <= 512) ? 16 : ((NF == 1024) ? 8 : 4);
+    static constexpr int THREADS = C * T;
+    static constexpr int NS = 3;
+    static constexpr int BOX_R = (NF < 256) ? NF : 256;
+    static constexpr int NBOX = NF / BOX_R;
+    static constexpr uint32_t STAGE_BYTES = (uint32_t)NF * C * sizeof(float2);
+    static constexpr size_t SMEM = (size_t)NS * STAGE_BYTES + NS * sizeof(uint64_t) + 128;
+    static constexpr int MIN_BLOCKS = (THREADS <= 256) ? 2 : 1;
+};
+
+template <int NF>
+__global__ void __launch_bounds__(TacawTmaCfg<NF>::THREADS, TacawTmaCfg<NF>::MIN_BLOCKS)
+k_tacaw_tma(const __grid_constant__ CUtensorMap emap, float* __restrict__ I, const int32_t* __restrict__ slot_of_bin,
+            const int n_out, const int nx, const int ny, const int32_t* __restrict__ nmax,
+            const int32_t* __restrict__ groups, const int n_groups, const int n_items) {
+    using Cfg = TacawTmaCfg<NF>;
+    constexpr int T = Cfg::T, C = Cfg::C, NS = Cfg::NS, PF = NS - 1;
+    extern __shared__ __align__(1024) float2 smem_t[];
+    float2* stage0 = smem_t;
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem_t + (size_t)NS * NF * C);
+    const int c = threadIdx.x % C, t = threadIdx.x / C;
+    const size_t npix = (size_t)nx * ny;
+
+    auto issue_load = [&](const int item, const int s) {
+        const int p = item / n_groups;
+        const int c0 = 2 * groups[item % n_groups], c1 = p * NF;
+        tma::mbar_arrive_expect_tx(&full[s], Cfg::STAGE_BYTES);
+#pragma unroll
+        for (int b = 0; b < Cfg::NBOX; ++b)
+            tma::tensor_load_2d(stage0 + (size_t)s * NF * C + (size_t)b * Cfg::BOX_R * C, &emap, c0,
+                                c1 + b * Cfg::BOX_R, &full[s]);
+    };
+
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int s = 0; s < NS; ++s) tma::mbar_init(&full[s], 1);
+        tma::fence_mbar_init();
+    }
+    Twiddles<NF> tw;
+    tw.init(t);
+    int slot[16];
+#pragma unroll
+    for (int e = 0; e < 16; ++e) slot[e] = slot_of_bin[t + e * T];
+    __syncthreads();
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int k = 0; k < PF; ++k)
+            if (blockIdx.x + k * gridDim.x < n_items) issue_load(blockIdx.x + k * gridDim.x, k);
+    }
+
+    int it = 0;
+    for (int item = blockIdx.x; item < n_items; item += gridDim.x, ++it) {
+        const int s = it % NS;
+        // every thread is past the exchange of item it-1, whose stage (it+PF)%NS is the next load's target
+        tma::fence_proxy_async();
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            const int nxt = item + PF * gridDim.x;
+            if (nxt < n_items) issue_load(nxt, (it + PF) % NS);
+        }
+        const int p = item / n_groups, pix0 = groups[item % n_groups];
+        const int ix = pix0 % nx + c, iy = pix0 / nx;
+        const int ay = iy < ny / 2 ? iy : ny - iy;
+        const bool mine = ay <= nmax[ix];                    // the group has in-band pixels; this one may not be
+        float* out = I + (size_t)p * n_out * npix + pix0 + c;
+        ColSlots<C> slots{stage0 + (size_t)s * NF * C + c};
+        tma::mbar_wait(&full[s], (it / NS) & 1);
+        const float2 ref = slots.at(0);                      // frame 0 (A14: mean removal, see header)
+        float2 v[16];
+#pragma unroll
+        for (int e = 0; e < 16; ++e) {
+            const float2 x = slots.at(t + e * T);
+            v[e] = make_float2(x.x - ref.x, x.y - ref.y);
+        }
+        fft_forward<NF, ColSlots<C>, BlockSync>(v, t, tw, slots);
+#pragma unroll
+        for (int e = 0; e < 16; ++e) {
+            if (slot[e] >= 0) {
+                const bool zero = (t + e * T) == 0 || !mine;
+                out[(size_t)slot[e] * npix] = zero ? 0.f : fmaf(v[e].x, v[e].x, v[e].y * v[e].y);
+            }
+        }
+    }
+}
+
+// I = 0 on the pixel groups that lie wholly outside the band limit (the exit wave is exactly zero there)
+__global__ void k_tacaw_zero(float* __restrict__ I, const int32_t* __restrict__ groups, const int n_groups, const int C,
+                             const size_t npix, const long long total /* P * n_out * n_groups * C */) {
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x) {
+        const int c = (int)(i % C);
+        const long long r = i / C;
+        const int g = (int)(r % n_groups);
+        const long long pb = r / n_groups;                  // p * n_out + slot
+        I[(size_t)pb * npix + groups[g] + c] = 0.f;
     }
 }
 
@@ -159,6 +266,68 @@ static cudaError_t launch_tacaw(ps_ctx* c, const float2* exitw, float* I, const 
     return cudaGetLastError();
 }
 
+// pixel groups of width C (first pixel of each): [active..., inactive...], cached per geometry
+static ps_status ensure_tacaw_groups(ps_ctx* c, int C) {
+    if (c->tacaw_groups_C == C) return PS_OK;
+    std::vector<int32_t> act, inact;
+    for (int iy = 0; iy < c->ny; ++iy) {
+        const int ay = iy < c->ny / 2 ? iy : c->ny - iy;
+        for (int ix0 = 0; ix0 < c->nx; ix0 += C) {
+            bool any = false;
+            for (int j = 0; j < C; ++j) any = any || (ay <= c->h_nmax[ix0 + j]);
+            (any ? act : inact).push_back(iy * c->nx + ix0);
+        }
+    }
+    c->tacaw_n_active = (int)act.size(); c->tacaw_n_inactive = (int)inact.size();
+    act.insert(act.end(), inact.begin(), inact.end());
+    ps_status st = ensure_buf(c, c->tacaw_groups, act.size() * sizeof(int32_t));
+    if (st != PS_OK) return st;
+    PSB_CUDA(c, cudaMemcpyAsync(c->tacaw_groups.p, act.data(), act.size() * sizeof(int32_t), cudaMemcpyHostToDevice, c->stream));
+    PSB_CUDA(c, cudaStreamSynchronize(c->stream));           // `act` dies at return
+    c->tacaw_groups_C = C;
+    return PS_OK;
+}
+
+template <int NF>
+static ps_status launch_tacaw_tma(ps_ctx* c, const float2* exitw, float* I, const int32_t* slot, int n_out, int P) {
+    using Cfg = TacawTmaCfg<NF>;
+    auto kern = k_tacaw_tma<NF>;
+    static int cap = 0;
+    if (!cap) {
+        PSB_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM));
+        int per_sm = 1, dev = 0, n_sm = kNumSM;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, Cfg::THREADS, Cfg::SMEM) != cudaSuccess || per_sm < 1)
+            per_sm = 1;
+        cap = n_sm * per_sm;
+    }
+    ps_status st = ensure_tacaw_groups(c, Cfg::C);
+    if (st != PS_OK) return st;
+    const size_t npix = (size_t)c->nx * c->ny;
+    if ((long long)P * NF > 0x7fffffffLL || 2 * npix > 0xffffffffULL)
+        return fail(c, PS_EUNSUPPORTED, "ps_tacaw: exit-wave stack has more than 2^31 rows");
+    CUtensorMap emap;
+    if (!tma::make_map_2d_f32(&emap, (void*)exitw, 2ull * npix, (uint64_t)P * NF, 2 * Cfg::C, Cfg::BOX_R))
+        return fail(c, PS_ECUDA, "ps_tacaw: cuTensorMapEncodeTiled failed (exit-wave array must be 16-byte aligned)");
+    const int32_t* groups = (const int32_t*)c->tacaw_groups.p;
+    const long long n_items = (long long)P * c->tacaw_n_active;
+    if (n_items > 0x7fffffffLL) return fail(c, PS_EUNSUPPORTED, "ps_tacaw: too many pixel groups");
+    if (c->tacaw_n_inactive > 0) {
+        const long long total = (long long)P * n_out * c->tacaw_n_inactive * Cfg::C;
+        const long long nb = (total + 255) / 256;
+        k_tacaw_zero<<<(unsigned)(nb < 148 * 32 ? nb : 148 * 32), 256, 0, c->stream>>>(
+            I, groups + c->tacaw_n_active, c->tacaw_n_inactive, Cfg::C, npix, total);
+        PSB_LAUNCH_CHECK(c, "k_tacaw_zero");
+    }
+    if (n_items > 0) {
+        kern<<<(int)(n_items < cap ? n_items : cap), Cfg::THREADS, Cfg::SMEM, c->stream>>>(
+            emap, I, slot, n_out, c->nx, c->ny, c->d_nmax, groups, c->tacaw_n_active, (int)n_items);
+        PSB_LAUNCH_CHECK(c, "k_tacaw_tma");
+    }
+    return PS_OK;
+}
+
 }  // namespace psb
 
 using namespace psb;
@@ -185,22 +354,40 @@ extern "C" ps_status ps_tacaw(ps_ctx* c, const void* d_exit, int exit_layout, in
     int32_t* d_slot = (int32_t*)((char*)c->misc.p + 4096);
     PSB_CUDA(c, cudaMemcpyAsync(d_slot, slot.data(), (size_t)n_frames * 4, cudaMemcpyHostToDevice, c->stream));
     PSB_CUDA(c, cudaStreamSynchronize(c->stream));           // `slot` dies at return; 16 KB at most
-    cudaError_t e = cudaErrorInvalidValue;
     ProfScope ps_(c, K_TACAW_FFT);
-    switch (n_frames) {
-        case 32: e = launch_tacaw<32>(c, (const float2*)d_exit, d_I, d_slot, n_bins, n_probes); break;
-        case 64: e = launch_tacaw<64>(c, (const float2*)d_exit, d_I, d_slot, n_bins, n_probes); break;
-        case 128: e = launch_tacaw<128>(c, (const float2*)d_exit, d_I, d_slot, n_bins, n_probes); break;
-        case 256: e = launch_tacaw<256>(c, (const float2*)d_exit, d_I, d_slot, n_bins, n_probes); break;
-        case 512: e = launch_tacaw<512>(c, (const float2*)d_exit, d_I, d_slot, n_bins, n_probes); break;
-        case 1024: e = launch_tacaw<1024>(c, (const float2*)d_exit, d_I, d_slot, n_bins, n_probes); break;
-        case 2048: e = launch_tacaw<2048>(c, (const float2*)d_exit, d_I, d_slot, n_bins, n_probes); break;
-        case 4096: e = launch_tacaw<4096>(c, (const float2*)d_exit, d_I, d_slot, n_bins, n_probes); break;
+    const float2* ex = (const float2*)d_exit;
+    // Kernel choice measured on B200 (profiles/r1_tacaw_kernels.md): the TMA-staged ring wins where one block per
+    // SM is all that fits anyway (2048 frames) and where few bins are written (reads dominate, 512-1024 frames);
+    // the register-staged kernel with several resident blocks wins for short stacks and when every bin is written.
+    const bool use_ring = n_frames == 2048 ||
+                          ((n_frames == 512 || n_frames == 1024) && 4 * n_bins <= n_frames);
+    if (!use_ring) {
+        cudaError_t e = cudaErrorInvalidValue;
+        switch (n_frames) {
+            case 32: e = launch_tacaw<32>(c, ex, d_I, d_slot, n_bins, n_probes); break;
+            case 64: e = launch_tacaw<64>(c, ex, d_I, d_slot, n_bins, n_probes); break;
+            case 128: e = launch_tacaw<128>(c, ex, d_I, d_slot, n_bins, n_probes); break;
+            case 256: e = launch_tacaw<256>(c, ex, d_I, d_slot, n_bins, n_probes); break;
+            case 512: e = launch_tacaw<512>(c, ex, d_I, d_slot, n_bins, n_probes); break;
+            case 1024: e = launch_tacaw<1024>(c, ex, d_I, d_slot, n_bins, n_probes); break;
+            case 4096: e = launch_tacaw<4096>(c, ex, d_I, d_slot, n_bins, n_probes); break;
+            default: break;
+        }
+        if (e != cudaSuccess) return fail(c, PS_ECUDA, std::string("k_tacaw_fft: ") + cudaGetErrorString(e));
+        c->launches++;
+        return PS_OK;
+    }
+    switch (n_frames) {                                       // TMA-staged ring up to 2048 frames (64 KB stages)
+        case 32: return launch_tacaw_tma<32>(c, ex, d_I, d_slot, n_bins, n_probes);
+        case 64: return launch_tacaw_tma<64>(c, ex, d_I, d_slot, n_bins, n_probes);
+        case 128: return launch_tacaw_tma<128>(c, ex, d_I, d_slot, n_bins, n_probes);
+        case 256: return launch_tacaw_tma<256>(c, ex, d_I, d_slot, n_bins, n_probes);
+        case 512: return launch_tacaw_tma<512>(c, ex, d_I, d_slot, n_bins, n_probes);
+        case 1024: return launch_tacaw_tma<1024>(c, ex, d_I, d_slot, n_bins, n_probes);
+        case 2048: return launch_tacaw_tma<2048>(c, ex, d_I, d_slot, n_bins, n_probes);
         default: break;
     }
-    if (e != cudaSuccess) return fail(c, PS_ECUDA, std::string("k_tacaw_fft: ") + cudaGetErrorString(e));
-    c->launches++;
-    return PS_OK;
+    return fail(c, PS_EUNSUPPORTED, "ps_tacaw: unsupported n_frames for this layout");
 }
 
 extern "C" ps_status ps_tacaw_begin(ps_ctx* c, int n_probes, int n_frames_total, double dt_fs, int n_bins,
