@@ -104,6 +104,11 @@ PS_API ps_status ps_set_workspace(ps_ctx* ctx, void* d_ws, size_t bytes);
  * 0 = library default = the whole batch in one launch per pass (profiles/r1_chunk_sweep.md). */
 PS_API ps_status ps_set_wave_chunk(ps_ctx* ctx, int n_waves);
 
+/* Tuning knob: how ps_build_slices forms the structure-factor sums of V(k).
+ *   1 = FP32 FMA pipes (k_vk);  2 = tensor cores, tcgen05.mma kind::tf32 with the 3xTF32 operand split, FP32
+ *   accumulation in TMEM (k_vk_tc);  0 = library default (2 when the mean (slice, element) group has >= 48 atoms). */
+PS_API ps_status ps_set_vk_mode(ps_ctx* ctx, int mode);
+
 /* ---------------------------------------------------------------- hot path */
 
 /* a0+a2+a3: projected potentials of every slice of every frame.

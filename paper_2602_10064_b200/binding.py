@@ -30,6 +30,7 @@ _PROTOTYPES = {
     "ps_workspace_bytes": (C.c_size_t, [C.c_void_p, C.c_int, C.c_int]),
     "ps_set_workspace": (C.c_int, [C.c_void_p, C.c_void_p, C.c_size_t]),
     "ps_set_wave_chunk": (C.c_int, [C.c_void_p, C.c_int]),
+    "ps_set_vk_mode": (C.c_int, [C.c_void_p, C.c_int]),
     "ps_build_slices": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p]),
     "ps_make_incident": (C.c_int, [C.c_void_p, C.c_double, C.c_double, C.c_int, C.c_void_p, C.c_int, C.c_void_p]),
     "ps_multislice": (C.c_int, [C.c_void_p, C.c_double, C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_void_p, C.c_int]),
@@ -177,6 +178,10 @@ class Context:
             self._check(self._lib.ps_set_workspace(self._h, C.c_void_p(0), 0))
         else:
             self._check(self._lib.ps_set_workspace(self._h, _ptr(ws), ws.numel() * ws.element_size()))
+
+    def set_vk_mode(self, mode: int):
+        """0 auto, 1 FP32 SIMT structure-factor sums, 2 tcgen05 3xTF32 sums."""
+        self._check(self._lib.ps_set_vk_mode(self._h, int(mode)))
 
     def set_wave_chunk(self, n_waves: int):
         self._check(self._lib.ps_set_wave_chunk(self._h, int(n_waves)))

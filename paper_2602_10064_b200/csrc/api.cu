@@ -243,6 +243,13 @@ extern "C" ps_status ps_set_wave_chunk(ps_ctx* c, int n_waves) {
     return PS_OK;
 }
 
+extern "C" ps_status ps_set_vk_mode(ps_ctx* c, int mode) {
+    if (!c) return PS_EINVAL;
+    if (mode < 0 || mode > 2) return fail(c, PS_EINVAL, "ps_set_vk_mode: mode must be 0 (auto), 1 (FP32 SIMT) or 2 (tcgen05 3xTF32)");
+    c->vk_mode = mode;
+    return PS_OK;
+}
+
 extern "C" ps_status ps_set_workspace(ps_ctx* c, void* d_ws, size_t bytes) {
     if (!c) return PS_EINVAL;
     if (d_ws && bytes == 0) return fail(c, PS_EINVAL, "ps_set_workspace: zero-sized workspace");

@@ -68,6 +68,7 @@ struct ps_ctx {
     uint8_t* d_tile_active = nullptr;       // [nx/kColTile]
     int n_tiles_active = 0;
     int wave_chunk = 0;
+    int vk_mode = 0;                        // ps_set_vk_mode: 0 auto, 1 FP32 SIMT sums, 2 tcgen05 3xTF32 sums
 
     // form factors
     bool have_ff = false;
@@ -149,6 +150,8 @@ inline int signed_index(int i, int n) { return i < (n + 1) / 2 ? i : i - n; }
 ps_status ensure_buf(ps_ctx* c, DeviceBuf& b, size_t bytes);
 ps_status ensure_kv(ps_ctx* c, double kV);
 ps_status ensure_ftab(ps_ctx* c);
+cudaError_t launch_vk_tc(ps_ctx* c, const uint32_t* sUx, const uint32_t* sUy, const int32_t* off, float2* Vk, int n_atoms,
+                         int nf);                                          // vk_tc.cu
 
 // physical constants (CODATA values; DESIGN.md §3 "Constants")
 constexpr double kHC_keVA = 12.398419843;

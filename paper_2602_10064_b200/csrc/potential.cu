@@ -521,11 +521,21 @@ extern "C" ps_status ps_build_slices(ps_ctx* c, const float* d_pos, const int32_
         }
         }
         PSB_LAUNCH_CHECK(c, "k_sort");
-        { ProfScope ps_(c, K_VK);
-        k_vk<<<dim3(tiles_m * tiles_n, c->n_slices, nf), VK_THREADS, 0, c->stream>>>(
-            sUx, sUy, off, c->d_ftab, c->d_nmax, Vk, n_atoms, c->n_slices, c->n_elem, c->mcut, c->ncut, tiles_m);
+        // tensor-core sums pay off once a (slice, element) group fills a few K = 16 stages
+        const bool use_tc = c->vk_mode == 2 ||
+                            (c->vk_mode == 0 && (long long)n_atoms >= 48LL * c->n_slices * c->n_elem);
+        if (use_tc) {
+            cudaError_t e;
+            { ProfScope ps_(c, K_VK); e = launch_vk_tc(c, sUx, sUy, off, Vk, n_atoms, nf); }
+            if (e != cudaSuccess) return fail(c, PS_ECUDA, std::string("k_vk_tc: ") + cudaGetErrorString(e));
+            c->launches++;
+        } else {
+            { ProfScope ps_(c, K_VK);
+            k_vk<<<dim3(tiles_m * tiles_n, c->n_slices, nf), VK_THREADS, 0, c->stream>>>(
+                sUx, sUy, off, c->d_ftab, c->d_nmax, Vk, n_atoms, c->n_slices, c->n_elem, c->mcut, c->ncut, tiles_m);
+            }
+            PSB_LAUNCH_CHECK(c, "k_vk");
         }
-        PSB_LAUNCH_CHECK(c, "k_vk");
         cudaError_t e = cudaErrorInvalidValue;
         { ProfScope ps_(c, K_V_COL);
         PSB_DISPATCH_N(c->ny, (e = launch_v_col<N_>(c, Vk, off, Zm, nf))); }

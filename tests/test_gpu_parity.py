@@ -38,11 +38,14 @@ MINIS = ["c1_si_128", "c2_hbn_256", "c3_si_probe_512", "c4_interface_1024", "c5_
 
 
 # ----------------------------------------------------------------------------- a0 + a2 + a3
+@pytest.mark.parametrize("vk_mode", [1, 2], ids=["fp32", "tcgen05"])
 @pytest.mark.parametrize("name", MINIS)
-def test_build_slices_matches_oracle(torch, name):
+def test_build_slices_matches_oracle(torch, name, vk_mode):
+    """Both ways of forming the structure-factor sums (FP32 FMA pipes; tcgen05 3xTF32 GEMMs) against the oracle."""
     import paper_2602_10064_b200 as ps
     w = make_workload(name, mini=True)
     ctx = make_ctx(w)
+    ctx.set_vk_mode(vk_mode)
     frames = [0, w.n_frames - 1]
     pos = w.positions()[frames]
     V, sidx = ps.ps_build_slices(ctx, _t(torch, pos), _t(torch, w.Z), want_slice_idx=True)
@@ -53,7 +56,8 @@ def test_build_slices_matches_oracle(torch, name):
         assert rel_l2(V[i], Vo) < TOL_V
 
 
-def test_build_slices_ragged_and_wrapped(torch):
+@pytest.mark.parametrize("vk_mode", [1, 2], ids=["fp32", "tcgen05"])
+def test_build_slices_ragged_and_wrapped(torch, vk_mode):
     """atom count not a multiple of anything, positions outside the cell (periodic wrap), odd slice count,
     non-square grid."""
     import paper_2602_10064_b200 as ps
@@ -62,6 +66,7 @@ def test_build_slices_ragged_and_wrapped(torch):
     keep = np.arange(w.n_atoms)[: w.n_atoms - 13]
     w.Z = w.Z[keep]; w.R0 = w.R0[keep]; w.mode_amp = w.mode_amp[:, keep]
     ctx = make_ctx(w)
+    ctx.set_vk_mode(vk_mode)
     pos = w.positions(0, 3)
     pos[1] += np.array([3 * w.cell[0], -2 * w.cell[1], 5 * w.cell[2]], dtype=np.float32)
     pos[2, ::7, 2] = 0.0                                       # atoms exactly on the cell boundary
