@@ -311,8 +311,14 @@ def main():
     achieved = alg_bytes_launch / (dom_ms / dom_n * 1e-3) / 1e9
     ms_pair = kern["k_row_transmit"][0] + kern["k_col_propagate"][0]
     pair_gbs = (ROW_BYTES + COL_BYTES) * px_slices_per_step * K / (ms_pair * 1e-3) / 1e9
+    traffic = None                                              # DRAM bytes per launch of that kernel, from ncu
+    tpath = os.path.join(ROOT, "profiles", "r1_traffic.json")
+    if w.name == "c2_hbn_256" and args.frames is None and args.grid is None and not args.wave_chunk and os.path.exists(tpath):
+        with open(tpath) as fh:
+            tj = json.load(fh)["dram_bytes_per_launch"]
+        traffic = next((v for k, v in tj.items() if k.startswith(dom + "<") and k.endswith(", 0>")), None)
     roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
                 "bytes_per_launch": alg_bytes_launch, "avg_launch_ms": dom_ms / dom_n,
                 "slice_step_pair": {"achieved": pair_gbs, "frac": pair_gbs / peak,
                                     "gpx_slice_s": px_slices_per_step * K / (ms_pair * 1e-3) / 1e9},

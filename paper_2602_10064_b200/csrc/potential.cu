@@ -336,7 +336,8 @@ k_v_row(const float2* __restrict__ Zm, const int32_t* __restrict__ offsets, floa
 #pragma unroll
         for (int e = 0; e < 16; ++e)
             v[e] = (any && ((amask >> e) & 1u)) ? src[t + e * T] : make_float2(0.f, 0.f);
-        fft_inverse<NX, RowSlots, typename Cfg::Sync>(v, t, tw, slots);
+        // both slices of every row of this block empty (vacuum): V = 0, no transform needed
+        if (__syncthreads_or(any)) fft_inverse<NX, RowSlots, typename Cfg::Sync>(v, t, tw, slots);
         if (valid) {
             float* va = V + (((size_t)f * n_slices + sa) * ny + y) * NX;
 #pragma unroll

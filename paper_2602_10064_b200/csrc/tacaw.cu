@@ -164,15 +164,16 @@ k_tacaw_tma(const __grid_constant__ CUtensorMap emap, float* __restrict__ I, con
     }
 }
 
-// I = 0 on the pixel groups that lie wholly outside the band limit (the exit wave is exactly zero there)
-__global__ void k_tacaw_zero(float* __restrict__ I, const int32_t* __restrict__ groups, const int n_groups, const int C,
-                             const size_t npix, const long long total /* P * n_out * n_groups * C */) {
+// I = 0 on the pixel groups that lie wholly outside the band limit (the exit wave is exactly zero there);
+// groups are C >= 4 pixels wide and C-aligned, so every store is one aligned float4
+__global__ void k_tacaw_zero(float* __restrict__ I, const int32_t* __restrict__ groups, const int n_groups, const int C4,
+                             const size_t npix, const long long total /* P * n_out * n_groups * C4 */) {
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x) {
-        const int c = (int)(i % C);
-        const long long r = i / C;
+        const int c = (int)(i % C4);
+        const long long r = i / C4;
         const int g = (int)(r % n_groups);
         const long long pb = r / n_groups;                  // p * n_out + slot
-        I[(size_t)pb * npix + groups[g] + c] = 0.f;
+        *reinterpret_cast<float4*>(I + (size_t)pb * npix + groups[g] + 4 * c) = make_float4(0.f, 0.f, 0.f, 0.f);
     }
 }
 
@@ -314,10 +315,10 @@ static ps_status launch_tacaw_tma(ps_ctx* c, const float2* exitw, float* I, cons
     const long long n_items = (long long)P * c->tacaw_n_active;
     if (n_items > 0x7fffffffLL) return fail(c, PS_EUNSUPPORTED, "ps_tacaw: too many pixel groups");
     if (c->tacaw_n_inactive > 0) {
-        const long long total = (long long)P * n_out * c->tacaw_n_inactive * Cfg::C;
+        const long long total = (long long)P * n_out * c->tacaw_n_inactive * (Cfg::C / 4);
         const long long nb = (total + 255) / 256;
-        k_tacaw_zero<<<(unsigned)(nb < 148 * 32 ? nb : 148 * 32), 256, 0, c->stream>>>(
-            I, groups + c->tacaw_n_active, c->tacaw_n_inactive, Cfg::C, npix, total);
+        k_tacaw_zero<<<(unsigned)(nb < 148 * 64 ? nb : 148 * 64), 256, 0, c->stream>>>(
+            I, groups + c->tacaw_n_active, c->tacaw_n_inactive, Cfg::C / 4, npix, total);
         PSB_LAUNCH_CHECK(c, "k_tacaw_zero");
     }
     if (n_items > 0) {

@@ -1,6 +1,7 @@
 // vk_tc.cu — k_vk_tc: the V(k) structure-factor sums as tcgen05 TF32 GEMMs (design: vk_tc.cuh).
 #include "common.cuh"
 #include "vk_tc.cuh"
+#include <type_traits>
 
 namespace psb {
 
@@ -13,7 +14,7 @@ __device__ __forceinline__ float2 phase_cs_tc(const int m, const uint32_t U) {
     return make_float2(__cosf(r), __sinf(r));
 }
 
-// grid = (tiles_m * tiles_n, n_slices, frames); block = 160 threads; dynamic smem = tc::SMEM_BYTES
+// grid = (tiles_m * tiles_n, n_slices, frames); block = 288 threads; dynamic smem = tc::SMEM_BYTES
 __global__ void __launch_bounds__(THREADS, 1)
 k_vk_tc(const uint32_t* __restrict__ sUx, const uint32_t* __restrict__ sUy, const int32_t* __restrict__ offsets,
         const float* __restrict__ ftab, const int32_t* __restrict__ nmax, float2* __restrict__ Vk, const int n_atoms,
@@ -38,18 +39,18 @@ k_vk_tc(const uint32_t* __restrict__ sUx, const uint32_t* __restrict__ sUy, cons
     const size_t abase = (size_t)f * n_atoms;
 
     if (threadIdx.x == 0) {
-        for (int i = 0; i < NS; ++i) { mbar_init(&full[i], 128); mbar_init(&empty[i], 1); }
+        for (int i = 0; i < NS; ++i) { mbar_init(&full[i], 32 * PROD_WARPS); mbar_init(&empty[i], 1); }
         mbar_init(acc_full, 1);
-        mbar_init(acc_free, 128);
+        mbar_init(acc_free, 32 * PROD_WARPS);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    if (warp == 4) tmem_alloc(tmem_slot);
+    if (warp == PROD_WARPS) tmem_alloc(tmem_slot);
     fence_before_sync();
     __syncthreads();
     fence_after_sync();
     const uint32_t tmem = *tmem_slot;
 
-    if (warp == 4) {
+    if (warp == PROD_WARPS) {
         // ------------------------------------------------------------ MMA issuer (one lane)
         const uint32_t idesc = instr_desc(2 * Tn);
         int c = 0, el = 0;
@@ -84,60 +85,71 @@ k_vk_tc(const uint32_t* __restrict__ sUx, const uint32_t* __restrict__ sUy, cons
             ++el;
         }
     } else {
-        // ------------------------------------------------------------ producers (warps 0-3), then epilogue
-        const int r = threadIdx.x;                                         // operand row = TMEM lane = m - m0
+        // ------------------------------------------------------------ producers (warps 0-7), then epilogue
+        const int r = threadIdx.x & 127;                                   // operand row = TMEM lane = m - m0
+        const int half = threadIdx.x >> 7;                                 // which 8 of the 16 atoms of a stage
         const int m = m0 + r;
         float2* out = Vk + ((size_t)f * n_slices + s) * nh * mw;
         const uint32_t row_off = (uint32_t)((r >> 3) * SBO + (r & 7) * 16);
         const uint32_t brow_c = row_off;                                   // B row r       : cos(2 pi (n0 + r) u_y)
         const uint32_t brow_s = (uint32_t)(((r + Tn) >> 3) * SBO + ((r + Tn) & 7) * 16);   // B row Tn + r: sin
+        // U of the first chunk (lanes 0..15: Ux of atom lane; 16..31: Uy), then always one chunk ahead
+        auto load_u = [&](const int j0, const int je) -> uint32_t {
+            return (j0 + (lane & 15) < je) ? (lane < 16 ? sUx : sUy)[abase + j0 + (lane & 15)] : 0u;
+        };
         int c = 0, el = 0;
         for (int e = 0; e < n_elem; ++e) {
             const int jb = off[e], je = off[e + 1];
             if (jb == je) continue;
+            uint32_t u_next = load_u(jb, je);
             for (int j0 = jb; j0 < je; j0 += KB, ++c) {
                 const int st = c % NS, cnt = min(KB, je - j0);
-                uint32_t u = 0;                                            // lanes 0..15: Ux of atom lane; 16..31: Uy
-                if ((lane & 15) < cnt) u = (lane < 16 ? sUx : sUy)[abase + j0 + (lane & 15)];
+                const uint32_t u = u_next;
+                u_next = load_u(j0 + KB, je);
                 if (c >= NS) mbar_wait(&empty[st], ((c / NS) - 1) & 1);
                 uint8_t* sb = stages + (size_t)st * STAGE_BYTES;
+                // phase factors of this thread's row for its atoms -> hi / lo operand tiles (K-major core matrices)
+                auto generate = [&](auto tail_tag) {
+                    constexpr bool TAIL = decltype(tail_tag)::value;       // last chunk of an element: atoms >= cnt are zero
 #pragma unroll
-                for (int kg = 0; kg < KB / 4; ++kg) {
-                    float ch[4], cl[4], sh[4], sl[4], bch[4], bcl[4], bsh[4], bsl[4];
+                    for (int kgi = 0; kgi < KB / 8; ++kgi) {
+                        const int kg = half * (KB / 8) + kgi;
+                        float ch[4], cl[4], sh[4], sl[4], bch[4], bcl[4], bsh[4], bsl[4];
 #pragma unroll
-                    for (int kk = 0; kk < 4; ++kk) {
-                        const int k = kg * 4 + kk;
-                        const uint32_t ux = __shfl_sync(0xffffffffu, u, k), uy = __shfl_sync(0xffffffffu, u, 16 + k);
-                        const bool live = k < cnt;
-                        float2 px = phase_cs_tc(m, ux), py = make_float2(0.f, 0.f);
-                        if (r < Tn) py = phase_cs_tc(n0 + r, uy);
-                        if (!live) { px = make_float2(0.f, 0.f); py = make_float2(0.f, 0.f); }
-                        split_tf32(px.x, ch[kk], cl[kk]); split_tf32(px.y, sh[kk], sl[kk]);
-                        split_tf32(py.x, bch[kk], bcl[kk]); split_tf32(py.y, bsh[kk], bsl[kk]);
+                        for (int kk = 0; kk < 4; ++kk) {
+                            const int k = kg * 4 + kk;
+                            const uint32_t ux = __shfl_sync(0xffffffffu, u, k), uy = __shfl_sync(0xffffffffu, u, 16 + k);
+                            float2 px = phase_cs_tc(m, ux), py = phase_cs_tc(n0 + r, uy);
+                            if (TAIL && k >= cnt) { px = make_float2(0.f, 0.f); py = make_float2(0.f, 0.f); }
+                            split_tf32(px.x, ch[kk], cl[kk]); split_tf32(px.y, sh[kk], sl[kk]);
+                            split_tf32(py.x, bch[kk], bcl[kk]); split_tf32(py.y, bsh[kk], bsl[kk]);
+                        }
+                        const uint32_t ko = kg * 128;
+                        *reinterpret_cast<float4*>(sb + 0 * A_BYTES + row_off + ko) = make_float4(ch[0], ch[1], ch[2], ch[3]);
+                        *reinterpret_cast<float4*>(sb + 1 * A_BYTES + row_off + ko) = make_float4(cl[0], cl[1], cl[2], cl[3]);
+                        *reinterpret_cast<float4*>(sb + 2 * A_BYTES + row_off + ko) = make_float4(sh[0], sh[1], sh[2], sh[3]);
+                        *reinterpret_cast<float4*>(sb + 3 * A_BYTES + row_off + ko) = make_float4(sl[0], sl[1], sl[2], sl[3]);
+                        if (r < Tn) {
+                            uint8_t* bh = sb + 4 * A_BYTES; uint8_t* bl = bh + B_BYTES;
+                            *reinterpret_cast<float4*>(bh + brow_c + ko) = make_float4(bch[0], bch[1], bch[2], bch[3]);
+                            *reinterpret_cast<float4*>(bl + brow_c + ko) = make_float4(bcl[0], bcl[1], bcl[2], bcl[3]);
+                            *reinterpret_cast<float4*>(bh + brow_s + ko) = make_float4(bsh[0], bsh[1], bsh[2], bsh[3]);
+                            *reinterpret_cast<float4*>(bl + brow_s + ko) = make_float4(bsl[0], bsl[1], bsl[2], bsl[3]);
+                        }
                     }
-                    const uint32_t ko = kg * 128;
-                    *reinterpret_cast<float4*>(sb + 0 * A_BYTES + row_off + ko) = make_float4(ch[0], ch[1], ch[2], ch[3]);
-                    *reinterpret_cast<float4*>(sb + 1 * A_BYTES + row_off + ko) = make_float4(cl[0], cl[1], cl[2], cl[3]);
-                    *reinterpret_cast<float4*>(sb + 2 * A_BYTES + row_off + ko) = make_float4(sh[0], sh[1], sh[2], sh[3]);
-                    *reinterpret_cast<float4*>(sb + 3 * A_BYTES + row_off + ko) = make_float4(sl[0], sl[1], sl[2], sl[3]);
-                    if (r < Tn) {
-                        uint8_t* bh = sb + 4 * A_BYTES; uint8_t* bl = bh + B_BYTES;
-                        *reinterpret_cast<float4*>(bh + brow_c + ko) = make_float4(bch[0], bch[1], bch[2], bch[3]);
-                        *reinterpret_cast<float4*>(bl + brow_c + ko) = make_float4(bcl[0], bcl[1], bcl[2], bcl[3]);
-                        *reinterpret_cast<float4*>(bh + brow_s + ko) = make_float4(bsh[0], bsh[1], bsh[2], bsh[3]);
-                        *reinterpret_cast<float4*>(bl + brow_s + ko) = make_float4(bsl[0], bsl[1], bsl[2], bsl[3]);
-                    }
-                }
+                };
+                if (cnt == KB) generate(std::false_type{}); else generate(std::true_type{});
                 fence_proxy_async_smem();                                  // generic-proxy stores -> tensor-core reads
                 mbar_arrive(&full[st]);
             }
             // ---- epilogue of this element: TMEM lane r = row m; columns n (cc), Tn + n (cs); D2: sc, ss
             mbar_wait(acc_full, el & 1);
             fence_after_sync();
-            const uint32_t tl = tmem + ((uint32_t)(warp * 32) << 16);
+            const uint32_t tl = tmem + ((uint32_t)((warp & 3) * 32) << 16);
+            const int q_mid = ((Tn / 2) + 7) & ~7, q_lo = half ? q_mid : 0, q_hi = half ? Tn : q_mid;
             const float* ft = ftab + (size_t)e * nh * mw;
             const int nm = (m <= mcut) ? nmax[m] : -1;
-            for (int q = 0; q < Tn; q += 8) {
+            for (int q = q_lo; q < q_hi; q += 8) {
                 float cc[8], cs[8], sc[8], ss[8];
                 tmem_ld8(tl + q, cc);
                 tmem_ld8(tl + Tn + q, cs);
@@ -169,7 +181,7 @@ k_vk_tc(const uint32_t* __restrict__ sUx, const uint32_t* __restrict__ sUy, cons
     }
     fence_before_sync();
     __syncthreads();
-    if (warp == 4) tmem_dealloc(tmem);
+    if (warp == PROD_WARPS) tmem_dealloc(tmem);
 }
 
 // host launcher (called from ps_build_slices): tiles of 128 m-values x Tn n-values over the quarter plane

@@ -6,14 +6,14 @@
 //     D1[m][0:Tn | Tn:2Tn] = cx[m][j] * [cy | sy][n][j]^T          D2[m][...] = sx[m][j] * [cy | sy][n][j]^T
 // issued as tcgen05.mma kind::tf32 (M = 128 m-values = the 128 TMEM lanes, N = 2 Tn <= 256, K = 8 atoms per
 // instruction), accumulators D1, D2 in TMEM.  FP32 accuracy comes from the 3xTF32 split: every operand x is stored
-// as hi = rna_tf32(x) and lo = rna_tf32(x - hi) and each product is issued as hi*hi + hi*lo + lo*hi (the dropped
+// as hi = tf32(x) (rounded to nearest) and lo = x - hi and each product is issued as hi*hi + hi*lo + lo*hi (the dropped
 // lo*lo term is 2^-22 relative).  Then, as in the SIMT kernel (potential.cu),
 //     V(+m, n) = f (cc - ss, -(cs + sc)),     V(-m, n) = f (cc + ss, sc - cs).
 //
-// One CTA = one (frame, slice, 128 x Tn tile of the quarter plane).  Warps 0-3 turn atoms into operand tiles in
+// One CTA = one (frame, slice, 128 x Tn tile of the quarter plane).  Warps 0-7 turn atoms into operand tiles in
 // shared memory (canonical K-major, no-swizzle UMMA layout: 8-row x 16-byte core matrices), ring of NS stages;
-// warp 4 owns TMEM (512 columns) and issues the MMAs from one lane; tcgen05.commit on mbarriers frees stages and
-// hands the accumulators to warps 0-3, which read them back with tcgen05.ld (warp w <-> TMEM lanes 32w..32w+31) and
+// warp 8 owns TMEM (512 columns) and issues the MMAs from one lane; tcgen05.commit on mbarriers frees stages and
+// hands the accumulators to warps 0-7, which read them back with tcgen05.ld (warp w <-> TMEM lanes 32 (w % 4) ...) and
 // write V(k).  No TMA: the operands do not exist in global memory, they are generated on the fly.
 #pragma once
 #include <cuda_runtime.h>
@@ -26,7 +26,8 @@ constexpr int TM = 128;                 // m values per tile = TMEM lanes = MMA 
 constexpr int KB = 16;                  // atoms per shared-memory stage (two K = 8 instructions)
 constexpr int NS = 3;                   // stages
 constexpr int TN_MAX = 128;             // n values per tile at most (MMA N = 2 Tn <= 256)
-constexpr int THREADS = 160;            // 4 producer / epilogue warps + 1 MMA warp
+constexpr int PROD_WARPS = 8;            // producer / epilogue warps: warp w and w + 4 share rows, split the atoms
+constexpr int THREADS = 32 * (PROD_WARPS + 1);   // + 1 MMA warp
 constexpr int A_BYTES = TM * KB * 4;                    // one A operand array of a stage (8 KB)
 constexpr int B_BYTES = 2 * TN_MAX * KB * 4;            // one B operand array of a stage (16 KB)
 constexpr int STAGE_BYTES = 4 * A_BYTES + 2 * B_BYTES;  // cx_hi cx_lo sx_hi sx_lo | b_hi b_lo  (64 KB)
@@ -102,13 +103,12 @@ __device__ __forceinline__ void tmem_ld8(const uint32_t taddr, float (&v)[8]) {
 }
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
-// x = hi + lo, both representable in TF32 (round to nearest)
+// x = hi + lo with hi representable in TF32 (10 mantissa bits, rounded to nearest by an integer add on the bit
+// pattern: cvt.rna.tf32.f32 is emulated with ~8 integer instructions on sm_100a) and lo = x - hi exact in FP32;
+// the tensor core reads the top 19 bits of lo, i.e. drops at most 2^-10 |lo| <= 2^-21 |x|.
 __device__ __forceinline__ void split_tf32(const float x, float& hi, float& lo) {
-    uint32_t h, l;
-    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(h) : "f"(x));
-    hi = __uint_as_float(h);
-    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(l) : "f"(x - hi));
-    lo = __uint_as_float(l);
+    hi = __uint_as_float((__float_as_uint(x) + 0x1000u) & 0xffffe000u);
+    lo = x - hi;
 }
 
 }  // namespace tc
