@@ -168,6 +168,13 @@ template <int C> struct ColSlots {   // C transforms interleaved (lane = column)
 };
 struct BlockSync { static __device__ __forceinline__ void sync() { __syncthreads(); } };
 struct WarpSync  { static __device__ __forceinline__ void sync() { __syncwarp(); } };
+// the T threads (whole warps) that carry one transform of a block holding several: named barrier 1 + threadIdx.x / T
+template <int T> struct GroupSync {
+    static_assert(T % 32 == 0, "a transform must be carried by whole warps");
+    static __device__ __forceinline__ void sync() {
+        asm volatile("bar.sync %0, %1;" ::"r"(1 + (int)threadIdx.x / T), "r"(T) : "memory");
+    }
+};
 
 template <int N> struct RowLine { static constexpr int LEN = N + N / 16; };      // padded line length (float2)
 

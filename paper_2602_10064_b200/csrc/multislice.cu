@@ -26,7 +26,9 @@ template <int NX> struct RowCfg {
     static constexpr int RPB = THREADS / T;                               // rows per block
     static constexpr int MIN_BLOCKS = (THREADS <= 256) ? 2 : 1;           // cap registers at 128
     static constexpr size_t SMEM = (size_t)RPB * RowLine<NX>::LEN * sizeof(float2);
-    using Sync = typename std::conditional<(T <= 32), WarpSync, BlockSync>::type;
+    // rows are independent: only the T threads of a row synchronise (a warp, or a named barrier per row)
+    using Sync = typename std::conditional<(T <= 32), WarpSync,
+                                           typename std::conditional<(RPB > 1), GroupSync<T>, BlockSync>::type>::type;
 };
 
 struct ChunkMap {           // chunk of waves: probes [p0,p0+np) x frames [f0,f0+nf); local l = lf*np + lp

@@ -300,7 +300,8 @@ template <int NX> struct VRowCfg {
     static constexpr int THREADS = 256;
     static constexpr int RPB = THREADS / T;
     static constexpr size_t SMEM = (size_t)RPB * RowLine<NX>::LEN * sizeof(float2);
-    using Sync = typename std::conditional<(T <= 32), WarpSync, BlockSync>::type;
+    using Sync = typename std::conditional<(T <= 32), WarpSync,
+                                           typename std::conditional<(RPB > 1), GroupSync<T>, BlockSync>::type>::type;
 };
 
 template <int NX>
