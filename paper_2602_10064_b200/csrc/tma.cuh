@@ -68,6 +68,10 @@ __device__ __forceinline__ void tensor_store_2d(const CUtensorMap* map, const in
                  "r"(c1), "r"(smem_u32(smem_src))
                  : "memory");
 }
+// asks the copy engine to bring [g, g + bytes) into L2 (16-byte aligned, size % 16 == 0); no completion to wait for
+__device__ __forceinline__ void bulk_prefetch_l2(const void* g, const uint32_t bytes) {
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(g), "r"(bytes) : "memory");
+}
 __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 // all but the newest N bulk groups of this thread have finished READING their shared-memory source
 template <int N>
