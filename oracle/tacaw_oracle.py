@@ -246,6 +246,27 @@ def spectrum_image(I: np.ndarray, cell, k_in: float, k_out: float) -> np.ndarray
     return (I * m[None, None]).sum(axis=(2, 3))
 
 
+def haadf(exit_waves: np.ndarray, cell, k_in: float, k_out: float) -> np.ndarray:
+    """Annular detector signal per probe position ("HAADFData ... annular dark field scanning probe
+    imaging", "integrates scattered intensity within configurable collection angle ranges"):
+        out[p] = (1/F) sum_f sum_{k_in <= |k| < k_out} |Psi_pf(k)|^2 / (nx ny)
+    for exit waves [P][F][ny][nx] in k-space, unitary (step 7): the fraction of the incident intensity (mean
+    intensity 1 per pixel) that lands on the detector, averaged over the frames (frozen-phonon average).
+    k_out <= 0: no outer limit.  [Reading: detector limits in 1/Angstrom like spectrum_image; theta = lambda k.]"""
+    P, F, ny, nx = exit_waves.shape
+    kx, ky = k_grids(cell, nx, ny)
+    k = np.sqrt(kx[None, :] ** 2 + ky[:, None] ** 2)
+    m = (k >= k_in) & ((k < k_out) if k_out > 0 else True)
+    inten = np.abs(exit_waves) ** 2
+    return (inten * m[None, None]).sum(axis=(2, 3)).mean(axis=1) / (nx * ny)
+
+
+def accumulate_intensity(acc: np.ndarray, I: np.ndarray, w_acc: float, w_new: float) -> np.ndarray:
+    """acc <- w_acc * acc + w_new * I: averaging |Psi(k,w)|^2 over independent trajectories or trajectory
+    segments (Suppl. PAPER.md:305).  Running mean over n results: w_acc = (n-1)/n, w_new = 1/n."""
+    return w_acc * acc + w_new * I
+
+
 def dispersion_pixels(cell, nx: int, ny: int, kx_path, ky_path) -> np.ndarray:
     """Linear pixel index iy*nx+ix of the nearest reciprocal-grid point to each path point:
     ix = floor(kx Lx + 0.5) mod Nx (A17). int32."""

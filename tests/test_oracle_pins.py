@@ -435,3 +435,43 @@ def test_aperture_mask_properties():
     assert abs(A.mean() - np.pi / 9) < 0.01
     assert A[0, 42] and not A[0, 43] and not A[64, 0]
     assert np.array_equal(A, A.T) and np.array_equal(A, np.roll(A[::-1, ::-1], (1, 1), (0, 1)))
+
+
+# ----------------------------------------------------------------------------- HAADF / averaging
+def test_haadf_closed_forms_and_brute_force():
+    """Free space: the whole beam stays at k = 0, so an annulus sees nothing and a disc that holds k = 0 sees the
+    whole incident intensity (fraction 1); a phase grating puts |J_n(sigma V0)|^2 on order n (Jacobi-Anger, P7);
+    and on random waves the definition is a plain double loop."""
+    cell = np.array([12.0, 9.0, 3.0]); nx, ny = 96, 32; kV = 100.0
+    E0 = O.multislice(O.plane_wave(nx, ny), np.zeros((2, ny, nx)), cell, kV)[None, None]
+    assert abs(O.haadf(E0, cell, 0.0, 0.05)[0] - 1.0) < 1e-12
+    assert O.haadf(E0, cell, 0.05, 0.0)[0] < 1e-24
+    g, V0 = 3, 900.0
+    x = np.arange(nx) * cell[0] / nx
+    V = np.tile(V0 * np.cos(2 * np.pi * g * x / cell[0])[None, None, :], (1, ny, 1))
+    E = O.multislice(O.plane_wave(nx, ny), V, cell, kV)[None, None]
+    sig = O.sigma_rad_per_VA(kV)
+    k1 = g / cell[0]                                                    # first diffraction order at |k| = g/Lx
+    got = O.haadf(E, cell, 0.5 * k1, 1.5 * k1)[0]
+    assert abs(got - 2.0 * jv(1, sig * V0) ** 2) < 1e-10                # orders +1 and -1
+    rng = np.random.default_rng(8)
+    W = rng.normal(size=(2, 3, 6, 8)) + 1j * rng.normal(size=(2, 3, 6, 8))
+    c2 = np.array([4.0, 3.0, 1.0]); kin, kout = 0.3, 0.9
+    want = np.zeros(2)
+    for p in range(2):
+        for f in range(3):
+            for iy in range(6):
+                for ix in range(8):
+                    kx = (ix if ix < 4 else ix - 8) / c2[0]; ky = (iy if iy < 3 else iy - 6) / c2[1]
+                    if kin <= np.hypot(kx, ky) < kout:
+                        want[p] += abs(W[p, f, iy, ix]) ** 2 / 3.0 / 48.0
+    assert np.allclose(O.haadf(W, c2, kin, kout), want, rtol=1e-13)
+
+
+def test_accumulate_intensity_running_mean():
+    rng = np.random.default_rng(9)
+    Is = rng.uniform(size=(5, 2, 3, 4, 4))
+    acc = np.zeros_like(Is[0])
+    for n, I in enumerate(Is, start=1):
+        acc = O.accumulate_intensity(acc, I, (n - 1) / n, 1.0 / n)
+    assert np.allclose(acc, Is.mean(axis=0), rtol=1e-13)
