@@ -169,6 +169,17 @@ PS_API ps_status ps_sdp(ps_ctx* ctx, const float* d_I, int P, int n_bins, int bi
  * no outer limit) of I[p][b][k] -> float32 [P][n_bins]. */
 PS_API ps_status ps_spectrum_image(ps_ctx* ctx, const float* d_I, int P, int n_bins, double k_in, double k_out,
                             float* d_out);
+/* ps_haadf: annular detector on the k-space exit waves,
+ *   d_out[p] = (1/F) sum_f sum_{k_in <= |k| < k_out} |Psi_pf(k)|^2 / (nx ny)      (k_out <= 0: no outer limit)
+ * = fraction of the incident intensity on the detector, averaged over frames -> float32 [n_probes].
+ * d_exit complex64 [n_probes][n_frames][ny][nx] as written by ps_multislice. */
+PS_API ps_status ps_haadf(ps_ctx* ctx, const void* d_exit, int exit_layout, int n_probes, int n_frames, double k_in,
+                   double k_out, float* d_out);
+/* ps_accumulate_intensity: d_acc <- w_acc * d_acc + w_new * d_I over
+ * n_values float32 (16-byte aligned, n_values % 4 == 0): averaging |Psi(k,w)|^2 over independent trajectories or
+ * trajectory segments; the running mean over n results uses w_acc = (n-1)/n, w_new = 1/n. */
+PS_API ps_status ps_accumulate_intensity(ps_ctx* ctx, float* d_acc, const float* d_I, size_t n_values, double w_acc,
+                                  double w_new);
 /* ps_dispersion: nearest grid pixel of each path point, ix = floor(kx Lx + 0.5) mod nx (A17);
  * d_pix int32 [n_path] = iy*nx+ix (bit-exact), d_out[b][i] = sum_p I[p][b][pix_i]. */
 PS_API ps_status ps_dispersion(ps_ctx* ctx, const float* d_I, int P, int n_bins, int n_path, const double* kx,

@@ -40,6 +40,8 @@ _PROTOTYPES = {
     "ps_tacaw_finish": (C.c_int, [C.c_void_p, C.c_void_p]),
     "ps_sdp": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_void_p]),
     "ps_spectrum_image": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_double, C.c_double, C.c_void_p]),
+    "ps_haadf": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_void_p]),
+    "ps_accumulate_intensity": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t, C.c_double, C.c_double]),
     "ps_dispersion": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
     "ps_qbin": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_double, C.c_int, C.c_void_p, C.c_void_p]),
     "ps_launch_count": (C.c_longlong, [C.c_void_p]),
@@ -290,6 +292,26 @@ def ps_spectrum_image(ctx: Context, d_I, k_in: float = 0.0, k_out: float = 0.0, 
         d_out = torch.empty((P, nb), dtype=torch.float32, device=ctx.device)
     ctx._check(ctx._lib.ps_spectrum_image(ctx._h, _ptr(d_I), P, nb, float(k_in), float(k_out), _ptr(d_out)))
     return d_out
+
+
+def ps_haadf(ctx: Context, d_exit, k_in: float, k_out: float = 0.0, d_out=None):
+    """exit waves complex64 [P][F][ny][nx] -> float32 [P]: frame-averaged fraction of the beam on the annulus."""
+    import torch
+    _need(d_exit, torch.complex64, "d_exit")
+    P, F = int(d_exit.shape[0]), int(d_exit.shape[1])
+    if d_out is None:
+        d_out = torch.empty((P,), dtype=torch.float32, device=ctx.device)
+    ctx._check(ctx._lib.ps_haadf(ctx._h, _ptr(d_exit), PS_LAYOUT_DENSE, P, F, float(k_in), float(k_out), _ptr(d_out)))
+    return d_out
+
+
+def ps_accumulate_intensity(ctx: Context, d_acc, d_I, w_acc: float, w_new: float):
+    """d_acc <- w_acc * d_acc + w_new * d_I (float32, same shape)."""
+    import torch
+    _need(d_acc, torch.float32, "d_acc"); _need(d_I, torch.float32, "d_I")
+    assert d_acc.shape == d_I.shape
+    ctx._check(ctx._lib.ps_accumulate_intensity(ctx._h, _ptr(d_acc), _ptr(d_I), d_I.numel(), float(w_acc), float(w_new)))
+    return d_acc
 
 
 def ps_dispersion(ctx: Context, d_I, kx, ky, d_out=None):

@@ -71,6 +71,44 @@ k_spectrum_image(const float* __restrict__ I, const uint8_t* __restrict__ mask, 
     if (threadIdx.x == 0) out[blockIdx.x] = s;
 }
 
+// ---------------------------------------------------------------- HAADF (annular detector on the exit waves)
+// tmp[p * F + f] = sum_{k in detector} |Psi_pf(k)|^2, fixed order; k_haadf_mean then averages over frames
+__global__ void __launch_bounds__(1024)
+k_haadf_frame(const float2* __restrict__ exitw, const uint8_t* __restrict__ mask, float* __restrict__ tmp, const size_t npix) {
+    __shared__ float sh[32];
+    const float4* src = reinterpret_cast<const float4*>(exitw + (size_t)blockIdx.x * npix);   // two pixels per float4
+    const uchar2* m2 = reinterpret_cast<const uchar2*>(mask);
+    float s = 0.f;
+    for (size_t i = threadIdx.x; i < npix / 2; i += blockDim.x) {
+        const float4 x = src[i];
+        const uchar2 m = m2[i];
+        float q = m.x ? fmaf(x.x, x.x, x.y * x.y) : 0.f;
+        q += m.y ? fmaf(x.z, x.z, x.w * x.w) : 0.f;
+        s += q;
+    }
+    s = block_sum(s, sh);
+    if (threadIdx.x == 0) tmp[blockIdx.x] = s;
+}
+__global__ void k_haadf_mean(const float* __restrict__ tmp, float* __restrict__ out, const int P, const int F, const float scale) {
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= P) return;
+    float s = 0.f;
+    for (int f = 0; f < F; ++f) s += tmp[(size_t)p * F + f];
+    out[p] = s * scale;
+}
+
+// acc <- w_acc * acc + w_new * I  (trajectory / segment averaging of |Psi(k,w)|^2)
+__global__ void k_accumulate(float* __restrict__ acc, const float* __restrict__ I, const size_t n4, const float w_acc,
+                             const float w_new) {
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += (size_t)gridDim.x * blockDim.x) {
+        float4 a = reinterpret_cast<float4*>(acc)[i];
+        const float4 x = reinterpret_cast<const float4*>(I)[i];
+        a.x = fmaf(w_acc, a.x, w_new * x.x); a.y = fmaf(w_acc, a.y, w_new * x.y);
+        a.z = fmaf(w_acc, a.z, w_new * x.z); a.w = fmaf(w_acc, a.w, w_new * x.w);
+        reinterpret_cast<float4*>(acc)[i] = a;
+    }
+}
+
 // ---------------------------------------------------------------- dispersion
 __global__ void k_path_pixels(const double* __restrict__ kx, const double* __restrict__ ky, int32_t* __restrict__ pix,
                               const int n_path, const int nx, const int ny, const double Lx, const double Ly) {
@@ -199,6 +237,45 @@ extern "C" ps_status ps_spectrum_image(ps_ctx* c, const float* d_I, int P, int n
     PSB_LAUNCH_CHECK(c, "k_detector_mask");
     k_spectrum_image<<<P * n_bins, 1024, 0, c->stream>>>(d_I, d_mask, d_out, npix);
     PSB_LAUNCH_CHECK(c, "k_spectrum_image");
+    return PS_OK;
+}
+
+extern "C" ps_status ps_haadf(ps_ctx* c, const void* d_exit, int exit_layout, int n_probes, int n_frames, double k_in,
+                              double k_out, float* d_out) {
+    if (!c) return PS_EINVAL;
+    if (!c->have_geom) return fail(c, PS_ESTATE, "ps_haadf: ps_set_geometry has not been called");
+    if (!d_exit || !d_out || n_probes < 1 || n_frames < 1) return fail(c, PS_EINVAL, "ps_haadf: null pointer or non-positive size");
+    if (exit_layout != PS_LAYOUT_DENSE) return fail(c, PS_EUNSUPPORTED, "ps_haadf: unknown exit layout");
+    if (k_in < 0.0) return fail(c, PS_EINVAL, "ps_haadf: k_in must be >= 0");
+    const size_t npix = (size_t)c->nx * c->ny;
+    const size_t tmp_off = (4096 + npix + 255) & ~(size_t)255;
+    ps_status st = ensure_buf(c, c->misc, tmp_off + (size_t)n_probes * n_frames * sizeof(float));
+    if (st != PS_OK) return st;
+    uint8_t* d_mask = (uint8_t*)c->misc.p + 4096;
+    float* d_tmp = (float*)((char*)c->misc.p + tmp_off);
+    ProfScope ps_(c, K_REDUCE);
+    k_detector_mask<<<(unsigned)((npix + 255) / 256), 256, 0, c->stream>>>(d_mask, c->nx, c->ny, c->cell[0], c->cell[1], k_in,
+                                                                           k_out, k_out > 0.0 ? 1 : 0);
+    PSB_LAUNCH_CHECK(c, "k_detector_mask");
+    k_haadf_frame<<<n_probes * n_frames, 1024, 0, c->stream>>>((const float2*)d_exit, d_mask, d_tmp, npix);
+    PSB_LAUNCH_CHECK(c, "k_haadf_frame");
+    k_haadf_mean<<<(n_probes + 127) / 128, 128, 0, c->stream>>>(d_tmp, d_out, n_probes, n_frames,
+                                                                 (float)(1.0 / ((double)n_frames * (double)npix)));
+    PSB_LAUNCH_CHECK(c, "k_haadf_mean");
+    return PS_OK;
+}
+
+extern "C" ps_status ps_accumulate_intensity(ps_ctx* c, float* d_acc, const float* d_I, size_t n_values, double w_acc,
+                                             double w_new) {
+    if (!c) return PS_EINVAL;
+    if (!d_acc || !d_I || n_values == 0) return fail(c, PS_EINVAL, "ps_accumulate_intensity: null pointer or zero size");
+    if (n_values % 4 != 0 || (((uintptr_t)d_acc | (uintptr_t)d_I) & 15u))
+        return fail(c, PS_EINVAL, "ps_accumulate_intensity: arrays must be 16-byte aligned with a multiple of 4 values");
+    const size_t n4 = n_values / 4;
+    const size_t nb = (n4 + 255) / 256;
+    ProfScope ps_(c, K_REDUCE);
+    k_accumulate<<<(unsigned)(nb < 148 * 16 ? nb : 148 * 16), 256, 0, c->stream>>>(d_acc, d_I, n4, (float)w_acc, (float)w_new);
+    PSB_LAUNCH_CHECK(c, "k_accumulate");
     return PS_OK;
 }
 

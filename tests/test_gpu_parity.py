@@ -256,3 +256,41 @@ def test_results_are_deterministic(torch):
         ex = ps.ps_multislice(ctx, w.kV, gpu_incident(ctx, w), V)
         outs.append(ps.ps_tacaw(ctx, ex, w.dt_fs, w.bins).clone())
     assert torch.equal(outs[0], outs[1])
+
+
+# ----------------------------------------------------------------------------- SURVEY §8(f) 2 and 4
+@pytest.mark.parametrize("name", ["c3_si_probe_512", "c2_hbn_256"])
+def test_haadf_matches_oracle(torch, name):
+    """Annular detector on the CUDA exit waves against the oracle's definition applied to the same array, and the
+    whole chain positions -> HAADF against the oracle's own exit waves."""
+    import paper_2602_10064_b200 as ps
+    from workloads import form_factor_coefficients
+    w = make_workload(name, mini=True)
+    ctx = make_ctx(w)
+    pos = w.positions(0, 6)
+    V = ps.ps_build_slices(ctx, _t(torch, pos), _t(torch, w.Z))
+    ex = ps.ps_multislice(ctx, w.kV, gpu_incident(ctx, w), V)
+    kc = O.k_cut(w.cell, w.nx, w.ny)
+    exn = ex.cpu().numpy().astype(np.complex128)
+    for k_in, k_out in ((0.0, 0.0), (0.25 * kc, 0.8 * kc), (0.5 * kc, 0.0)):
+        g = ps.ps_haadf(ctx, ex, k_in, k_out).cpu().numpy()
+        assert rel_l2(g, O.haadf(exn, w.cell, k_in, k_out)) < TOL_RED
+    nl, ng, coef = form_factor_coefficients(w.elements, w.ff_kind)
+    _, exo = O.run_path(pos, np.searchsorted(w.elements, w.Z), coef, nl, ng, w.cell, w.nx, w.ny, w.n_slices, w.kV,
+                        oracle_incident(w), None)
+    g = ps.ps_haadf(ctx, ex, 0.25 * kc, 0.8 * kc).cpu().numpy()
+    assert rel_l2(g, O.haadf(exo, w.cell, 0.25 * kc, 0.8 * kc)) < 2e-4      # 2 x the exit-wave tolerance (intensity)
+
+
+def test_accumulate_intensity_running_mean(torch):
+    import paper_2602_10064_b200 as ps
+    rng = np.random.default_rng(3)
+    w = make_workload("c1_si_128", mini=True)
+    ctx = make_ctx(w)
+    Is = rng.uniform(size=(4, 2, 5, w.ny, w.nx)).astype(np.float32)
+    acc = torch.zeros((2, 5, w.ny, w.nx), dtype=torch.float32, device="cuda")
+    ref = np.zeros((2, 5, w.ny, w.nx))
+    for n, I in enumerate(Is, start=1):
+        ps.ps_accumulate_intensity(ctx, acc, _t(torch, I), (n - 1) / n, 1.0 / n)
+        ref = O.accumulate_intensity(ref, I.astype(np.float64), (n - 1) / n, 1.0 / n)
+    assert rel_l2(acc.cpu().numpy(), ref) < 1e-6
