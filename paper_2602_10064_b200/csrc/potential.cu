@@ -471,7 +471,19 @@ extern "C" ps_status ps_build_slices(ps_ctx* c, const float* d_pos, const int32_
 
     // scratch: installed workspace or library-owned buffer; frames are processed in chunks that fit
     const size_t per_frame = scratch_layout(c, 1, n_atoms).total;
-    size_t avail = c->user_ws ? c->user_ws_bytes : (size_t)768 * 1024 * 1024;
+    // library-owned scratch: an eighth of the free device memory, between 768 MB and 16 GB (at 1024^2 x 120 slices
+    // one frame needs 0.6 GB: with less, frames go one per launch and the sort / V(k) launches cannot fill the GPU)
+    size_t avail = c->user_ws_bytes;
+    if (!c->user_ws) {
+        size_t free_b = 0, total_b = 0;
+        avail = (size_t)768 << 20;
+        if (c->scratch.bytes > avail) avail = c->scratch.bytes;           // keep what a previous call already holds
+        else if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess) {
+            size_t want = (free_b + c->scratch.bytes) / 8;
+            if (want > ((size_t)16 << 30)) want = (size_t)16 << 30;
+            if (want > avail) avail = want;
+        }
+    }
     int nfc = (int)(avail / per_frame);
     if (nfc < 1) {
         if (c->user_ws) return fail(c, PS_EWORKSPACE, "ps_build_slices: workspace smaller than one frame needs (" +
