@@ -259,6 +259,17 @@ k_v_col(const float2* __restrict__ Vk, const int32_t* __restrict__ offsets, floa
     tw.init(t);
     const int per_pair = n_tiles * SUB;
     const int mw = 2 * mcut + 1, nh = ncut + 1, n_bins = n_slices * n_elem;
+    // item-invariant part of the gather: row iy = t + e T  ->  |n| and the row offset |n| * mw in the half-plane box;
+    // rows with n < 0 (bit e of negmask) are read through V(-k) = conj V(k)
+    int absn[16];
+    unsigned negmask = 0;
+#pragma unroll
+    for (int e = 0; e < 16; ++e) {
+        const int iy = t + e * T;
+        const int n = iy < NY / 2 ? iy : iy - NY;
+        absn[e] = abs(n);
+        negmask |= (n < 0 ? 1u : 0u) << e;
+    }
 
     for (int item = blockIdx.x; item < n_items; item += gridDim.x) {
         const int fp = item / per_pair, rem = item % per_pair;
@@ -271,20 +282,23 @@ k_v_col(const float2* __restrict__ Vk, const int32_t* __restrict__ offsets, floa
         const int kx = tiles[rem / SUB] * kColTile + (rem % SUB) * C + c;
         const int m = kx < nx / 2 ? kx : kx - nx;
         const int nm = nmax[kx];
-        const float2* Va = Vk + ((size_t)f * n_slices + sa) * nh * mw;
-        const float2* Vb = Vk + ((size_t)f * n_slices + sb) * nh * mw;
+        // vacuum slices read slice sa's box with weight 0 (no branch in the loop)
+        const float2* Va = Vk + ((size_t)f * n_slices + (has_a ? sa : sb)) * nh * mw;
+        const float2* Vb = Vk + ((size_t)f * n_slices + (has_b ? sb : sa)) * nh * mw;
+        const float wa = has_a ? 1.f : 0.f, wb = has_b ? 1.f : 0.f;
+        const int col_dir = mcut + m, col_mir = mcut - m;
+        const unsigned mirmask = negmask | ((m < 0 && t == 0) ? 1u : 0u);  // n == 0 (t == 0, e == 0) with m < 0: mirrored too
         float2 v[16];
 #pragma unroll
         for (int e = 0; e < 16; ++e) {
-            const int iy = t + e * T;
-            const int n = iy < NY / 2 ? iy : iy - NY;
             float2 z = make_float2(0.f, 0.f);
-            if (abs(n) <= nm) {
-                const bool direct = (n > 0) || (n == 0 && m >= 0);
-                const size_t idx = direct ? (size_t)n * mw + (m + mcut) : (size_t)(-n) * mw + (mcut - m);
-                const float2 a = has_a ? __ldg(Va + idx) : make_float2(0.f, 0.f);
-                const float2 b = has_b ? __ldg(Vb + idx) : make_float2(0.f, 0.f);
-                z = direct ? make_float2(a.x - b.y, a.y + b.x) : make_float2(a.x + b.y, b.x - a.y);
+            if (absn[e] <= nm) {
+                const bool mir = (mirmask >> e) & 1u;
+                const int idx = absn[e] * mw + (mir ? col_mir : col_dir);
+                float2 a = __ldg(Va + idx), b = __ldg(Vb + idx);
+                a.x *= wa; a.y *= wa; b.x *= wb; b.y *= wb;
+                const float sg = mir ? -1.f : 1.f;                         // conj of both for mirrored rows
+                z = make_float2(fmaf(-sg, b.y, a.x), fmaf(sg, a.y, b.x));
             }
             v[e] = z;
         }
