@@ -14,7 +14,7 @@ __device__ __forceinline__ float2 phase_cs_tc(const int m, const uint32_t U) {
     return make_float2(__cosf(r), __sinf(r));
 }
 
-// grid = (tiles_m * tiles_n, n_slices, frames); block = 288 threads; dynamic smem = tc::SMEM_BYTES
+// grid = (tiles_m * tiles_n, n_slices, frames); block = 544 threads; dynamic smem = tc::SMEM_BYTES
 __global__ void __launch_bounds__(THREADS, 1)
 k_vk_tc(const uint32_t* __restrict__ sUx, const uint32_t* __restrict__ sUy, const int32_t* __restrict__ offsets,
         const float* __restrict__ ftab, const int32_t* __restrict__ nmax, float2* __restrict__ Vk, const int n_atoms,
@@ -85,9 +85,9 @@ k_vk_tc(const uint32_t* __restrict__ sUx, const uint32_t* __restrict__ sUy, cons
             ++el;
         }
     } else {
-        // ------------------------------------------------------------ producers (warps 0-7), then epilogue
+        // ------------------------------------------------------------ producers (warps 0-15), then epilogue
         const int r = threadIdx.x & 127;                                   // operand row = TMEM lane = m - m0
-        const int half = threadIdx.x >> 7;                                 // which 8 of the 16 atoms of a stage
+        const int part = threadIdx.x >> 7;                                 // which atoms of a stage (KG_PER groups of 4)
         const int m = m0 + r;
         float2* out = Vk + ((size_t)f * n_slices + s) * nh * mw;
         const uint32_t row_off = (uint32_t)((r >> 3) * SBO + (r & 7) * 16);
@@ -112,8 +112,8 @@ k_vk_tc(const uint32_t* __restrict__ sUx, const uint32_t* __restrict__ sUy, cons
                 auto generate = [&](auto tail_tag) {
                     constexpr bool TAIL = decltype(tail_tag)::value;       // last chunk of an element: atoms >= cnt are zero
 #pragma unroll
-                    for (int kgi = 0; kgi < KB / 8; ++kgi) {
-                        const int kg = half * (KB / 8) + kgi;
+                    for (int kgi = 0; kgi < KG_PER; ++kgi) {
+                        const int kg = part * KG_PER + kgi;
                         float ch[4], cl[4], sh[4], sl[4], bch[4], bcl[4], bsh[4], bsl[4];
 #pragma unroll
                         for (int kk = 0; kk < 4; ++kk) {
@@ -146,7 +146,8 @@ k_vk_tc(const uint32_t* __restrict__ sUx, const uint32_t* __restrict__ sUy, cons
             mbar_wait(acc_full, el & 1);
             fence_after_sync();
             const uint32_t tl = tmem + ((uint32_t)((warp & 3) * 32) << 16);
-            const int q_mid = ((Tn / 2) + 7) & ~7, q_lo = half ? q_mid : 0, q_hi = half ? Tn : q_mid;
+            const int q_step = ((Tn + PARTS - 1) / PARTS + 7) & ~7;         // columns split between the row's threads
+            const int q_lo = min(part * q_step, Tn), q_hi = min(q_lo + q_step, Tn);
             const float* ft = ftab + (size_t)e * nh * mw;
             const int nm = (m <= mcut) ? nmax[m] : -1;
             for (int q = q_lo; q < q_hi; q += 8) {

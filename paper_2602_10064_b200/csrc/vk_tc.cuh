@@ -10,10 +10,10 @@
 // lo*lo term is 2^-22 relative).  Then, as in the SIMT kernel (potential.cu),
 //     V(+m, n) = f (cc - ss, -(cs + sc)),     V(-m, n) = f (cc + ss, sc - cs).
 //
-// One CTA = one (frame, slice, 128 x Tn tile of the quarter plane).  Warps 0-7 turn atoms into operand tiles in
+// One CTA = one (frame, slice, 128 x Tn tile of the quarter plane).  Warps 0-15 turn atoms into operand tiles in
 // shared memory (canonical K-major, no-swizzle UMMA layout: 8-row x 16-byte core matrices), ring of NS stages;
-// warp 8 owns TMEM (512 columns) and issues the MMAs from one lane; tcgen05.commit on mbarriers frees stages and
-// hands the accumulators to warps 0-7, which read them back with tcgen05.ld (warp w <-> TMEM lanes 32 (w % 4) ...) and
+// warp 16 owns TMEM (512 columns) and issues the MMAs from one lane; tcgen05.commit on mbarriers frees stages and
+// hands the accumulators to warps 0-15, which read them back with tcgen05.ld (warp w <-> TMEM lanes 32 (w % 4) ...) and
 // write V(k).  No TMA: the operands do not exist in global memory, they are generated on the fly.
 #pragma once
 #include <cuda_runtime.h>
@@ -26,7 +26,9 @@ constexpr int TM = 128;                 // m values per tile = TMEM lanes = MMA 
 constexpr int KB = 16;                  // atoms per shared-memory stage (two K = 8 instructions)
 constexpr int NS = 3;                   // stages
 constexpr int TN_MAX = 128;             // n values per tile at most (MMA N = 2 Tn <= 256)
-constexpr int PROD_WARPS = 8;            // producer / epilogue warps: warp w and w + 4 share rows, split the atoms
+constexpr int PROD_WARPS = 16;          // producer / epilogue warps: warps w, w + 4, ... share rows, split the atoms
+constexpr int PARTS = PROD_WARPS / 4;   // producer threads per operand row
+constexpr int KG_PER = (KB / 4) / PARTS; // 4-atom groups per producer thread and stage
 constexpr int THREADS = 32 * (PROD_WARPS + 1);   // + 1 MMA warp
 constexpr int A_BYTES = TM * KB * 4;                    // one A operand array of a stage (8 KB)
 constexpr int B_BYTES = 2 * TN_MAX * KB * 4;            // one B operand array of a stage (16 KB)
