@@ -491,12 +491,15 @@ extern "C" ps_status ps_build_slices(ps_ctx* c, const float* d_pos, const int32_
     if (!c->user_ws) {
         size_t free_b = 0, total_b = 0;
         avail = (size_t)768 << 20;
-        if (c->scratch.bytes > avail) avail = c->scratch.bytes;           // keep what a previous call already holds
-        else if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess) {
+        const int f_all = n_frames < 65535 ? n_frames : 65535;
+        if (c->scratch.bytes >= scratch_layout(c, f_all, n_atoms).total) {
+            avail = c->scratch.bytes;                                      // everything fits what is already held
+        } else if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess) {
             size_t want = (free_b + c->scratch.bytes) / 8;
             if (want > ((size_t)16 << 30)) want = (size_t)16 << 30;
             if (want > avail) avail = want;
         }
+        if (c->scratch.bytes > avail) avail = c->scratch.bytes;           // never less than what is already held
     }
     int nfc = (int)(avail / per_frame);
     if (nfc < 1) {
@@ -506,6 +509,7 @@ extern "C" ps_status ps_build_slices(ps_ctx* c, const float* d_pos, const int32_
     }
     if (nfc > n_frames) nfc = n_frames;
     if (nfc > 65535) nfc = 65535;                                          // grid.z limit of k_vk
+    nfc = (n_frames + (n_frames + nfc - 1) / nfc - 1) / ((n_frames + nfc - 1) / nfc);   // equal chunks, no short tail
     ScratchLayout L = scratch_layout(c, nfc, n_atoms);
     while (c->user_ws && L.total > c->user_ws_bytes && nfc > 1) L = scratch_layout(c, --nfc, n_atoms);
     char* ws = (char*)c->user_ws;
