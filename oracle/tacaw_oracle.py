@@ -171,14 +171,41 @@ def tilted_plane_wave(nx: int, ny: int, mt: int, nt: int) -> np.ndarray:
     return np.exp(2j * np.pi * (mt * i / nx + nt * j / ny))
 
 
-def probe_wave(cell, nx: int, ny: int, kV: float, semi_angle_mrad: float, x0: float, y0: float) -> np.ndarray:
-    """Focused probe (A12): Psi0(k) = [lambda |k| <= alpha] A(k) exp(-2 pi i k.r_p),
-    psi0 = ifft2(Psi0) scaled so sum |psi0|^2 = Nx Ny."""
+def aberration_function(cell, nx: int, ny: int, kV: float, coef) -> np.ndarray:
+    """chi(k) in radians ("the standard aberration function supporting defocus, astigmatism, coma,
+    spherical aberration"; the paper prints no formula: reading A24, Krivanek-style coefficients in Angstrom):
+        chi = (2 pi / lambda) [ C10 th^2/2 + C12 th^2/2 cos(2(phi - phi12)) + C21 th^3/3 cos(phi - phi21)
+                                + C23 th^3/3 cos(3(phi - phi23)) + C30 th^4/4 ],
+    th = lambda |k|, phi = atan2(ky, kx); coef = (C10, C12, phi12, C21, phi21, C23, phi23, C30).
+    With C10 = -defocus and C30 = Cs this is the textbook chi = pi lambda k^2 (Cs lambda^2 k^2 / 2 - defocus)."""
+    C10, C12, p12, C21, p21, C23, p23, C30 = [float(x) for x in coef]
+    kx, ky = k_grids(cell, nx, ny)
+    KX, KY = np.meshgrid(kx, ky)
+    lam = wavelength_A(kV)
+    th = lam * np.sqrt(KX ** 2 + KY ** 2)
+    phi = np.arctan2(KY, KX)
+    return (2.0 * np.pi / lam) * (0.5 * C10 * th ** 2 + 0.5 * C12 * th ** 2 * np.cos(2.0 * (phi - p12))
+                                  + C21 * th ** 3 / 3.0 * np.cos(phi - p21)
+                                  + C23 * th ** 3 / 3.0 * np.cos(3.0 * (phi - p23)) + 0.25 * C30 * th ** 4)
+
+
+def apply_aberrations(waves_k: np.ndarray, cell, kV: float, coef) -> np.ndarray:
+    """Post-hoc aberrations on stored k-space waves [..., ny, nx]: Psi(k) <- Psi(k) exp(-i chi(k))."""
+    ny, nx = waves_k.shape[-2:]
+    return waves_k * np.exp(-1j * aberration_function(cell, nx, ny, kV, coef))
+
+
+def probe_wave(cell, nx: int, ny: int, kV: float, semi_angle_mrad: float, x0: float, y0: float,
+               aberrations=None) -> np.ndarray:
+    """Focused probe (A12): Psi0(k) = [lambda |k| <= alpha] A(k) exp(-i chi(k)) exp(-2 pi i k.r_p),
+    psi0 = ifft2(Psi0) scaled so sum |psi0|^2 = Nx Ny; chi = 0 without `aberrations`."""
     kx, ky = k_grids(cell, nx, ny)
     lam = wavelength_A(kV)
     k2 = kx[None, :] ** 2 + ky[:, None] ** 2
     Psi0 = ((lam * np.sqrt(k2) <= semi_angle_mrad * 1.0e-3) & aperture_mask(cell, nx, ny)).astype(np.complex128)
     Psi0 = Psi0 * np.exp(-2j * np.pi * (kx[None, :] * x0 + ky[:, None] * y0))
+    if aberrations is not None:
+        Psi0 = Psi0 * np.exp(-1j * aberration_function(cell, nx, ny, kV, aberrations))
     psi0 = np.fft.ifft2(Psi0)
     return psi0 * np.sqrt(nx * ny / np.sum(np.abs(psi0) ** 2))
 

@@ -475,3 +475,37 @@ def test_accumulate_intensity_running_mean():
     for n, I in enumerate(Is, start=1):
         acc = O.accumulate_intensity(acc, I, (n - 1) / n, 1.0 / n)
     assert np.allclose(acc, Is.mean(axis=0), rtol=1e-13)
+
+
+# ----------------------------------------------------------------------------- aberrations
+def test_aberration_function_against_propagator_and_textbook():
+    """(i) pure C10: exp(-i chi) = exp(-i pi lambda C10 k^2) is the free-space propagator over the distance C10, so the
+    defocused probe equals the focused probe sent through one vacuum slice of that thickness (ties sign and factor
+    to the propagator pinned by P5/P7); (ii) C10 + C30 against Scherzer's form pi lambda k^2 (Cs lambda^2 k^2/2 - df)
+    at a hand-picked k; (iii) rotating the astigmatism axis by 90 degrees flips its sign, coma by 180 degrees;
+    (iv) a pure phase: the probe keeps its norm."""
+    cell = np.array([14.0, 11.0, 5.0]); nx, ny = 64, 48; kV = 100.0
+    lam = O.wavelength_A(kV)
+    z = np.zeros(8)
+    c = z.copy(); c[0] = 37.5                                          # C10 = 37.5 A
+    p_ab = O.probe_wave(cell, nx, ny, kV, 25.0, 3.0, 4.0, aberrations=c)
+    p0 = O.probe_wave(cell, nx, ny, kV, 25.0, 3.0, 4.0)
+    cell_dz = np.array([cell[0], cell[1], 37.5])
+    via_prop = O.multislice(p0, np.zeros((1, ny, nx)), cell_dz, kV, return_real_space=True)
+    assert rel_l2(p_ab, via_prop) < 1e-12
+    c = z.copy(); c[0] = -120.0; c[7] = 1.3e7                          # defocus 120 A, Cs = 1.3 mm
+    chi = O.aberration_function(cell, nx, ny, kV, c)
+    kx, ky = O.k_grids(cell, nx, ny)
+    k2 = kx[5] ** 2 + ky[3] ** 2
+    assert abs(chi[3, 5] - np.pi * lam * k2 * (0.5 * 1.3e7 * lam ** 2 * k2 - 120.0)) < 1e-9 * abs(chi[3, 5])
+    a = z.copy(); a[1] = 50.0; a[2] = 0.3
+    b = z.copy(); b[1] = -50.0; b[2] = 0.3 + np.pi / 2
+    assert np.allclose(O.aberration_function(cell, nx, ny, kV, a), O.aberration_function(cell, nx, ny, kV, b), atol=1e-9)
+    a = z.copy(); a[3] = 900.0; a[4] = 0.2
+    b = z.copy(); b[3] = -900.0; b[4] = 0.2 + np.pi
+    assert np.allclose(O.aberration_function(cell, nx, ny, kV, a), O.aberration_function(cell, nx, ny, kV, b), atol=1e-9)
+    full = np.array([30.0, 20.0, 0.4, 500.0, 1.0, 300.0, -0.7, 2.0e5])
+    p = O.probe_wave(cell, nx, ny, kV, 25.0, 3.0, 4.0, aberrations=full)
+    assert abs(np.sum(np.abs(p) ** 2) - nx * ny) < 1e-9 * nx * ny
+    W = RNG.normal(size=(2, ny, nx)) + 1j * RNG.normal(size=(2, ny, nx))
+    assert np.allclose(np.abs(O.apply_aberrations(W, cell, kV, full)), np.abs(W), rtol=1e-12)
