@@ -109,6 +109,15 @@ PS_API ps_status ps_set_wave_chunk(ps_ctx* ctx, int n_waves);
  *   accumulation in TMEM (k_vk_tc);  0 = library default (2 when the mean (slice, element) group has >= 48 atoms). */
 PS_API ps_status ps_set_vk_mode(ps_ctx* ctx, int mode);
 
+/* Aberrations (A24).  coef = {C10, C12, phi12, C21, phi21, C23, phi23,
+ * C30} in Angstrom / radians (host, 8 doubles; NULL switches aberrations off):
+ *   chi(k) = (2 pi/lambda) [C10 th^2/2 + C12 th^2/2 cos 2(phi-phi12) + C21 th^3/3 cos(phi-phi21)
+ *                           + C23 th^3/3 cos 3(phi-phi23) + C30 th^4/4],   th = lambda |k|, phi = atan2(ky, kx).
+ * While set, ps_make_incident builds probes as A(k) exp(-i chi) exp(-2 pi i k.r_p).  ps_apply_aberrations multiplies
+ * n_waves stored k-space waves complex64 [n_waves][ny][nx] (exit waves of ps_multislice) by exp(-i chi) in place. */
+PS_API ps_status ps_set_aberrations(ps_ctx* ctx, const double* coef);
+PS_API ps_status ps_apply_aberrations(ps_ctx* ctx, double kV, void* d_waves_k, long long n_waves);
+
 /* ---------------------------------------------------------------- hot path */
 
 /* a0+a2+a3: projected potentials of every slice of every frame.

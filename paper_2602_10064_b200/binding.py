@@ -31,6 +31,8 @@ _PROTOTYPES = {
     "ps_set_workspace": (C.c_int, [C.c_void_p, C.c_void_p, C.c_size_t]),
     "ps_set_wave_chunk": (C.c_int, [C.c_void_p, C.c_int]),
     "ps_set_vk_mode": (C.c_int, [C.c_void_p, C.c_int]),
+    "ps_set_aberrations": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "ps_apply_aberrations": (C.c_int, [C.c_void_p, C.c_double, C.c_void_p, C.c_longlong]),
     "ps_build_slices": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p]),
     "ps_make_incident": (C.c_int, [C.c_void_p, C.c_double, C.c_double, C.c_int, C.c_void_p, C.c_int, C.c_void_p]),
     "ps_multislice": (C.c_int, [C.c_void_p, C.c_double, C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_void_p, C.c_int]),
@@ -180,6 +182,23 @@ class Context:
             self._check(self._lib.ps_set_workspace(self._h, C.c_void_p(0), 0))
         else:
             self._check(self._lib.ps_set_workspace(self._h, _ptr(ws), ws.numel() * ws.element_size()))
+
+    def set_aberrations(self, coef=None):
+        """coef = (C10, C12, phi12, C21, phi21, C23, phi23, C30) in Angstrom / rad, or None to switch them off."""
+        if coef is None:
+            self._check(self._lib.ps_set_aberrations(self._h, C.c_void_p(0)))
+        else:
+            ch, cp = _host(coef, np.float64)
+            assert ch.shape == (8,)
+            self._check(self._lib.ps_set_aberrations(self._h, cp))
+
+    def apply_aberrations(self, kV: float, d_waves_k):
+        """In place: k-space waves complex64 [..., ny, nx] *= exp(-i chi(k))."""
+        import torch
+        _need(d_waves_k, torch.complex64, "d_waves_k")
+        n = d_waves_k.numel() // (self.nx * self.ny)
+        self._check(self._lib.ps_apply_aberrations(self._h, float(kV), _ptr(d_waves_k), n))
+        return d_waves_k
 
     def set_vk_mode(self, mode: int):
         """0 auto, 1 FP32 SIMT structure-factor sums, 2 tcgen05 3xTF32 sums."""

@@ -223,6 +223,7 @@ extern "C" ps_status ps_set_geometry(ps_ctx* c, const double cell[3], int nx, in
     c->ftab_valid = false;
     c->qorder_valid = false;
     c->tacaw_groups_C = 0;
+    c->ab_kV = -1.0;
     c->have_geom = true;
     return PS_OK;
 }

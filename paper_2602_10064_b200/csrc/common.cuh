@@ -81,6 +81,12 @@ struct ps_ctx {
 
     psb::KvTables kv;
 
+    // aberrations (ps_set_aberrations): C10, C12, phi12, C21, phi21, C23, phi23, C30 (Angstrom / rad)
+    bool have_ab = false;
+    double ab[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    psb::DeviceBuf abtab;                   // complex64 [ny][nx] exp(-i chi(k)) for ab_kV
+    double ab_kV = -1.0;
+
     // scratch
     psb::DeviceBuf scratch;                 // library-owned
     void* user_ws = nullptr;
@@ -150,6 +156,7 @@ inline int signed_index(int i, int n) { return i < (n + 1) / 2 ? i : i - n; }
 ps_status ensure_buf(ps_ctx* c, DeviceBuf& b, size_t bytes);
 ps_status ensure_kv(ps_ctx* c, double kV);
 ps_status ensure_ftab(ps_ctx* c);
+ps_status ensure_abtab(ps_ctx* c, double kV);                           // incident.cu
 cudaError_t launch_vk_tc(ps_ctx* c, const uint32_t* sUx, const uint32_t* sUy, const int32_t* off, float2* Vk, int n_atoms,
                          int nf);                                          // vk_tc.cu
 

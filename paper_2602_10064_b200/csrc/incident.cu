@@ -39,7 +39,7 @@ __global__ void __launch_bounds__(PColCfg<NY>::THREADS)
 k_probe_col(float2* __restrict__ psi, const int nx, const int32_t* __restrict__ tiles, const int n_tiles,
             const int32_t* __restrict__ pmax /* [nx] per-column limit of |n| inside probe aperture and band limit */,
             const uint32_t* __restrict__ U0 /* [n][2] fixed-point probe positions */, const float scale,
-            const int n_items) {
+            const float2* __restrict__ abtab /* [NY][nx] exp(-i chi) or NULL */, const int n_items) {
     using Cfg = PColCfg<NY>;
     constexpr int T = Cfg::T, C = Cfg::C, SUB = kColTile / C;
     extern __shared__ float2 smem[];
@@ -65,6 +65,7 @@ k_probe_col(float2* __restrict__ psi, const int nx, const int32_t* __restrict__ 
                 float s, cc;
                 sincospif((float)(ph >> 8) * (2.0f / 16777216.0f), &s, &cc);
                 z = make_float2(cc * scale, -s * scale);
+                if (abtab) z = cmul(z, __ldg(abtab + (size_t)iy * nx + kx));
             }
             v[e] = z;
         }
@@ -125,7 +126,8 @@ static int blocks_cap_i(K kernel, int threads, size_t smem) {
 }
 
 template <int NY>
-static cudaError_t launch_probe_col(ps_ctx* c, float2* psi, const int32_t* pmax, const uint32_t* U0, float scale, int n) {
+static cudaError_t launch_probe_col(ps_ctx* c, float2* psi, const int32_t* pmax, const uint32_t* U0, float scale,
+                                    const float2* abtab, int n) {
     using Cfg = PColCfg<NY>;
     auto kern = k_probe_col<NY>;
     static int cap = 0;
@@ -136,7 +138,7 @@ static cudaError_t launch_probe_col(ps_ctx* c, float2* psi, const int32_t* pmax,
     }
     const int n_items = n * c->n_tiles_active * (kColTile / Cfg::C);
     kern<<<n_items < cap ? n_items : cap, Cfg::THREADS, Cfg::SMEM, c->stream>>>(psi, c->nx, c->d_tiles, c->n_tiles_active,
-                                                                               pmax, U0, scale, n_items);
+                                                                               pmax, U0, scale, abtab, n_items);
     return cudaGetLastError();
 }
 
@@ -179,6 +181,70 @@ static uint32_t host_fixed(double pos, double L) {
 }  // namespace psb
 
 using namespace psb;
+
+// ---------------------------------------------------------------- aberrations (A24)
+namespace psb {
+
+// exp(-i chi(k)) on the full grid, float64 on the host, complex64 on the device; cached per (geometry, kV, coefficients)
+ps_status ensure_abtab(ps_ctx* c, double kV) {
+    if (c->ab_kV == kV && c->abtab.p) return PS_OK;
+    const int nx = c->nx, ny = c->ny;
+    const double lam = kHC_keVA / sqrt(kV * (2.0 * kM0C2_keV + kV));
+    const double* a = c->ab;
+    std::vector<float2> h((size_t)nx * ny);
+    for (int iy = 0; iy < ny; ++iy) {
+        const double ky = signed_index(iy, ny) / c->cell[1];
+        for (int ix = 0; ix < nx; ++ix) {
+            const double kx = signed_index(ix, nx) / c->cell[0];
+            const double th = lam * sqrt(kx * kx + ky * ky), phi = atan2(ky, kx);
+            const double th2 = th * th;
+            const double chi = (2.0 * M_PI / lam) * (0.5 * a[0] * th2 + 0.5 * a[1] * th2 * cos(2.0 * (phi - a[2])) +
+                                                    a[3] * th2 * th / 3.0 * cos(phi - a[4]) +
+                                                    a[5] * th2 * th / 3.0 * cos(3.0 * (phi - a[6])) + 0.25 * a[7] * th2 * th2);
+            h[(size_t)iy * nx + ix] = make_float2((float)cos(chi), (float)(-sin(chi)));
+        }
+    }
+    ps_status st = ensure_buf(c, c->abtab, h.size() * sizeof(float2));
+    if (st != PS_OK) return st;
+    PSB_CUDA(c, cudaMemcpyAsync(c->abtab.p, h.data(), h.size() * sizeof(float2), cudaMemcpyHostToDevice, c->stream));
+    PSB_CUDA(c, cudaStreamSynchronize(c->stream));           // `h` dies at return
+    c->ab_kV = kV;
+    return PS_OK;
+}
+
+__global__ void k_apply_table(float2* __restrict__ w, const float2* __restrict__ tab, const size_t npix, const size_t total) {
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x)
+        w[i] = cmul(w[i], __ldg(tab + i % npix));
+}
+
+}  // namespace psb
+
+extern "C" ps_status ps_set_aberrations(ps_ctx* c, const double* coef) {
+    if (!c) return PS_EINVAL;
+    c->have_ab = coef != nullptr;
+    for (int i = 0; i < 8; ++i) {
+        const double v = coef ? coef[i] : 0.0;
+        if (!(v == v) || fabs(v) > 1e300) return fail(c, PS_EINVAL, "ps_set_aberrations: coefficient is not finite");
+        c->ab[i] = v;
+    }
+    c->ab_kV = -1.0;
+    return PS_OK;
+}
+
+extern "C" ps_status ps_apply_aberrations(ps_ctx* c, double kV, void* d_waves_k, long long n_waves) {
+    if (!c) return PS_EINVAL;
+    if (!c->have_geom) return fail(c, PS_ESTATE, "ps_apply_aberrations: ps_set_geometry has not been called");
+    if (!c->have_ab) return fail(c, PS_ESTATE, "ps_apply_aberrations: ps_set_aberrations has not been called");
+    if (!d_waves_k || n_waves < 1 || !(kV > 0.0)) return fail(c, PS_EINVAL, "ps_apply_aberrations: null pointer or non-positive size / voltage");
+    ps_status st = ensure_abtab(c, kV);
+    if (st != PS_OK) return st;
+    const size_t npix = (size_t)c->nx * c->ny, total = npix * (size_t)n_waves;
+    const size_t nb = (total + 255) / 256;
+    ProfScope ps_(c, K_INCIDENT);
+    k_apply_table<<<(unsigned)(nb < 148 * 32 ? nb : 148 * 32), 256, 0, c->stream>>>((float2*)d_waves_k, (const float2*)c->abtab.p, npix, total);
+    PSB_LAUNCH_CHECK(c, "k_apply_table");
+    return PS_OK;
+}
 
 extern "C" ps_status ps_make_incident(ps_ctx* c, double kV, double semi_angle_mrad, int n, const double* xy_or_tilt,
                                       int is_tilt, void* d_psi0) {
@@ -245,7 +311,12 @@ extern "C" ps_status ps_make_incident(ps_ctx* c, double kV, double semi_angle_mr
     PSB_CUDA(c, cudaStreamSynchronize(c->stream));
     const float scale = (float)(1.0 / sqrt((double)n_ap));
     cudaError_t e = cudaErrorInvalidValue;
-    PSB_DISPATCH_N(ny, (e = launch_probe_col<N_>(c, psi, d_pmax, d_U0, scale, n)));
+    const float2* abtab = nullptr;
+    if (c->have_ab) {
+        if ((st = ensure_abtab(c, kV)) != PS_OK) return st;
+        abtab = (const float2*)c->abtab.p;
+    }
+    PSB_DISPATCH_N(ny, (e = launch_probe_col<N_>(c, psi, d_pmax, d_U0, scale, abtab, n)));
     if (e != cudaSuccess) return fail(c, PS_ECUDA, std::string("k_probe_col: ") + cudaGetErrorString(e));
     c->launches++;
     e = cudaErrorInvalidValue;

@@ -294,3 +294,24 @@ def test_accumulate_intensity_running_mean(torch):
         ps.ps_accumulate_intensity(ctx, acc, _t(torch, I), (n - 1) / n, 1.0 / n)
         ref = O.accumulate_intensity(ref, I.astype(np.float64), (n - 1) / n, 1.0 / n)
     assert rel_l2(acc.cpu().numpy(), ref) < 1e-6
+
+
+def test_aberrated_probes_and_post_hoc_aberrations(torch):
+    """probes formed with chi(k) and exp(-i chi) applied to stored k-space waves, against the oracle."""
+    import paper_2602_10064_b200 as ps
+    w = make_workload("c3_si_probe_512", mini=True)
+    ctx = make_ctx(w)
+    coef = np.array([40.0, 15.0, 0.4, 600.0, 1.0, 350.0, -0.7, 3.0e5])
+    ctx.set_aberrations(coef)
+    g = gpu_incident(ctx, w).cpu().numpy()
+    o = np.stack([O.probe_wave(w.cell, w.nx, w.ny, w.kV, w.semi_angle_mrad, x, y, aberrations=coef) for x, y in w.probe_xy])
+    assert rel_l2(g, o) < TOL_PSI0
+    rng = np.random.default_rng(11)
+    W = (rng.normal(size=(3, 2, w.ny, w.nx)) + 1j * rng.normal(size=(3, 2, w.ny, w.nx))).astype(np.complex64)
+    Wg = ctx.apply_aberrations(w.kV, _t(torch, W)).cpu().numpy()
+    assert rel_l2(Wg, O.apply_aberrations(W.astype(np.complex128), w.cell, w.kV, coef)) < TOL_PSI0
+    ctx.set_aberrations(None)                                         # off again: plain probes
+    g0 = gpu_incident(ctx, w).cpu().numpy()
+    assert rel_l2(g0, np.stack(oracle_incident(w))) < TOL_PSI0
+    with pytest.raises(ps.PSError):
+        ctx.apply_aberrations(w.kV, _t(torch, W))
