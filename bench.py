@@ -52,7 +52,7 @@ def measured_peaks():
 class ClockSampler(threading.Thread):
     """Samples SM clock and throttle reasons through NVML while the timed region runs."""
 
-    def __init__(self, index: int, period_s: float = 0.02):
+    def __init__(self, index: int, period_s: float = 0.002):
         super().__init__(daemon=True)
         self.index, self.period, self.stop_flag = index, period_s, threading.Event()
         self.sm, self.reasons, self.max_mhz, self.ok = [], set(), None, False
@@ -329,6 +329,20 @@ def main():
         tms = kern["k_tacaw_fft"][0] / kern["k_tacaw_fft"][1]
         roofline["tacaw"] = {"achieved": tb / (tms * 1e-3) / 1e9, "frac": tb / (tms * 1e-3) / 1e9 / peak,
                              "bytes_per_launch": tb, "avg_launch_ms": tms}
+
+    if "k_vk" in kern:
+        # V(k) structure-factor sums: 4 real sums per quarter-plane point and atom, x3 for the 3xTF32 split (tensor path)
+        bf16 = 1590.0                                           # fallback of B200_PROFILING.md
+        mp = os.path.join(ROOT, "MEASURED_PEAKS.json")
+        if os.path.exists(mp):
+            with open(mp) as fh:
+                bf16 = float(json.load(fh).get("bf16_tflops", bf16))
+        flop = 24.0 * (ctx.n_k_aperture / 4.0) * float(w.n_atoms) * F
+        tms = kern["k_vk"][0] / K
+        roofline["vk"] = {"bound": "tensor", "unit": "TFLOP/s", "achieved": flop / (tms * 1e-3) / 1e12,
+                          "peak": 0.5 * bf16, "frac": flop / (tms * 1e-3) / 1e12 / (0.5 * bf16),
+                          "note": "algorithmic 3xTF32 flops over the in-aperture quarter plane; peak = measured bf16 x 0.5 "
+                                  "(guide's nominal tf32:bf16 ratio); FP32 path when ps_set_vk_mode(1) or few atoms per slice"}
 
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
