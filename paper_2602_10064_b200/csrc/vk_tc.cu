@@ -39,9 +39,9 @@ k_vk_tc(const uint32_t* __restrict__ sUx, const uint32_t* __restrict__ sUy, cons
     const size_t abase = (size_t)f * n_atoms;
 
     if (threadIdx.x == 0) {
-        for (int i = 0; i < NS; ++i) { mbar_init(&full[i], 32 * PROD_WARPS); mbar_init(&empty[i], 1); }
+        for (int i = 0; i < NS; ++i) { mbar_init(&full[i], PROD_WARPS); mbar_init(&empty[i], 1); }   // one arrival per warp
         mbar_init(acc_full, 1);
-        mbar_init(acc_free, 32 * PROD_WARPS);
+        mbar_init(acc_free, PROD_WARPS);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == PROD_WARPS) tmem_alloc(tmem_slot);
@@ -140,7 +140,8 @@ k_vk_tc(const uint32_t* __restrict__ sUx, const uint32_t* __restrict__ sUy, cons
                 };
                 if (cnt == KB) generate(std::false_type{}); else generate(std::true_type{});
                 fence_proxy_async_smem();                                  // generic-proxy stores -> tensor-core reads
-                mbar_arrive(&full[st]);
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&full[st]);                     // one arrival per warp (512 would serialise)
             }
             // ---- epilogue of this element: TMEM lane r = row m; columns n (cc), Tn + n (cs); D2: sc, ss
             mbar_wait(acc_full, el & 1);
@@ -176,7 +177,8 @@ k_vk_tc(const uint32_t* __restrict__ sUx, const uint32_t* __restrict__ sUy, cons
                 }
             }
             fence_before_sync();
-            mbar_arrive(acc_free);
+            __syncwarp();
+            if (lane == 0) mbar_arrive(acc_free);
             ++el;
         }
     }
