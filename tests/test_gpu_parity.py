@@ -315,3 +315,54 @@ def test_aberrated_probes_and_post_hoc_aberrations(torch):
     assert rel_l2(g0, np.stack(oracle_incident(w))) < TOL_PSI0
     with pytest.raises(ps.PSError):
         ctx.apply_aberrations(w.kV, _t(torch, W))
+
+
+# ----------------------------------------------------------------------------- degenerate sizes and error paths
+def test_degenerate_single_atom_single_slice_single_frame(torch):
+    """One atom, one slice, one frame, smallest grid: the whole path against the oracle (V, exit wave)."""
+    import paper_2602_10064_b200 as ps
+    from workloads import form_factor_coefficients
+    w = make_workload("c1_si_128", mini=True)
+    w.nx = w.ny = 32; w.n_slices = 1
+    w.Z = w.Z[:1]; w.R0 = w.R0[:1]; w.mode_amp = w.mode_amp[:, :1]
+    ctx = make_ctx(w)
+    pos = w.positions(0, 1)
+    for mode in (1, 2):
+        ctx.set_vk_mode(mode)
+        V = ps.ps_build_slices(ctx, _t(torch, pos), _t(torch, w.Z))
+        Vo, _ = oracle_potential(w, pos[0])
+        assert rel_l2(V[0].cpu().numpy(), Vo) < TOL_V
+    ex = ps.ps_multislice(ctx, w.kV, gpu_incident(ctx, w), V)
+    eo = O.multislice(O.plane_wave(32, 32), Vo, w.cell, w.kV)
+    assert rel_l2(ex[0, 0].cpu().numpy(), eo) < TOL_EXIT
+
+
+def test_error_statuses(torch):
+    """Every failure is a negative status with a message (include/pyslice_b200.h): no abort, no silent fallback."""
+    import paper_2602_10064_b200 as ps
+    w = make_workload("c1_si_128", mini=True)
+    ctx = make_ctx(w)
+    with pytest.raises(ps.PSError) as ei:                                  # non power-of-two grid
+        ctx.set_geometry(w.cell, 48, 64, w.slice_dz)
+    assert ei.value.status == -2
+    ctx.set_geometry(w.cell, w.nx, w.ny, w.slice_dz)
+    pos = _t(torch, w.positions(0, 2)); Z = _t(torch, w.Z)
+    with pytest.raises(ps.PSError) as ei:                                  # empty input
+        ps.ps_build_slices(ctx, pos[:0].contiguous(), Z)
+    assert ei.value.status == -1
+    x = torch.zeros((1, 48, w.ny, w.nx), dtype=torch.complex64, device="cuda")
+    with pytest.raises(ps.PSError) as ei:                                  # 48 frames: not a power of two (path A)
+        ps.ps_tacaw(ctx, x, 2.0)
+    assert ei.value.status == -2
+    x = torch.zeros((1, 64, w.ny, w.nx), dtype=torch.complex64, device="cuda")
+    with pytest.raises(ps.PSError) as ei:                                  # duplicate bin (5 and 5 - 64)
+        ps.ps_tacaw(ctx, x, 2.0, np.array([5, 5 - 64], dtype=np.int32))
+    assert ei.value.status == -1
+    ws = torch.empty(4096, dtype=torch.uint8, device="cuda")
+    ctx.set_workspace(ws)
+    with pytest.raises(ps.PSError) as ei:                                  # caller workspace too small for one frame
+        ps.ps_build_slices(ctx, pos, Z)
+    assert ei.value.status == -3
+    ctx.set_workspace(None)
+    V = ps.ps_build_slices(ctx, pos, Z)                                    # and the context is still usable
+    assert torch.isfinite(V).all()
