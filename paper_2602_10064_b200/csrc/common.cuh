@@ -89,6 +89,7 @@ struct ps_ctx {
 
     // scratch
     psb::DeviceBuf scratch;                 // library-owned
+    size_t scratch_budget = 0;              // bytes the library may use for scratch (decided at the first need)
     void* user_ws = nullptr;
     size_t user_ws_bytes = 0;
 

@@ -494,10 +494,16 @@ extern "C" ps_status ps_build_slices(ps_ctx* c, const float* d_pos, const int32_
         const int f_all = n_frames < 65535 ? n_frames : 65535;
         if (c->scratch.bytes >= scratch_layout(c, f_all, n_atoms).total) {
             avail = c->scratch.bytes;                                      // everything fits what is already held
-        } else if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess) {
-            size_t want = (free_b + c->scratch.bytes) / 8;
-            if (want > ((size_t)16 << 30)) want = (size_t)16 << 30;
-            if (want > avail) avail = want;
+        } else {
+            if (c->scratch_budget == 0) {                                  // one driver query per context
+                c->scratch_budget = avail;
+                if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess) {
+                    size_t want = (free_b + c->scratch.bytes) / 8;
+                    if (want > ((size_t)16 << 30)) want = (size_t)16 << 30;
+                    if (want > c->scratch_budget) c->scratch_budget = want;
+                }
+            }
+            avail = c->scratch_budget;
         }
         if (c->scratch.bytes > avail) avail = c->scratch.bytes;           // never less than what is already held
     }
