@@ -156,6 +156,41 @@ def run_reference(args, w, rank):
         "gpu_launches": 0}))
 
 
+# --------------------------------------------------------------------------------------------- ps_tacaw alone
+def tacaw_micro():
+    """ps_tacaw on random complex64 stacks [P][F][n][n] (every pixel non-zero; only in-band pixels are read):
+    median of 5 runs after 3 warm-ups, L2 flushed between runs; one JSON line per shape."""
+    import torch
+    import paper_2602_10064_b200 as ps
+    peak, _ = measured_peaks()
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")
+    w0 = make_workload("c1_si_128", mini=True)
+    nl, ng, coef = form_factor_coefficients(w0.elements, w0.ff_kind)
+    for P, F, n, nb in [(1, 512, 256, 50), (1, 512, 256, 512), (4, 1024, 512, 1024), (4, 1024, 512, 128), (1, 2048, 512, 2048),
+                        (1, 4096, 256, 256), (8, 256, 512, 256), (16, 128, 512, 128), (1, 256, 1024, 256)]:
+        ctx = ps.Context(0)
+        ctx.set_form_factors(w0.elements, nl, ng, coef)
+        ctx.set_geometry(np.array([n * 0.1, n * 0.1, 8.0]), n, n, 2.0)
+        ex = torch.view_as_complex(torch.randn((P, F, n, n, 2), device="cuda"))
+        bins = None if nb == F else np.arange(nb, dtype=np.int32)
+        I = torch.empty((P, nb, n, n), dtype=torch.float32, device="cuda")
+        for _ in range(3):
+            ps.ps_tacaw(ctx, ex, 2.0, bins, d_I=I)
+        ts = []
+        for _ in range(5):
+            flush.zero_()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(); ps.ps_tacaw(ctx, ex, 2.0, bins, d_I=I); b.record()
+            torch.cuda.synchronize()
+            ts.append(a.elapsed_time(b))
+        ms = float(np.median(ts))
+        nk = ctx.n_k_aperture
+        byts = (8.0 * F + 4.0 * nb) * nk * P + 4.0 * nb * (n * n - nk) * P
+        print(json.dumps({"micro": "ps_tacaw", "P": P, "frames": F, "grid": n, "bins": nb, "ms": ms,
+                          "algorithmic_GB": byts / 1e9, "GBps": byts / ms / 1e6, "frac_of_hbm_peak": byts / ms / 1e6 / peak}))
+        del ex, I, ctx
+
+
 # --------------------------------------------------------------------------------------------- our arm
 def main():
     ap = argparse.ArgumentParser()
@@ -169,6 +204,8 @@ def main():
     ap.add_argument("--probes-side", type=int, default=None, help="override probes per scan side / number of tilts")
     ap.add_argument("--wave-chunk", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--tacaw-micro", action="store_true",
+                    help="time ps_tacaw alone on synthetic stacks of several shapes (profiles/r1_tacaw_kernels.md) and exit")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -178,6 +215,9 @@ def main():
 
     if args.impl == "reference":
         run_reference(args, w, rank)
+        return
+    if args.tacaw_micro:
+        tacaw_micro()
         return
 
     import torch
