@@ -31,6 +31,7 @@ _PROTOTYPES = {
     "ps_set_workspace": (C.c_int, [C.c_void_p, C.c_void_p, C.c_size_t]),
     "ps_set_wave_chunk": (C.c_int, [C.c_void_p, C.c_int]),
     "ps_set_vk_mode": (C.c_int, [C.c_void_p, C.c_int]),
+    "ps_set_vacuum_shortcut": (C.c_int, [C.c_void_p, C.c_int]),
     "ps_set_aberrations": (C.c_int, [C.c_void_p, C.c_void_p]),
     "ps_apply_aberrations": (C.c_int, [C.c_void_p, C.c_double, C.c_void_p, C.c_longlong]),
     "ps_build_slices": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p]),
@@ -199,6 +200,10 @@ class Context:
         n = d_waves_k.numel() // (self.nx * self.ny)
         self._check(self._lib.ps_apply_aberrations(self._h, float(kV), _ptr(d_waves_k), n))
         return d_waves_k
+
+    def set_vacuum_shortcut(self, on: bool):
+        """Rows with V == 0 are only rescaled by ps_multislice (exact; default off)."""
+        self._check(self._lib.ps_set_vacuum_shortcut(self._h, int(bool(on))))
 
     def set_vk_mode(self, mode: int):
         """0 auto, 1 FP32 SIMT structure-factor sums, 2 tcgen05 3xTF32 sums."""

@@ -244,6 +244,12 @@ extern "C" ps_status ps_set_wave_chunk(ps_ctx* c, int n_waves) {
     return PS_OK;
 }
 
+extern "C" ps_status ps_set_vacuum_shortcut(ps_ctx* c, int on) {
+    if (!c) return PS_EINVAL;
+    c->vacuum_shortcut = on ? 1 : 0;
+    return PS_OK;
+}
+
 extern "C" ps_status ps_set_vk_mode(ps_ctx* c, int mode) {
     if (!c) return PS_EINVAL;
     if (mode < 0 || mode > 2) return fail(c, PS_EINVAL, "ps_set_vk_mode: mode must be 0 (auto), 1 (FP32 SIMT) or 2 (tcgen05 3xTF32)");

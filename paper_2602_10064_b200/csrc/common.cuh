@@ -68,6 +68,7 @@ struct ps_ctx {
     uint8_t* d_tile_active = nullptr;       // [nx/kColTile]
     int n_tiles_active = 0;
     int wave_chunk = 0;
+    int vacuum_shortcut = 0;                // ps_set_vacuum_shortcut: rows with V == 0 skip the transmit + FFT pair (exact)
     int vk_mode = 0;                        // ps_set_vk_mode: 0 auto, 1 FP32 SIMT sums, 2 tcgen05 3xTF32 sums
 
     // form factors

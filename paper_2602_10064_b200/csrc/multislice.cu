@@ -39,7 +39,8 @@ template <int NX, bool FIRST>
 __global__ void __launch_bounds__(RowCfg<NX>::THREADS, RowCfg<NX>::MIN_BLOCKS)
 k_row_transmit(float2* __restrict__ W, const float2* __restrict__ psi0, const float* __restrict__ V,
                const uint8_t* __restrict__ tile_active, const ChunkMap cm, const int ny, const int n_slices,
-               const int slice, const float sigma, const int n_items, const int col_lo, const int col_hi) {
+               const int slice, const float sigma, const int n_items, const int col_lo, const int col_hi,
+               const int vacuum_shortcut) {
     using Cfg = RowCfg<NX>;
     constexpr int T = Cfg::T;
     extern __shared__ float2 smem[];
@@ -92,6 +93,23 @@ k_row_transmit(float2* __restrict__ W, const float2* __restrict__ psi0, const fl
 #pragma unroll
             for (int e = 0; e < 16; ++e)
                 v[e] = (valid && ((amask >> e) & 1u)) ? wrow[t + e * T] : make_float2(0.f, 0.f);
+            if (vacuum_shortcut) {
+                // V == 0 on the whole row (vacuum): exp(i sigma V) = 1 and FFT_x[IFFT_x[M]] = NX * M exactly, so the
+                // row is only rescaled (NX is a power of two: no rounding).  Decided per warp (T <= 32: the rows this
+                // warp carries) or per block, from the potential itself: any input with vacuum rows benefits.
+                bool z = true;
+#pragma unroll
+                for (int e = 0; e < 16; ++e) z = z && (sv[e] == 0.f);
+                const bool all_z = (T <= 32) ? (bool)__all_sync(0xffffffffu, z) : (bool)__syncthreads_and(z);
+                if (all_z) {
+                    if (valid) {
+#pragma unroll
+                        for (int e = 0; e < 16; ++e)
+                            if ((amask >> e) & 1u) wrow[t + e * T] = make_float2(v[e].x * (float)NX, v[e].y * (float)NX);
+                    }
+                    continue;
+                }
+            }
             fft_inverse<NX, RowSlots, typename Cfg::Sync>(v, t, tw, slots);
         }
 #pragma unroll
@@ -256,7 +274,7 @@ static cudaError_t launch_row(ps_ctx* c, float2* W, const float2* psi0, const fl
     const int n_items = (int)((n_rows + Cfg::RPB - 1) / Cfg::RPB);
     const int grid = n_items < per_sm_grid ? n_items : per_sm_grid;
     kern<<<grid, Cfg::THREADS, Cfg::SMEM, c->stream>>>(W, psi0, V, c->d_tile_active, cm, c->ny, c->n_slices, slice,
-                                                      sigma, n_items, col_lo, col_hi);
+                                                      sigma, n_items, col_lo, col_hi, c->vacuum_shortcut);
     return cudaGetLastError();
 }
 

@@ -366,3 +366,30 @@ def test_error_statuses(torch):
     ctx.set_workspace(None)
     V = ps.ps_build_slices(ctx, pos, Z)                                    # and the context is still usable
     assert torch.isfinite(V).all()
+
+
+@pytest.mark.parametrize("nx,ny", [(64, 64), (256, 64), (512, 32), (1024, 32)])
+def test_vacuum_row_shortcut_is_exact(torch, nx, ny):
+    """Rows on which V == 0 are only rescaled (ps_set_vacuum_shortcut): same exit waves as the full transforms to
+    rounding, and the oracle's within tolerance; mixed slices (some rows vacuum, some not) and fully empty slices."""
+    import paper_2602_10064_b200 as ps
+    rng = np.random.default_rng(nx + ny)
+    w = make_workload("c1_si_128", mini=True)
+    w.nx, w.ny, w.n_slices = nx, ny, 4
+    w.cell = np.array([nx * 0.12, ny * 0.12, 8.0])
+    ctx = make_ctx(w)
+    F = 3
+    V32 = (60.0 * rng.normal(size=(F, 4, ny, nx))).astype(np.float32)
+    V32[:, 1] = 0.0                                                      # a vacuum slice
+    V32[:, 2, ::3] = 0.0                                                 # every third row of slice 2
+    V32[1, 3, ny // 2:] = 0.0                                            # half of slice 3 in one frame
+    psi0 = O.tilted_plane_wave(nx, ny, 2, -1).astype(np.complex64)[None]
+    ctx.set_vacuum_shortcut(True)
+    a = ps.ps_multislice(ctx, 80.0, _t(torch, psi0), _t(torch, V32)).clone()
+    ctx.set_vacuum_shortcut(False)
+    b = ps.ps_multislice(ctx, 80.0, _t(torch, psi0), _t(torch, V32)).clone()
+    assert rel_l2(a.cpu().numpy(), b.cpu().numpy()) < 2e-6
+    for i in range(F):
+        eo = O.multislice(psi0[0].astype(np.complex128), V32[i].astype(np.float64), w.cell, 80.0)
+        assert rel_l2(a[0, i].cpu().numpy(), eo) < TOL_EXIT
+        assert rel_l2(b[0, i].cpu().numpy(), eo) < TOL_EXIT
