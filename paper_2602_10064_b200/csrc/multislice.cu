@@ -51,24 +51,31 @@ k_row_transmit(float2* __restrict__ W, const float2* __restrict__ psi0, const fl
     unsigned amask = 0;                                  // bit e: column t+e*T lies in an active tile
 #pragma unroll
     for (int e = 0; e < 16; ++e) amask |= (tile_active[(t + e * T) / kColTile] ? 1u : 0u) << e;
-    const long long n_rows = (long long)cm.np * cm.nf * ny;
+    // 32-bit index arithmetic (ps_multislice checks n_probes * n_frames * ny < 2^31; ny is a power of two):
+    // 64-bit divisions here cost about a tenth of the kernel's instructions
+    const unsigned n_rows = (unsigned)cm.np * (unsigned)cm.nf * (unsigned)ny;
+    const int ny_shift = __ffs(ny) - 1;
+    const unsigned np_u = (unsigned)cm.np;
 
     for (int item = blockIdx.x; item < n_items; item += gridDim.x) {
-        const long long rho = (long long)item * Cfg::RPB + r;
+        const unsigned rho = (unsigned)item * Cfg::RPB + r;
         const bool valid = rho < n_rows;
         int y = 0, p = 0, f = 0;
         if (valid) {
-            const int l = (int)(rho / ny);
-            y = (int)(rho % ny);
-            p = cm.p0 + l % cm.np;
-            f = cm.f0 + l / cm.np;
+            const unsigned l = rho >> ny_shift;
+            y = (int)(rho & (unsigned)(ny - 1));
+            const unsigned lf = (np_u == 1u) ? l : l / np_u;
+            p = cm.p0 + (int)(l - lf * np_u);
+            f = cm.f0 + (int)lf;
         }
         if (NX >= 512 && t == 0) {                           // this block's next row: HBM -> L2 while this one is transformed
                                                              // (measured: +3 % at 512^2, +4 % at 2048^2, -4 % at 256^2)
-            const long long rn = rho + (long long)gridDim.x * Cfg::RPB;
+            const unsigned rn = rho + gridDim.x * Cfg::RPB;
             if (rn < n_rows) {
-                const int ln = (int)(rn / ny), yn = (int)(rn % ny);
-                const int pn = cm.p0 + ln % cm.np, fn = cm.f0 + ln / cm.np;
+                const unsigned ln = rn >> ny_shift;
+                const int yn = (int)(rn & (unsigned)(ny - 1));
+                const unsigned lfn = (np_u == 1u) ? ln : ln / np_u;
+                const int pn = cm.p0 + (int)(ln - lfn * np_u), fn = cm.f0 + (int)lfn;
                 tma::bulk_prefetch_l2(V + (((size_t)fn * n_slices + slice) * ny + yn) * NX, NX * sizeof(float));
                 if (!FIRST) {
                     const float2* wn = W + (((size_t)pn * cm.F + fn) * ny + yn) * NX;
