@@ -191,6 +191,8 @@ k_col_propagate(const __grid_constant__ CUtensorMap wmap, const int tiles_lo, co
     }
 
     int it = 0;
+    int rem = blockIdx.x % per_wave;                         // item % per_wave, kept incrementally (no division per item)
+    const int rem_step = gridDim.x % per_wave;
     for (int item = blockIdx.x; item < n_items; item += gridDim.x, ++it) {
         const int s = it % NS;
         if (threadIdx.x == 0) {
@@ -200,7 +202,6 @@ k_col_propagate(const __grid_constant__ CUtensorMap wmap, const int tiles_lo, co
                 issue_load(nxt, (it + PF) % NS);
             }
         }
-        const int l = item / per_wave, rem = item % per_wave;
         const int tj = rem / SUB;
         const int kx0 = (tj < tiles_lo ? tj : tj + tile_gap) * kColTile + (rem % SUB) * C;
         const int kx = kx0 + c;
@@ -226,6 +227,7 @@ k_col_propagate(const __grid_constant__ CUtensorMap wmap, const int tiles_lo, co
         tma::fence_proxy_async();
         __syncthreads();
         if (threadIdx.x == 0) {
+            const int l = item / per_wave;
             const int p = cm.p0 + l % cm.np, f = cm.f0 + l / cm.np;
             const int row0 = (p * cm.F + f) * NY;
 #pragma unroll
@@ -233,6 +235,8 @@ k_col_propagate(const __grid_constant__ CUtensorMap wmap, const int tiles_lo, co
                 tma::tensor_store_2d(&wmap, 2 * kx0, row0 + b * Cfg::BOX_R, st + (size_t)b * Cfg::BOX_R * C);
             tma::bulk_commit();
         }
+        rem += rem_step;
+        if (rem >= per_wave) rem -= per_wave;
     }
     if (threadIdx.x == 0) tma::bulk_wait_all<0>();
 }

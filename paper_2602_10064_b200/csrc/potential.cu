@@ -334,12 +334,13 @@ k_v_row(const float2* __restrict__ Zm, const int32_t* __restrict__ offsets, floa
 #pragma unroll
     for (int e = 0; e < 16; ++e) amask |= (tile_active[(t + e * T) / kColTile] ? 1u : 0u) << e;
     const int n_bins = n_slices * n_elem;
+    const int ny_shift = __ffs(ny) - 1;                       // ny is a power of two
 
     for (int item = blockIdx.x; item < n_items; item += gridDim.x) {
-        const long long rho = (long long)item * Cfg::RPB + r;
-        const bool valid = rho < n_rows;
+        const unsigned rho = (unsigned)item * Cfg::RPB + r;       // < 2^31: the mixed array lives in scratch
+        const bool valid = (long long)rho < n_rows;
         int y = 0, fp = 0;
-        if (valid) { fp = (int)(rho / ny); y = (int)(rho % ny); }
+        if (valid) { fp = (int)(rho >> ny_shift); y = (int)(rho & (unsigned)(ny - 1)); }
         const int f = fp / n_pairs, pr = fp % n_pairs;
         const int sa = 2 * pr, sb = 2 * pr + 1;
         const int32_t* off = offsets + (size_t)f * (n_bins + 1);
