@@ -38,9 +38,11 @@ k_tacaw_fft(const float2* __restrict__ exitw, float* __restrict__ I, const int32
 #pragma unroll
     for (int e = 0; e < 16; ++e) slot[e] = slot_of_bin[t + e * T];
 
+    // nx, ny and C are powers of two: shifts instead of four integer divisions per item and thread
+    const int gpr_shift = __ffs(groups_per_row) - 1, gpp_shift = __ffs(groups_per_probe) - 1;
     for (int item = blockIdx.x; item < n_items; item += gridDim.x) {
-        const int p = item / groups_per_probe, g = item % groups_per_probe;
-        const int iy = g / groups_per_row, ix0 = (g % groups_per_row) * C;
+        const int p = item >> gpp_shift, g = item & (groups_per_probe - 1);
+        const int iy = g >> gpr_shift, ix0 = (g & (groups_per_row - 1)) * C;
         const int ay = iy < ny / 2 ? iy : ny - iy;
         const size_t pix = (size_t)iy * nx + ix0 + c;
         float* out = I + (size_t)p * n_out * npix + pix;
@@ -130,6 +132,9 @@ k_tacaw_tma(const __grid_constant__ CUtensorMap emap, float* __restrict__ I, con
     }
 
     int it = 0;
+    const int nx_shift = __ffs(nx) - 1;
+    int g_rem = blockIdx.x % n_groups, p_cur = blockIdx.x / n_groups;
+    const int g_step = gridDim.x % n_groups, p_step = gridDim.x / n_groups;
     for (int item = blockIdx.x; item < n_items; item += gridDim.x, ++it) {
         const int s = it % NS;
         // every thread is past the exchange of item it-1, whose stage (it+PF)%NS is the next load's target
@@ -139,8 +144,9 @@ k_tacaw_tma(const __grid_constant__ CUtensorMap emap, float* __restrict__ I, con
             const int nxt = item + PF * gridDim.x;
             if (nxt < n_items) issue_load(nxt, (it + PF) % NS);
         }
-        const int p = item / n_groups, pix0 = groups[item % n_groups];
-        const int ix = pix0 % nx + c, iy = pix0 / nx;
+        const int pix0 = groups[g_rem];                      // g_rem = item % n_groups, p_cur = item / n_groups (incremental)
+        const int p = p_cur;
+        const int ix = (pix0 & (nx - 1)) + c, iy = pix0 >> nx_shift;
         const int ay = iy < ny / 2 ? iy : ny - iy;
         const bool mine = ay <= nmax[ix];                    // the group has in-band pixels; this one may not be
         float* out = I + (size_t)p * n_out * npix + pix0 + c;
@@ -161,6 +167,8 @@ k_tacaw_tma(const __grid_constant__ CUtensorMap emap, float* __restrict__ I, con
                 out[(size_t)slot[e] * npix] = zero ? 0.f : fmaf(v[e].x, v[e].x, v[e].y * v[e].y);
             }
         }
+        g_rem += g_step; p_cur += p_step;
+        if (g_rem >= n_groups) { g_rem -= n_groups; ++p_cur; }
     }
 }
 
