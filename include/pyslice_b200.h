@@ -66,6 +66,8 @@ typedef enum {
 
 /* ---------------------------------------------------------------- life cycle */
 
+/* One context per host thread and one CUDA device per process (the multi-GPU model is one process per GPU): kernel
+ * attributes and occupancy-derived grid sizes are cached per process on first use. */
 /* Create a context bound to CUDA device `device` and to `cuda_stream` (a cudaStream_t; NULL =
  * the legacy default stream).  Fails with PS_ECUDA when no usable device exists. */
 PS_API ps_status ps_create(ps_ctx** out, int device, void* cuda_stream);
