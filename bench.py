@@ -191,6 +191,82 @@ def tacaw_micro():
         del ex, I, ctx
 
 
+# --------------------------------------------------------------------------------------------- configs 3 / 4 at full size
+def full_config(which):
+    """Config 4: 4096 frames x 1024^2 x 120 slices, V built and propagated 64 frames at a time, exit waves folded into the
+    streaming per-bin DFT (path B, 256 bins) chunk by chunk (SURVEY.md 8(d) capacity plan).  Config 3: 1024 frames x
+    256 probes x 512^2 x 80 slices: V of all frames resident (86 GB), probes 16 at a time (34 GB of exit waves),
+    path A per probe chunk, spectrum image and probe-summed diffraction pattern accumulated on the fly."""
+    import torch
+    import paper_2602_10064_b200 as ps
+    from paper_2602_10064_b200.binding import TacawStream
+    t_host = time.perf_counter()
+    w = make_workload("c4_interface_1024" if which == "c4" else "c3_si_probe_512")
+    F, P, S, nx, ny = w.n_frames, w.n_probes, w.n_slices, w.nx, w.ny
+    ctx = ps.Context(0)
+    nl, ng, coef = form_factor_coefficients(w.elements, w.ff_kind)
+    ctx.set_form_factors(w.elements, nl, ng, coef)
+    ctx.set_geometry(w.cell, nx, ny, w.slice_dz)
+    step = 256
+    pos_d = torch.cat([torch.from_numpy(w.positions(f0, min(F, f0 + step))).cuda() for f0 in range(0, F, step)])
+    Z_d = torch.from_numpy(w.Z.copy()).cuda()
+    t_host = time.perf_counter() - t_host
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    l0 = ctx.launches
+    if which == "c4":
+        chunk = 64
+        bins = w.bins
+        V = torch.empty((chunk, S, ny, nx), dtype=torch.float32, device="cuda")
+        ex = torch.empty((1, chunk, ny, nx), dtype=torch.complex64, device="cuda")
+        psi0 = ps.ps_make_incident(ctx, w.kV)
+        ts0 = TacawStream(ctx, 1, F, w.dt_fs, bins)                      # warm-up of every kernel on one chunk
+        ps.ps_build_slices(ctx, pos_d[:chunk], Z_d, d_V=V); ps.ps_multislice(ctx, w.kV, psi0, V, d_exit=ex); ts0.add(ex, 0)
+        del ts0
+        torch.cuda.synchronize()
+        a.record()
+        ts = TacawStream(ctx, 1, F, w.dt_fs, bins)
+        for f0 in range(0, F, chunk):
+            ps.ps_build_slices(ctx, pos_d[f0:f0 + chunk], Z_d, d_V=V)
+            ps.ps_multislice(ctx, w.kV, psi0, V, d_exit=ex)
+            ts.add(ex, f0)
+        I = ts.finish()
+        simg = ps.ps_spectrum_image(ctx, I)
+        b.record()
+        torch.cuda.synchronize()
+        check = float(simg.sum())
+        plan = f"{F // chunk} chunks of {chunk} frames: build V (30 GB) -> multislice -> ps_tacaw_add (path B, {len(bins)} bins)"
+    else:
+        pc = 16
+        V = ps.ps_build_slices(ctx, pos_d[:8], Z_d)                      # warm-up
+        del V
+        torch.cuda.synchronize()
+        ex = torch.empty((pc, F, ny, nx), dtype=torch.complex64, device="cuda")
+        I = torch.empty((pc, F, ny, nx), dtype=torch.float32, device="cuda")
+        simg = torch.empty((P, F), dtype=torch.float32, device="cuda")
+        sdp = torch.zeros((ny, nx), dtype=torch.float32, device="cuda")
+        sdp_c = torch.empty((ny, nx), dtype=torch.float32, device="cuda")
+        a.record()
+        V = torch.empty((F, S, ny, nx), dtype=torch.float32, device="cuda")
+        ps.ps_build_slices(ctx, pos_d, Z_d, d_V=V)
+        for p0 in range(0, P, pc):
+            psi0 = ps.ps_make_incident(ctx, w.kV, w.semi_angle_mrad, w.probe_xy[p0:p0 + pc])
+            ps.ps_multislice(ctx, w.kV, psi0, V, d_exit=ex)
+            ps.ps_tacaw(ctx, ex, w.dt_fs, d_I=I)
+            ps.ps_spectrum_image(ctx, I, d_out=simg[p0:p0 + pc])
+            ps.ps_sdp(ctx, I, 1, 32, d_out=sdp_c)
+            ps.ps_accumulate_intensity(ctx, sdp, sdp_c, 1.0, 1.0)
+        b.record()
+        torch.cuda.synchronize()
+        check = float(simg.sum())
+        plan = f"V of all {F} frames resident (86 GB); {P // pc} chunks of {pc} probes: incident -> multislice (34 GB) -> ps_tacaw -> reductions"
+    sec = a.elapsed_time(b) * 1e-3
+    units = float(nx) * ny * S * F * P
+    print(json.dumps({"full_config": w.name, "grid": [nx, ny], "n_slices": S, "frames": F, "probes": P, "atoms": int(w.n_atoms),
+                      "tacaw_end_to_end_s": sec, "value": units / sec / 1e9, "unit": UNIT, "plan": plan,
+                      "gpu_launches": int(ctx.launches - l0), "host_setup_s": t_host, "checksum_spectrum_image": check,
+                      "hbm_peak_allocated_GB": torch.cuda.max_memory_allocated() / 1e9}))
+
+
 # --------------------------------------------------------------------------------------------- our arm
 def main():
     ap = argparse.ArgumentParser()
@@ -204,6 +280,9 @@ def main():
     ap.add_argument("--probes-side", type=int, default=None, help="override probes per scan side / number of tilts")
     ap.add_argument("--wave-chunk", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--full-config", choices=["c3", "c4"], default=None,
+                    help="run config 3 or 4 at its FULL size (all frames, all probes) in chunks that fit 180 GB, one step, "
+                         "and print one JSON line (minutes of host-side trajectory generation before the timed region)")
     ap.add_argument("--tacaw-micro", action="store_true",
                     help="time ps_tacaw alone on synthetic stacks of several shapes (profiles/r1_tacaw_kernels.md) and exit")
     args = ap.parse_args()
@@ -218,6 +297,9 @@ def main():
         return
     if args.tacaw_micro:
         tacaw_micro()
+        return
+    if args.full_config:
+        full_config(args.full_config)
         return
 
     import torch
