@@ -352,8 +352,23 @@ k_v_row(const float2* __restrict__ Zm, const int32_t* __restrict__ offsets, floa
 #pragma unroll
         for (int e = 0; e < 16; ++e)
             v[e] = (any && ((amask >> e) & 1u)) ? src[t + e * T] : make_float2(0.f, 0.f);
-        // both slices of every row of this block empty (vacuum): V = 0, no transform needed
-        if (__syncthreads_or(any)) fft_inverse<NX, RowSlots, typename Cfg::Sync>(v, t, tw, slots);
+        // both slices of every row of this block empty (vacuum): V = 0, no transform; the block's RPB rows are
+        // contiguous in V (ny is a multiple of RPB), so they are cleared with 16-byte stores
+        if (!__syncthreads_or(any)) {
+            const unsigned rho0 = (unsigned)item * Cfg::RPB;
+            if ((long long)rho0 < n_rows) {
+                const int fp0 = (int)(rho0 >> ny_shift), y0 = (int)(rho0 & (unsigned)(ny - 1));
+                const int f0 = fp0 / n_pairs, s0 = 2 * (fp0 % n_pairs);
+                float4* za = reinterpret_cast<float4*>(V + (((size_t)f0 * n_slices + s0) * ny + y0) * NX);
+                float4* zb = reinterpret_cast<float4*>(V + (((size_t)f0 * n_slices + s0 + 1) * ny + y0) * NX);
+                for (int k = threadIdx.x; k < Cfg::RPB * NX / 4; k += Cfg::THREADS) {
+                    za[k] = make_float4(0.f, 0.f, 0.f, 0.f);
+                    if (s0 + 1 < n_slices) zb[k] = make_float4(0.f, 0.f, 0.f, 0.f);
+                }
+            }
+            continue;
+        }
+        fft_inverse<NX, RowSlots, typename Cfg::Sync>(v, t, tw, slots);
         if (valid) {
             float* va = V + (((size_t)f * n_slices + sa) * ny + y) * NX;
 #pragma unroll
