@@ -145,7 +145,7 @@ extern "C" void ps_destroy(ps_ctx* c) {
     cudaFree(c->d_ftab); cudaFree(c->d_elem_of_Z);
     cudaFree(c->kv.d_px_mid); cudaFree(c->kv.d_px_last); cudaFree(c->kv.d_py);
     cudaFree(c->scratch.p); cudaFree(c->misc.p); cudaFree(c->qorder.p); cudaFree(c->ts.d_bins);
-    cudaFree(c->tacaw_groups.p); cudaFree(c->abtab.p);
+    cudaFree(c->tacaw_groups.p); cudaFree(c->abtab.p); cudaFree(c->tacaw_slot.p);
     for (auto& r : c->prof_pending) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
     for (auto e : c->prof_pool) cudaEventDestroy(e);
     delete c;

@@ -98,6 +98,8 @@ struct ps_ctx {
     psb::DeviceBuf tacaw_groups;            // ps_tacaw: pixel-group lists [active..., inactive...] (first pixel of each)
     int tacaw_groups_C = 0;                 // group width the lists were built for (0 = not built)
     int tacaw_n_active = 0, tacaw_n_inactive = 0;
+    psb::DeviceBuf tacaw_slot;              // ps_tacaw: output slot of every FFT bin (-1 = not requested)
+    std::vector<int32_t> tacaw_slot_host;   // its host copy (uploaded again only when the bin list changes)
     psb::DeviceBuf misc;                    // small per-call tables (bin slots, path pixels)
     psb::DeviceBuf qorder;                  // ps_qbin: cursor, offsets and pixel order by q bin (cached)
     bool qorder_valid = false;

@@ -358,11 +358,16 @@ extern "C" ps_status ps_tacaw(ps_ctx* c, const void* d_exit, int exit_layout, in
         if (slot[n] >= 0) return fail(c, PS_EINVAL, "ps_tacaw: duplicate bin in list");
         slot[n] = b;
     }
-    ps_status st = ensure_buf(c, c->misc, 4096 + (size_t)n_frames * 4);
-    if (st != PS_OK) return st;
-    int32_t* d_slot = (int32_t*)((char*)c->misc.p + 4096);
-    PSB_CUDA(c, cudaMemcpyAsync(d_slot, slot.data(), (size_t)n_frames * 4, cudaMemcpyHostToDevice, c->stream));
-    PSB_CUDA(c, cudaStreamSynchronize(c->stream));           // `slot` dies at return; 16 KB at most
+    // the bin -> output-slot table lives in its own buffer and is uploaded only when it changes: repeated calls with
+    // the same bin list (every step of a run) enqueue work without a host-side wait
+    if (slot != c->tacaw_slot_host || !c->tacaw_slot.p) {
+        ps_status st = ensure_buf(c, c->tacaw_slot, (size_t)n_frames * 4);
+        if (st != PS_OK) return st;
+        PSB_CUDA(c, cudaMemcpyAsync(c->tacaw_slot.p, slot.data(), (size_t)n_frames * 4, cudaMemcpyHostToDevice, c->stream));
+        PSB_CUDA(c, cudaStreamSynchronize(c->stream));       // `slot` is a host temporary; 16 KB at most
+        c->tacaw_slot_host = slot;
+    }
+    int32_t* d_slot = (int32_t*)c->tacaw_slot.p;
     ProfScope ps_(c, K_TACAW_FFT);
     const float2* ex = (const float2*)d_exit;
     // Kernel choice measured on B200 (profiles/r1_tacaw_kernels.md): the TMA-staged ring wins where one block per
