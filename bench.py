@@ -434,6 +434,7 @@ def main():
     ms_pair = kern["k_row_transmit"][0] + kern["k_col_propagate"][0]
     pair_gbs = (ROW_BYTES + COL_BYTES) * px_slices_per_step * K / (ms_pair * 1e-3) / 1e9
     traffic = None                                              # DRAM bytes per launch of that kernel, from ncu
+    tj = {}
     tpath = os.path.join(ROOT, "profiles", "r1_traffic.json")
     if w.name == "c2_hbn_256" and args.frames is None and args.grid is None and not args.wave_chunk and os.path.exists(tpath):
         with open(tpath) as fh:
@@ -450,7 +451,8 @@ def main():
         tb = (8.0 * F + 4.0 * nb) * ctx.n_k_aperture * P + 4.0 * nb * (nx * ny - ctx.n_k_aperture) * P
         tms = kern["k_tacaw_fft"][0] / kern["k_tacaw_fft"][1]
         roofline["tacaw"] = {"achieved": tb / (tms * 1e-3) / 1e9, "frac": tb / (tms * 1e-3) / 1e9 / peak,
-                             "bytes_per_launch": tb, "avg_launch_ms": tms}
+                             "bytes_per_launch": tb, "avg_launch_ms": tms,
+                             "traffic": next((v for k, v in tj.items() if k.startswith("k_tacaw_tma") or k.startswith("k_tacaw_fft")), None)}
 
     if "k_vk" in kern:
         # V(k) structure-factor sums: 4 real sums per quarter-plane point and atom, x3 for the 3xTF32 split (tensor path)
