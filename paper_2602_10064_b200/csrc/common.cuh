@@ -10,7 +10,8 @@
 
 namespace psb {
 
-constexpr int kColTile = 16;        // columns per tile of the column passes / activity granularity
+constexpr int kColTile = 8;         // columns per tile of the column passes / activity granularity (16 measured
+                                    // 2 % slower at 256^2: 192 instead of 176 of 256 columns touched)
 constexpr int kMaxGrid = 2048;
 constexpr int kMinGrid = 32;
 constexpr int kNumSM = 148;         // B200

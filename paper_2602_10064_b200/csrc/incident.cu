@@ -28,7 +28,7 @@ __global__ void k_fill_plane_tilt(float2* __restrict__ psi, const int nx, const 
 
 template <int NY> struct PColCfg {
     static constexpr int T = Plan<NY>::T;
-    static constexpr int C = (NY <= 512) ? 16 : ((NY == 1024) ? 8 : 4);
+    static constexpr int C = (NY <= 1024) ? 8 : 4;
     static constexpr int THREADS = C * T;
     static constexpr size_t SMEM = (size_t)NY * C * sizeof(float2);
 };

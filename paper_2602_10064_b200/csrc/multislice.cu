@@ -138,7 +138,7 @@ k_row_transmit(float2* __restrict__ W, const float2* __restrict__ psi0, const fl
 // transforms of item i and no register is spent on staging.
 template <int NY> struct ColCfg {
     static constexpr int T = Plan<NY>::T;
-    static constexpr int C = (NY <= 256) ? 16 : ((NY <= 1024) ? 8 : 4);   // columns per block
+    static constexpr int C = (NY <= 1024) ? 8 : 4;   // columns per block
     static constexpr int THREADS = C * T;
     static constexpr int NS = 3;                                          // pipeline stages
     static constexpr int BOX_R = (NY < 256) ? NY : 256;                   // TMA box rows (<= 256)

@@ -238,7 +238,7 @@ k_vk(const uint32_t* __restrict__ sUx, const uint32_t* __restrict__ sUy, const i
 // ------------------------------------------------------------------------------------ a3: inverse FFT of slice pairs
 template <int NY> struct VColCfg {
     static constexpr int T = Plan<NY>::T;
-    static constexpr int C = (NY <= 512) ? 16 : ((NY == 1024) ? 8 : 4);
+    static constexpr int C = (NY <= 1024) ? 8 : 4;
     static constexpr int THREADS = C * T;
     static constexpr size_t SMEM = (size_t)NY * C * sizeof(float2);
 };
