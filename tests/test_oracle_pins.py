@@ -509,3 +509,85 @@ def test_aberration_function_against_propagator_and_textbook():
     assert abs(np.sum(np.abs(p) ** 2) - nx * ny) < 1e-9 * nx * ny
     W = RNG.normal(size=(2, ny, nx)) + 1j * RNG.normal(size=(2, ny, nx))
     assert np.allclose(np.abs(O.apply_aberrations(W, cell, kV, full)), np.abs(W), rtol=1e-12)
+
+
+def test_aberration_function_hand_evaluated_C12_C21_C23():
+    """Pins the 1/2, 1/3 prefactors and the cos 2(phi-phi12), cos(phi-phi21), cos 3(phi-phi23) factors of reading A24
+    (PAPER.md:143 "standard aberration function supporting defocus, astigmatism, coma, spherical aberration"): chi is
+    hand-evaluated from the Krivanek polynomial chi = (2 pi/lambda) sum_{n,m} C_nm theta^(n+1)/(n+1) cos m(phi-phi_nm)
+    at explicit grid points of a 10 x 10 A cell (k = m/10 1/A), with theta = lambda |k| and phi worked out by hand:
+        lambda(100 kV) = 0.037014 A (textbook value, tests/golden/electron_constants.txt)
+        (kx, ky) = (0, 0.4):     |k| = 0.4,          theta = 0.0148056,   phi = 90 deg
+        (kx, ky) = (-0.2, 0):    |k| = 0.2,          theta = 0.0074028,   phi = 180 deg
+        (kx, ky) = (0.3, 0.3):   |k| = 0.424264069,  theta = 0.0157037102, phi = 45 deg
+        (kx, ky) = (-0.3, 0.3):  same |k|,                                phi = 135 deg
+    A wrong prefactor (1/2 <-> 1/3), a wrong power of theta or a wrong angular multiplicity fails one of the lines."""
+    cell = np.array([10.0, 10.0, 5.0]); nx = ny = 32; kV = 100.0
+    lam = 0.037014
+    two_pi_over_lam = 2.0 * np.pi / lam
+    z = np.zeros(8)
+
+    def chi_at(coef, m, n):                                            # chi[iy][ix] at kx = m/10, ky = n/10
+        return O.aberration_function(cell, nx, ny, kV, coef)[n % ny, m % nx]
+
+    def close(got, want):
+        return abs(got - want) <= 1e-4 * abs(want) + 1e-12
+
+    # ---- pure C12 = 50 A, phi12 = 0.3 rad:  chi = (2 pi/lam) * 50 * theta^2/2 * cos 2(phi - 0.3)
+    c = z.copy(); c[1] = 50.0; c[2] = 0.3
+    # phi = 90 deg: cos(pi - 0.6) = -cos 0.6 = -0.8253356149
+    assert close(chi_at(c, 0, 4), two_pi_over_lam * 50.0 * 0.0148056 ** 2 / 2.0 * (-0.8253356149))
+    # phi = 180 deg: cos(2 pi - 0.6) = +0.8253356149
+    assert close(chi_at(c, -2, 0), two_pi_over_lam * 50.0 * 0.0074028 ** 2 / 2.0 * 0.8253356149)
+    # phi = 45 deg: cos(pi/2 - 0.6) = sin 0.6 = 0.5646424734  (a cos(phi - phi12) would give 0.8816)
+    assert close(chi_at(c, 3, 3), two_pi_over_lam * 50.0 * 0.0157037102 ** 2 / 2.0 * 0.5646424734)
+    # ---- pure C21 = 900 A, phi21 = 0.2 rad:  chi = (2 pi/lam) * 900 * theta^3/3 * cos(phi - 0.2)
+    c = z.copy(); c[3] = 900.0; c[4] = 0.2
+    # phi = 180 deg: cos(pi - 0.2) = -0.9800665778
+    assert close(chi_at(c, -2, 0), two_pi_over_lam * 900.0 * 0.0074028 ** 3 / 3.0 * (-0.9800665778))
+    # phi = 90 deg: cos(pi/2 - 0.2) = sin 0.2 = 0.1986693308
+    assert close(chi_at(c, 0, 4), two_pi_over_lam * 900.0 * 0.0148056 ** 3 / 3.0 * 0.1986693308)
+    # ---- pure C23 = 350 A, phi23 = 0:  chi = (2 pi/lam) * 350 * theta^3/3 * cos 3 phi
+    c = z.copy(); c[5] = 350.0
+    # phi = 45 deg: cos 135 deg = -0.7071067812;  phi = 135 deg: cos 405 deg = +0.7071067812 (cos phi would flip both signs)
+    assert close(chi_at(c, 3, 3), two_pi_over_lam * 350.0 * 0.0157037102 ** 3 / 3.0 * (-0.7071067812))
+    assert close(chi_at(c, -3, 3), two_pi_over_lam * 350.0 * 0.0157037102 ** 3 / 3.0 * 0.7071067812)
+    # phi = 180 deg: cos 540 deg = -1;  phi = 90 deg: cos 270 deg = 0
+    assert close(chi_at(c, -2, 0), two_pi_over_lam * 350.0 * 0.0074028 ** 3 / 3.0 * (-1.0))
+    assert abs(chi_at(c, 0, 4)) < 1e-9
+    # ---- with phi23 = -0.7: phi = 90 deg -> cos(3 pi/2 + 2.1) = sin 2.1 = 0.8632093666
+    c[6] = -0.7
+    assert close(chi_at(c, 0, 4), two_pi_over_lam * 350.0 * 0.0148056 ** 3 / 3.0 * 0.8632093666)
+    # ---- the terms add: everything on at once equals the sum of the single-term values at one point
+    full = np.array([30.0, 50.0, 0.3, 900.0, 0.2, 350.0, -0.7, 2.0e5])
+    parts = 0.0
+    for idx in ((0,), (1, 2), (3, 4), (5, 6), (7,)):
+        c = z.copy(); c[list(idx)] = full[list(idx)]
+        parts += chi_at(c, 3, 3)
+    assert abs(chi_at(full, 3, 3) - parts) < 1e-9 * abs(parts)
+
+
+# ----------------------------------------------------------------------------- tilted illumination (reading A18)
+def test_tilted_plane_wave_is_one_reciprocal_grid_point():
+    """A18 (BASELINE.json config 5; the paper has no tilt): psi0 = exp(2 pi i (mt x/Lx + nt y/Ly)) sits on ONE point of
+    the reciprocal grid: fft2(psi0) is a single delta of height nx*ny at [nt mod ny][mt mod nx] (pins sign and axis
+    order), and through V = 0 it stays that plane wave times exp(-i pi lambda Lz ((mt/Lx)^2 + (nt/Ly)^2)) — the
+    free-space propagator of PAPER.md:79 (pinned by P5/P7) evaluated by hand on a NON-square cell:
+        lambda(100 kV) = 0.037014 A, Lx = 9, Ly = 12, Lz = 30 A, (mt, nt) = (-3, 2):
+        k^2 = (3/9)^2 + (2/12)^2 = 0.1111111111 + 0.0277777778 = 0.1388888889
+        phase = -pi * 0.037014 * 30 * 0.1388888889 = -0.4845121 rad."""
+    nx, ny = 24, 16
+    for mt, nt in ((-3, 2), (5, 0), (0, -7), (1, 1)):
+        psi = O.tilted_plane_wave(nx, ny, mt, nt)
+        spec = np.fft.fft2(psi)
+        want = np.zeros((ny, nx), complex); want[nt % ny, mt % nx] = nx * ny
+        assert np.abs(spec - want).max() < 1e-9
+    cell = np.array([9.0, 12.0, 30.0])
+    psi = O.tilted_plane_wave(nx, ny, -3, 2)
+    ex = O.multislice(psi, np.zeros((5, ny, nx)), cell, 100.0)           # five vacuum slices of 6 A
+    want = np.zeros((ny, nx), complex)
+    want[2, nx - 3] = np.sqrt(nx * ny) * np.exp(1j * (-0.4845121))        # unitary k-space exit wave (A13)
+    assert np.abs(ex - want).max() < 2e-5 * np.sqrt(nx * ny)
+    # a tilt outside the band limit is removed by the first propagator (kc = (2/3) * min(24/18, 16/24) = 0.4444)
+    out = O.multislice(O.tilted_plane_wave(nx, ny, 0, -7), np.zeros((1, ny, nx)), cell, 100.0)   # |k| = 7/12 = 0.583
+    assert np.abs(out).max() < 1e-12
