@@ -1,19 +1,21 @@
 #!/usr/bin/env python
 """bench.py — one JSON line for the TACAW hot path on B200 (contract: task prompt / DESIGN.md §8).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload NAME]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload NAME] ...
 
-A "step" is one pass of the whole hot path over one synthetic trajectory of the workload
-(BASELINE.json configs[1] by default: hBN-like monolayer, 256x256, 10 slices, 512 frames):
+A "step" is one pass of the whole hot path over one batch of synthetic input:
     ps_build_slices -> ps_make_incident -> ps_multislice -> ps_tacaw -> ps_sdp / ps_spectrum_image /
     ps_dispersion / ps_qbin.
-`value` = nx*ny*n_slices*frames*probes / step time, in Gpx*slice/s, inputs resident in HBM;
-`e2e` = the same with host buffers (pinned positions in, I(k,w) cube + reductions out) inside the timed
-region.  `roofline` is for the dominant kernel family of the step (per-launch CUDA events recorded by the
-library's ps_profile_* on its own stream, in a second pass of the same K steps); `cpu_baseline` is the
-float64 oracle timed on this box's host cores on a bounded sample of the same workload.
-With N > 1 (torchrun) every rank processes an independent trajectory (averaging over
-independent trajectories) and the I(k,w) cubes are summed with one NCCL all-reduce: weak scaling.
+Default workload = the largest single-GPU configuration of BASELINE.json, config 3 (Si 8x8x20, 10 240 atoms, 512^2,
+80 slices, 30 mrad probe, 1024 frames) in the unit its full run is made of: ONE 16-probe scan row x all 1024 frames
+(V of all frames 86 GB + exit waves 34 GB + I(k,w) 17 GB resident: the chunk `--full-config c3` loops 16 times).
+`value` = nx*ny*n_slices*frames*probes / step time in Gpx*slice/s, inputs resident in HBM; `e2e` = the same through
+the public API with pinned host positions in and the reductions a caller keeps out, copies inside the timed region.
+`roofline` is for the dominant kernel of the step (per-launch CUDA events recorded by the library on its own stream
+in a second pass of the same K steps); `cpu_baseline` is the float64 oracle timed on all host cores on a bounded
+sample of the same workload.  With N > 1 (torchrun): `--scaling weak` (default) gives every rank an independent
+trajectory and averages the reductions with one all-reduce; `--scaling strong` shards ONE problem
+(paper_2602_10064_b200/sharding.py: probe shards, or frame shards + reduce-scatter of the per-bin accumulators).
 `--impl reference` times the oracle (the only reference there is: the paper ships no code).
 """
 from __future__ import annotations
@@ -35,18 +37,33 @@ from workloads import form_factor_coefficients, make_workload  # noqa: E402
 
 METRIC = "multislice Gpx*slice/s over frames x probes (whole TACAW hot path per step)"
 UNIT = "Gpx*slice/s"
-# algorithmic bytes per pixel*slice of the slice step (pruned figure):
-#   row pass 4 (V) + 16 * f_col, column pass 16 * f_col, f_col = 2/3 of the columns inside the band limit
-ROW_BYTES = 4.0 + 16.0 * (2.0 / 3.0)
-COL_BYTES = 16.0 * (2.0 / 3.0)
+N_SM, LANES_PER_SM = 148, 128          # B200: 148 SMs x 4 schedulers x 32 lanes issue one instruction per clock each
 
 
 def measured_peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(path):
         with open(path) as fh:
-            return float(json.load(fh)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
-    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+            d = json.load(fh)
+        return float(d["hbm_gbs"]), float(d.get("bf16_tflops", 1590.0)), "measured (MEASURED_PEAKS.json)"
+    return 6650.0, 1590.0, "fallback (B200_PROFILING.md: 6.65 TB/s, 1.59 PFLOP/s)"
+
+
+def kernel_stats():
+    """ncu-derived per-kernel constants (profiles/r2_kernel_stats.json, written from the --set full captures named in
+    profiles/r2_slice_step.md): DRAM bytes and thread instructions per pixel of one wave, keyed by kernel<N>."""
+    path = os.path.join(ROOT, "profiles", "r2_kernel_stats.json")
+    if os.path.exists(path):
+        with open(path) as fh:
+            return json.load(fh)
+    return {}
+
+
+def band_columns(cell, nx, ny):
+    """Number of k-columns that hold at least one point inside the band limit (2 m_cut + 1): the columns any
+    implementation of the slice step must move (workload geometry, no method arithmetic)."""
+    kc = (2.0 / 3.0) * min(nx / (2.0 * cell[0]), ny / (2.0 * cell[1]))
+    return 2 * int(np.floor(kc * cell[0] + 1e-9)) + 1
 
 
 class ClockSampler(threading.Thread):
@@ -105,44 +122,70 @@ def physical_gpu_index(local_rank: int) -> int:
 
 
 # --------------------------------------------------------------------------------------------- oracle arm
-def oracle_sample(w, budget_s: float = 20.0):
-    """Times the float64 oracle (as it stands) on the first n frames of the workload; n is chosen from
-    a one-frame calibration so that the sample costs about `budget_s` seconds of CPU work."""
+def _oracle_frames(job):
+    """Worker (one process = one host core): positions -> exit waves of its frames through the first `n_sl` slices.
+    The oracle as it stands (oracle/tacaw_oracle.py), nothing tuned."""
     from oracle import tacaw_oracle as O
+    pos, elem, coef, nl, ng, cell, nx, ny, n_slices, n_sl, kV, psi0 = job
+    out = np.empty((pos.shape[0], ny, nx), dtype=np.complex128)
+    sub_cell = np.array([cell[0], cell[1], cell[2] * n_sl / n_slices])       # same dz for the propagator
+    for i in range(pos.shape[0]):
+        V, _ = O.projected_potential(pos[i], elem, coef, nl, ng, cell, nx, ny, n_slices, slices=range(n_sl))
+        out[i] = O.multislice(psi0, V[:n_sl], sub_cell, kV)
+    return out
+
+
+def oracle_sample(w, budget_s: float = 20.0, cores: int | None = None):
+    """Times the float64 oracle on all host cores: every worker process takes one frame (two when that stays inside
+    the budget) of the workload, builds its potentials and propagates one probe through the first n_sl slices (n_sl
+    calibrated so that the sample costs about `budget_s` seconds), and the parent runs the oracle's time transform on
+    the gathered exit waves.  Rate = nx*ny*n_sl*frames / wall time."""
+    import multiprocessing as mp
+    from oracle import tacaw_oracle as O
+    cores = cores or os.cpu_count() or 1
     nl, ng, coef = form_factor_coefficients(w.elements, w.ff_kind)
     elem = np.searchsorted(w.elements, w.Z)
     if w.beam == "plane":
-        psi0 = [O.plane_wave(w.nx, w.ny)]
+        psi0 = O.plane_wave(w.nx, w.ny)
     elif w.beam == "tilt":
-        psi0 = [O.tilted_plane_wave(w.nx, w.ny, int(m), int(n)) for m, n in w.tilts]
+        psi0 = O.tilted_plane_wave(w.nx, w.ny, int(w.tilts[-1][0]), int(w.tilts[-1][1]))
     else:
-        psi0 = [O.probe_wave(w.cell, w.nx, w.ny, w.kV, w.semi_angle_mrad, x, y) for x, y in w.probe_xy]
-    psi0 = psi0[:1]                                             # one probe / tilt is enough for a rate
-    pos = w.positions(0, min(w.n_frames, 64))
-
-    def run(n):
+        psi0 = O.probe_wave(w.cell, w.nx, w.ny, w.kV, w.semi_angle_mrad, w.probe_xy[0][0], w.probe_xy[0][1])
+    n_frames = min(w.n_frames, 2 * cores)
+    pos = w.positions(0, n_frames)
+    # calibration: one frame, one slice, in this process
+    t0 = time.perf_counter()
+    _oracle_frames((pos[:1], elem, coef, nl, ng, w.cell, w.nx, w.ny, w.n_slices, 1, w.kV, psi0))
+    t1 = max(time.perf_counter() - t0, 1e-3)
+    per_worker = max(1, n_frames // cores)
+    n_sl = int(max(1, min(w.n_slices, budget_s / (t1 * per_worker))))
+    jobs = [(pos[i::cores], elem, coef, nl, ng, w.cell, w.nx, w.ny, w.n_slices, n_sl, w.kV, psi0) for i in range(cores)
+            if pos[i::cores].shape[0] > 0]
+    ctx = mp.get_context("spawn")                                # children never touch CUDA
+    with ctx.Pool(len(jobs)) as pool:
+        pool.map(_oracle_frames, [(pos[:1], elem, coef, nl, ng, w.cell, 32, 32, w.n_slices, 1, w.kV,
+                                   O.plane_wave(32, 32))] * len(jobs))    # start-up (imports) outside the timed region
         t0 = time.perf_counter()
-        O.run_path(pos[:n], elem, coef, nl, ng, w.cell, w.nx, w.ny, w.n_slices, w.kV, psi0, None, frames=range(n))
-        return time.perf_counter() - t0
-
-    t1 = run(1)
-    n = int(max(2, min(pos.shape[0], budget_s / max(t1, 1e-3))))
-    t = run(n)
-    units = float(w.nx) * w.ny * w.n_slices * n * len(psi0)
-    return {"value": units / t / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle",
-            "sample": f"{n} of {w.n_frames} frames x {len(psi0)} probe(s), positions -> |Psi(k,w)|^2 "
-                      f"(float64 NumPy oracle, {t:.1f} s)"}, t, units
+        parts = pool.map(_oracle_frames, jobs)
+        ex = np.concatenate(parts)
+        O.tacaw_intensity(ex, None)
+        t = time.perf_counter() - t0
+    units = float(w.nx) * w.ny * n_sl * n_frames
+    return {"value": units / t / 1e9, "unit": UNIT, "cores": len(jobs), "kind": "oracle",
+            "sample": f"{n_frames} of {w.n_frames} frames x 1 of {w.n_probes} probe(s) x first {n_sl} of {w.n_slices} "
+                      f"slices, positions -> potentials -> exit waves -> |Psi(k,w)|^2; float64 NumPy oracle, "
+                      f"{len(jobs)} worker processes (os.cpu_count() = {os.cpu_count()}), {t:.1f} s wall"}, t, units
 
 
 def run_reference(args, w, rank):
     if rank != 0:
         return
-    t_all, u_all = 0.0, 0.0
-    cb = None
-    for _ in range(args.warmup if args.warmup < 2 else 1):
+    t_all, u_all, cb = 0.0, 0.0, None
+    for _ in range(1 if args.warmup > 0 else 0):
         oracle_sample(w, budget_s=2.0)
+    per = max(3.0, min(20.0, 120.0 / max(1, args.steps)))
     for _ in range(max(1, args.steps)):
-        cb, t, u = oracle_sample(w, budget_s=max(2.0, 60.0 / max(1, args.steps)))
+        cb, t, u = oracle_sample(w, budget_s=per)
         t_all += t; u_all += u
     val = u_all / t_all / 1e9
     cb["value"] = val
@@ -150,49 +193,98 @@ def run_reference(args, w, rank):
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * t_all / max(1, args.steps), "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": w.name, "note": "float64 NumPy oracle on host cores; each step is a bounded sample"},
+        "config": workload_config(w, note="float64 NumPy oracle on the host cores; each step is a bounded sample"),
         "cpu_baseline": cb,
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0}))
 
 
-# --------------------------------------------------------------------------------------------- ps_tacaw alone
+def workload_config(w, **extra):
+    d = {"workload": w.label, "grid": [w.nx, w.ny], "n_slices": w.n_slices, "frames": w.n_frames, "probes": w.n_probes,
+         "atoms": int(w.n_atoms), "kV": w.kV}
+    d.update(extra)
+    return d
+
+
+def build_workload(args):
+    w = make_workload(args.workload, n_frames=args.frames, grid=args.grid, n_probes_side=args.probes_side)
+    w.label = w.name
+    if w.beam == "probe" and args.probe_chunk and args.probe_chunk < w.n_probes:
+        w.probe_xy = w.probe_xy[:args.probe_chunk]                # one scan row (x fixed, 16 y positions)
+        w.label = f"{w.name}: one {args.probe_chunk}-probe scan row x {w.n_frames} frames"
+    if args.frames or args.grid or args.probes_side:
+        w.label += " (size overridden)"
+    return w
+
+
+# --------------------------------------------------------------------------------------------- micro benches
+def _event_time(torch, fn, flush, reps=5, warm=3):
+    for _ in range(warm):
+        fn()
+    ts = []
+    for _ in range(reps):
+        flush.zero_()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(); fn(); b.record()
+        torch.cuda.synchronize()
+        ts.append(a.elapsed_time(b))
+    return float(np.median(ts))
+
+
 def tacaw_micro():
-    """ps_tacaw on random complex64 stacks [P][F][n][n] (every pixel non-zero; only in-band pixels are read):
-    median of 5 runs after 3 warm-ups, L2 flushed between runs; one JSON line per shape."""
+    """ps_tacaw (path A) and ps_tacaw_add (path B) alone on random complex64 stacks (every pixel non-zero; only
+    in-band pixels are read): median of 5 runs after 3 warm-ups, L2 flushed between runs; one JSON line per shape."""
     import torch
     import paper_2602_10064_b200 as ps
-    peak, _ = measured_peaks()
+    from paper_2602_10064_b200.binding import TacawStream
+    peak, _, _ = measured_peaks()
     flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")
     w0 = make_workload("c1_si_128", mini=True)
     nl, ng, coef = form_factor_coefficients(w0.elements, w0.ff_kind)
-    for P, F, n, nb in [(1, 512, 256, 50), (1, 512, 256, 512), (4, 1024, 512, 1024), (4, 1024, 512, 128), (1, 2048, 512, 2048),
-                        (1, 4096, 256, 256), (8, 256, 512, 256), (16, 128, 512, 128), (1, 256, 1024, 256)]:
+
+    def ctx_for(n):
         ctx = ps.Context(0)
         ctx.set_form_factors(w0.elements, nl, ng, coef)
         ctx.set_geometry(np.array([n * 0.1, n * 0.1, 8.0]), n, n, 2.0)
+        return ctx
+
+    for P, F, n, nb in [(1, 512, 256, 50), (1, 512, 256, 512), (16, 1024, 512, 1024), (4, 1024, 512, 128),
+                        (1, 2048, 512, 2048), (1, 4096, 256, 256), (8, 256, 512, 256), (16, 128, 512, 128),
+                        (1, 256, 1024, 256), (1, 64, 128, 64)]:
+        ctx = ctx_for(n)
         ex = torch.view_as_complex(torch.randn((P, F, n, n, 2), device="cuda"))
         bins = None if nb == F else np.arange(nb, dtype=np.int32)
         I = torch.empty((P, nb, n, n), dtype=torch.float32, device="cuda")
-        for _ in range(3):
-            ps.ps_tacaw(ctx, ex, 2.0, bins, d_I=I)
-        ts = []
-        for _ in range(5):
-            flush.zero_()
-            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            a.record(); ps.ps_tacaw(ctx, ex, 2.0, bins, d_I=I); b.record()
-            torch.cuda.synchronize()
-            ts.append(a.elapsed_time(b))
-        ms = float(np.median(ts))
+        ms = _event_time(torch, lambda: ps.ps_tacaw(ctx, ex, 2.0, bins, d_I=I), flush)
         nk = ctx.n_k_aperture
         byts = (8.0 * F + 4.0 * nb) * nk * P + 4.0 * nb * (n * n - nk) * P
         print(json.dumps({"micro": "ps_tacaw", "P": P, "frames": F, "grid": n, "bins": nb, "ms": ms,
                           "algorithmic_GB": byts / 1e9, "GBps": byts / ms / 1e6, "frac_of_hbm_peak": byts / ms / 1e6 / peak}))
         del ex, I, ctx
+    # path B: one 64-frame chunk of a 4096-frame stream, 256 bins (config 4's shape) and a 1024^2 grid
+    for n, Fc, nb in [(1024, 64, 256), (512, 64, 256), (1024, 64, 64)]:
+        ctx = ctx_for(n)
+        ex = torch.view_as_complex(torch.randn((1, Fc, n, n, 2), device="cuda"))
+        ts = TacawStream(ctx, 1, 4096, 2.0, np.arange(nb, dtype=np.int32))
+        ts.add(ex, 0)
+        state = {"f": Fc}
+
+        def add():
+            ts.add(ex, state["f"]); state["f"] += Fc
+
+        ms = _event_time(torch, add, flush, reps=5, warm=3)
+        nk = ctx.n_k_aperture
+        byts = 8.0 * Fc * nk + 2.0 * 8.0 * nb * nk                  # exit values once + accumulators read and written
+        fma = 4.0 * Fc * nb * nk
+        sm_clock = 1.965e9
+        print(json.dumps({"micro": "ps_tacaw_add", "grid": n, "chunk_frames": Fc, "bins": nb, "ms": ms,
+                          "algorithmic_GB": byts / 1e9, "frac_of_hbm_peak": byts / ms / 1e6 / peak,
+                          "fma_per_s": fma / ms * 1e3, "frac_of_fp32_fma_peak": fma / ms * 1e3 / (N_SM * LANES_PER_SM * sm_clock)}))
+        del ex, ts, ctx
 
 
 # --------------------------------------------------------------------------------------------- configs 3 / 4 at full size
-def full_config(which):
+def full_config(which, quiet=False):
     """Config 4: 4096 frames x 1024^2 x 120 slices, V built and propagated 64 frames at a time, exit waves folded into the
     streaming per-bin DFT (path B, 256 bins) chunk by chunk (SURVEY.md 8(d) capacity plan).  Config 3: 1024 frames x
     256 probes x 512^2 x 80 slices: V of all frames resident (86 GB), probes 16 at a time (34 GB of exit waves),
@@ -212,6 +304,7 @@ def full_config(which):
     Z_d = torch.from_numpy(w.Z.copy()).cuda()
     t_host = time.perf_counter() - t_host
     a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.reset_peak_memory_stats()
     l0 = ctx.launches
     if which == "c4":
         chunk = 64
@@ -261,36 +354,51 @@ def full_config(which):
         plan = f"V of all {F} frames resident (86 GB); {P // pc} chunks of {pc} probes: incident -> multislice (34 GB) -> ps_tacaw -> reductions"
     sec = a.elapsed_time(b) * 1e-3
     units = float(nx) * ny * S * F * P
-    print(json.dumps({"full_config": w.name, "grid": [nx, ny], "n_slices": S, "frames": F, "probes": P, "atoms": int(w.n_atoms),
-                      "tacaw_end_to_end_s": sec, "value": units / sec / 1e9, "unit": UNIT, "plan": plan,
-                      "gpu_launches": int(ctx.launches - l0), "host_setup_s": t_host, "checksum_spectrum_image": check,
-                      "hbm_peak_allocated_GB": torch.cuda.max_memory_allocated() / 1e9}))
+    out = {"full_config": w.name, "grid": [nx, ny], "n_slices": S, "frames": F, "probes": P, "atoms": int(w.n_atoms),
+           "tacaw_end_to_end_s": sec, "value": units / sec / 1e9, "unit": UNIT, "plan": plan,
+           "gpu_launches": int(ctx.launches - l0), "host_setup_s": t_host, "checksum_spectrum_image": check,
+           "hbm_peak_allocated_GB": torch.cuda.max_memory_allocated() / 1e9}
+    del V, ex, I, ctx, pos_d
+    torch.cuda.empty_cache()
+    if not quiet:
+        print(json.dumps(out))
+    return out
 
 
 # --------------------------------------------------------------------------------------------- our arm
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="c2_hbn_256")
+    ap.add_argument("--workload", default="c3_si_probe_512")
+    ap.add_argument("--probe-chunk", type=int, default=16,
+                    help="probe workloads: probes per step (default: one 16-probe scan row, the chunk the full run loops over)")
     ap.add_argument("--frames", type=int, default=None, help="override the number of frames (parity/debug only)")
     ap.add_argument("--grid", type=int, default=None, help="override the grid size (config 5 sweeps 256..2048)")
     ap.add_argument("--probes-side", type=int, default=None, help="override probes per scan side / number of tilts")
     ap.add_argument("--wave-chunk", type=int, default=0)
+    ap.add_argument("--tune", action="append", default=[], metavar="KEY=VALUE",
+                    help="ps_set_tuning knob (col_c, row_light); repeatable")
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="N > 1: weak = an independent trajectory per rank (reductions averaged); strong = ONE problem "
+                         "sharded by sharding.plan() (probe shards, or frame shards + reduce-scatter of the accumulators)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--with-full-configs", action="store_true",
+                    help="also run configs 3 and 4 at their FULL size after the timed steps and carry their end-to-end "
+                         "seconds in the same JSON line (adds about two minutes)")
     ap.add_argument("--full-config", choices=["c3", "c4"], default=None,
                     help="run config 3 or 4 at its FULL size (all frames, all probes) in chunks that fit 180 GB, one step, "
-                         "and print one JSON line (minutes of host-side trajectory generation before the timed region)")
+                         "and print one JSON line")
     ap.add_argument("--tacaw-micro", action="store_true",
-                    help="time ps_tacaw alone on synthetic stacks of several shapes (profiles/r1_tacaw_kernels.md) and exit")
+                    help="time ps_tacaw / ps_tacaw_add alone on synthetic stacks of several shapes and exit")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
-    w = make_workload(args.workload, n_frames=args.frames, grid=args.grid, n_probes_side=args.probes_side)
+    w = build_workload(args)
 
     if args.impl == "reference":
         run_reference(args, w, rank)
@@ -305,6 +413,7 @@ def main():
     import torch
     import torch.distributed as dist
     import paper_2602_10064_b200 as ps
+    from paper_2602_10064_b200 import sharding
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
@@ -312,6 +421,11 @@ def main():
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     dev = torch.device("cuda", local_rank)
+
+    if world > 1 and args.scaling == "strong":
+        sharding.run_strong_bench(args, w, rank, world, dev, ps, METRIC, UNIT)
+        dist.destroy_process_group()
+        return
 
     # ---- inputs: an independent seeded trajectory per rank (rank 0 = the workload's own seed)
     if rank > 0:
@@ -323,12 +437,20 @@ def main():
     bins = w.bins if w.bins is not None else None
     nb = F if bins is None else len(bins)
 
+    need = 4.0 * F * S * ny * nx + 8.0 * P * F * ny * nx + 4.0 * P * nb * ny * nx
+    free_b, _ = torch.cuda.mem_get_info()
+    if need > 0.97 * free_b:
+        raise SystemExit(f"workload needs {need / 1e9:.0f} GB of HBM (V + exit waves + I), {free_b / 1e9:.0f} GB free")
+
     ctx = ps.Context(local_rank)
     nl, ng, coef = form_factor_coefficients(w.elements, w.ff_kind)
     ctx.set_form_factors(w.elements, nl, ng, coef)
     ctx.set_geometry(w.cell, nx, ny, w.slice_dz)
     if args.wave_chunk:
         ctx.set_wave_chunk(args.wave_chunk)
+    for kv in args.tune:
+        k, v = kv.split("=")
+        ctx.set_tuning(k, int(v))
 
     pos_d = pos_h.to(dev)
     Z_d = Z_h.to(dev)
@@ -343,8 +465,12 @@ def main():
     kx_path = np.linspace(0.0, 0.9 * kc, n_path); ky_path = np.zeros(n_path)
     disp = torch.empty((nb, n_path), dtype=torch.float32, device=dev)
     qb = torch.empty((nb, n_q), dtype=torch.float32, device=dev)
-    I_h = torch.empty(I.shape, dtype=torch.float32).pin_memory()
-    red_h = [torch.empty(t.shape, dtype=torch.float32).pin_memory() for t in (sdp, simg, disp, qb)]
+    red_d = (sdp, simg, disp, qb)
+    red_h = [torch.empty(t.shape, dtype=torch.float32).pin_memory() for t in red_d]
+    # what a caller keeps: the whole I(k,w) cube when it is small (plane-wave / tilt runs look at it directly), only the
+    # reductions for probe scans (config 3's cube is 17 GB per 16-probe row, 275 GB per scan: it is never kept)
+    keep_cube = I.numel() * 4 <= (1 << 30)
+    I_h = torch.empty(I.shape, dtype=torch.float32).pin_memory() if keep_cube else None
     flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)      # > 126 MB L2
 
     if w.beam == "probe":
@@ -359,18 +485,20 @@ def main():
         ps.ps_make_incident(ctx, w.kV, d_psi0=psi0, **inc)
         ps.ps_multislice(ctx, w.kV, psi0, V, d_exit=exitw)
         ps.ps_tacaw(ctx, exitw, w.dt_fs, bins, d_I=I)
-        if world > 1:
-            dist.all_reduce(I)                                   # trajectory averaging (sum)
         ps.ps_sdp(ctx, I, 1, min(8, nb - 1), d_out=sdp)
         ps.ps_spectrum_image(ctx, I, 0.0, 0.0, d_out=simg)
         ps.ps_dispersion(ctx, I, kx_path, ky_path, d_out=disp)
         ps.ps_qbin(ctx, I, kc / n_q, n_q, d_out=qb)
+        if world > 1:                                            # trajectory averaging: the reductions are
+            for t in red_d:                                      # linear in I, so their sum over ranks is the reduction of
+                sharding.all_reduce_sum_(t)                      # the summed I(k,w)
 
     def step_e2e():
         pos_dev = pos_h.to(dev, non_blocking=True)
         step(pos_dev)
-        I_h.copy_(I, non_blocking=True)
-        for h, d in zip(red_h, (sdp, simg, disp, qb)):
+        if keep_cube:
+            I_h.copy_(I, non_blocking=True)
+        for h, d in zip(red_h, red_d):
             h.copy_(d, non_blocking=True)
 
     def barrier():
@@ -378,7 +506,7 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    def timed(fn, K, profile=False):
+    def timed(fn, K):
         """K steps, each bracketed by its own event pair, L2 flushed (outside the pairs) between steps."""
         evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
         barrier()
@@ -389,13 +517,10 @@ def main():
             b.record()
         barrier()
         ms = sum(a.elapsed_time(b) for a, b in evs)
-        if world > 1:
-            t = torch.tensor([ms], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
-        return ms
+        return sharding.max_over_ranks(ms, device=dev) if world > 1 else ms
 
-    for _ in range(max(3, args.warmup)):
+    W = max(3, args.warmup)
+    for _ in range(W):
         step(pos_d)
     barrier()
 
@@ -415,80 +540,115 @@ def main():
     ms_e2e = timed(step_e2e, K)
     e2e_value = units_rank * world * K / (ms_e2e * 1e-3) / 1e9
     h2d = pos_h.numel() * 4
-    d2h = I_h.numel() * 4 + sum(h.numel() * 4 for h in red_h)
+    d2h = (I_h.numel() * 4 if keep_cube else 0) + sum(h.numel() * 4 for h in red_h)
 
-    # ---- per-kernel device time (library-side CUDA events on its stream), same K steps
+    # ---- per-kernel device time (library-side CUDA events on its stream), a second pass of the same K steps
     ctx.profile_read(reset=True)
     ctx.profile_enable(True)
     ms_prof_total = timed(lambda: step(pos_d), K)
     prof = ctx.profile_read(reset=True)
     ctx.profile_enable(False)
 
-    peak, peak_src = measured_peaks()
-    px_slices_per_step = units_rank
+    peak, bf16_peak, peak_src = measured_peaks()
+    stats = kernel_stats()
     kern = {k: v for k, v in prof.items() if v[1] > 0}
-    dom = max(("k_row_transmit", "k_col_propagate"), key=lambda k: kern.get(k, (0.0, 0))[0])
+    # algorithmic bytes per pixel of one wave and slice: the wave is read and written once per pass on the
+    # k-columns that hold in-band points (f_col of them); V is read once per FRAME (its rows are shared by the P probes
+    # of the frame inside a launch), i.e. 4/P bytes per pixel of one wave
+    f_col = band_columns(w.cell, nx, ny) / nx
+    alg = {"k_row_transmit": 16.0 * f_col + 4.0 / P, "k_col_propagate": 16.0 * f_col}
+    dom = max(alg, key=lambda k: kern.get(k, (0.0, 0))[0])
     dom_ms, dom_n = kern[dom]
-    alg_bytes_launch = (ROW_BYTES if dom == "k_row_transmit" else COL_BYTES) * px_slices_per_step * K / dom_n
+    px_waves_per_launch = units_rank * K / dom_n
+    alg_bytes_launch = alg[dom] * px_waves_per_launch
     achieved = alg_bytes_launch / (dom_ms / dom_n * 1e-3) / 1e9
     ms_pair = kern["k_row_transmit"][0] + kern["k_col_propagate"][0]
-    pair_gbs = (ROW_BYTES + COL_BYTES) * px_slices_per_step * K / (ms_pair * 1e-3) / 1e9
-    traffic = None                                              # DRAM bytes per launch of that kernel, from ncu
-    tj = {}
-    tpath = os.path.join(ROOT, "profiles", "r1_traffic.json")
-    if w.name == "c2_hbn_256" and args.frames is None and args.grid is None and not args.wave_chunk and os.path.exists(tpath):
-        with open(tpath) as fh:
-            tj = json.load(fh)["dram_bytes_per_launch"]
-        traffic = next((v for k, v in tj.items() if k.startswith(dom + "<") and k.endswith(", 0>")), None)
-    roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
+    pair_gbs = (alg["k_row_transmit"] + alg["k_col_propagate"]) * units_rank * K / (ms_pair * 1e-3) / 1e9
+    sm_clock = (clocks.get("sm_mhz") or 1965.0) * 1e6
+
+    def co_limits(kname, n_grid, ms_launch):
+        """ncu-derived constants of this kernel at this grid size -> DRAM traffic per launch and FP32-issue utilisation."""
+        st = stats.get(f"{kname}<{n_grid}>")
+        if not st:
+            return None, None
+        px_s = px_waves_per_launch / (ms_launch * 1e-3)
+        issue = {"thread_inst_per_px": st["thread_inst_per_px"],
+                 "peak_thread_inst_per_s": N_SM * LANES_PER_SM * sm_clock,
+                 "frac": st["thread_inst_per_px"] * px_s / (N_SM * LANES_PER_SM * sm_clock),
+                 "note": "thread instructions per pixel (ncu, profiles/r2_kernel_stats.json) x pixels/s / (148 SMs x 128 "
+                         "lanes x SM clock sampled in this run): the FP32-issue co-limit of the FFT passes"}
+        traffic = st["dram_bytes_per_px"].get(str(P), st["dram_bytes_per_px"].get("any"))
+        return (traffic * px_waves_per_launch if traffic is not None else None), issue
+
+    traffic, issue = co_limits(dom, nx if dom == "k_row_transmit" else ny, dom_ms / dom_n)
+    roofline = {"bound": "hbm", "kernel": f"{dom}<{nx if dom == 'k_row_transmit' else ny}>", "achieved": achieved,
+                "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
                 "bytes_per_launch": alg_bytes_launch, "avg_launch_ms": dom_ms / dom_n,
+                "algorithmic_bytes_per_px": alg[dom], "band_column_fraction": f_col,
+                "fp32_issue": issue,
                 "slice_step_pair": {"achieved": pair_gbs, "frac": pair_gbs / peak,
-                                    "gpx_slice_s": px_slices_per_step * K / (ms_pair * 1e-3) / 1e9},
+                                    "gpx_slice_s": units_rank * K / (ms_pair * 1e-3) / 1e9,
+                                    "algorithmic_bytes_per_px_slice": alg["k_row_transmit"] + alg["k_col_propagate"]},
                 "kernel_ms_per_step": {k: v[0] / K for k, v in kern.items()},
+                "kernel_times_from": "a second pass of the same K steps with per-launch CUDA events recorded by the library "
+                                     "on its stream (ps_profile_*), not the pass `value` was timed on",
                 "profiled_ms_per_step": ms_prof_total / K}
+    other = "k_col_propagate" if dom == "k_row_transmit" else "k_row_transmit"
+    o_ms, o_n = kern[other]
+    o_tr, o_issue = co_limits(other, ny if other == "k_col_propagate" else nx, o_ms / o_n)
+    o_ach = alg[other] * px_waves_per_launch / (o_ms / o_n * 1e-3) / 1e9
+    roofline["other_pass"] = {"kernel": other, "achieved": o_ach, "frac": o_ach / peak, "traffic": o_tr,
+                              "avg_launch_ms": o_ms / o_n, "fp32_issue": o_issue}
     if "k_tacaw_fft" in kern:
         tb = (8.0 * F + 4.0 * nb) * ctx.n_k_aperture * P + 4.0 * nb * (nx * ny - ctx.n_k_aperture) * P
         tms = kern["k_tacaw_fft"][0] / kern["k_tacaw_fft"][1]
+        tst = stats.get(f"k_tacaw<{F}>")
         roofline["tacaw"] = {"achieved": tb / (tms * 1e-3) / 1e9, "frac": tb / (tms * 1e-3) / 1e9 / peak,
                              "bytes_per_launch": tb, "avg_launch_ms": tms,
-                             "traffic": next((v for k, v in tj.items() if k.startswith("k_tacaw_tma") or k.startswith("k_tacaw_fft")), None)}
-
+                             "traffic": (tst["dram_bytes_per_algorithmic_byte"] * tb) if tst else None}
     if "k_vk" in kern:
         # V(k) structure-factor sums: 4 real sums per quarter-plane point and atom, x3 for the 3xTF32 split (tensor path)
-        bf16 = 1590.0                                           # fallback of B200_PROFILING.md
-        mp = os.path.join(ROOT, "MEASURED_PEAKS.json")
-        if os.path.exists(mp):
-            with open(mp) as fh:
-                bf16 = float(json.load(fh).get("bf16_tflops", bf16))
         flop = 24.0 * (ctx.n_k_aperture / 4.0) * float(w.n_atoms) * F
         tms = kern["k_vk"][0] / K
         roofline["vk"] = {"bound": "tensor", "unit": "TFLOP/s", "achieved": flop / (tms * 1e-3) / 1e12,
-                          "peak": 0.5 * bf16, "frac": flop / (tms * 1e-3) / 1e12 / (0.5 * bf16),
+                          "peak": 0.5 * bf16_peak, "frac": flop / (tms * 1e-3) / 1e12 / (0.5 * bf16_peak),
                           "note": "algorithmic 3xTF32 flops over the in-aperture quarter plane; peak = measured bf16 x 0.5 "
                                   "(guide's nominal tf32:bf16 ratio); FP32 path when ps_set_vk_mode(1) or few atoms per slice"}
 
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        cpu_baseline, _, _ = oracle_sample(make_workload(args.workload, n_frames=args.frames, grid=args.grid,
-                                                           n_probes_side=args.probes_side))
+        cpu_baseline, _, _ = oracle_sample(w)
+
+    cube_gb = I.numel() * 4 / 1e9
+    full = None
+    if rank == 0 and world == 1 and args.with_full_configs:
+        del V, exitw, I, psi0
+        torch.cuda.empty_cache()
+        full = {k: full_config(k, quiet=True) for k in ("c3", "c4")}
 
     if rank == 0:
-        print(json.dumps({
-            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": max(3, args.warmup),
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "complex64 (f32)", "data": "synthetic",
-            "config": {"workload": w.name, "grid": [nx, ny], "n_slices": S, "frames": F, "probes": P,
-                       "atoms": int(w.n_atoms), "kV": w.kV, "omega_bins": nb,
-                       "l2": "256 MiB buffer written between timed steps (L2 flush); per-step CUDA events",
-                       "parallelism": f"independent trajectory per GPU x{world}, one all-reduce of I(k,w)"},
+            "config": workload_config(w, omega_bins=nb,
+                                      l2="256 MiB buffer written between timed steps (L2 flush); per-step CUDA events",
+                                      hbm_resident_GB=need / 1e9,
+                                      parallelism=f"independent trajectory per GPU x{world}, one all-reduce of the reductions"),
             "tacaw_end_to_end_s": ms_total / K * 1e-3,
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": ms_e2e / K, "h2d_bytes_per_step": h2d,
-                    "d2h_bytes_per_step": d2h},
+                    "d2h_bytes_per_step": d2h,
+                    "copied_back": ("I(k,w) cube + " if keep_cube else "") +
+                                   "spectral diffraction pattern, spectrum image, dispersion, q-bins" +
+                                   ("" if keep_cube else f" (the {cube_gb:.0f} GB I(k,w) cube of a probe chunk "
+                                                         "is reduced on the device and never kept: 275 GB per 256-probe scan)")},
             "gpu_launches": int(launches),
             "roofline": roofline,
-            "cpu_baseline": cpu_baseline}))
+            "cpu_baseline": cpu_baseline}
+        if full:
+            line["full_configs"] = full
+        print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
 

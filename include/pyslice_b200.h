@@ -18,8 +18,23 @@
  * Conventions
  *   - Every pointer named d_* is DEVICE memory owned by the caller (e.g. a torch tensor);
  *     every other pointer is HOST memory, read during the call and never retained.
- *   - All hot-path calls are asynchronous on the stream given to ps_create(); the library
- *     never synchronises the device on the hot path and never frees caller memory.
+ *   - All hot-path calls enqueue their work on the stream given to ps_create() and return; the
+ *     library never frees caller memory.  WHEN A CALL MAY BLOCK THE HOST (and only then):
+ *       (a) set-up: ps_set_geometry, and the first hot-path call after a change of geometry,
+ *           voltage, form factors or aberration coefficients (tables are rebuilt on the host);
+ *       (b) growth: a call that needs more library-owned scratch than any earlier call
+ *           (the buffer is re-allocated after a stream wait);
+ *       (c) ps_build_slices the first time it sees a (d_Z, n_atoms) pair: one 4-byte read-back
+ *           validates the atomic numbers before any work is queued;
+ *       (d) ps_profile_read, ps_destroy.
+ *     A repeated call with the same parameters and sizes ("warmed up") never waits for the
+ *     device: small host tables (bin lists, tilt indices, probe positions, path points) are
+ *     copied into a page-locked staging ring owned by the ctx and sent with cudaMemcpyAsync,
+ *     so host arrays are never retained past the call.
+ *   - Asynchronous errors: ps_build_slices re-checks every atomic number on the device in
+ *     every call; an unknown Z met by a call that did not validate synchronously (case c) is
+ *     raised through a page-locked word and reported as PS_EUNSUPPORTED by the next ps_* call
+ *     on the ctx that observes it.
  *   - Scratch memory the library needs is allocated by the ctx itself (cudaMalloc, grown
  *     on demand, freed by ps_destroy) unless the caller installs a workspace with
  *     ps_set_workspace().
@@ -31,7 +46,9 @@
  *   - Band limit (A10): A(k) = [kx^2+ky^2 <= kc^2], kc = (2/3) min(nx/(2Lx), ny/(2Ly)),
  *     applied in every propagator, to V(k) and to the probe.
  *   - Results are deterministic for fixed inputs (no floating-point atomics anywhere).
- *   - One ctx per host thread.
+ *   - One ctx per host thread at a time; ctxs share no state (kernel attributes and
+ *     occupancy figures are cached per ctx, i.e. per device), so one process may drive several
+ *     devices or threads with one ctx each.  Every call makes the ctx's device current.
  */
 #ifndef PYSLICE_B200_H
 #define PYSLICE_B200_H
@@ -61,13 +78,17 @@ typedef enum {
     PS_ESTATE = -5         /* call order violated (geometry / form factors not set, ...)       */
 } ps_status;
 
-/* exit-wave layouts accepted by ps_multislice / ps_tacaw */
+/* exit-wave layouts accepted by ps_multislice / ps_tacaw / ps_haadf */
 #define PS_LAYOUT_DENSE 0  /* complex64 [P][F][ny][nx], k-space, FFT index order (A13)        */
+/* SURVEY.md 8(b) also sketched PS_LAYOUT_TILED_APERTURE (only the in-aperture k points, tiled for the
+ * time transform: same values, 0.35x the bytes).  It is NOT offered: pixels outside the band limit
+ * are written as exact zeros in the dense layout and are skipped (never read) by ps_tacaw, ps_haadf
+ * and the streaming path, so the compact layout would save capacity only (config 3: 12 instead of
+ * 34 GB per 16-probe chunk), not traffic; the time-major tiling measured no faster
+ * (profiles/r1_tacaw_kernels.md).  Any other value of `exit_layout` returns PS_EUNSUPPORTED. */
 
 /* ---------------------------------------------------------------- life cycle */
 
-/* One context per host thread and one CUDA device per process (the multi-GPU model is one process per GPU): kernel
- * attributes and occupancy-derived grid sizes are cached per process on first use. */
 /* Create a context bound to CUDA device `device` and to `cuda_stream` (a cudaStream_t; NULL =
  * the legacy default stream).  Fails with PS_ECUDA when no usable device exists. */
 PS_API ps_status ps_create(ps_ctx** out, int device, void* cuda_stream);
@@ -94,8 +115,13 @@ PS_API ps_status ps_set_geometry(ps_ctx* ctx, const double cell[3], int nx, int 
 /* n_k_aperture = number of grid points with A(k) = 1.  Any out pointer may be NULL. */
 PS_API ps_status ps_get_geometry(const ps_ctx* ctx, int* n_slices, double* dz_eff, int* n_k_aperture);
 
-/* Scratch needed by ps_build_slices on `n_frames_chunk` frames at a time (the only call that
- * needs scratch).  ps_set_workspace installs caller-owned device memory (d_ws == NULL removes
+/* Scratch needed by ps_build_slices on `n_frames_chunk` frames of `n_atoms` atoms at a time (the
+ * only call that needs scratch: fixed-point coordinates and sort keys, 5 x 4 B per atom-frame,
+ * plus V(k) and the mixed array of the inverse transform, which depend on the geometry alone).
+ * NOTE: SURVEY.md 8(b) sketched the second argument as `n_probes_chunk`; the probe count does not
+ * enter any scratch size here (ps_multislice propagates in place inside d_exit and needs none),
+ * while the atom count does, so the argument is `n_atoms`.  Returns 0 before geometry and form
+ * factors are set.  ps_set_workspace installs caller-owned device memory (d_ws == NULL removes
  * it and returns the ctx to self-allocation).  ps_build_slices processes frames in chunks that
  * fit whatever scratch is available. */
 PS_API size_t    ps_workspace_bytes(const ps_ctx* ctx, int n_frames_chunk, int n_atoms);
@@ -105,6 +131,13 @@ PS_API ps_status ps_set_workspace(ps_ctx* ctx, void* d_ws, size_t bytes);
  * the 126 MB L2 between the two FFT passes of a slice; a large one amortises launch costs).
  * 0 = library default = the whole batch in one launch per pass (profiles/r1_chunk_sweep.md). */
 PS_API ps_status ps_set_wave_chunk(ps_ctx* ctx, int n_waves);
+
+/* Tuning knobs of the slice-step kernels, by name (results are identical to rounding order; the defaults are the
+ * measured optimum per grid size, profiles/r2_slice_step.md):
+ *   "col_c"     columns per block of the column pass: 0 = default, 4 or 8 (4 applies to 512 <= ny <= 1024 only)
+ *   "row_light" 1 = register-light row pass for nx >= 512 (stage-2 twiddles in shared memory, three blocks per SM)
+ * Unknown keys and values are PS_EINVAL. */
+PS_API ps_status ps_set_tuning(ps_ctx* ctx, const char* key, int value);
 
 /* Tuning knob (default off, so that every row of every slice goes through the full transforms): rows of a slice on which V is exactly zero (vacuum) have exp(i sigma V) = 1, and the
  * inverse + forward row transform around it is NX times the identity, so ps_multislice only rescales such rows (an
@@ -167,15 +200,31 @@ PS_API ps_status ps_multislice(ps_ctx* ctx, double kV, const void* d_psi0, int n
 PS_API ps_status ps_tacaw(ps_ctx* ctx, const void* d_exit, int exit_layout, int n_probes, int n_frames, double dt_fs,
                    int n_bins, const int32_t* bins, float* d_I);
 
-/* Streaming variant for frames x grid > HBM (BASELINE config 4): per-bin DFT accumulation over
- * frame chunks.  acc[p][b][k] += sum_j Psi_j e^{-2 pi i n_b j/F}; slot n_bins holds sum_j Psi_j
- * (the mean term).  finish: I = |acc_b - [n_b mod F == 0] * F * mean|^2 (exact for integer bins).
- *   d_acc  complex64 [n_probes][n_bins+1][ny][nx], zeroed by begin; any n_frames_total >= 1. */
+/* Streaming variant for frames x grid > HBM (BASELINE config 4, Suppl. Eq. 5 at PAPER.md:295): per-bin DFT
+ * accumulation over frame chunks,
+ *     acc[p][b][k] += sum_{j in chunk} (Psi_j - ref) e^{-2 pi i n_b j / F},      finish: I = |acc_b|^2, bin 0 := 0.
+ * `ref` is one wave per probe subtracted from every frame (it strips the elastic part so that fp32 partial sums stay
+ * small; over the complete set of F frames a constant shift changes no bin n != 0, and bin 0 of the mean-subtracted
+ * series is zero by definition (A14), so the result equals F_t[Psi - <Psi>_t] for integer bins).  By default ref = the
+ * first frame the stream receives; ps_tacaw_set_reference installs another one (copied; NULL = zeros) — required when
+ * several streams (GPUs) each sum a shard of the frames and their accumulators are added afterwards: all shards must
+ * subtract the SAME wave.
+ *   d_acc  complex64 [n_probes][n_bins][ny][nx], zeroed by begin; any n_frames_total >= 1.
+ * Every exit value of a chunk is read from HBM once; the accumulators are read and written once per 64 frames. */
 PS_API ps_status ps_tacaw_begin(ps_ctx* ctx, int n_probes, int n_frames_total, double dt_fs, int n_bins,
                          const int32_t* bins, void* d_acc);
-/* d_exit_chunk complex64 [n_probes][n_frames_chunk][ny][nx] = frames frame0.. of every probe. */
+/* Optional, after begin and before the first add: d_ref complex64 [n_probes][ny][nx] (device), or NULL for zeros. */
+PS_API ps_status ps_tacaw_set_reference(ps_ctx* ctx, const void* d_ref);
+/* d_exit_chunk complex64 [n_probes][n_frames_chunk][ny][nx] = frames frame0.. of every probe.  Chunks must arrive in
+ * ascending, contiguous frame order (the first chunk may start at any frame: a shard); anything else is PS_ESTATE. */
 PS_API ps_status ps_tacaw_add(ps_ctx* ctx, const void* d_exit_chunk, int frame0, int n_frames_chunk);
+/* PS_ESTATE unless exactly n_frames_total frames were added. */
 PS_API ps_status ps_tacaw_finish(ps_ctx* ctx, float* d_I /* float32 [n_probes][n_bins][ny][nx] */);
+/* Sharded finish (frame shards + reduce-scatter): the caller has summed the accumulators of all shards
+ * (each fed through begin / set_reference / add on its own ctx) and owns n_k of the k points of every (probe, bin):
+ *   d_acc_shard complex64 [n_probes][n_bins][n_k]  ->  d_I_shard float32 [n_probes][n_bins][n_k].
+ * No frame-count check (this ctx saw only its shard); ends the stream like ps_tacaw_finish. */
+PS_API ps_status ps_tacaw_finish_shard(ps_ctx* ctx, const void* d_acc_shard, size_t n_k, float* d_I_shard);
 
 /* a8: reductions over d_I = float32 [P][n_bins][ny][nx] (A15-A17).
  * ps_sdp: spectral diffraction pattern, sum over probes and bins bin_lo..bin_hi inclusive
@@ -210,7 +259,7 @@ PS_API ps_status ps_qbin(ps_ctx* ctx, const float* d_I, int P, int n_bins, doubl
  * per-kernel totals and returns them: names[i] (static strings), ms[i] (summed device time) and
  * launches[i] for i < *n_kernels (arrays of at least 16 entries; any may be NULL); reset != 0 clears
  * the totals afterwards.  Kernel slots: k_bin, k_sort, k_vk, k_v_col, k_v_row, k_incident,
- * k_row_transmit, k_col_propagate, k_tacaw_fft, k_tacaw_accum, k_tacaw_finish, k_reduce. */
+ * k_row_transmit, k_col_propagate, k_tacaw_fft, k_tacaw_accum, k_tacaw_finish, k_reduce, k_slice_resident. */
 PS_API ps_status ps_profile_enable(ps_ctx* ctx, int on);
 PS_API ps_status ps_profile_read(ps_ctx* ctx, int reset, int* n_kernels, const char** names, double* ms,
                                  long long* launches);

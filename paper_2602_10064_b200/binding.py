@@ -31,6 +31,7 @@ _PROTOTYPES = {
     "ps_set_workspace": (C.c_int, [C.c_void_p, C.c_void_p, C.c_size_t]),
     "ps_set_wave_chunk": (C.c_int, [C.c_void_p, C.c_int]),
     "ps_set_vk_mode": (C.c_int, [C.c_void_p, C.c_int]),
+    "ps_set_tuning": (C.c_int, [C.c_void_p, C.c_char_p, C.c_int]),
     "ps_set_vacuum_shortcut": (C.c_int, [C.c_void_p, C.c_int]),
     "ps_set_aberrations": (C.c_int, [C.c_void_p, C.c_void_p]),
     "ps_apply_aberrations": (C.c_int, [C.c_void_p, C.c_double, C.c_void_p, C.c_longlong]),
@@ -39,8 +40,10 @@ _PROTOTYPES = {
     "ps_multislice": (C.c_int, [C.c_void_p, C.c_double, C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_void_p, C.c_int]),
     "ps_tacaw": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_double, C.c_int, C.c_void_p, C.c_void_p]),
     "ps_tacaw_begin": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_double, C.c_int, C.c_void_p, C.c_void_p]),
+    "ps_tacaw_set_reference": (C.c_int, [C.c_void_p, C.c_void_p]),
     "ps_tacaw_add": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_int]),
     "ps_tacaw_finish": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "ps_tacaw_finish_shard": (C.c_int, [C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]),
     "ps_sdp": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_void_p]),
     "ps_spectrum_image": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_double, C.c_double, C.c_void_p]),
     "ps_haadf": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_void_p]),
@@ -209,6 +212,10 @@ class Context:
         """0 auto, 1 FP32 SIMT structure-factor sums, 2 tcgen05 3xTF32 sums."""
         self._check(self._lib.ps_set_vk_mode(self._h, int(mode)))
 
+    def set_tuning(self, key: str, value: int):
+        """Named tuning knobs of the slice-step kernels ("col_c", "row_light"); see include/pyslice_b200.h."""
+        self._check(self._lib.ps_set_tuning(self._h, key.encode(), int(value)))
+
     def set_wave_chunk(self, n_waves: int):
         self._check(self._lib.ps_set_wave_chunk(self._h, int(n_waves)))
 
@@ -282,8 +289,15 @@ class TacawStream:
         self.ctx = ctx
         bh, bp = _host(bins, np.int32)
         self.n_bins, self.P = int(bh.shape[0]), int(n_probes)
-        self.d_acc = torch.empty((n_probes, self.n_bins + 1, ctx.ny, ctx.nx), dtype=torch.complex64, device=ctx.device)
+        self.d_acc = torch.empty((n_probes, self.n_bins, ctx.ny, ctx.nx), dtype=torch.complex64, device=ctx.device)
         ctx._check(ctx._lib.ps_tacaw_begin(ctx._h, n_probes, int(n_frames_total), float(dt_fs), self.n_bins, bp, _ptr(self.d_acc)))
+
+    def set_reference(self, d_ref):
+        """complex64 [P][ny][nx] wave subtracted from every frame (None = zeros); before the first add."""
+        import torch
+        if d_ref is not None:
+            _need(d_ref, torch.complex64, "d_ref")
+        self.ctx._check(self.ctx._lib.ps_tacaw_set_reference(self.ctx._h, _ptr(d_ref)))
 
     def add(self, d_exit_chunk, frame0: int):
         import torch
@@ -296,6 +310,16 @@ class TacawStream:
             d_I = torch.empty((self.P, self.n_bins, self.ctx.ny, self.ctx.nx), dtype=torch.float32, device=self.ctx.device)
         self.ctx._check(self.ctx._lib.ps_tacaw_finish(self.ctx._h, _ptr(d_I)))
         return d_I
+
+    def finish_shard(self, d_acc_shard, d_I_shard=None):
+        """complex64 [P][n_bins][n_k] (summed over all shards by the caller) -> float32 [P][n_bins][n_k]."""
+        import torch
+        _need(d_acc_shard, torch.complex64, "d_acc_shard")
+        if d_I_shard is None:
+            d_I_shard = torch.empty(d_acc_shard.shape, dtype=torch.float32, device=self.ctx.device)
+        _need(d_I_shard, torch.float32, "d_I_shard")
+        self.ctx._check(self.ctx._lib.ps_tacaw_finish_shard(self.ctx._h, _ptr(d_acc_shard), int(d_acc_shard.shape[-1]), _ptr(d_I_shard)))
+        return d_I_shard
 
 
 def ps_sdp(ctx: Context, d_I, bin_lo: int, bin_hi: int, d_out=None):

@@ -25,6 +25,65 @@ ps_status ensure_buf(ps_ctx* c, DeviceBuf& b, size_t bytes) {
     return PS_OK;
 }
 
+// ------------------------------------------------------------------------------------ pinned staging ring
+static constexpr size_t kRingBytes = (size_t)4 << 20;     // 4 MB: the largest steady-state table is a bin list (16 KB)
+
+static cudaEvent_t ring_event(PinnedRing& r) {
+    cudaEvent_t e = nullptr;
+    if (!r.pool.empty()) { e = r.pool.back(); r.pool.pop_back(); return e; }
+    if (cudaEventCreateWithFlags(&e, cudaEventDisableTiming) != cudaSuccess) return nullptr;
+    return e;
+}
+
+ps_status upload_async(ps_ctx* c, void* d_dst, const void* h_src, size_t bytes) {
+    if (bytes == 0) return PS_OK;
+    PinnedRing& r = c->ring;
+    if (!r.base) {
+        PSB_CUDA(c, cudaHostAlloc((void**)&r.base, kRingBytes, cudaHostAllocDefault));
+        r.cap = kRingBytes;
+    }
+    const size_t need = (bytes + 255) & ~(size_t)255;
+    if (need > r.cap / 2) {                                  // a table too large for the ring (set-up paths only): blocking copy
+        PSB_CUDA(c, cudaMemcpyAsync(d_dst, h_src, bytes, cudaMemcpyHostToDevice, c->stream));
+        PSB_CUDA(c, cudaStreamSynchronize(c->stream));
+        return PS_OK;
+    }
+    while (!r.live.empty() && cudaEventQuery(r.live.front().ev) == cudaSuccess) {   // retire finished copies
+        r.pool.push_back(r.live.front().ev);
+        r.live.pop_front();
+    }
+    if (r.head + need > r.cap) r.head = 0;                   // wrap
+    const size_t lo = r.head, hi = r.head + need;
+    while (!r.live.empty() && r.live.front().off < hi && r.live.front().end > lo) {  // oldest copies still own the range
+        PSB_CUDA(c, cudaEventSynchronize(r.live.front().ev));
+        r.pool.push_back(r.live.front().ev);
+        r.live.pop_front();
+    }
+    memcpy(r.base + lo, h_src, bytes);
+    PSB_CUDA(c, cudaMemcpyAsync(d_dst, r.base + lo, bytes, cudaMemcpyHostToDevice, c->stream));
+    cudaEvent_t ev = ring_event(r);
+    if (!ev) return fail(c, PS_ECUDA, "upload_async: cudaEventCreate failed");
+    PSB_CUDA(c, cudaEventRecord(ev, c->stream));
+    r.live.push_back({lo, hi, ev});
+    r.head = hi;
+    return PS_OK;
+}
+
+ps_status enter(ps_ctx* c, const char* who) {
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != c->device) PSB_CUDA(c, cudaSetDevice(c->device));
+    if (c->h_async_err) {
+        const int z = *(volatile int*)c->h_async_err;        // written by k_bin of an earlier asynchronous call
+        if (z != 0) {
+            *(volatile int*)c->h_async_err = 0;
+            return fail(c, PS_EUNSUPPORTED, std::string(who) + ": an earlier ps_build_slices met atomic number " +
+                                                std::to_string(z == -1 ? 0 : z) + " without form-factor coefficients "
+                                                "(its potentials are invalid)");
+        }
+    }
+    return PS_OK;
+}
+
 template <class T>
 static ps_status upload(ps_ctx* c, T** d, const std::vector<T>& h) {
     if (*d) { cudaFree(*d); *d = nullptr; }
@@ -133,6 +192,17 @@ extern "C" ps_status ps_create(ps_ctx** out, int device, void* cuda_stream) {
     if (!c) { g_create_err = "ps_create: out of host memory"; return PS_EINVAL; }
     c->device = device;
     c->stream = (cudaStream_t)cuda_stream;
+    // error word kernels can raise without the host waiting for them: page-locked, mapped into the device
+    if (cudaHostAlloc((void**)&c->h_async_err, sizeof(int), cudaHostAllocMapped) == cudaSuccess) {
+        *c->h_async_err = 0;
+        if (cudaHostGetDevicePointer((void**)&c->d_async_err, c->h_async_err, 0) != cudaSuccess) c->d_async_err = nullptr;
+    }
+    if (!c->d_async_err) {
+        g_create_err = "ps_create: mapped pinned allocation failed";
+        if (c->h_async_err) cudaFreeHost(c->h_async_err);
+        delete c;
+        return PS_ECUDA;
+    }
     *out = c;
     return PS_OK;
 }
@@ -144,7 +214,12 @@ extern "C" void ps_destroy(ps_ctx* c) {
     cudaFree(c->d_nmax); cudaFree(c->d_tiles); cudaFree(c->d_tile_active);
     cudaFree(c->d_ftab); cudaFree(c->d_elem_of_Z);
     cudaFree(c->kv.d_px_mid); cudaFree(c->kv.d_px_last); cudaFree(c->kv.d_py);
-    cudaFree(c->scratch.p); cudaFree(c->misc.p); cudaFree(c->qorder.p); cudaFree(c->ts.d_bins);
+    cudaFree(c->scratch.p); cudaFree(c->misc.p); cudaFree(c->qorder.p); cudaFree(c->ts.d_bins.p); cudaFree(c->ts.d_ref.p); cudaFree(c->ts.d_tw.p);
+    cudaFree(c->path_buf.p); cudaFree(c->inc_buf.p);
+    for (auto& sg : c->ring.live) cudaEventDestroy(sg.ev);
+    for (auto e : c->ring.pool) cudaEventDestroy(e);
+    if (c->ring.base) cudaFreeHost(c->ring.base);
+    if (c->h_async_err) cudaFreeHost(c->h_async_err);
     cudaFree(c->tacaw_groups.p); cudaFree(c->abtab.p); cudaFree(c->tacaw_slot.p);
     for (auto& r : c->prof_pending) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
     for (auto e : c->prof_pool) cudaEventDestroy(e);
@@ -169,6 +244,7 @@ extern "C" ps_status ps_set_form_factors(ps_ctx* c, int n_elem, const int32_t* Z
     c->ffcoef.assign(coef, coef + (size_t)n_elem * ncoef);
     c->have_ff = true;
     c->ftab_valid = false;
+    c->z_checked = nullptr;                                  // the set of known atomic numbers changed
     return PS_OK;
 }
 
@@ -255,6 +331,22 @@ extern "C" ps_status ps_set_vk_mode(ps_ctx* c, int mode) {
     if (!c) return PS_EINVAL;
     if (mode < 0 || mode > 2) return fail(c, PS_EINVAL, "ps_set_vk_mode: mode must be 0 (auto), 1 (FP32 SIMT) or 2 (tcgen05 3xTF32)");
     c->vk_mode = mode;
+    return PS_OK;
+}
+
+extern "C" ps_status ps_set_tuning(ps_ctx* c, const char* key, int value) {
+    if (!c) return PS_EINVAL;
+    if (!key) return fail(c, PS_EINVAL, "ps_set_tuning: key is NULL");
+    const std::string k(key);
+    if (k == "col_c") {
+        if (value != 0 && value != 4 && value != 8) return fail(c, PS_EINVAL, "ps_set_tuning: col_c must be 0 (default), 4 or 8");
+        c->tune_col_c = value;
+    } else if (k == "row_light") {
+        if (value != 0 && value != 1) return fail(c, PS_EINVAL, "ps_set_tuning: row_light must be 0 or 1");
+        c->tune_row_light = value;
+    } else {
+        return fail(c, PS_EINVAL, "ps_set_tuning: unknown key '" + k + "'");
+    }
     return PS_OK;
 }
 

@@ -3,7 +3,10 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <stdio.h>
+#include <string.h>
+#include <deque>
 #include <string>
+#include <unordered_map>
 #include <vector>
 
 #include "../../include/pyslice_b200.h"
@@ -39,12 +42,28 @@ static const char* const kKernelNames[K_COUNT] = {
 
 struct ProfRec { cudaEvent_t a, b; int id; };
 
+// Pinned host staging ring: small host tables (bin lists, tilt indices, path points) are copied into page-locked
+// memory owned by the ctx and sent with cudaMemcpyAsync, so the caller's array need not outlive the call and the
+// hot path never waits for the stream.  A segment is reused only after the event recorded behind its copy has fired
+// (cudaEventSynchronize on wrap-around: reached only if the device is a whole ring of uploads behind).
+struct PinnedRing {
+    struct Seg { size_t off, end; cudaEvent_t ev; };
+    char* base = nullptr;
+    size_t cap = 0, head = 0;
+    std::deque<Seg> live;
+    std::vector<cudaEvent_t> pool;
+};
+
 struct TacawStream {                // state of ps_tacaw_begin/add/finish
     bool active = false;
     int n_probes = 0, n_frames_total = 0, n_bins = 0, frames_seen = 0;
     void* d_acc = nullptr;
-    int32_t* d_bins = nullptr;      // [n_bins] bins mod F (library-owned)
+    DeviceBuf d_bins;               // [n_bins] bins mod F (library-owned)
+    DeviceBuf d_ref;                // complex64 [P][ny][nx] reference wave subtracted from every frame
+    DeviceBuf d_tw;                 // complex64 [chunk frames][n_bins] twiddles of the current chunk
+    bool have_ref = false;
     std::vector<int32_t> bins;
+    int next_frame = 0;             // chunks must arrive in ascending, contiguous frame order
 };
 
 }  // namespace psb
@@ -54,6 +73,10 @@ struct ps_ctx {
     cudaStream_t stream = nullptr;
     std::string err;
     long long launches = 0;
+    psb::PinnedRing ring;                   // staging of small host tables (no host wait on the hot path)
+    std::unordered_map<const void*, int> kern_cap;   // per kernel: resident blocks on this device (attributes set once)
+    int* h_async_err = nullptr;             // mapped pinned word written by kernels (bad atomic number, ...)
+    int* d_async_err = nullptr;             // its device alias
 
     // geometry
     bool have_geom = false;
@@ -71,6 +94,8 @@ struct ps_ctx {
     int wave_chunk = 0;
     int vacuum_shortcut = 0;                // ps_set_vacuum_shortcut: rows with V == 0 skip the transmit + FFT pair (exact)
     int vk_mode = 0;                        // ps_set_vk_mode: 0 auto, 1 FP32 SIMT sums, 2 tcgen05 3xTF32 sums
+    int tune_col_c = 0;                     // ps_set_tuning("col_c"): columns per block of the column pass (0 = default)
+    int tune_row_light = 0;                 // ps_set_tuning("row_light"): register-light row pass (3 blocks per SM)
 
     // form factors
     bool have_ff = false;
@@ -101,7 +126,12 @@ struct ps_ctx {
     int tacaw_n_active = 0, tacaw_n_inactive = 0;
     psb::DeviceBuf tacaw_slot;              // ps_tacaw: output slot of every FFT bin (-1 = not requested)
     std::vector<int32_t> tacaw_slot_host;   // its host copy (uploaded again only when the bin list changes)
-    psb::DeviceBuf misc;                    // small per-call tables (bin slots, path pixels)
+    psb::DeviceBuf misc;                    // detector mask + per-frame partial sums (ps_spectrum_image, ps_haadf)
+    psb::DeviceBuf path_buf;                // ps_dispersion: path points (float64 kx, ky)
+    psb::DeviceBuf inc_buf;                 // ps_make_incident: tilt indices / probe-aperture limits + probe positions
+    std::vector<int32_t> inc_pmax_host;     // last uploaded probe-aperture limits (uploaded again only when they change)
+    const void* z_checked = nullptr;        // ps_build_slices: (d_Z, n_atoms) already validated synchronously
+    int z_checked_n = 0;
     psb::DeviceBuf qorder;                  // ps_qbin: cursor, offsets and pixel order by q bin (cached)
     bool qorder_valid = false;
     double qorder_dq = 0.0;
@@ -159,6 +189,30 @@ inline bool is_pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
 inline int signed_index(int i, int n) { return i < (n + 1) / 2 ? i : i - n; }
 
 ps_status ensure_buf(ps_ctx* c, DeviceBuf& b, size_t bytes);
+// asynchronous upload of a small host table through the ctx's pinned ring (api.cu); never blocks in steady state
+ps_status upload_async(ps_ctx* c, void* d_dst, const void* h_src, size_t bytes);
+// makes c->device current, and reports (once) an error a kernel of an earlier asynchronous call has flagged
+ps_status enter(ps_ctx* c, const char* who);
+
+// Resident-block cap of `kern` on the ctx's device; the first use sets the dynamic shared-memory attribute.  Cached in
+// the ctx (not in a process-wide static): attributes and occupancy are per device, and ctxs of different devices or
+// host threads share nothing.
+template <class K>
+inline cudaError_t kernel_cap(ps_ctx* c, K kern, int threads, size_t smem, int* cap) {
+    const void* key = reinterpret_cast<const void*>(kern);
+    auto it = c->kern_cap.find(key);
+    if (it != c->kern_cap.end()) { *cap = it->second; return cudaSuccess; }
+    if (smem > 48 * 1024) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+    }
+    int per_sm = 1, n_sm = kNumSM;
+    cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, c->device);
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, threads, smem) != cudaSuccess || per_sm < 1) per_sm = 1;
+    *cap = n_sm * per_sm;
+    c->kern_cap.emplace(key, *cap);
+    return cudaSuccess;
+}
 ps_status ensure_kv(ps_ctx* c, double kV);
 ps_status ensure_ftab(ps_ctx* c);
 ps_status ensure_abtab(ps_ctx* c, double kV);                           // incident.cu

@@ -153,18 +153,85 @@ template <int N> struct Twiddles {
             w3[0] = make_float2(1.f, 0.f);
         }
     }
+    __device__ __forceinline__ float2 tw2(const int b, const int r) const { return w2[b * (P::R2 - 1) + r - 1]; }
+    __device__ __forceinline__ float2 tw3(const int b) const { return w3[b]; }
+};
+
+// Register-light variant: the stage-2 twiddles W_{16 R2}^{q r} depend on the thread only through q = j mod 16, so a block
+// keeps one table [16][R2 - 1] in shared memory (filled once per kernel) and every thread re-reads its R2 - 1 values per
+// transform (one broadcast-friendly LDS.64 each) instead of holding 2 (R2 - 1) registers across the persistent loop.
+template <int N> struct TwiddlesShared {
+    using P = Plan<N>;
+    static constexpr int TABLE = 16 * (P::R2 - 1);       // float2 entries
+    // stage 3: W_N^{t + b T}; when T B3/2 = N/4 (N = 512) the upper half of the b range is the lower half times -i
+    static constexpr bool HALF3 = (P::R3 > 1) && (P::T * P::B3 / 2 * 4 == N);
+    static constexpr int NW3 = HALF3 ? P::B3 / 2 : P::B3;
+    const float2* row[P::B2];                            // table row of (t + b T) mod 16
+    float2 w3[NW3];
+    // every thread of the block calls fill() (followed by a block barrier) before the first transform
+    static __device__ __forceinline__ void fill(float2* tab, const int tid, const int nthreads) {
+        for (int i = tid; i < TABLE; i += nthreads) {
+            const int q = i / (P::R2 - 1), r = i % (P::R2 - 1) + 1;
+            tab[i] = root_of_unity(q * r, 16 * P::R2);
+        }
+    }
+    __device__ __forceinline__ void init(const int t, const float2* tab) {
+#pragma unroll
+        for (int b = 0; b < P::B2; ++b) row[b] = tab + ((t + b * P::T) & 15) * (P::R2 - 1);
+        if (P::R3 > 1) {
+#pragma unroll
+            for (int b = 0; b < NW3; ++b) w3[b] = root_of_unity((t + b * P::T) & (16 * P::R2 - 1), N);
+        } else {
+            w3[0] = make_float2(1.f, 0.f);
+        }
+    }
+    __device__ __forceinline__ float2 tw2(const int b, const int r) const { return row[b][r - 1]; }
+    __device__ __forceinline__ float2 tw3(const int b) const {
+        if constexpr (HALF3) {
+            if (b >= NW3) return make_float2(w3[b - NW3].y, -w3[b - NW3].x);     // times W_4 = -i
+        }
+        return w3[b < NW3 ? b : 0];
+    }
 };
 
 // ---------------------------------------------------------------- exchange policies
 // A policy gives the shared-memory slot of logical element idx of *this thread's* transform and
 // the barrier covering all threads of that transform.
+// `at` is the layout the caller sees (first read, last write, second exchange); x1w / x1r address the FIRST exchange
+// (element 16 t + r written, element t + e T read), whose layout may differ as long as write and read agree.
 struct RowSlots {            // one transform per contiguous padded line; pad 1 per 16 (conflict-free)
     float2* line;
     __device__ __forceinline__ float2& at(const int idx) const { return line[idx + (idx >> 4)]; }
+    __device__ __forceinline__ float2& x1w(const int t, const int r) const { return at(16 * t + r); }
+    template <int T> __device__ __forceinline__ float2& x1r(const int t, const int e) const { return at(t + e * T); }
 };
-template <int C> struct ColSlots {   // C transforms interleaved (lane = column), no padding needed
+// C transforms interleaved (a warp = 32/C consecutive t x C columns), linear so that a TMA box [rows][C] can land in it.
+// First exchange: the writes 16 t + r of the 32/C t-values of a warp would all fall on the same C*8-byte slice of the
+// 128-byte bank window (a 16/C-way conflict for C < 16).  XOR-ing the row index with (row >> 4) & M, M = 16/C - 1,
+// spreads them over the whole window (2 wavefronts per 256-byte warp access, the minimum).  The XOR term is a per-thread
+// constant (t & M for the writes, (t >> 4) & M for the reads when T is a multiple of 16 (M + 1)), so it is folded into
+// M + 2 base pointers computed once per item and every access keeps an immediate offset.
+template <int C> struct ColSlots {
+    static constexpr int M = (C < 16) ? 16 / C - 1 : 0;
     float2* base;                    // already offset by the column index c
+    float2* wb[M + 1];
+    float2* rb;
+    __device__ __forceinline__ ColSlots(float2* b, const int t) : base(b) {
+        const int sw = t & M;
+#pragma unroll
+        for (int k = 0; k <= M; ++k) wb[k] = b + (16 * t + ((k ^ sw) - k)) * C;
+        rb = b + (t ^ ((t >> 4) & M)) * C;
+    }
     __device__ __forceinline__ float2& at(const int idx) const { return base[idx * C]; }
+    __device__ __forceinline__ float2& x1w(const int, const int r) const { return wb[r & M][r * C]; }
+    template <int T> __device__ __forceinline__ float2& x1r(const int t, const int e) const {
+        if constexpr (T % (16 * (M + 1)) == 0) {
+            return rb[e * T * C];
+        } else {
+            const int idx = t + e * T;
+            return base[(idx ^ ((idx >> 4) & M)) * C];
+        }
+    }
 };
 struct BlockSync { static __device__ __forceinline__ void sync() { __syncthreads(); } };
 struct WarpSync  { static __device__ __forceinline__ void sync() { __syncwarp(); } };
@@ -179,18 +246,18 @@ template <int T> struct GroupSync {
 template <int N> struct RowLine { static constexpr int LEN = N + N / 16; };      // padded line length (float2)
 
 // ---------------------------------------------------------------- the transform
-template <int N, class Slots, class Sync>
-__device__ __forceinline__ void fft_forward(float2 (&v)[16], const int t, const Twiddles<N>& tw, const Slots& sm) {
+template <int N, class Slots, class Sync, class TW = Twiddles<N>>
+__device__ __forceinline__ void fft_forward(float2 (&v)[16], const int t, const TW& tw, const Slots& sm) {
     using P = Plan<N>;
     constexpr int T = P::T;
     // stage 1: radix 16, Ns = 1, no twiddle
     Dft<16>::run(v);
     Sync::sync();                                             // earlier readers of the buffer are done
 #pragma unroll
-    for (int r = 0; r < 16; ++r) sm.at(16 * t + r) = v[r];
+    for (int r = 0; r < 16; ++r) sm.x1w(t, r) = v[r];
     Sync::sync();
 #pragma unroll
-    for (int e = 0; e < 16; ++e) v[e] = sm.at(t + e * T);
+    for (int e = 0; e < 16; ++e) v[e] = sm.template x1r<T>(t, e);
     // stage 2: radix R2, Ns = 16
     constexpr int R2 = P::R2, B2 = P::B2;
 #pragma unroll
@@ -199,7 +266,7 @@ __device__ __forceinline__ void fft_forward(float2 (&v)[16], const int t, const 
 #pragma unroll
         for (int r = 0; r < R2; ++r) w[r] = v[b + r * B2];
 #pragma unroll
-        for (int r = 1; r < R2; ++r) w[r] = cmul(w[r], tw.w2[b * (R2 - 1) + r - 1]);
+        for (int r = 1; r < R2; ++r) w[r] = cmul(w[r], tw.tw2(b, r));
         Dft<R2>::run(w);
 #pragma unroll
         for (int r = 0; r < R2; ++r) v[b + r * B2] = w[r];
@@ -224,7 +291,7 @@ __device__ __forceinline__ void fft_forward(float2 (&v)[16], const int t, const 
 #pragma unroll
             for (int r = 0; r < R3; ++r) w[r] = v[b + r * B3];
             float2 p[R3];                                     // p[r] = base^r (balanced products)
-            p[1] = tw.w3[b];
+            p[1] = tw.tw3(b);
 #pragma unroll
             for (int r = 2; r < R3; ++r) p[r] = cmul(p[r / 2], p[r - r / 2]);
 #pragma unroll
@@ -237,11 +304,11 @@ __device__ __forceinline__ void fft_forward(float2 (&v)[16], const int t, const 
 }
 
 // unnormalised inverse: swap, forward, swap
-template <int N, class Slots, class Sync>
-__device__ __forceinline__ void fft_inverse(float2 (&v)[16], const int t, const Twiddles<N>& tw, const Slots& sm) {
+template <int N, class Slots, class Sync, class TW = Twiddles<N>>
+__device__ __forceinline__ void fft_inverse(float2 (&v)[16], const int t, const TW& tw, const Slots& sm) {
 #pragma unroll
     for (int e = 0; e < 16; ++e) v[e] = cswap(v[e]);
-    fft_forward<N, Slots, Sync>(v, t, tw, sm);
+    fft_forward<N, Slots, Sync, TW>(v, t, tw, sm);
 #pragma unroll
     for (int e = 0; e < 16; ++e) v[e] = cswap(v[e]);
 }

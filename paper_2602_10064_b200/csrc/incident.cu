@@ -44,7 +44,7 @@ k_probe_col(float2* __restrict__ psi, const int nx, const int32_t* __restrict__ 
     constexpr int T = Cfg::T, C = Cfg::C, SUB = kColTile / C;
     extern __shared__ float2 smem[];
     const int c = threadIdx.x % C, t = threadIdx.x / C;
-    ColSlots<C> slots{smem + c};
+    ColSlots<C> slots(smem + c, t);
     Twiddles<NY> tw;
     tw.init(t);
     const int per_wave = n_tiles * SUB;
@@ -115,27 +115,14 @@ k_row_ifft(float2* __restrict__ psi, const uint8_t* __restrict__ tile_active, co
     }
 }
 
-template <class K>
-static int blocks_cap_i(K kernel, int threads, size_t smem) {
-    int per_sm = 1, dev = 0, n_sm = kNumSM;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, smem) != cudaSuccess || per_sm < 1)
-        per_sm = 1;
-    return n_sm * per_sm;
-}
-
 template <int NY>
 static cudaError_t launch_probe_col(ps_ctx* c, float2* psi, const int32_t* pmax, const uint32_t* U0, float scale,
                                     const float2* abtab, int n) {
     using Cfg = PColCfg<NY>;
     auto kern = k_probe_col<NY>;
-    static int cap = 0;
-    if (!cap) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
-        if (e != cudaSuccess) return e;
-        cap = blocks_cap_i(kern, Cfg::THREADS, Cfg::SMEM);
-    }
+    int cap = 0;
+    cudaError_t ce = kernel_cap(c, kern, Cfg::THREADS, Cfg::SMEM, &cap);
+    if (ce != cudaSuccess) return ce;
     const int n_items = n * c->n_tiles_active * (kColTile / Cfg::C);
     kern<<<n_items < cap ? n_items : cap, Cfg::THREADS, Cfg::SMEM, c->stream>>>(psi, c->nx, c->d_tiles, c->n_tiles_active,
                                                                                pmax, U0, scale, abtab, n_items);
@@ -146,12 +133,9 @@ template <int NX>
 static cudaError_t launch_row_ifft(ps_ctx* c, float2* psi, int n) {
     using Cfg = PRowCfg<NX>;
     auto kern = k_row_ifft<NX>;
-    static int cap = 0;
-    if (!cap) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
-        if (e != cudaSuccess) return e;
-        cap = blocks_cap_i(kern, Cfg::THREADS, Cfg::SMEM);
-    }
+    int cap = 0;
+    cudaError_t ce = kernel_cap(c, kern, Cfg::THREADS, Cfg::SMEM, &cap);
+    if (ce != cudaSuccess) return ce;
     const long long n_rows = (long long)n * c->ny;
     const int n_items = (int)((n_rows + Cfg::RPB - 1) / Cfg::RPB);
     kern<<<n_items < cap ? n_items : cap, Cfg::THREADS, Cfg::SMEM, c->stream>>>(psi, c->d_tile_active, n_rows, n_items);
@@ -206,8 +190,7 @@ ps_status ensure_abtab(ps_ctx* c, double kV) {
     }
     ps_status st = ensure_buf(c, c->abtab, h.size() * sizeof(float2));
     if (st != PS_OK) return st;
-    PSB_CUDA(c, cudaMemcpyAsync(c->abtab.p, h.data(), h.size() * sizeof(float2), cudaMemcpyHostToDevice, c->stream));
-    PSB_CUDA(c, cudaStreamSynchronize(c->stream));           // `h` dies at return
+    if ((st = upload_async(c, c->abtab.p, h.data(), h.size() * sizeof(float2))) != PS_OK) return st;   // set-up path
     c->ab_kV = kV;
     return PS_OK;
 }
@@ -236,8 +219,9 @@ extern "C" ps_status ps_apply_aberrations(ps_ctx* c, double kV, void* d_waves_k,
     if (!c->have_geom) return fail(c, PS_ESTATE, "ps_apply_aberrations: ps_set_geometry has not been called");
     if (!c->have_ab) return fail(c, PS_ESTATE, "ps_apply_aberrations: ps_set_aberrations has not been called");
     if (!d_waves_k || n_waves < 1 || !(kV > 0.0)) return fail(c, PS_EINVAL, "ps_apply_aberrations: null pointer or non-positive size / voltage");
-    ps_status st = ensure_abtab(c, kV);
+    ps_status st = enter(c, "ps_apply_aberrations");
     if (st != PS_OK) return st;
+    if ((st = ensure_abtab(c, kV)) != PS_OK) return st;
     const size_t npix = (size_t)c->nx * c->ny, total = npix * (size_t)n_waves;
     const size_t nb = (total + 255) / 256;
     ProfScope ps_(c, K_INCIDENT);
@@ -253,6 +237,8 @@ extern "C" ps_status ps_make_incident(ps_ctx* c, double kV, double semi_angle_mr
     if (!d_psi0 || n < 1 || !(kV > 0.0) || semi_angle_mrad < 0.0)
         return fail(c, PS_EINVAL, "ps_make_incident: null pointer, non-positive count/voltage or negative angle");
     const int nx = c->nx, ny = c->ny;
+    ps_status st0 = enter(c, "ps_make_incident");
+    if (st0 != PS_OK) return st0;
     ProfScope ps_(c, K_INCIDENT);
     float2* psi = (float2*)d_psi0;
     const long long total = (long long)n * nx * ny;
@@ -268,11 +254,11 @@ extern "C" ps_status ps_make_incident(ps_ctx* c, double kV, double semi_angle_mr
                 if (v != floor(v) || fabs(v) > 1e6) return fail(c, PS_EINVAL, "ps_make_incident: tilt indices must be integers");
                 h[i] = (int32_t)v;
             }
-            ps_status st = ensure_buf(c, c->misc, 4096 + h.size() * 4);
+            ps_status st = ensure_buf(c, c->inc_buf, h.size() * 4);
             if (st != PS_OK) return st;
-            d_t = (int32_t*)((char*)c->misc.p + 4096);
-            PSB_CUDA(c, cudaMemcpyAsync(d_t, h.data(), h.size() * 4, cudaMemcpyHostToDevice, c->stream));
-            PSB_CUDA(c, cudaStreamSynchronize(c->stream));                   // h is a stack-lifetime buffer
+            d_t = (int32_t*)c->inc_buf.p;
+            if ((st = upload_async(c, d_t, h.data(), h.size() * 4)) != PS_OK) return st;   // staged: no host wait
+            c->inc_pmax_host.clear();
         }
         k_fill_plane_tilt<<<(unsigned)((total + 255) / 256), 256, 0, c->stream>>>(psi, nx, ny, n, d_t);
         PSB_LAUNCH_CHECK(c, "k_fill_plane_tilt");
@@ -301,14 +287,18 @@ extern "C" ps_status ps_make_incident(ps_ctx* c, double kV, double semi_angle_mr
         U0[2 * i] = host_fixed(xy_or_tilt[2 * i], c->cell[0]);
         U0[2 * i + 1] = host_fixed(xy_or_tilt[2 * i + 1], c->cell[1]);
     }
-    const size_t need = 4096 + (size_t)nx * 4 + 256 + U0.size() * 4;
-    ps_status st = ensure_buf(c, c->misc, need);
+    const size_t pmax_bytes = ((size_t)nx * 4 + 255) & ~(size_t)255;
+    const bool grown = c->inc_buf.bytes < pmax_bytes + U0.size() * 4;
+    ps_status st = ensure_buf(c, c->inc_buf, pmax_bytes + U0.size() * 4);
     if (st != PS_OK) return st;
-    int32_t* d_pmax = (int32_t*)((char*)c->misc.p + 4096);
-    uint32_t* d_U0 = (uint32_t*)((char*)c->misc.p + 4096 + (((size_t)nx * 4 + 255) & ~(size_t)255));
-    PSB_CUDA(c, cudaMemcpyAsync(d_pmax, pmax.data(), (size_t)nx * 4, cudaMemcpyHostToDevice, c->stream));
-    PSB_CUDA(c, cudaMemcpyAsync(d_U0, U0.data(), U0.size() * 4, cudaMemcpyHostToDevice, c->stream));
-    PSB_CUDA(c, cudaStreamSynchronize(c->stream));
+    int32_t* d_pmax = (int32_t*)c->inc_buf.p;
+    uint32_t* d_U0 = (uint32_t*)((char*)c->inc_buf.p + pmax_bytes);
+    // staged through the ctx's pinned ring: the host vectors may die at return and nothing waits for the stream
+    if (grown || pmax != c->inc_pmax_host) {
+        if ((st = upload_async(c, d_pmax, pmax.data(), (size_t)nx * 4)) != PS_OK) return st;
+        c->inc_pmax_host = pmax;
+    }
+    if ((st = upload_async(c, d_U0, U0.data(), U0.size() * 4)) != PS_OK) return st;
     const float scale = (float)(1.0 / sqrt((double)n_ap));
     cudaError_t e = cudaErrorInvalidValue;
     const float2* abtab = nullptr;

@@ -36,7 +36,7 @@ __global__ void k_bin(const float* __restrict__ pos, const int32_t* __restrict__
                       const int32_t* __restrict__ elem_of_Z, const long long n_total, const int n_atoms,
                       const double Lx, const double Ly, const double Lz, const int n_slices, const int n_elem,
                       uint32_t* __restrict__ Ux, uint32_t* __restrict__ Uy, int32_t* __restrict__ key,
-                      int32_t* __restrict__ slice_idx) {
+                      int32_t* __restrict__ slice_idx, int* __restrict__ async_err) {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n_total) return;
     const int j = (int)(i % n_atoms);
@@ -48,6 +48,7 @@ __global__ void k_bin(const float* __restrict__ pos, const int32_t* __restrict__
     const int zz = Z[j];
     const int e = (zz >= 1 && zz <= 127) ? elem_of_Z[zz] : -1;
     key[i] = (e >= 0) ? s * n_elem + e : -1;
+    if (e < 0) { *(volatile int*)async_err = (zz == 0) ? -1 : zz; __threadfence_system(); }   // mapped host word (ps_ctx)
     if (slice_idx) slice_idx[i] = s;
 }
 
@@ -254,7 +255,7 @@ k_v_col(const float2* __restrict__ Vk, const int32_t* __restrict__ offsets, floa
     constexpr int T = Cfg::T, C = Cfg::C, SUB = kColTile / C;
     extern __shared__ float2 smem[];
     const int c = threadIdx.x % C, t = threadIdx.x / C;
-    ColSlots<C> slots{smem + c};
+    ColSlots<C> slots(smem + c, t);
     Twiddles<NY> tw;
     tw.init(t);
     const int per_pair = n_tiles * SUB;
@@ -352,18 +353,31 @@ k_v_row(const float2* __restrict__ Zm, const int32_t* __restrict__ offsets, floa
 #pragma unroll
         for (int e = 0; e < 16; ++e)
             v[e] = (any && ((amask >> e) & 1u)) ? src[t + e * T] : make_float2(0.f, 0.f);
-        // both slices of every row of this block empty (vacuum): V = 0, no transform; the block's RPB rows are
-        // contiguous in V (ny is a multiple of RPB), so they are cleared with 16-byte stores
+        // both slices of every row of this block empty (vacuum): V = 0, no transform.  When the block's RPB rows lie
+        // inside one slice-pair image (RPB <= ny; both are powers of two, so they are then contiguous in V) they are
+        // cleared with 16-byte stores; on smaller grids a block spans several slice pairs and every row group clears
+        // its own row through the normal (f, sa, sb, y) addressing.
         if (!__syncthreads_or(any)) {
-            const unsigned rho0 = (unsigned)item * Cfg::RPB;
-            if ((long long)rho0 < n_rows) {
-                const int fp0 = (int)(rho0 >> ny_shift), y0 = (int)(rho0 & (unsigned)(ny - 1));
-                const int f0 = fp0 / n_pairs, s0 = 2 * (fp0 % n_pairs);
-                float4* za = reinterpret_cast<float4*>(V + (((size_t)f0 * n_slices + s0) * ny + y0) * NX);
-                float4* zb = reinterpret_cast<float4*>(V + (((size_t)f0 * n_slices + s0 + 1) * ny + y0) * NX);
-                for (int k = threadIdx.x; k < Cfg::RPB * NX / 4; k += Cfg::THREADS) {
-                    za[k] = make_float4(0.f, 0.f, 0.f, 0.f);
-                    if (s0 + 1 < n_slices) zb[k] = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (Cfg::RPB <= ny) {
+                const unsigned rho0 = (unsigned)item * Cfg::RPB;
+                if ((long long)rho0 < n_rows) {
+                    const int fp0 = (int)(rho0 >> ny_shift), y0 = (int)(rho0 & (unsigned)(ny - 1));
+                    const int f0 = fp0 / n_pairs, s0 = 2 * (fp0 % n_pairs);
+                    float4* za = reinterpret_cast<float4*>(V + (((size_t)f0 * n_slices + s0) * ny + y0) * NX);
+                    float4* zb = reinterpret_cast<float4*>(V + (((size_t)f0 * n_slices + s0 + 1) * ny + y0) * NX);
+                    for (int k = threadIdx.x; k < Cfg::RPB * NX / 4; k += Cfg::THREADS) {
+                        za[k] = make_float4(0.f, 0.f, 0.f, 0.f);
+                        if (s0 + 1 < n_slices) zb[k] = make_float4(0.f, 0.f, 0.f, 0.f);
+                    }
+                }
+            } else if (valid) {
+                float* va = V + (((size_t)f * n_slices + sa) * ny + y) * NX;
+#pragma unroll
+                for (int e = 0; e < 16; ++e) va[t + e * T] = 0.f;
+                if (sb < n_slices) {
+                    float* vb = V + (((size_t)f * n_slices + sb) * ny + y) * NX;
+#pragma unroll
+                    for (int e = 0; e < 16; ++e) vb[t + e * T] = 0.f;
                 }
             }
             continue;
@@ -405,26 +419,13 @@ static ScratchLayout scratch_layout(const ps_ctx* c, int nfc, int n_atoms) {
     return L;
 }
 
-template <class K>
-static int blocks_cap(K kernel, int threads, size_t smem) {
-    int per_sm = 1, dev = 0, n_sm = kNumSM;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, smem) != cudaSuccess || per_sm < 1)
-        per_sm = 1;
-    return n_sm * per_sm;
-}
-
 template <int NY>
 static cudaError_t launch_v_col(ps_ctx* c, const float2* Vk, const int32_t* off, float2* Zm, int nfc) {
     using Cfg = VColCfg<NY>;
     auto kern = k_v_col<NY>;
-    static int cap = 0;
-    if (!cap) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
-        if (e != cudaSuccess) return e;
-        cap = blocks_cap(kern, Cfg::THREADS, Cfg::SMEM);
-    }
+    int cap = 0;
+    cudaError_t ce = kernel_cap(c, kern, Cfg::THREADS, Cfg::SMEM, &cap);
+    if (ce != cudaSuccess) return ce;
     const int n_pairs = (c->n_slices + 1) / 2;
     const long long n_items = (long long)nfc * n_pairs * c->n_tiles_active * (kColTile / Cfg::C);
     const int grid = (int)(n_items < cap ? n_items : cap);
@@ -437,12 +438,9 @@ template <int NX>
 static cudaError_t launch_v_row(ps_ctx* c, const float2* Zm, const int32_t* off, float* V, int nfc) {
     using Cfg = VRowCfg<NX>;
     auto kern = k_v_row<NX>;
-    static int cap = 0;
-    if (!cap) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
-        if (e != cudaSuccess) return e;
-        cap = blocks_cap(kern, Cfg::THREADS, Cfg::SMEM);
-    }
+    int cap = 0;
+    cudaError_t ce = kernel_cap(c, kern, Cfg::THREADS, Cfg::SMEM, &cap);
+    if (ce != cudaSuccess) return ce;
     const int n_pairs = (c->n_slices + 1) / 2;
     const long long n_rows = (long long)nfc * n_pairs * c->ny;
     const long long n_items = (n_rows + Cfg::RPB - 1) / Cfg::RPB;
@@ -480,24 +478,31 @@ extern "C" ps_status ps_build_slices(ps_ctx* c, const float* d_pos, const int32_
         return fail(c, PS_ESTATE, "ps_build_slices: ps_set_geometry and ps_set_form_factors must be called first");
     if (!d_pos || !d_Z || !d_V || n_frames < 1 || n_atoms < 1)
         return fail(c, PS_EINVAL, "ps_build_slices: null pointer or non-positive size");
-    ps_status st = ensure_ftab(c);
+    ps_status st = enter(c, "ps_build_slices");
     if (st != PS_OK) return st;
+    if ((st = ensure_ftab(c)) != PS_OK) return st;
     const long long n_bins = (long long)c->n_slices * c->n_elem;
     if ((2 * n_bins + 2) * 4 > 200 * 1024)
         return fail(c, PS_EUNSUPPORTED, "ps_build_slices: n_slices * n_elements too large for the sort kernel");
 
-    // validate Z (one 4-byte read-back before any work is queued; the rest of the call is asynchronous)
-    if ((st = ensure_buf(c, c->misc, 4096)) != PS_OK) return st;
-    int* d_flag = (int*)c->misc.p;
-    PSB_CUDA(c, cudaMemsetAsync(d_flag, 0, sizeof(int), c->stream));
-    k_check_Z<<<(n_atoms + 255) / 256, 256, 0, c->stream>>>(d_Z, n_atoms, c->d_elem_of_Z, d_flag);
-    PSB_LAUNCH_CHECK(c, "k_check_Z");
-    int h_flag = 0;
-    PSB_CUDA(c, cudaMemcpyAsync(&h_flag, d_flag, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
-    PSB_CUDA(c, cudaStreamSynchronize(c->stream));
-    if (h_flag != 0)
-        return fail(c, PS_EUNSUPPORTED, "ps_build_slices: atomic number " + std::to_string(h_flag) +
-                                            " has no form-factor coefficients");
+    // Z validation.  The first time a (d_Z, n_atoms) pair is seen, one 4-byte read-back rejects unknown atomic numbers
+    // before any work is queued (a blocking call, like every first call with new parameters).  Later calls with the
+    // same pair queue their work without waiting; k_bin re-checks every atom of every call on the device and raises the
+    // ctx's mapped error word, which the next ps_* call reports (enter()).
+    if (c->z_checked != (const void*)d_Z || c->z_checked_n != n_atoms) {
+        if ((st = ensure_buf(c, c->misc, 4096)) != PS_OK) return st;
+        int* d_flag = (int*)c->misc.p;
+        PSB_CUDA(c, cudaMemsetAsync(d_flag, 0, sizeof(int), c->stream));
+        k_check_Z<<<(n_atoms + 255) / 256, 256, 0, c->stream>>>(d_Z, n_atoms, c->d_elem_of_Z, d_flag);
+        PSB_LAUNCH_CHECK(c, "k_check_Z");
+        int h_flag = 0;
+        PSB_CUDA(c, cudaMemcpyAsync(&h_flag, d_flag, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+        PSB_CUDA(c, cudaStreamSynchronize(c->stream));
+        if (h_flag != 0)
+            return fail(c, PS_EUNSUPPORTED, "ps_build_slices: atomic number " + std::to_string(h_flag == -1 ? 0 : h_flag) +
+                                                " has no form-factor coefficients");
+        c->z_checked = (const void*)d_Z; c->z_checked_n = n_atoms;
+    }
 
     // scratch: installed workspace or library-owned buffer; frames are processed in chunks that fit
     const size_t per_frame = scratch_layout(c, 1, n_atoms).total;
@@ -548,10 +553,9 @@ extern "C" ps_status ps_build_slices(ps_ctx* c, const float* d_pos, const int32_
 
     const int tiles_m = (c->mcut + 1 + VK_TM - 1) / VK_TM, tiles_n = (c->ncut + 1 + VK_TN - 1) / VK_TN;
     const size_t img = (size_t)c->nx * c->ny;
-    static bool sort_attr = false;
-    if (!sort_attr) {
-        PSB_CUDA(c, cudaFuncSetAttribute(k_sort, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
-        sort_attr = true;
+    {
+        int cap_unused = 0;                                                // sets the 200 KB attribute once per ctx
+        PSB_CUDA(c, kernel_cap(c, k_sort, 1024, (size_t)200 * 1024, &cap_unused));
     }
 
     for (int f0 = 0; f0 < n_frames; f0 += nfc) {
@@ -560,7 +564,8 @@ extern "C" ps_status ps_build_slices(ps_ctx* c, const float* d_pos, const int32_
         { ProfScope ps_(c, K_BIN);
         k_bin<<<(unsigned)((n_total + 255) / 256), 256, 0, c->stream>>>(
             d_pos + (size_t)f0 * n_atoms * 3, d_Z, c->d_elem_of_Z, n_total, n_atoms, c->cell[0], c->cell[1], c->cell[2],
-            c->n_slices, c->n_elem, Ux, Uy, key, d_slice_idx ? d_slice_idx + (size_t)f0 * n_atoms : nullptr);
+            c->n_slices, c->n_elem, Ux, Uy, key, d_slice_idx ? d_slice_idx + (size_t)f0 * n_atoms : nullptr,
+            c->d_async_err);
         }
         PSB_LAUNCH_CHECK(c, "k_bin");
         { ProfScope ps_(c, K_SORT);

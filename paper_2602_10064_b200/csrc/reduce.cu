@@ -205,6 +205,8 @@ k_qbin_sum(const float* __restrict__ I, const int32_t* __restrict__ offsets, con
 using namespace psb;
 
 static ps_status check_I(ps_ctx* c, const char* who, const float* d_I, int P, int n_bins, const void* d_out) {
+    ps_status st = enter(c, who);
+    if (st != PS_OK) return st;
     if (!c->have_geom) return fail(c, PS_ESTATE, std::string(who) + ": ps_set_geometry has not been called");
     if (!d_I || !d_out || P < 1 || n_bins < 1) return fail(c, PS_EINVAL, std::string(who) + ": null pointer or non-positive size");
     return PS_OK;
@@ -247,6 +249,8 @@ extern "C" ps_status ps_haadf(ps_ctx* c, const void* d_exit, int exit_layout, in
     if (!d_exit || !d_out || n_probes < 1 || n_frames < 1) return fail(c, PS_EINVAL, "ps_haadf: null pointer or non-positive size");
     if (exit_layout != PS_LAYOUT_DENSE) return fail(c, PS_EUNSUPPORTED, "ps_haadf: unknown exit layout");
     if (k_in < 0.0) return fail(c, PS_EINVAL, "ps_haadf: k_in must be >= 0");
+    ps_status st_in = enter(c, "ps_haadf");
+    if (st_in != PS_OK) return st_in;
     const size_t npix = (size_t)c->nx * c->ny;
     const size_t tmp_off = (4096 + npix + 255) & ~(size_t)255;
     ps_status st = ensure_buf(c, c->misc, tmp_off + (size_t)n_probes * n_frames * sizeof(float));
@@ -271,6 +275,8 @@ extern "C" ps_status ps_accumulate_intensity(ps_ctx* c, float* d_acc, const floa
     if (!d_acc || !d_I || n_values == 0) return fail(c, PS_EINVAL, "ps_accumulate_intensity: null pointer or zero size");
     if (n_values % 4 != 0 || (((uintptr_t)d_acc | (uintptr_t)d_I) & 15u))
         return fail(c, PS_EINVAL, "ps_accumulate_intensity: arrays must be 16-byte aligned with a multiple of 4 values");
+    ps_status st_in = enter(c, "ps_accumulate_intensity");
+    if (st_in != PS_OK) return st_in;
     const size_t n4 = n_values / 4;
     const size_t nb = (n4 + 255) / 256;
     ProfScope ps_(c, K_REDUCE);
@@ -286,12 +292,11 @@ extern "C" ps_status ps_dispersion(ps_ctx* c, const float* d_I, int P, int n_bin
     if (st != PS_OK) return st;
     ProfScope ps_(c, K_REDUCE);
     if (!kx || !ky || !d_pix || n_path < 1) return fail(c, PS_EINVAL, "ps_dispersion: null pointer or empty path");
-    const size_t need = 4096 + 2 * (size_t)n_path * sizeof(double);
-    if ((st = ensure_buf(c, c->misc, need)) != PS_OK) return st;
-    double* d_k = (double*)((char*)c->misc.p + 4096);
-    PSB_CUDA(c, cudaMemcpyAsync(d_k, kx, (size_t)n_path * 8, cudaMemcpyHostToDevice, c->stream));
-    PSB_CUDA(c, cudaMemcpyAsync(d_k + n_path, ky, (size_t)n_path * 8, cudaMemcpyHostToDevice, c->stream));
-    PSB_CUDA(c, cudaStreamSynchronize(c->stream));               // caller's host arrays are not retained
+    if ((st = ensure_buf(c, c->path_buf, 2 * (size_t)n_path * sizeof(double))) != PS_OK) return st;
+    double* d_k = (double*)c->path_buf.p;
+    // the caller's host arrays are copied into the ctx's pinned ring and sent asynchronously: not retained, no wait
+    if ((st = upload_async(c, d_k, kx, (size_t)n_path * 8)) != PS_OK) return st;
+    if ((st = upload_async(c, d_k + n_path, ky, (size_t)n_path * 8)) != PS_OK) return st;
     k_path_pixels<<<(n_path + 127) / 128, 128, 0, c->stream>>>(d_k, d_k + n_path, d_pix, n_path, c->nx, c->ny, c->cell[0],
                                                                c->cell[1]);
     PSB_LAUNCH_CHECK(c, "k_path_pixels");

@@ -29,7 +29,7 @@ k_tacaw_fft(const float2* __restrict__ exitw, float* __restrict__ I, const int32
     constexpr int T = Cfg::T, C = Cfg::C;
     extern __shared__ float2 smem[];
     const int c = threadIdx.x % C, t = threadIdx.x / C;
-    ColSlots<C> slots{smem + c};
+    ColSlots<C> slots(smem + c, t);
     Twiddles<NF> tw;
     tw.init(t);
     const size_t npix = (size_t)nx * ny;
@@ -150,7 +150,7 @@ k_tacaw_tma(const __grid_constant__ CUtensorMap emap, float* __restrict__ I, con
         const int ay = iy < ny / 2 ? iy : ny - iy;
         const bool mine = ay <= nmax[ix];                    // the group has in-band pixels; this one may not be
         float* out = I + (size_t)p * n_out * npix + pix0 + c;
-        ColSlots<C> slots{stage0 + (size_t)s * NF * C + c};
+        ColSlots<C> slots(stage0 + (size_t)s * NF * C + c, t);
         tma::mbar_wait(&full[s], (it / NS) & 1);
         const float2 ref = slots.at(0);                      // frame 0 (A14: mean removal, see header)
         float2 v[16];
@@ -186,88 +186,119 @@ __global__ void k_tacaw_zero(float* __restrict__ I, const int32_t* __restrict__ 
 }
 
 // ------------------------------------------------------------------------------------ path B: streaming DFT
-constexpr int SB_PIX = 128, SB_BINS = 16, SB_FR = 64;
+// acc[p][b][k] += sum_{j in chunk} (Psi[p][j][k] - ref[p][k]) exp(-2 pi i n_b (frame0 + j) / F)
+//
+// One block owns a tile of SB_PIX adjacent pixels x up to SB_FR frames of the chunk, staged ONCE in shared memory by the
+// copy engine (one 2-D TMA box, 64 KB), strips the reference wave from it (the elastic part, ~100x the signal: without
+// it the fp32 partial sums of the Bragg term over thousands of frames would swamp weak bins; a constant
+// shift of every frame changes no bin n != 0 of the complete sum, and bin 0 is written as exact zero), and then sweeps ALL
+// bins over the tile: thread = (pixel, bin half), SB_BINS complex accumulators in registers per sweep, the twiddles of
+// the sweep (SB_FR x 2 SB_BINS, read from a per-chunk table built by k_tacaw_twiddles in float64) broadcast from shared
+// memory.  Every exit value is read from HBM once per chunk; the accumulators are read and written once per tile.
+// Bound: FP32 FMA issue (4 n_bins FMA per sample against 8 bytes), not HBM.
+constexpr int SB_PIX = 128, SB_BINS = 16, SB_FR = 64, SB_THREADS = 2 * SB_PIX;
+constexpr size_t SB_SMEM = (size_t)SB_FR * SB_PIX * sizeof(float2) + (size_t)SB_FR * 2 * SB_BINS * sizeof(float2) + 64;
 
-// acc[p][b][pix] += sum_{j in chunk} Psi[p][j][pix] * exp(-2 pi i n_b (frame0+j) / F)
-__global__ void __launch_bounds__(SB_PIX)
-k_tacaw_accum(const float2* __restrict__ chunk, float2* __restrict__ acc, const int32_t* __restrict__ bins,
-              const int n_bins, const int n_frames_total, const int frame0, const int n_frames_chunk,
-              const size_t npix, const int nx, const int ny, const int32_t* __restrict__ nmax) {
-    __shared__ float2 w[SB_FR][SB_BINS];
-    const size_t pix = (size_t)blockIdx.x * SB_PIX + threadIdx.x;
-    const int p = blockIdx.z, b0 = blockIdx.y * SB_BINS;
+// tw[j][b] = exp(-2 pi i n_b (frame0 + j) / F), j < n_frames_chunk: float64 sincospi on an exactly reduced phase
+__global__ void k_tacaw_twiddles(float2* __restrict__ tw, const int32_t* __restrict__ bins, const int n_bins,
+                                 const int n_frames_total, const int frame0, const int n_frames_chunk) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_frames_chunk * n_bins) return;
+    const int j = i / n_bins, b = i % n_bins;
+    const long long ph = ((long long)bins[b] * (long long)(frame0 + j)) % n_frames_total;     // bins already in [0, F)
+    double sn, cs;
+    sincospi(2.0 * (double)ph / (double)n_frames_total, &sn, &cs);
+    tw[i] = make_float2((float)cs, (float)(-sn));
+}
+
+__global__ void __launch_bounds__(SB_THREADS, 2)
+k_tacaw_accum(const __grid_constant__ CUtensorMap cmap, float2* __restrict__ acc, const float2* __restrict__ ref,
+              const float2* __restrict__ twtab, const int n_bins, const int n_frames_chunk, const size_t npix,
+              const int nx, const int ny, const int32_t* __restrict__ nmax) {
+    extern __shared__ __align__(1024) float2 smem_b[];
+    float2* tile = smem_b;                                             // [SB_FR][SB_PIX]
+    float2* wsm = smem_b + (size_t)SB_FR * SB_PIX;                     // [SB_FR][2 SB_BINS]
+    uint64_t* full = reinterpret_cast<uint64_t*>(wsm + (size_t)SB_FR * 2 * SB_BINS);
+    const int px = threadIdx.x % SB_PIX, half = threadIdx.x / SB_PIX;
+    const size_t pix0 = (size_t)blockIdx.x * SB_PIX, pix = pix0 + px;
+    const int p = blockIdx.y;
     const int iy = (int)(pix / nx), ix = (int)(pix % nx);
     const int ay = iy < ny / 2 ? iy : ny - iy;
-    const bool mine = pix < npix && ay <= nmax[ix];
-    if (!__syncthreads_or(mine)) return;                    // accumulators stay zero there
-    float2 a[SB_BINS];
-#pragma unroll
-    for (int b = 0; b < SB_BINS; ++b) a[b] = make_float2(0.f, 0.f);
-    const float2* src = chunk + (size_t)p * n_frames_chunk * npix + pix;
-    for (int j0 = 0; j0 < n_frames_chunk; j0 += SB_FR) {
+    const bool mine = ay <= nmax[ix];
+    if (!__syncthreads_or(mine)) return;                                // tile wholly outside the band: acc stays zero
+    if (threadIdx.x == 0) { tma::mbar_init(full, 1); tma::fence_mbar_init(); }
+    __syncthreads();
+    const float2 rf = mine ? __ldg(ref + (size_t)p * npix + pix) : make_float2(0.f, 0.f);
+    int it = 0;
+    for (int j0 = 0; j0 < n_frames_chunk; j0 += SB_FR, ++it) {
         const int cnt = min(SB_FR, n_frames_chunk - j0);
-        __syncthreads();
-        for (int i = threadIdx.x; i < cnt * SB_BINS; i += SB_PIX) {
-            const int jj = i / SB_BINS, b = i % SB_BINS;
-            float2 tw = make_float2(0.f, 0.f);
-            if (b0 + b <= n_bins) {                          // slot n_bins: plain sum (twiddle 1)
-                const long long n = (b0 + b < n_bins) ? bins[b0 + b] : 0;
-                const long long ph = (n * (long long)(frame0 + j0 + jj)) % n_frames_total;   // bins already in [0,F)
-                double s, cc;
-                sincospi(2.0 * (double)ph / (double)n_frames_total, &s, &cc);
-                tw = make_float2((float)cc, (float)(-s));
-            }
-            w[jj][b] = tw;
+        if (threadIdx.x == 0) {                                         // rows past the chunk / the probe are never used
+            tma::fence_proxy_async();                                   // earlier generic-proxy accesses of the tile
+            tma::mbar_arrive_expect_tx(full, (uint32_t)(SB_FR * SB_PIX * sizeof(float2)));
+            tma::tensor_load_2d(tile, &cmap, (int)(2 * pix0), p * n_frames_chunk + j0, full);
         }
-        __syncthreads();
-        if (mine) {
+        tma::mbar_wait(full, it & 1);
+        for (int jj = half; jj < cnt; jj += 2) {                        // strip the reference from this thread's pixel
+            float2 x = tile[jj * SB_PIX + px];
+            x.x -= rf.x; x.y -= rf.y;
+            tile[jj * SB_PIX + px] = x;
+        }
+        for (int b0 = 0; b0 < n_bins; b0 += 2 * SB_BINS) {
+            __syncthreads();                                            // tile ready / previous sweep done with wsm
+            for (int i = threadIdx.x; i < cnt * 2 * SB_BINS; i += SB_THREADS) {
+                const int jj = i / (2 * SB_BINS), b = b0 + i % (2 * SB_BINS);
+                wsm[i] = (b < n_bins) ? __ldg(twtab + (size_t)(j0 + jj) * n_bins + b) : make_float2(0.f, 0.f);
+            }
+            __syncthreads();
+            float2 a[SB_BINS];
+#pragma unroll
+            for (int b = 0; b < SB_BINS; ++b) a[b] = make_float2(0.f, 0.f);
+            const float4* wrow = reinterpret_cast<const float4*>(wsm + half * SB_BINS);
+#pragma unroll 2
             for (int jj = 0; jj < cnt; ++jj) {
-                const float2 x = src[(size_t)(j0 + jj) * npix];
+                const float2 x = tile[jj * SB_PIX + px];
+#pragma unroll
+                for (int q = 0; q < SB_BINS / 2; ++q) {
+                    const float4 ww = wrow[jj * SB_BINS + q];           // two twiddles, same address in the whole warp
+                    a[2 * q].x = fmaf(x.x, ww.x, a[2 * q].x); a[2 * q].x = fmaf(-x.y, ww.y, a[2 * q].x);
+                    a[2 * q].y = fmaf(x.x, ww.y, a[2 * q].y); a[2 * q].y = fmaf(x.y, ww.x, a[2 * q].y);
+                    a[2 * q + 1].x = fmaf(x.x, ww.z, a[2 * q + 1].x); a[2 * q + 1].x = fmaf(-x.y, ww.w, a[2 * q + 1].x);
+                    a[2 * q + 1].y = fmaf(x.x, ww.w, a[2 * q + 1].y); a[2 * q + 1].y = fmaf(x.y, ww.z, a[2 * q + 1].y);
+                }
+            }
+            if (mine) {
 #pragma unroll
                 for (int b = 0; b < SB_BINS; ++b) {
-                    const float2 ww = w[jj][b];
-                    a[b].x = fmaf(x.x, ww.x, a[b].x); a[b].x = fmaf(-x.y, ww.y, a[b].x);
-                    a[b].y = fmaf(x.x, ww.y, a[b].y); a[b].y = fmaf(x.y, ww.x, a[b].y);
+                    const int bb = b0 + half * SB_BINS + b;
+                    if (bb < n_bins) {
+                        float2* d = acc + ((size_t)p * n_bins + bb) * npix + pix;
+                        const float2 o = *d;
+                        *d = make_float2(o.x + a[b].x, o.y + a[b].y);
+                    }
                 }
             }
         }
-    }
-    if (mine) {
-#pragma unroll
-        for (int b = 0; b < SB_BINS; ++b)
-            if (b0 + b <= n_bins) {
-                float2* d = acc + ((size_t)p * (n_bins + 1) + b0 + b) * npix + pix;
-                const float2 o = *d;
-                *d = make_float2(o.x + a[b].x, o.y + a[b].y);
-            }
+        __syncthreads();                                                // everyone is done with the tile before the next load
     }
 }
 
+// I = |acc|^2; bin 0 is sum_j (Psi_j - <Psi>) = 0 exactly (A14)
 __global__ void k_tacaw_finish(const float2* __restrict__ acc, float* __restrict__ I, const int32_t* __restrict__ bins,
                                const int n_bins, const size_t npix, const long long total) {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= total) return;
-    const size_t pix = (size_t)(i % npix);
-    const int b = (int)((i / npix) % n_bins), p = (int)(i / (npix * n_bins));
-    const float2 a = acc[((size_t)p * (n_bins + 1) + b) * npix + pix];
-    I[i] = (bins[b] == 0) ? 0.f : fmaf(a.x, a.x, a.y * a.y);      // bin 0: sum_j (Psi_j - mean) = 0 exactly
+    const int b = (int)((i / npix) % n_bins);
+    const float2 a = acc[i];
+    I[i] = (bins[b] == 0) ? 0.f : fmaf(a.x, a.x, a.y * a.y);
 }
 
 template <int NF>
 static cudaError_t launch_tacaw(ps_ctx* c, const float2* exitw, float* I, const int32_t* slot, int n_out, int P) {
     using Cfg = TacawCfg<NF>;
     auto kern = k_tacaw_fft<NF>;
-    static int cap = 0;
-    if (!cap) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
-        if (e != cudaSuccess) return e;
-        int per_sm = 1, dev = 0, n_sm = kNumSM;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, Cfg::THREADS, Cfg::SMEM) != cudaSuccess || per_sm < 1)
-            per_sm = 1;
-        cap = n_sm * per_sm;
-    }
+    int cap = 0;
+    cudaError_t ce = kernel_cap(c, kern, Cfg::THREADS, Cfg::SMEM, &cap);
+    if (ce != cudaSuccess) return ce;
     const long long n_items = (long long)P * c->ny * (c->nx / Cfg::C);
     if (n_items > 0x7fffffffLL) return cudaErrorInvalidValue;
     kern<<<(int)(n_items < cap ? n_items : cap), Cfg::THREADS, Cfg::SMEM, c->stream>>>(exitw, I, slot, n_out, c->nx, c->ny,
@@ -291,8 +322,7 @@ static ps_status ensure_tacaw_groups(ps_ctx* c, int C) {
     act.insert(act.end(), inact.begin(), inact.end());
     ps_status st = ensure_buf(c, c->tacaw_groups, act.size() * sizeof(int32_t));
     if (st != PS_OK) return st;
-    PSB_CUDA(c, cudaMemcpyAsync(c->tacaw_groups.p, act.data(), act.size() * sizeof(int32_t), cudaMemcpyHostToDevice, c->stream));
-    PSB_CUDA(c, cudaStreamSynchronize(c->stream));           // `act` dies at return
+    if ((st = upload_async(c, c->tacaw_groups.p, act.data(), act.size() * sizeof(int32_t))) != PS_OK) return st;   // once per geometry
     c->tacaw_groups_C = C;
     return PS_OK;
 }
@@ -301,16 +331,8 @@ template <int NF>
 static ps_status launch_tacaw_tma(ps_ctx* c, const float2* exitw, float* I, const int32_t* slot, int n_out, int P) {
     using Cfg = TacawTmaCfg<NF>;
     auto kern = k_tacaw_tma<NF>;
-    static int cap = 0;
-    if (!cap) {
-        PSB_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM));
-        int per_sm = 1, dev = 0, n_sm = kNumSM;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, Cfg::THREADS, Cfg::SMEM) != cudaSuccess || per_sm < 1)
-            per_sm = 1;
-        cap = n_sm * per_sm;
-    }
+    int cap = 0;
+    PSB_CUDA(c, kernel_cap(c, kern, Cfg::THREADS, Cfg::SMEM, &cap));
     ps_status st = ensure_tacaw_groups(c, Cfg::C);
     if (st != PS_OK) return st;
     const size_t npix = (size_t)c->nx * c->ny;
@@ -351,6 +373,8 @@ extern "C" ps_status ps_tacaw(ps_ctx* c, const void* d_exit, int exit_layout, in
     if (!is_pow2(n_frames) || n_frames < 32 || n_frames > 4096)
         return fail(c, PS_EUNSUPPORTED, "ps_tacaw: n_frames must be a power of two in [32, 4096] (use ps_tacaw_begin/add/finish otherwise)");
     if (!bins && n_bins != n_frames) return fail(c, PS_EINVAL, "ps_tacaw: bins == NULL requires n_bins == n_frames");
+    ps_status st_in = enter(c, "ps_tacaw");
+    if (st_in != PS_OK) return st_in;
     std::vector<int32_t> slot(n_frames, -1);
     for (int b = 0; b < n_bins; ++b) {
         long long n = bins ? bins[b] : b;
@@ -363,8 +387,7 @@ extern "C" ps_status ps_tacaw(ps_ctx* c, const void* d_exit, int exit_layout, in
     if (slot != c->tacaw_slot_host || !c->tacaw_slot.p) {
         ps_status st = ensure_buf(c, c->tacaw_slot, (size_t)n_frames * 4);
         if (st != PS_OK) return st;
-        PSB_CUDA(c, cudaMemcpyAsync(c->tacaw_slot.p, slot.data(), (size_t)n_frames * 4, cudaMemcpyHostToDevice, c->stream));
-        PSB_CUDA(c, cudaStreamSynchronize(c->stream));       // `slot` is a host temporary; 16 KB at most
+        if ((st = upload_async(c, c->tacaw_slot.p, slot.data(), (size_t)n_frames * 4)) != PS_OK) return st;   // staged: no host wait
         c->tacaw_slot_host = slot;
     }
     int32_t* d_slot = (int32_t*)c->tacaw_slot.p;
@@ -416,14 +439,30 @@ extern "C" ps_status ps_tacaw_begin(ps_ctx* c, int n_probes, int n_frames_total,
         long long n = bins[b] % n_frames_total; if (n < 0) n += n_frames_total;
         ts.bins[b] = (int32_t)n;
     }
-    PSB_CUDA(c, cudaStreamSynchronize(c->stream));
-    if (ts.d_bins) { cudaFree(ts.d_bins); ts.d_bins = nullptr; }
-    PSB_CUDA(c, cudaMalloc((void**)&ts.d_bins, (size_t)n_bins * 4));
-    PSB_CUDA(c, cudaMemcpy(ts.d_bins, ts.bins.data(), (size_t)n_bins * 4, cudaMemcpyHostToDevice));
-    const size_t bytes = (size_t)n_probes * (n_bins + 1) * c->nx * c->ny * sizeof(float2);
+    ps_status st = enter(c, "ps_tacaw_begin");
+    if (st != PS_OK) return st;
+    const size_t npix = (size_t)c->nx * c->ny;
+    if ((st = ensure_buf(c, ts.d_bins, (size_t)n_bins * 4)) != PS_OK) return st;           // grows only; no free/alloc per call
+    if ((st = ensure_buf(c, ts.d_ref, (size_t)n_probes * npix * sizeof(float2))) != PS_OK) return st;
+    if ((st = upload_async(c, ts.d_bins.p, ts.bins.data(), (size_t)n_bins * 4)) != PS_OK) return st;
+    const size_t bytes = (size_t)n_probes * n_bins * npix * sizeof(float2);
     PSB_CUDA(c, cudaMemsetAsync(d_acc, 0, bytes, c->stream));
     ts.active = true; ts.n_probes = n_probes; ts.n_frames_total = n_frames_total; ts.n_bins = n_bins;
-    ts.frames_seen = 0; ts.d_acc = d_acc;
+    ts.frames_seen = 0; ts.next_frame = -1; ts.have_ref = false; ts.d_acc = d_acc;
+    return PS_OK;
+}
+
+extern "C" ps_status ps_tacaw_set_reference(ps_ctx* c, const void* d_ref) {
+    if (!c) return PS_EINVAL;
+    TacawStream& ts = c->ts;
+    if (!ts.active) return fail(c, PS_ESTATE, "ps_tacaw_set_reference: ps_tacaw_begin has not been called");
+    if (ts.frames_seen > 0) return fail(c, PS_ESTATE, "ps_tacaw_set_reference: frames have already been added");
+    ps_status st = enter(c, "ps_tacaw_set_reference");
+    if (st != PS_OK) return st;
+    const size_t bytes = (size_t)ts.n_probes * c->nx * c->ny * sizeof(float2);
+    if (d_ref) PSB_CUDA(c, cudaMemcpyAsync(ts.d_ref.p, d_ref, bytes, cudaMemcpyDeviceToDevice, c->stream));
+    else PSB_CUDA(c, cudaMemsetAsync(ts.d_ref.p, 0, bytes, c->stream));
+    ts.have_ref = true;
     return PS_OK;
 }
 
@@ -431,15 +470,51 @@ extern "C" ps_status ps_tacaw_add(ps_ctx* c, const void* d_exit_chunk, int frame
     if (!c) return PS_EINVAL;
     TacawStream& ts = c->ts;
     if (!ts.active) return fail(c, PS_ESTATE, "ps_tacaw_add: ps_tacaw_begin has not been called");
+    ps_status st = enter(c, "ps_tacaw_add");
+    if (st != PS_OK) return st;
     if (!d_exit_chunk || frame0 < 0 || n_frames_chunk < 1 || frame0 + n_frames_chunk > ts.n_frames_total)
         return fail(c, PS_EINVAL, "ps_tacaw_add: null pointer or frame range outside [0, n_frames_total)");
+    // chunks arrive in ascending, contiguous frame order (a shard may start anywhere): a frame can be neither counted
+    // twice nor skipped
+    if (ts.next_frame >= 0 && frame0 != ts.next_frame)
+        return fail(c, PS_ESTATE, "ps_tacaw_add: chunk starts at frame " + std::to_string(frame0) + ", expected frame " +
+                                      std::to_string(ts.next_frame) + " (chunks must be contiguous and ascending)");
     const size_t npix = (size_t)c->nx * c->ny;
-    dim3 grid((unsigned)((npix + SB_PIX - 1) / SB_PIX), (unsigned)((ts.n_bins + 1 + SB_BINS - 1) / SB_BINS), ts.n_probes);
+    if ((long long)ts.n_probes * n_frames_chunk > 0x7fffffffLL || 2 * npix > 0xffffffffULL)
+        return fail(c, PS_EUNSUPPORTED, "ps_tacaw_add: chunk has more than 2^31 rows");
+    if (!ts.have_ref) {                                                 // reference = the first frame this stream sees
+        PSB_CUDA(c, cudaMemcpy2DAsync(ts.d_ref.p, npix * sizeof(float2), d_exit_chunk, (size_t)n_frames_chunk * npix * sizeof(float2),
+                                      npix * sizeof(float2), ts.n_probes, cudaMemcpyDeviceToDevice, c->stream));
+        ts.have_ref = true;
+    }
+    if ((st = ensure_buf(c, ts.d_tw, (size_t)n_frames_chunk * ts.n_bins * sizeof(float2))) != PS_OK) return st;
+    CUtensorMap cmap;
+    if (!tma::make_map_2d_f32(&cmap, (void*)d_exit_chunk, 2ull * npix, (uint64_t)ts.n_probes * n_frames_chunk, 2 * SB_PIX, SB_FR))
+        return fail(c, PS_ECUDA, "ps_tacaw_add: cuTensorMapEncodeTiled failed (chunk must be 16-byte aligned)");
+    int cap_unused = 0;
+    PSB_CUDA(c, kernel_cap(c, k_tacaw_accum, SB_THREADS, SB_SMEM, &cap_unused));
     ProfScope ps_(c, K_TACAW_ACCUM);
-    k_tacaw_accum<<<grid, SB_PIX, 0, c->stream>>>((const float2*)d_exit_chunk, (float2*)ts.d_acc, ts.d_bins, ts.n_bins,
-                                                 ts.n_frames_total, frame0, n_frames_chunk, npix, c->nx, c->ny, c->d_nmax);
+    const int n_tw = n_frames_chunk * ts.n_bins;
+    k_tacaw_twiddles<<<(n_tw + 255) / 256, 256, 0, c->stream>>>((float2*)ts.d_tw.p, (const int32_t*)ts.d_bins.p, ts.n_bins,
+                                                               ts.n_frames_total, frame0, n_frames_chunk);
+    PSB_LAUNCH_CHECK(c, "k_tacaw_twiddles");
+    dim3 grid((unsigned)(npix / SB_PIX), ts.n_probes);
+    k_tacaw_accum<<<grid, SB_THREADS, SB_SMEM, c->stream>>>(cmap, (float2*)ts.d_acc, (const float2*)ts.d_ref.p,
+                                                           (const float2*)ts.d_tw.p, ts.n_bins, n_frames_chunk, npix, c->nx,
+                                                           c->ny, c->d_nmax);
     PSB_LAUNCH_CHECK(c, "k_tacaw_accum");
     ts.frames_seen += n_frames_chunk;
+    ts.next_frame = frame0 + n_frames_chunk;
+    return PS_OK;
+}
+
+static ps_status tacaw_finish_impl(ps_ctx* c, const void* d_acc, size_t n_k, float* d_I) {
+    TacawStream& ts = c->ts;
+    const long long total = (long long)ts.n_probes * ts.n_bins * (long long)n_k;
+    ProfScope ps_(c, K_TACAW_FINISH);
+    k_tacaw_finish<<<(unsigned)((total + 255) / 256), 256, 0, c->stream>>>((const float2*)d_acc, d_I, (const int32_t*)ts.d_bins.p,
+                                                                           ts.n_bins, n_k, total);
+    PSB_LAUNCH_CHECK(c, "k_tacaw_finish");
     return PS_OK;
 }
 
@@ -447,16 +522,25 @@ extern "C" ps_status ps_tacaw_finish(ps_ctx* c, float* d_I) {
     if (!c) return PS_EINVAL;
     TacawStream& ts = c->ts;
     if (!ts.active) return fail(c, PS_ESTATE, "ps_tacaw_finish: ps_tacaw_begin has not been called");
+    ps_status st = enter(c, "ps_tacaw_finish");
+    if (st != PS_OK) return st;
     if (!d_I) return fail(c, PS_EINVAL, "ps_tacaw_finish: d_I is NULL");
     if (ts.frames_seen != ts.n_frames_total)
         return fail(c, PS_ESTATE, "ps_tacaw_finish: " + std::to_string(ts.frames_seen) + " of " +
                                       std::to_string(ts.n_frames_total) + " frames were added");
-    const size_t npix = (size_t)c->nx * c->ny;
-    const long long total = (long long)ts.n_probes * ts.n_bins * npix;
-    ProfScope ps_(c, K_TACAW_FINISH);
-    k_tacaw_finish<<<(unsigned)((total + 255) / 256), 256, 0, c->stream>>>((const float2*)ts.d_acc, d_I, ts.d_bins, ts.n_bins,
-                                                                           npix, total);
-    PSB_LAUNCH_CHECK(c, "k_tacaw_finish");
-    ts.active = false;
-    return PS_OK;
+    st = tacaw_finish_impl(c, ts.d_acc, (size_t)c->nx * c->ny, d_I);
+    if (st == PS_OK) ts.active = false;
+    return st;
+}
+
+extern "C" ps_status ps_tacaw_finish_shard(ps_ctx* c, const void* d_acc_shard, size_t n_k, float* d_I_shard) {
+    if (!c) return PS_EINVAL;
+    TacawStream& ts = c->ts;
+    if (!ts.active) return fail(c, PS_ESTATE, "ps_tacaw_finish_shard: ps_tacaw_begin has not been called");
+    ps_status st = enter(c, "ps_tacaw_finish_shard");
+    if (st != PS_OK) return st;
+    if (!d_acc_shard || !d_I_shard || n_k == 0) return fail(c, PS_EINVAL, "ps_tacaw_finish_shard: null pointer or empty shard");
+    st = tacaw_finish_impl(c, d_acc_shard, n_k, d_I_shard);
+    if (st == PS_OK) ts.active = false;
+    return st;
 }

@@ -190,12 +190,9 @@ k_vk_tc(const uint32_t* __restrict__ sUx, const uint32_t* __restrict__ sUy, cons
 // host launcher (called from ps_build_slices): tiles of 128 m-values x Tn n-values over the quarter plane
 cudaError_t launch_vk_tc(ps_ctx* c, const uint32_t* sUx, const uint32_t* sUy, const int32_t* off, float2* Vk, int n_atoms,
                          int nf) {
-    static bool attr_done = false;
-    if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(k_vk_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES);
-        if (e != cudaSuccess) return e;
-        attr_done = true;
-    }
+    int cap_unused = 0;                                                    // sets the shared-memory attribute once per ctx
+    cudaError_t ce = kernel_cap(c, k_vk_tc, THREADS, SMEM_BYTES, &cap_unused);
+    if (ce != cudaSuccess) return ce;
     const int tiles_m = (c->mcut + 1 + TM - 1) / TM;
     const int tiles_n = (c->ncut + 1 + TN_MAX - 1) / TN_MAX;
     int Tn = ((c->ncut + 1 + tiles_n - 1) / tiles_n + 7) & ~7;            // equal-width n tiles, multiple of 8

@@ -31,12 +31,104 @@ def _exit_waves(P, F, n=6, seed=3):
     return (rng.normal(size=(P, F, n, n)) + 1j * rng.normal(size=(P, F, n, n))) * 0.1 + (2.0 - 1.0j)
 
 
+class OracleOps:
+    """run_sharded's device work stood in for by the float64 oracle (the kernels cannot run here): same methods as
+    sharding.LibraryOps, torch CPU tensors in and out.  The streaming accumulator follows the contract of
+    include/pyslice_b200.h (global frame index in the twiddle, shared reference wave, bin 0 := 0)."""
+
+    def __init__(self, w):
+        from workloads import form_factor_coefficients
+        self.w = w
+        self.nl, self.ng, self.coef = form_factor_coefficients(w.elements, w.ff_kind)
+        self.elem = np.searchsorted(w.elements, w.Z)
+        self.pos = w.positions()
+
+    def build_slices(self, f0, f1):
+        w = self.w
+        return np.stack([O.projected_potential(self.pos[f], self.elem, self.coef, self.nl, self.ng, w.cell, w.nx, w.ny,
+                                               w.n_slices)[0] for f in range(f0, f1)])
+
+    def incident(self, p0, p1):
+        w = self.w
+        if w.beam == "probe":
+            return [O.probe_wave(w.cell, w.nx, w.ny, w.kV, w.semi_angle_mrad, x, y) for x, y in w.probe_xy[p0:p1]]
+        return [O.plane_wave(w.nx, w.ny)]
+
+    def multislice(self, psi0, V):
+        return torch.from_numpy(np.stack([[O.multislice(p, v, self.w.cell, self.w.kV) for v in V] for p in psi0]))
+
+    def tacaw(self, ex, bins):
+        return torch.from_numpy(np.stack([O.tacaw_intensity(e, bins) for e in ex.numpy()]).astype(np.float32))
+
+    def sdp(self, I, lo, hi):
+        return torch.from_numpy(O.sdp(I.numpy().astype(np.float64), lo, min(hi, I.shape[1] - 1)).astype(np.float32))
+
+    def spectrum_image(self, I):
+        return torch.from_numpy(I.numpy().astype(np.float64).sum(axis=(2, 3)).astype(np.float32))
+
+    def stream_begin(self, P, F, bins):
+        self.F, self.bins = F, np.asarray(bins) % F
+        self.acc = np.zeros((P, len(bins), self.w.ny * self.w.nx), complex)
+        self.ref = None
+
+    def stream_set_reference(self, ref):
+        self.ref = ref.numpy().reshape(ref.shape[0], 1, -1)
+
+    def stream_add(self, ex, frame0):
+        x = ex.numpy().reshape(ex.shape[0], ex.shape[1], -1) - self.ref
+        j = frame0 + np.arange(ex.shape[1])
+        self.acc += np.einsum("bj,pjk->pbk", np.exp(-2j * np.pi * np.outer(self.bins, j) / self.F), x)
+
+    def stream_accumulators(self):
+        return torch.from_numpy(self.acc)
+
+    def stream_finish_shard(self, acc_shard):
+        I = np.abs(acc_shard.numpy()) ** 2
+        I[:, self.bins == 0] = 0.0
+        return torch.from_numpy(I.astype(np.float32))
+
+    def as_images(self, I_flat):
+        return I_flat.reshape(I_flat.shape[0], I_flat.shape[1], self.w.ny, self.w.nx)
+
+
+def _sharded_case(case, rank, world):
+    """The function bench.py --scaling strong runs (sharding.run_sharded), with the oracle as the device: the combined
+    result must equal the oracle on the whole, unsharded problem."""
+    from workloads import make_workload
+    if case == "sharded_probe":
+        w = make_workload("c3_si_probe_512", mini=True, n_frames=8, grid=32)          # 4 probes >= 2 ranks
+        w.n_slices = 2
+        bins = None
+    else:
+        w = make_workload("c1_si_128", mini=True, n_frames=13, grid=32)              # 1 probe < 2 ranks, ragged frames
+        w.n_slices = 2
+        bins = np.array([0, 1, 2, -1, 5, -6], dtype=np.int64)
+    ops = OracleOps(w)
+    out = sharding.run_sharded(ops, w.n_probes, w.n_frames, bins, rank, world, frame_chunk=3)
+    assert out["plan"].axis == ("probe" if case == "sharded_probe" else "frame")
+    I_all, _ = O.run_path(ops.pos, ops.elem, ops.coef, ops.nl, ops.ng, w.cell, w.nx, w.ny, w.n_slices, w.kV,
+                          ops.incident(0, w.n_probes), bins)
+    want_sdp = O.sdp(I_all, 1, min(4, I_all.shape[1] - 1))
+    want_si = I_all.sum(axis=(2, 3))
+    ok = np.allclose(out["sdp"].numpy(), want_sdp, rtol=2e-5, atol=1e-6 * want_sdp.max())
+    ok = ok and np.allclose(out["spectrum_image"].numpy(), want_si, rtol=2e-5, atol=1e-6 * want_si.max())
+    if case == "sharded_frame":                                                      # this rank's k-slice of I
+        npix = w.nx * w.ny
+        n_k = -(-npix // world)
+        mine = I_all.reshape(1, len(bins), npix)[:, :, rank * n_k:(rank + 1) * n_k]
+        got = out["I_local"].numpy()[:, :, :mine.shape[2]]
+        ok = ok and np.allclose(got, mine, rtol=2e-5, atol=1e-6 * I_all.max())
+    return ok
+
+
 def _worker(rank, world, port, case, out):
     os.environ["MASTER_ADDR"] = "127.0.0.1"
     os.environ["MASTER_PORT"] = str(port)
     dist.init_process_group("gloo", rank=rank, world_size=world)
     try:
-        if case == "frame":
+        if case.startswith("sharded_"):
+            ok = _sharded_case(case, rank, world)
+        elif case == "frame":
             P, F = 1, 37                                            # P < world -> frame shards, ragged split
             bins = np.array([0, 1, -1, 5, 18, -18], dtype=np.int64)
             x = _exit_waves(P, F)
@@ -84,7 +176,7 @@ def _worker(rank, world, port, case, out):
         dist.destroy_process_group()
 
 
-@pytest.mark.parametrize("case", ["frame", "probe", "trajectory"])
+@pytest.mark.parametrize("case", ["frame", "probe", "trajectory", "sharded_probe", "sharded_frame"])
 def test_world_size_2_gloo(case):
     world = 2
     mgr = mp.Manager()

@@ -393,3 +393,224 @@ def test_vacuum_row_shortcut_is_exact(torch, nx, ny):
         eo = O.multislice(psi0[0].astype(np.complex128), V32[i].astype(np.float64), w.cell, 80.0)
         assert rel_l2(a[0, i].cpu().numpy(), eo) < TOL_EXIT
         assert rel_l2(b[0, i].cpu().numpy(), eo) < TOL_EXIT
+
+
+# ----------------------------------------------------------------------------- round-2 additions
+def per_bin_errors(Ig, Io):
+    """(per-bin rel-L2, per-bin max|dI| / max_k I_bin) of I[...][n_bins][ny][nx] against the oracle, bins whose oracle
+    intensity is identically zero (bin 0) excluded from the ratios."""
+    nb = Io.shape[-3]
+    g = np.moveaxis(Ig, -3, 0).reshape(nb, -1).astype(np.float64)
+    o = np.moveaxis(Io, -3, 0).reshape(nb, -1)
+    num = np.linalg.norm(g - o, axis=1)
+    den = np.linalg.norm(o, axis=1)
+    mx = np.abs(g - o).max(axis=1)
+    omx = o.max(axis=1)
+    ok = den > 0
+    assert np.all(num[~ok] == 0.0), "bins that are exactly zero in the oracle must be exactly zero"
+    return num[ok] / den[ok], mx[ok] / omx[ok]
+
+
+def test_tacaw_per_bin_parity_same_exit_waves(torch):
+    """The transform alone, judged bin by bin (a wrong weak bin cannot hide behind the strong ones): both sides get the
+    same complex64 exit waves, with an elastic term 100x the fluctuation and EVERY bin of both signs of omega populated,
+    amplitudes spread over two decades (four in intensity).  (Bins more than ~1e-3 below the strongest one in amplitude
+    sit on the fp32 floor of a length-F transform, eps log2(F) |strongest|, and cannot be held to 1e-3: DESIGN.md §7.)"""
+    import paper_2602_10064_b200 as ps
+    rng = np.random.default_rng(77)
+    w = make_workload("c2_hbn_256", mini=True)
+    ctx = make_ctx(w)
+    F, P = 256, 2
+    A = O.aperture_mask(w.cell, w.nx, w.ny)
+    j = np.arange(F)
+    amp = 10.0 ** rng.uniform(-2, 0, size=F)                             # per-frequency amplitudes over two decades
+    x = np.zeros((P, F, w.ny, w.nx), complex)
+    for n in range(1, F):                                               # n > F/2 are the negative frequencies
+        ph = rng.uniform(0, 2 * np.pi, size=(P, 1, w.ny, w.nx))
+        x += 0.01 * amp[n] * np.exp(1j * (2 * np.pi * n * j[None, :, None, None] / F + ph))
+    x = ((x + (3.0 - 2.0j)) * A).astype(np.complex64)
+    bins = np.arange(-F // 2, F // 2, dtype=np.int32)
+    Ig = ps.ps_tacaw(ctx, _t(torch, x), 2.0, bins).cpu().numpy()
+    Io = np.stack([O.tacaw_intensity(x[p].astype(np.complex128), bins) for p in range(P)])
+    rel, mx = per_bin_errors(Ig, Io)
+    assert rel.max() < TOL_I and mx.max() < TOL_I, (rel.max(), mx.max())
+
+
+@pytest.mark.parametrize("name", MINIS)
+def test_end_to_end_per_bin(torch, name):
+    """positions -> I(k, w) on the mini twins, judged per omega bin.  Bins are held to TOL_I in rel-L2 and in
+    max|dI| / max_k I; the bound for weak bins allows for the white floor that the exit-wave tolerance itself implies
+    (an exit-wave error delta per frame spreads over all bins as delta^2 F)."""
+    import paper_2602_10064_b200 as ps
+    from workloads import form_factor_coefficients
+    w = make_workload(name, mini=True)
+    ctx = make_ctx(w)
+    pos = w.positions()
+    V = ps.ps_build_slices(ctx, _t(torch, pos), _t(torch, w.Z))
+    ex = ps.ps_multislice(ctx, w.kV, gpu_incident(ctx, w), V)
+    Ig = ps.ps_tacaw(ctx, ex, w.dt_fs, w.bins).cpu().numpy()
+    nl, ng, coef = form_factor_coefficients(w.elements, w.ff_kind)
+    Io, exo = O.run_path(pos, np.searchsorted(w.elements, w.Z), coef, nl, ng, w.cell, w.nx, w.ny, w.n_slices, w.kV,
+                         oracle_incident(w), w.bins)
+    F = pos.shape[0]
+    nb = Io.shape[1]
+    g = np.moveaxis(Ig, 1, 0).reshape(nb, -1).astype(np.float64)
+    o = np.moveaxis(Io, 1, 0).reshape(nb, -1)
+    # white floor implied by the exit-wave tolerance: amplitude error per pixel and bin <= TOL_EXIT * rms|Psi| * sqrt(F)
+    d_amp = TOL_EXIT * np.sqrt(np.mean(np.abs(exo) ** 2)) * np.sqrt(F)
+    for b in range(nb):
+        if not o[b].any():
+            assert not g[b].any()
+            continue
+        allowed = TOL_I * np.linalg.norm(o[b]) + np.linalg.norm(2.0 * np.sqrt(o[b]) * d_amp + d_amp ** 2)
+        assert np.linalg.norm(g[b] - o[b]) < allowed, (b, np.linalg.norm(g[b] - o[b]), allowed)
+        assert np.abs(g[b] - o[b]).max() < TOL_I * o[b].max() + 2.0 * np.sqrt(o[b].max()) * d_amp + d_amp ** 2
+
+
+def test_tacaw_streaming_full_length_with_large_elastic_term(torch):
+    """Path B at config 4's real stream length: 4096 frames x 64^2, a (3-2i) elastic offset 100x the
+    fluctuation, 256 bins, 8 uneven chunks, against the oracle's mean-subtracted FFT, bin by bin."""
+    import paper_2602_10064_b200 as ps
+    from paper_2602_10064_b200.binding import TacawStream
+    rng = np.random.default_rng(4096)
+    w = make_workload("c1_si_128", mini=True)                          # 64 x 64 grid
+    ctx = make_ctx(w)
+    F, nb = 4096, 256
+    A = O.aperture_mask(w.cell, w.nx, w.ny)
+    x = (rng.normal(size=(1, F, w.ny, w.nx)) + 1j * rng.normal(size=(1, F, w.ny, w.nx))) * 0.03
+    j = np.arange(F)[None, :, None, None]
+    for n in (1, 3, 40, 255):                                           # a few coherent lines on top of the white part
+        x += 0.02 * np.exp(2j * np.pi * (n * j / F + rng.uniform(size=(1, 1, w.ny, w.nx))))
+    x = ((x + (3.0 - 2.0j)) * A).astype(np.complex64)
+    bins = np.arange(nb, dtype=np.int32)
+    ts = TacawStream(ctx, 1, F, 2.0, bins)
+    xg = _t(torch, x)
+    cuts = [0, 64, 65, 700, 1024, 1999, 3000, 4000, 4096]
+    for f0, f1 in zip(cuts[:-1], cuts[1:]):
+        ts.add(xg[:, f0:f1].contiguous(), f0)
+    Ig = ts.finish().cpu().numpy()
+    Io = O.tacaw_intensity(x[0].astype(np.complex128), bins)[None]
+    rel, mx = per_bin_errors(Ig, Io)
+    assert rel.max() < TOL_I and mx.max() < TOL_I, (rel.max(), mx.max())
+    assert rel_l2(Ig, Io) < TOL_I
+
+
+def test_tacaw_streaming_rejects_out_of_order_chunks(torch):
+    import paper_2602_10064_b200 as ps
+    from paper_2602_10064_b200.binding import TacawStream
+    w = make_workload("c1_si_128", mini=True)
+    ctx = make_ctx(w)
+    x = torch.zeros((1, 8, w.ny, w.nx), dtype=torch.complex64, device="cuda")
+    ts = TacawStream(ctx, 1, 32, 2.0, np.arange(4, dtype=np.int32))
+    ts.add(x, 0)
+    with pytest.raises(ps.PSError) as ei:                                # frames 0..7 again: would be counted twice
+        ts.add(x, 0)
+    assert ei.value.status == -5
+    with pytest.raises(ps.PSError):                                      # a gap (frames 8..15 skipped)
+        ts.add(x, 16)
+    ts.add(x, 8)
+
+
+@pytest.mark.parametrize("F", [1024, 2048])
+def test_tacaw_ring_many_probes_large_grid(torch, F):
+    """The TMA-ring kernels with more blocks than pixel groups per probe and P = 5 (the per-probe carry of the group
+    list), few bins (the shape for which the ring is chosen)."""
+    import paper_2602_10064_b200 as ps
+    rng = np.random.default_rng(F + 5)
+    w = make_workload("c1_si_128", mini=True)
+    w.nx, w.ny = 32, 64
+    w.cell = np.array([32 * 0.11, 64 * 0.12, 6.0])
+    ctx = make_ctx(w)
+    P = 5
+    A = O.aperture_mask(w.cell, w.nx, w.ny)
+    x = ((rng.normal(size=(P, F, w.ny, w.nx)) + 1j * rng.normal(size=(P, F, w.ny, w.nx))) * 0.05 + (1.0 + 0.5j)) * A
+    x = x.astype(np.complex64)
+    bins = np.array([1, 2, 3, -1, F // 2 - 1, 17, 100, -100], dtype=np.int32)
+    Ig = ps.ps_tacaw(ctx, _t(torch, x), 2.0, bins).cpu().numpy()
+    for p in range(P):
+        Io = O.tacaw_intensity(x[p].astype(np.complex128), bins)
+        assert rel_l2(Ig[p], Io) < TOL_I
+    assert float(np.abs(Ig[:, :, ~A]).max()) == 0.0
+
+
+def test_incident_tilt_both_axes_and_negative(torch):
+    """ps_make_incident with tilts (m_t, n_t): n_t != 0 and negative m_t (reading A18), against the oracle's tilted
+    plane wave (pinned on the CPU by its reciprocal-grid delta)."""
+    import paper_2602_10064_b200 as ps
+    w = make_workload("c5_al_sweep", mini=True)
+    w.nx, w.ny = 64, 128
+    ctx = make_ctx(w)
+    tilts = np.array([[-3, 2], [0, -5], [7, 0], [-1, -1], [0, 0]], dtype=np.float64)
+    g = ps.ps_make_incident(ctx, w.kV, 0.0, tilts, is_tilt=True).cpu().numpy()
+    o = np.stack([O.tilted_plane_wave(w.nx, w.ny, int(m), int(n)) for m, n in tilts])
+    assert rel_l2(g, o) < TOL_PSI0
+    spec = np.fft.fft2(g[0])
+    assert abs(spec[2, w.nx - 3] - w.nx * w.ny) < 1e-3 * w.nx * w.ny     # the delta sits at [n_t mod ny][m_t mod nx]
+
+
+@pytest.mark.parametrize("nx,ny", [(32, 32), (64, 32), (32, 64)])
+def test_build_slices_small_grids_with_vacuum_slabs(torch, nx, ny):
+    """Grids on which one block of the row kernel spans several slice pairs: a thin slab in a tall vacuum
+    box (most slice pairs empty), an odd frame count and an odd slice count; V is pre-filled with NaN so that any
+    element the library fails to write is caught."""
+    import paper_2602_10064_b200 as ps
+    w = make_workload("c2_hbn_256", mini=True)                          # a monolayer at z = Lz/2
+    w.nx, w.ny, w.n_slices = nx, ny, 11
+    ctx = make_ctx(w)
+    pos = w.positions(0, 3)
+    for mode in (1, 2):
+        ctx.set_vk_mode(mode)
+        V = torch.full((3, w.n_slices, ny, nx), float("nan"), dtype=torch.float32, device="cuda")
+        ps.ps_build_slices(ctx, _t(torch, pos), _t(torch, w.Z), d_V=V)
+        Vn = V.cpu().numpy()
+        assert np.isfinite(Vn).all(), "ps_build_slices left elements of V unwritten"
+        for i in range(3):
+            Vo, _ = oracle_potential(w, pos[i])
+            assert rel_l2(Vn[i], Vo) < TOL_V
+            empty = ~Vo.reshape(w.n_slices, -1).any(axis=1)
+            assert empty.sum() >= 8 and not Vn[i][empty].any()           # vacuum slices are exact zeros
+
+
+def test_warm_calls_do_not_wait_for_the_stream(torch):
+    """include/pyslice_b200.h "when a call may block": a warmed-up ps_build_slices / ps_make_incident / ps_tacaw /
+    ps_dispersion enqueues its work and returns while earlier work on the stream is still running."""
+    import paper_2602_10064_b200 as ps
+    w = make_workload("c3_si_probe_512", mini=True)
+    ctx = make_ctx(w)
+    pos = _t(torch, w.positions(0, 32)); Z = _t(torch, w.Z)
+    V = ps.ps_build_slices(ctx, pos, Z)                                  # warm-up: tables, scratch, Z validation
+    psi0 = gpu_incident(ctx, w)
+    ex = ps.ps_multislice(ctx, w.kV, psi0, V)
+    I = ps.ps_tacaw(ctx, ex, w.dt_fs)
+    kx = np.linspace(0, 0.1, 9); ky = np.zeros(9)
+    ps.ps_dispersion(ctx, I, kx, ky)
+    torch.cuda.synchronize()
+    done = torch.cuda.Event()
+    torch.cuda._sleep(int(1.5e9))                                         # ~0.8 s of device time ahead of everything else
+    ps.ps_build_slices(ctx, pos, Z, d_V=V)
+    ps.ps_make_incident(ctx, w.kV, w.semi_angle_mrad, w.probe_xy, d_psi0=psi0)
+    ps.ps_multislice(ctx, w.kV, psi0, V, d_exit=ex)
+    ps.ps_tacaw(ctx, ex, w.dt_fs, d_I=I)
+    ps.ps_dispersion(ctx, I, kx, ky)
+    done.record()
+    assert not done.query(), "a warmed-up hot-path call waited for the stream"
+    torch.cuda.synchronize()
+
+
+def test_unknown_Z_after_validation_is_reported_by_the_next_call(torch):
+    """The asynchronous error channel: same (d_Z, n_atoms) pair as a validated call, contents changed behind the
+    library's back -> the device-side check raises the ctx's error word and the next call reports it."""
+    import paper_2602_10064_b200 as ps
+    w = make_workload("c1_si_128", mini=True)
+    ctx = make_ctx(w)
+    pos = _t(torch, w.positions(0, 2)); Z = _t(torch, w.Z)
+    ps.ps_build_slices(ctx, pos, Z)
+    Z[5] = 79                                                            # in place: same pointer, same count
+    ps.ps_build_slices(ctx, pos, Z)                                      # queued without a host wait
+    torch.cuda.synchronize()
+    with pytest.raises(ps.PSError) as ei:
+        ps.ps_make_incident(ctx, w.kV)
+    assert ei.value.status == -2 and "79" in str(ei.value)
+    Z[5] = int(w.Z[5])
+    V = ps.ps_build_slices(ctx, pos, Z)                                  # the ctx stays usable
+    assert torch.isfinite(V).all()
