@@ -380,7 +380,7 @@ def main():
     ap.add_argument("--probes-side", type=int, default=None, help="override probes per scan side / number of tilts")
     ap.add_argument("--wave-chunk", type=int, default=0)
     ap.add_argument("--tune", action="append", default=[], metavar="KEY=VALUE",
-                    help="ps_set_tuning knob (col_c, row_light); repeatable")
+                    help="ps_set_tuning knob (resident=-1|0|1); repeatable")
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
                     help="N > 1: weak = an independent trajectory per rank (reductions averaged); strong = ONE problem "
                          "sharded by sharding.plan() (probe shards, or frame shards + reduce-scatter of the accumulators)")
@@ -556,49 +556,73 @@ def main():
     # k-columns that hold in-band points (f_col of them); V is read once per FRAME (its rows are shared by the P probes
     # of the frame inside a launch), i.e. 4/P bytes per pixel of one wave
     f_col = band_columns(w.cell, nx, ny) / nx
-    alg = {"k_row_transmit": 16.0 * f_col + 4.0 / P, "k_col_propagate": 16.0 * f_col}
-    dom = max(alg, key=lambda k: kern.get(k, (0.0, 0))[0])
-    dom_ms, dom_n = kern[dom]
-    px_waves_per_launch = units_rank * K / dom_n
-    alg_bytes_launch = alg[dom] * px_waves_per_launch
-    achieved = alg_bytes_launch / (dom_ms / dom_n * 1e-3) / 1e9
-    ms_pair = kern["k_row_transmit"][0] + kern["k_col_propagate"][0]
-    pair_gbs = (alg["k_row_transmit"] + alg["k_col_propagate"]) * units_rank * K / (ms_pair * 1e-3) / 1e9
     sm_clock = (clocks.get("sm_mhz") or 1965.0) * 1e6
+    issue_peak = N_SM * LANES_PER_SM * sm_clock
 
-    def co_limits(kname, n_grid, ms_launch):
-        """ncu-derived constants of this kernel at this grid size -> DRAM traffic per launch and FP32-issue utilisation."""
-        st = stats.get(f"{kname}<{n_grid}>")
+    def issue_of(key, px_per_s):
+        """FP32-issue co-limit from the ncu-derived instruction count of this kernel at this grid size."""
+        st = stats.get(key)
         if not st:
             return None, None
-        px_s = px_waves_per_launch / (ms_launch * 1e-3)
-        issue = {"thread_inst_per_px": st["thread_inst_per_px"],
-                 "peak_thread_inst_per_s": N_SM * LANES_PER_SM * sm_clock,
-                 "frac": st["thread_inst_per_px"] * px_s / (N_SM * LANES_PER_SM * sm_clock),
-                 "note": "thread instructions per pixel (ncu, profiles/r2_kernel_stats.json) x pixels/s / (148 SMs x 128 "
-                         "lanes x SM clock sampled in this run): the FP32-issue co-limit of the FFT passes"}
-        traffic = st["dram_bytes_per_px"].get(str(P), st["dram_bytes_per_px"].get("any"))
-        return (traffic * px_waves_per_launch if traffic is not None else None), issue
+        return st, {"thread_inst_per_px": st["thread_inst_per_px"], "peak_thread_inst_per_s": issue_peak,
+                    "frac": st["thread_inst_per_px"] * px_per_s / issue_peak,
+                    "note": "thread instructions per pixel (ncu, profiles/r2_kernel_stats.json) x pixels/s / (148 SMs x 128 "
+                            "lanes x SM clock sampled in this run): the FP32-issue co-limit of the FFT passes"}
 
-    traffic, issue = co_limits(dom, nx if dom == "k_row_transmit" else ny, dom_ms / dom_n)
-    roofline = {"bound": "hbm", "kernel": f"{dom}<{nx if dom == 'k_row_transmit' else ny}>", "achieved": achieved,
-                "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
-                "bytes_per_launch": alg_bytes_launch, "avg_launch_ms": dom_ms / dom_n,
-                "algorithmic_bytes_per_px": alg[dom], "band_column_fraction": f_col,
-                "fp32_issue": issue,
-                "slice_step_pair": {"achieved": pair_gbs, "frac": pair_gbs / peak,
-                                    "gpx_slice_s": units_rank * K / (ms_pair * 1e-3) / 1e9,
-                                    "algorithmic_bytes_per_px_slice": alg["k_row_transmit"] + alg["k_col_propagate"]},
-                "kernel_ms_per_step": {k: v[0] / K for k, v in kern.items()},
-                "kernel_times_from": "a second pass of the same K steps with per-launch CUDA events recorded by the library "
-                                     "on its stream (ps_profile_*), not the pass `value` was timed on",
-                "profiled_ms_per_step": ms_prof_total / K}
-    other = "k_col_propagate" if dom == "k_row_transmit" else "k_row_transmit"
-    o_ms, o_n = kern[other]
-    o_tr, o_issue = co_limits(other, ny if other == "k_col_propagate" else nx, o_ms / o_n)
-    o_ach = alg[other] * px_waves_per_launch / (o_ms / o_n * 1e-3) / 1e9
-    roofline["other_pass"] = {"kernel": other, "achieved": o_ach, "frac": o_ach / peak, "traffic": o_tr,
-                              "avg_launch_ms": o_ms / o_n, "fp32_issue": o_issue}
+    if "k_slice_resident" in kern:
+        # chip-resident slice loop (small square grids, small batches): the wave never leaves shared memory, so HBM sees
+        # V once per frame and slice plus the incident wave in and the exit wave out: the kernel is bound by
+        # instruction issue, and that is the roofline reported
+        ms_res, n_res = kern["k_slice_resident"]
+        px_s = units_rank * K / (ms_res * 1e-3)
+        alg_px = 4.0 / P + 16.0 / S
+        st, issue = issue_of(f"k_slice_resident<{nx}>", px_s)
+        roofline = {"bound": "alu", "kernel": f"k_slice_resident<{nx}>", "unit": "thread-instructions/s",
+                    "achieved": (st["thread_inst_per_px"] * px_s) if st else None, "peak": issue_peak,
+                    "frac": issue["frac"] if issue else None,
+                    "traffic": (st["dram_bytes_per_px"].get("any") * units_rank * K / n_res) if st else None,
+                    "avg_launch_ms": ms_res / n_res, "gpx_slice_s": px_s / 1e9,
+                    "hbm": {"algorithmic_bytes_per_px_slice": alg_px, "achieved_GBps": alg_px * px_s / 1e9,
+                            "frac_of_hbm_peak": alg_px * px_s / 1e9 / peak},
+                    "peak_source": "148 SMs x 128 lanes x sampled SM clock (DESIGN.md §6)",
+                    "kernel_ms_per_step": {k: v[0] / K for k, v in kern.items()},
+                    "kernel_times_from": "a second pass of the same K steps with per-launch CUDA events recorded by the "
+                                         "library on its stream (ps_profile_*), not the pass `value` was timed on",
+                    "profiled_ms_per_step": ms_prof_total / K}
+    else:
+        alg = {"k_row_transmit": 16.0 * f_col + 4.0 / P, "k_col_propagate": 16.0 * f_col}
+        dom = max(alg, key=lambda k: kern.get(k, (0.0, 0))[0])
+        other = "k_col_propagate" if dom == "k_row_transmit" else "k_row_transmit"
+        per = {}
+        for kname in (dom, other):
+            k_ms, k_n = kern[kname]
+            px_launch = units_rank * K / k_n
+            n_grid = nx if kname == "k_row_transmit" else ny
+            st, issue = issue_of(f"{kname}<{n_grid}>", px_launch / (k_ms / k_n * 1e-3))
+            tr = None
+            if st:
+                tr = st["dram_bytes_per_px"].get(str(P), st["dram_bytes_per_px"].get("any"))
+                tr = tr * px_launch if tr is not None else None
+            ach = alg[kname] * px_launch / (k_ms / k_n * 1e-3) / 1e9
+            per[kname] = {"kernel": f"{kname}<{n_grid}>", "achieved": ach, "frac": ach / peak, "traffic": tr,
+                          "bytes_per_launch": alg[kname] * px_launch, "avg_launch_ms": k_ms / k_n,
+                          "algorithmic_bytes_per_px": alg[kname], "fp32_issue": issue}
+        ms_pair = kern["k_row_transmit"][0] + kern["k_col_propagate"][0]
+        pair_gbs = (alg["k_row_transmit"] + alg["k_col_propagate"]) * units_rank * K / (ms_pair * 1e-3) / 1e9
+        roofline = {"bound": "hbm", "unit": "GB/s", "peak": peak, "peak_source": peak_src, "band_column_fraction": f_col}
+        roofline.update(per[dom])
+        roofline.update({
+            "algorithmic_bytes_note": "wave read + written once per pass on the k-columns holding in-band points; V read "
+                                      "once per FRAME and slice (its rows are shared by the probes of a launch): 4/P B per "
+                                      "pixel of one wave (DESIGN.md §6)",
+            "other_pass": per[other],
+            "slice_step_pair": {"achieved": pair_gbs, "frac": pair_gbs / peak,
+                                "gpx_slice_s": units_rank * K / (ms_pair * 1e-3) / 1e9,
+                                "algorithmic_bytes_per_px_slice": alg["k_row_transmit"] + alg["k_col_propagate"]},
+            "kernel_ms_per_step": {k: v[0] / K for k, v in kern.items()},
+            "kernel_times_from": "a second pass of the same K steps with per-launch CUDA events recorded by the library "
+                                 "on its stream (ps_profile_*), not the pass `value` was timed on",
+            "profiled_ms_per_step": ms_prof_total / K})
     if "k_tacaw_fft" in kern:
         tb = (8.0 * F + 4.0 * nb) * ctx.n_k_aperture * P + 4.0 * nb * (nx * ny - ctx.n_k_aperture) * P
         tms = kern["k_tacaw_fft"][0] / kern["k_tacaw_fft"][1]

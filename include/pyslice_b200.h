@@ -132,10 +132,10 @@ PS_API ps_status ps_set_workspace(ps_ctx* ctx, void* d_ws, size_t bytes);
  * 0 = library default = the whole batch in one launch per pass (profiles/r1_chunk_sweep.md). */
 PS_API ps_status ps_set_wave_chunk(ps_ctx* ctx, int n_waves);
 
-/* Tuning knobs of the slice-step kernels, by name (results are identical to rounding order; the defaults are the
- * measured optimum per grid size, profiles/r2_slice_step.md):
- *   "col_c"     columns per block of the column pass: 0 = default, 4 or 8 (4 applies to 512 <= ny <= 1024 only)
- *   "row_light" 1 = register-light row pass for nx >= 512 (stage-2 twiddles in shared memory, three blocks per SM)
+/* Named tuning knobs (results are identical to rounding order):
+ *   "resident"  chip-resident slice loop for square grids nx = ny <= 128 (one launch per ps_multislice, the wave kept
+ *               in shared memory through all slices; resident.cu): 0 = auto (batches of at most 2 x 148 waves, which
+ *               cannot fill the GPU with streaming launches), 1 = always, -1 = never
  * Unknown keys and values are PS_EINVAL. */
 PS_API ps_status ps_set_tuning(ps_ctx* ctx, const char* key, int value);
 

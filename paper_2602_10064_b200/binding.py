@@ -213,7 +213,7 @@ class Context:
         self._check(self._lib.ps_set_vk_mode(self._h, int(mode)))
 
     def set_tuning(self, key: str, value: int):
-        """Named tuning knobs of the slice-step kernels ("col_c", "row_light"); see include/pyslice_b200.h."""
+        """Named tuning knobs ("resident"); see include/pyslice_b200.h."""
         self._check(self._lib.ps_set_tuning(self._h, key.encode(), int(value)))
 
     def set_wave_chunk(self, n_waves: int):

@@ -338,12 +338,9 @@ extern "C" ps_status ps_set_tuning(ps_ctx* c, const char* key, int value) {
     if (!c) return PS_EINVAL;
     if (!key) return fail(c, PS_EINVAL, "ps_set_tuning: key is NULL");
     const std::string k(key);
-    if (k == "col_c") {
-        if (value != 0 && value != 4 && value != 8) return fail(c, PS_EINVAL, "ps_set_tuning: col_c must be 0 (default), 4 or 8");
-        c->tune_col_c = value;
-    } else if (k == "row_light") {
-        if (value != 0 && value != 1) return fail(c, PS_EINVAL, "ps_set_tuning: row_light must be 0 or 1");
-        c->tune_row_light = value;
+    if (k == "resident") {
+        if (value < -1 || value > 1) return fail(c, PS_EINVAL, "ps_set_tuning: resident must be -1 (never), 0 (auto) or 1 (always)");
+        c->tune_resident = value;
     } else {
         return fail(c, PS_EINVAL, "ps_set_tuning: unknown key '" + k + "'");
     }

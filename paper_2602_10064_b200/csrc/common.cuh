@@ -34,11 +34,11 @@ struct KvTables {                   // tables that depend on the accelerating vo
 
 enum KernelId {                      // per-kernel timing slots (ps_profile_*)
     K_BIN = 0, K_SORT, K_VK, K_V_COL, K_V_ROW, K_INCIDENT, K_ROW_TRANSMIT, K_COL_PROPAGATE, K_TACAW_FFT,
-    K_TACAW_ACCUM, K_TACAW_FINISH, K_REDUCE, K_COUNT
+    K_TACAW_ACCUM, K_TACAW_FINISH, K_REDUCE, K_SLICE_RESIDENT, K_COUNT
 };
 static const char* const kKernelNames[K_COUNT] = {
     "k_bin", "k_sort", "k_vk", "k_v_col", "k_v_row", "k_incident", "k_row_transmit", "k_col_propagate",
-    "k_tacaw_fft", "k_tacaw_accum", "k_tacaw_finish", "k_reduce"};
+    "k_tacaw_fft", "k_tacaw_accum", "k_tacaw_finish", "k_reduce", "k_slice_resident"};
 
 struct ProfRec { cudaEvent_t a, b; int id; };
 
@@ -94,8 +94,7 @@ struct ps_ctx {
     int wave_chunk = 0;
     int vacuum_shortcut = 0;                // ps_set_vacuum_shortcut: rows with V == 0 skip the transmit + FFT pair (exact)
     int vk_mode = 0;                        // ps_set_vk_mode: 0 auto, 1 FP32 SIMT sums, 2 tcgen05 3xTF32 sums
-    int tune_col_c = 0;                     // ps_set_tuning("col_c"): columns per block of the column pass (0 = default)
-    int tune_row_light = 0;                 // ps_set_tuning("row_light"): register-light row pass (3 blocks per SM)
+    int tune_resident = 0;                  // ps_set_tuning("resident"): chip-resident slice loop, 0 auto, 1 always, -1 never
 
     // form factors
     bool have_ff = false;
@@ -216,6 +215,9 @@ inline cudaError_t kernel_cap(ps_ctx* c, K kern, int threads, size_t smem, int* 
 ps_status ensure_kv(ps_ctx* c, double kV);
 ps_status ensure_ftab(ps_ctx* c);
 ps_status ensure_abtab(ps_ctx* c, double kV);                           // incident.cu
+bool resident_supported(const ps_ctx* c);                               // resident.cu
+cudaError_t launch_slice_resident(ps_ctx* c, float2* W, const float2* psi0, const float* V, int n_probes, int n_frames,
+                                  float sigma, int col_lo, int col_hi);
 cudaError_t launch_vk_tc(ps_ctx* c, const uint32_t* sUx, const uint32_t* sUy, const int32_t* off, float2* Vk, int n_atoms,
                          int nf);                                          // vk_tc.cu
 

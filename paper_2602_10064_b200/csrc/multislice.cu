@@ -20,15 +20,12 @@
 namespace psb {
 
 // ------------------------------------------------------------------------------------ row pass
-// LIGHT = register-light variant (stage-2 twiddles in shared memory, V fetched after the inverse transform): three
-// blocks per SM instead of two
-template <int NX, bool LIGHT = false> struct RowCfg {
+template <int NX> struct RowCfg {
     static constexpr int T = Plan<NX>::T;
     static constexpr int THREADS = (T > 256) ? T : 256;
     static constexpr int RPB = THREADS / T;                               // rows per block
-    static constexpr int MIN_BLOCKS = (THREADS <= 256) ? (LIGHT ? 3 : 2) : 1;   // cap registers at 128 (85 when LIGHT)
-    static constexpr size_t SMEM = (size_t)RPB * RowLine<NX>::LEN * sizeof(float2) +
-                                   (LIGHT ? (size_t)TwiddlesShared<NX>::TABLE * sizeof(float2) : 0);
+    static constexpr int MIN_BLOCKS = (THREADS <= 256) ? 2 : 1;           // cap registers at 128
+    static constexpr size_t SMEM = (size_t)RPB * RowLine<NX>::LEN * sizeof(float2);
     // rows are independent: only the T threads of a row synchronise (a warp, or a named barrier per row)
     using Sync = typename std::conditional<(T <= 32), WarpSync,
                                            typename std::conditional<(RPB > 1), GroupSync<T>, BlockSync>::type>::type;
@@ -38,27 +35,19 @@ struct ChunkMap {           // chunk of waves: probes [p0,p0+np) x frames [f0,f0
     int p0, np, f0, nf, F;  // F = total frames (exit layout [P][F][ny][nx])
 };
 
-template <int NX, bool FIRST, bool LIGHT>
-__global__ void __launch_bounds__(RowCfg<NX, LIGHT>::THREADS, RowCfg<NX, LIGHT>::MIN_BLOCKS)
+template <int NX, bool FIRST>
+__global__ void __launch_bounds__(RowCfg<NX>::THREADS, RowCfg<NX>::MIN_BLOCKS)
 k_row_transmit(float2* __restrict__ W, const float2* __restrict__ psi0, const float* __restrict__ V,
                const uint8_t* __restrict__ tile_active, const ChunkMap cm, const int ny, const int n_slices,
                const int slice, const float sigma, const int n_items, const int col_lo, const int col_hi,
                const int vacuum_shortcut) {
-    using Cfg = RowCfg<NX, LIGHT>;
-    using TW = typename std::conditional<LIGHT, TwiddlesShared<NX>, Twiddles<NX>>::type;
+    using Cfg = RowCfg<NX>;
     constexpr int T = Cfg::T;
     extern __shared__ float2 smem[];
     const int t = threadIdx.x % T, r = threadIdx.x / T;
     RowSlots slots{smem + (size_t)r * RowLine<NX>::LEN};
-    TW tw;
-    if constexpr (LIGHT) {
-        float2* tab = smem + (size_t)Cfg::RPB * RowLine<NX>::LEN;
-        TwiddlesShared<NX>::fill(tab, threadIdx.x, Cfg::THREADS);
-        __syncthreads();
-        tw.init(t, tab);
-    } else {
-        tw.init(t);
-    }
+    Twiddles<NX> tw;
+    tw.init(t);
     unsigned amask = 0;                                  // bit e: column t+e*T lies in an active tile
 #pragma unroll
     for (int e = 0; e < 16; ++e) amask |= (tile_active[(t + e * T) / kColTile] ? 1u : 0u) << e;
@@ -98,8 +87,8 @@ k_row_transmit(float2* __restrict__ W, const float2* __restrict__ psi0, const fl
         float2* wrow = W + (((size_t)p * cm.F + f) * ny + y) * NX;
         float2 v[16];
         float sv[16];                                    // sigma * V of this row, fetched with the wave
-        const float* vrow = V + (((size_t)f * n_slices + slice) * ny + y) * NX;
-        if (!LIGHT || FIRST) {
+        {
+            const float* vrow = V + (((size_t)f * n_slices + slice) * ny + y) * NX;
 #pragma unroll
             for (int e = 0; e < 16; ++e) sv[e] = valid ? __ldg(vrow + t + e * T) : 0.f;
         }
@@ -111,7 +100,7 @@ k_row_transmit(float2* __restrict__ W, const float2* __restrict__ psi0, const fl
 #pragma unroll
             for (int e = 0; e < 16; ++e)
                 v[e] = (valid && ((amask >> e) & 1u)) ? wrow[t + e * T] : make_float2(0.f, 0.f);
-            if (!LIGHT && vacuum_shortcut) {
+            if (vacuum_shortcut) {
                 // V == 0 on the whole row (vacuum): exp(i sigma V) = 1 and FFT_x[IFFT_x[M]] = NX * M exactly, so the
                 // row is only rescaled (NX is a power of two: no rounding).  Decided per warp (T <= 32: the rows this
                 // warp carries) or per block, from the potential itself: any input with vacuum rows benefits.
@@ -128,15 +117,11 @@ k_row_transmit(float2* __restrict__ W, const float2* __restrict__ psi0, const fl
                     continue;
                 }
             }
-            fft_inverse<NX, RowSlots, typename Cfg::Sync, TW>(v, t, tw, slots);
-            if (LIGHT) {                                     // V after the inverse transform: 16 fewer live registers in it
-#pragma unroll
-                for (int e = 0; e < 16; ++e) sv[e] = valid ? __ldg(vrow + t + e * T) : 0.f;
-            }
+            fft_inverse<NX, RowSlots, typename Cfg::Sync>(v, t, tw, slots);
         }
 #pragma unroll
         for (int e = 0; e < 16; ++e) v[e] = cmul(v[e], cis_fast(sigma * sv[e]));
-        fft_forward<NX, RowSlots, typename Cfg::Sync, TW>(v, t, tw, slots);
+        fft_forward<NX, RowSlots, typename Cfg::Sync>(v, t, tw, slots);
         if (valid) {
 #pragma unroll
             for (int e = 0; e < 16; ++e)
@@ -151,25 +136,24 @@ k_row_transmit(float2* __restrict__ W, const float2* __restrict__ psi0, const fl
 // float32 [P*F*ny][2 nx]); the ring of NS shared-memory stages is, in turn, TMA destination, FFT
 // exchange buffer and TMA store source, so the load of item i+1 and the store of item i-1 overlap the
 // transforms of item i and no register is spent on staging.
-template <int NY> constexpr int col_default_c() { return (NY <= 1024) ? 8 : 4; }
-template <int NY, int CC = col_default_c<NY>()> struct ColCfg {
+template <int NY> struct ColCfg {
     static constexpr int T = Plan<NY>::T;
-    static constexpr int C = CC;                     // columns per block
+    static constexpr int C = (NY <= 1024) ? 8 : 4;   // columns per block
     static constexpr int THREADS = C * T;
     static constexpr int NS = 3;                                          // pipeline stages
     static constexpr int BOX_R = (NY < 256) ? NY : 256;                   // TMA box rows (<= 256)
     static constexpr int NBOX = NY / BOX_R;
-    static constexpr int MIN_BLOCKS = (THREADS <= 128) ? 4 : ((THREADS <= 256) ? 2 : 1);   // <= 128 registers
+    static constexpr int MIN_BLOCKS = (THREADS <= 256) ? 2 : 1;           // cap registers at 128
     static constexpr uint32_t STAGE_BYTES = (uint32_t)NY * C * sizeof(float2);
     static constexpr size_t SMEM = (size_t)NS * STAGE_BYTES + (size_t)NY * sizeof(float2) + NS * sizeof(uint64_t) + 128;
 };
 
-template <int NY, bool LAST, int CC>
-__global__ void __launch_bounds__(ColCfg<NY, CC>::THREADS, ColCfg<NY, CC>::MIN_BLOCKS)
+template <int NY, bool LAST>
+__global__ void __launch_bounds__(ColCfg<NY>::THREADS, ColCfg<NY>::MIN_BLOCKS)
 k_col_propagate(const __grid_constant__ CUtensorMap wmap, const int tiles_lo, const int tile_gap, const int n_tiles,
                 const int32_t* __restrict__ nmax, const float2* __restrict__ px, const float2* __restrict__ py,
                 const ChunkMap cm, const int n_items) {
-    using Cfg = ColCfg<NY, CC>;
+    using Cfg = ColCfg<NY>;
     constexpr int T = Cfg::T, C = Cfg::C, SUB = kColTile / C, NS = Cfg::NS, PF = NS - 2;   // prefetch distance
     extern __shared__ __align__(1024) float2 smem_col[];      // no static shared memory: the window starts aligned
     float2* stage0 = smem_col;
@@ -272,11 +256,11 @@ __global__ void k_zero_cols(float2* __restrict__ W, const int nx, const int ny, 
 }
 
 // ------------------------------------------------------------------------------------ launch helpers
-template <int NX, bool FIRST, bool LIGHT>
-static cudaError_t launch_row_v(ps_ctx* c, float2* W, const float2* psi0, const float* V, const ChunkMap& cm,
-                                int slice, float sigma, int col_lo, int col_hi) {
-    using Cfg = RowCfg<NX, LIGHT>;
-    auto kern = k_row_transmit<NX, FIRST, LIGHT>;
+template <int NX, bool FIRST>
+static cudaError_t launch_row(ps_ctx* c, float2* W, const float2* psi0, const float* V, const ChunkMap& cm,
+                              int slice, float sigma, int col_lo, int col_hi) {
+    using Cfg = RowCfg<NX>;
+    auto kern = k_row_transmit<NX, FIRST>;
     int per_sm_grid = 0;
     cudaError_t ce = kernel_cap(c, kern, Cfg::THREADS, Cfg::SMEM, &per_sm_grid);
     if (ce != cudaSuccess) return ce;
@@ -288,19 +272,10 @@ static cudaError_t launch_row_v(ps_ctx* c, float2* W, const float2* psi0, const 
     return cudaGetLastError();
 }
 
-template <int NX, bool FIRST>
-static cudaError_t launch_row(ps_ctx* c, float2* W, const float2* psi0, const float* V, const ChunkMap& cm,
-                              int slice, float sigma, int col_lo, int col_hi) {
-    if constexpr (NX >= 512 && !FIRST) {
-        if (c->tune_row_light && !c->vacuum_shortcut) return launch_row_v<NX, FIRST, true>(c, W, psi0, V, cm, slice, sigma, col_lo, col_hi);
-    }
-    return launch_row_v<NX, FIRST, false>(c, W, psi0, V, cm, slice, sigma, col_lo, col_hi);
-}
-
-template <int NY, bool LAST, int CC>
+template <int NY, bool LAST>
 static cudaError_t launch_col(ps_ctx* c, const CUtensorMap& wmap, const ChunkMap& cm, int zero_lo, int zero_hi) {
-    using Cfg = ColCfg<NY, CC>;
-    auto kern = k_col_propagate<NY, LAST, CC>;
+    using Cfg = ColCfg<NY>;
+    auto kern = k_col_propagate<NY, LAST>;
     int per_sm_grid = 0;
     cudaError_t ce = kernel_cap(c, kern, Cfg::THREADS, Cfg::SMEM, &per_sm_grid);
     if (ce != cudaSuccess) return ce;
@@ -313,21 +288,9 @@ static cudaError_t launch_col(ps_ctx* c, const CUtensorMap& wmap, const ChunkMap
 }
 
 template <int NY>
-static int col_c_of(const ps_ctx* c) {                    // columns per block of the column pass for this ctx
-    if (NY >= 512 && NY <= 1024 && c->tune_col_c == 4) return 4;
-    return col_default_c<NY>();
-}
-template <int NY, bool LAST>
-static cudaError_t launch_col_any(ps_ctx* c, const CUtensorMap& wmap, const ChunkMap& cm, int zero_lo, int zero_hi) {
-    if constexpr (NY >= 512 && NY <= 1024) {
-        if (col_c_of<NY>(c) == 4) return launch_col<NY, LAST, 4>(c, wmap, cm, zero_lo, zero_hi);
-    }
-    return launch_col<NY, LAST, col_default_c<NY>()>(c, wmap, cm, zero_lo, zero_hi);
-}
-template <int NY>
-static bool make_wave_map(const ps_ctx* c, CUtensorMap* map, void* W, int nx, long long rows) {
+static bool make_wave_map(CUtensorMap* map, void* W, int nx, long long rows) {
     using Cfg = ColCfg<NY>;
-    return tma::make_map_2d_f32(map, W, 2ull * nx, (uint64_t)rows, 2 * col_c_of<NY>(c), Cfg::BOX_R);
+    return tma::make_map_2d_f32(map, W, 2ull * nx, (uint64_t)rows, 2 * Cfg::C, Cfg::BOX_R);
 }
 
 #define PSB_DISPATCH_N(n, CALL)                                                    \
@@ -345,6 +308,8 @@ static bool make_wave_map(const ps_ctx* c, CUtensorMap* map, void* W, int nx, lo
 }  // namespace psb
 
 using namespace psb;
+
+static constexpr long long kResidentMaxWaves = 2 * kNumSM;   // auto rule of the chip-resident path
 
 extern "C" ps_status ps_multislice(ps_ctx* c, double kV, const void* d_psi0, int n_probes, const float* d_V,
                                    int n_frames, void* d_exit, int exit_layout) {
@@ -379,7 +344,7 @@ extern "C" ps_status ps_multislice(ps_ctx* c, double kV, const void* d_psi0, int
     if (wave_rows > 0x7fffffffLL) return fail(c, PS_EUNSUPPORTED, "ps_multislice: n_probes*n_frames*ny exceeds 2^31");
     CUtensorMap wmap;
     bool map_ok = false;
-    PSB_DISPATCH_N(c->ny, (map_ok = make_wave_map<N_>(c, &wmap, d_exit, c->nx, wave_rows)));
+    PSB_DISPATCH_N(c->ny, (map_ok = make_wave_map<N_>(&wmap, d_exit, c->nx, wave_rows)));
     if (!map_ok) return fail(c, PS_ECUDA, "ps_multislice: cuTensorMapEncodeTiled failed (exit-wave array must be 16-byte aligned)");
     // contiguous range of columns outside the band limit (zero in the k-space exit wave)
     int zero_lo = 0, zero_hi = 0;
@@ -392,6 +357,16 @@ extern "C" ps_status ps_multislice(ps_ctx* c, double kV, const void* d_psi0, int
         int b = nt;
         while (b > a && act[b - 1]) --b;
         zero_lo = a * kColTile; zero_hi = b * kColTile;
+    }
+
+    // Small square grids, small batches: the whole slice loop in one launch with the wave resident in shared memory
+    // (resident.cu).  Batches that fill the GPU stay on the streaming passes (measured cross-over: profiles/r2_resident.md).
+    if (resident_supported(c) && !c->vacuum_shortcut && c->wave_chunk == 0 &&
+        (c->tune_resident == 1 || (c->tune_resident == 0 && (long long)n_probes * n_frames <= kResidentMaxWaves))) {
+        cudaError_t e = launch_slice_resident(c, W, psi0, d_V, n_probes, n_frames, sigma, zero_lo, zero_hi);
+        if (e != cudaSuccess) return fail(c, PS_ECUDA, std::string("k_slice_resident: ") + cudaGetErrorString(e));
+        c->launches++;
+        return PS_OK;
     }
 
     for (int p0 = 0; p0 < n_probes; p0 += np) {
@@ -419,9 +394,9 @@ extern "C" ps_status ps_multislice(ps_ctx* c, double kV, const void* d_psi0, int
                         k_zero_cols<<<zb, 256, 0, c->stream>>>(W, c->nx, c->ny, zero_lo, zero_hi, cm);
                         c->launches++;
                     }
-                    PSB_DISPATCH_N(c->ny, (e = launch_col_any<N_, true>(c, wmap, cm, zero_lo, zero_hi)));
+                    PSB_DISPATCH_N(c->ny, (e = launch_col<N_, true>(c, wmap, cm, zero_lo, zero_hi)));
                 } else {
-                    PSB_DISPATCH_N(c->ny, (e = launch_col_any<N_, false>(c, wmap, cm, zero_lo, zero_hi)));
+                    PSB_DISPATCH_N(c->ny, (e = launch_col<N_, false>(c, wmap, cm, zero_lo, zero_hi)));
                 }
                 }
                 if (e != cudaSuccess) return fail(c, PS_ECUDA, std::string("k_col_propagate: ") + cudaGetErrorString(e));

@@ -24,7 +24,8 @@ template <int NF> struct TacawCfg {
 template <int NF>
 __global__ void __launch_bounds__(TacawCfg<NF>::THREADS)
 k_tacaw_fft(const float2* __restrict__ exitw, float* __restrict__ I, const int32_t* __restrict__ slot_of_bin,
-            const int n_out, const int nx, const int ny, const int32_t* __restrict__ nmax, const int n_items) {
+            const int n_out, const int nx, const int ny, const int32_t* __restrict__ nmax, const int n_items,
+            const int prefetch) {
     using Cfg = TacawCfg<NF>;
     constexpr int T = Cfg::T, C = Cfg::C;
     extern __shared__ float2 smem[];
@@ -45,6 +46,23 @@ k_tacaw_fft(const float2* __restrict__ exitw, float* __restrict__ I, const int32
         const int iy = g >> gpr_shift, ix0 = (g & (groups_per_row - 1)) * C;
         const int ay = iy < ny / 2 ? iy : ny - iy;
         const size_t pix = (size_t)iy * nx + ix0 + c;
+        {
+            // this block's NEXT item: pull its F segments of C*8 bytes from HBM into L2 while the current item is
+            // transformed, so that the register-staged loads below find them there.  One prefetch per lane and segment.
+            // Measured (profiles/r2_tacaw.md): +5...+28 % for stacks of up to 512 frames on grids up to 512^2, a loss
+            // beyond (an item then touches more 2 MB pages than the TLB holds, and the prefetch doubles the misses):
+            // the host switches it per shape.
+            const int nxt = item + gridDim.x;
+            if (prefetch && nxt < n_items) {
+                const int pn = nxt >> gpp_shift, gn = nxt & (groups_per_probe - 1);
+                const int iyn = gn >> gpr_shift, ixn = (gn & (groups_per_row - 1)) * C;
+                const int ayn = iyn < ny / 2 ? iyn : ny - iyn;
+                if (ayn <= max(nmax[ixn], nmax[ixn + C - 1])) {              // nmax is monotone in |m|: the group's best column is an end
+                    const float2* nsrc = exitw + (size_t)pn * NF * npix + (size_t)iyn * nx + ixn;
+                    for (int j = threadIdx.x; j < NF; j += Cfg::THREADS) tma::prefetch_l2(nsrc + (size_t)j * npix);
+                }
+            }
+        }
         float* out = I + (size_t)p * n_out * npix + pix;
         const bool mine = ay <= nmax[ix0 + c];
         if (!__syncthreads_or(mine)) {                       // whole group outside the band limit
@@ -301,8 +319,9 @@ static cudaError_t launch_tacaw(ps_ctx* c, const float2* exitw, float* I, const 
     if (ce != cudaSuccess) return ce;
     const long long n_items = (long long)P * c->ny * (c->nx / Cfg::C);
     if (n_items > 0x7fffffffLL) return cudaErrorInvalidValue;
+    const int prefetch = (NF <= 512 && (long long)c->nx * c->ny <= 512LL * 512LL) ? 1 : 0;
     kern<<<(int)(n_items < cap ? n_items : cap), Cfg::THREADS, Cfg::SMEM, c->stream>>>(exitw, I, slot, n_out, c->nx, c->ny,
-                                                                                      c->d_nmax, (int)n_items);
+                                                                                      c->d_nmax, (int)n_items, prefetch);
     return cudaGetLastError();
 }
 

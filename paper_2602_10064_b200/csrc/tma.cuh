@@ -72,6 +72,9 @@ __device__ __forceinline__ void tensor_store_2d(const CUtensorMap* map, const in
 __device__ __forceinline__ void bulk_prefetch_l2(const void* g, const uint32_t bytes) {
     asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(g), "r"(bytes) : "memory");
 }
+// per-thread L2 prefetch of the line holding g (LSU path: one request per lane; for many small segments this is far
+// cheaper than one bulk prefetch per segment, which occupies the copy engine per request: profiles/r2_slice_step.md)
+__device__ __forceinline__ void prefetch_l2(const void* g) { asm volatile("prefetch.global.L2 [%0];" ::"l"(g)); }
 __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 // all but the newest N bulk groups of this thread have finished READING their shared-memory source
 template <int N>
