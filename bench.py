@@ -231,9 +231,11 @@ def _event_time(torch, fn, flush, reps=5, warm=3):
     return float(np.median(ts))
 
 
-def tacaw_micro():
+def tacaw_micro(shapes_a=None, shapes_b=None):
     """ps_tacaw (path A) and ps_tacaw_add (path B) alone on random complex64 stacks (every pixel non-zero; only
-    in-band pixels are read): median of 5 runs after 3 warm-ups, L2 flushed between runs; one JSON line per shape."""
+    in-band pixels are read): median of 5 runs after 3 warm-ups, L2 flushed between runs; one JSON line per shape.
+    `shapes_a` = [(P, frames, grid, bins)], `shapes_b` = [(grid, chunk frames, bins)] override the default lists
+    (--micro-a / --micro-b: one shape per ncu capture)."""
     import torch
     import paper_2602_10064_b200 as ps
     from paper_2602_10064_b200.binding import TacawStream
@@ -248,9 +250,12 @@ def tacaw_micro():
         ctx.set_geometry(np.array([n * 0.1, n * 0.1, 8.0]), n, n, 2.0)
         return ctx
 
-    for P, F, n, nb in [(1, 512, 256, 50), (1, 512, 256, 512), (16, 1024, 512, 1024), (4, 1024, 512, 128),
-                        (1, 2048, 512, 2048), (1, 4096, 256, 256), (8, 256, 512, 256), (16, 128, 512, 128),
-                        (1, 256, 1024, 256), (1, 64, 128, 64)]:
+    if shapes_a is None and shapes_b is None:
+        shapes_a = [(1, 512, 256, 50), (1, 512, 256, 512), (16, 1024, 512, 1024), (4, 1024, 512, 128),
+                    (1, 2048, 512, 2048), (1, 4096, 256, 256), (8, 256, 512, 256), (16, 128, 512, 128),
+                    (1, 256, 1024, 256), (1, 64, 128, 64)]
+        shapes_b = [(1024, 64, 256), (512, 64, 256), (1024, 64, 64)]
+    for P, F, n, nb in shapes_a or []:
         ctx = ctx_for(n)
         ex = torch.view_as_complex(torch.randn((P, F, n, n, 2), device="cuda"))
         bins = None if nb == F else np.arange(nb, dtype=np.int32)
@@ -262,7 +267,7 @@ def tacaw_micro():
                           "algorithmic_GB": byts / 1e9, "GBps": byts / ms / 1e6, "frac_of_hbm_peak": byts / ms / 1e6 / peak}))
         del ex, I, ctx
     # path B: one 64-frame chunk of a 4096-frame stream, 256 bins (config 4's shape) and a 1024^2 grid
-    for n, Fc, nb in [(1024, 64, 256), (512, 64, 256), (1024, 64, 64)]:
+    for n, Fc, nb in shapes_b or []:
         ctx = ctx_for(n)
         ex = torch.view_as_complex(torch.randn((1, Fc, n, n, 2), device="cuda"))
         ts = TacawStream(ctx, 1, 4096, 2.0, np.arange(nb, dtype=np.int32))
@@ -393,6 +398,10 @@ def main():
                          "and print one JSON line")
     ap.add_argument("--tacaw-micro", action="store_true",
                     help="time ps_tacaw / ps_tacaw_add alone on synthetic stacks of several shapes and exit")
+    ap.add_argument("--micro-a", action="append", default=None, metavar="P,FRAMES,GRID,BINS",
+                    help="--tacaw-micro: this path-A shape instead of the default list (repeatable)")
+    ap.add_argument("--micro-b", action="append", default=None, metavar="GRID,CHUNK_FRAMES,BINS",
+                    help="--tacaw-micro: this path-B shape instead of the default list (repeatable)")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -404,7 +413,11 @@ def main():
         run_reference(args, w, rank)
         return
     if args.tacaw_micro:
-        tacaw_micro()
+        parse = lambda xs: None if xs is None else [tuple(int(v) for v in x.split(",")) for x in xs]
+        if args.micro_a is None and args.micro_b is None:
+            tacaw_micro()
+        else:
+            tacaw_micro(parse(args.micro_a) or [], parse(args.micro_b) or [])
         return
     if args.full_config:
         full_config(args.full_config)

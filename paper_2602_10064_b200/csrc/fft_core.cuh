@@ -199,11 +199,35 @@ template <int N> struct TwiddlesShared {
 // the barrier covering all threads of that transform.
 // `at` is the layout the caller sees (first read, last write, second exchange); x1w / x1r address the FIRST exchange
 // (element 16 t + r written, element t + e T read), whose layout may differ as long as write and read agree.
+// x2w / x2r address the SECOND exchange (element j0 + 16 r written by butterfly b, element t + e T read).
 struct RowSlots {            // one transform per contiguous padded line; pad 1 per 16 (conflict-free)
     float2* line;
     __device__ __forceinline__ float2& at(const int idx) const { return line[idx + (idx >> 4)]; }
     __device__ __forceinline__ float2& x1w(const int t, const int r) const { return at(16 * t + r); }
     template <int T> __device__ __forceinline__ float2& x1r(const int t, const int e) const { return at(t + e * T); }
+    template <int N> __device__ __forceinline__ float2& x2w(const int t, const int b, const int r) const {
+        const int j = t + b * Plan<N>::T;
+        return at((j >> 4) * (16 * Plan<N>::R2) + (j & 15) + 16 * r);
+    }
+    template <int T> __device__ __forceinline__ float2& x2r(const int t, const int e) const { return at(t + e * T); }
+};
+// The same padded line with every access written as (per-thread base pointer) + (compile-time offset): for
+// T = N/16 a multiple of 16 the pad term of t + e T and of the second-exchange index separates into a part that depends
+// on the thread only and a part that depends on the unrolled loop index only.  (With at() the compiler rebuilt
+// idx + (idx >> 4) per element and per item: ncu showed ~130 of the 1650 warp instructions of a 512-point row pass
+// spent there.)  Three base registers per thread, zero address arithmetic per access.
+template <int N> struct RowSlotsF {
+    static constexpr int T = Plan<N>::T, R2 = Plan<N>::R2;
+    static_assert(T % 16 == 0, "RowSlotsF needs N >= 256");
+    float2 *w1, *rd, *w2;
+    __device__ __forceinline__ RowSlotsF(float2* line, const int t)
+        : w1(line + 17 * t), rd(line + t + (t >> 4)), w2(line + (t >> 4) * (17 * R2) + (t & 15)) {}
+    __device__ __forceinline__ float2& x1w(const int, const int r) const { return w1[r]; }                  // 16 t + r, r < 16
+    template <int T_> __device__ __forceinline__ float2& x1r(const int, const int e) const { return rd[e * T + e * T / 16]; }
+    template <int N_> __device__ __forceinline__ float2& x2w(const int, const int b, const int r) const {
+        return w2[b * (T / 16) * (17 * R2) + 17 * r];
+    }
+    template <int T_> __device__ __forceinline__ float2& x2r(const int, const int e) const { return rd[e * T + e * T / 16]; }
 };
 // C transforms interleaved (a warp = 32/C consecutive t x C columns), linear so that a TMA box [rows][C] can land in it.
 // First exchange: the writes 16 t + r of the 32/C t-values of a warp would all fall on the same C*8-byte slice of the
@@ -223,6 +247,11 @@ template <int C> struct ColSlots {
         rb = b + (t ^ ((t >> 4) & M)) * C;
     }
     __device__ __forceinline__ float2& at(const int idx) const { return base[idx * C]; }
+    template <int N> __device__ __forceinline__ float2& x2w(const int t, const int b, const int r) const {
+        const int j = t + b * Plan<N>::T;
+        return at((j >> 4) * (16 * Plan<N>::R2) + (j & 15) + 16 * r);
+    }
+    template <int T> __device__ __forceinline__ float2& x2r(const int t, const int e) const { return at(t + e * T); }
     __device__ __forceinline__ float2& x1w(const int, const int r) const { return wb[r & M][r * C]; }
     template <int T> __device__ __forceinline__ float2& x1r(const int t, const int e) const {
         if constexpr (T % (16 * (M + 1)) == 0) {
@@ -276,14 +305,12 @@ __device__ __forceinline__ void fft_forward(float2 (&v)[16], const int t, const 
         Sync::sync();
 #pragma unroll
         for (int b = 0; b < B2; ++b) {
-            const int j = t + b * T;
-            const int j0 = (j >> 4) * (16 * R2) + (j & 15);
 #pragma unroll
-            for (int r = 0; r < R2; ++r) sm.at(j0 + 16 * r) = v[b + r * B2];
+            for (int r = 0; r < R2; ++r) sm.template x2w<N>(t, b, r) = v[b + r * B2];
         }
         Sync::sync();
 #pragma unroll
-        for (int e = 0; e < 16; ++e) v[e] = sm.at(t + e * T);
+        for (int e = 0; e < 16; ++e) v[e] = sm.template x2r<T>(t, e);
         // stage 3: radix R3, Ns = 16 R2, twiddle base^r
 #pragma unroll
         for (int b = 0; b < B3; ++b) {

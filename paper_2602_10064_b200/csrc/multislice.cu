@@ -17,6 +17,10 @@
 #include "tma.cuh"
 #include <type_traits>
 
+#ifndef PSB_ROW_VLATE
+#define PSB_ROW_VLATE 1
+#endif
+
 namespace psb {
 
 // ------------------------------------------------------------------------------------ row pass
@@ -35,72 +39,110 @@ struct ChunkMap {           // chunk of waves: probes [p0,p0+np) x frames [f0,f0
     int p0, np, f0, nf, F;  // F = total frames (exit layout [P][F][ny][nx])
 };
 
-template <int NX, bool FIRST>
+// Row coordinates of a persistent thread group: rho = (lf * np + lp) * ny + y, advanced by a constant stride per item.
+// The stride is decomposed once (one integer division per kernel, none per item), so that an item costs a handful of
+// integer instructions instead of the two 32-bit divisions and the 64-bit address chains it cost in round 1
+// (ncu: 400 of the 1650 warp instructions of a 512-point row were index arithmetic).
+struct RowCursor {
+    unsigned y, lp, lf;
+    __device__ __forceinline__ void init(const unsigned rho, const int ny_shift, const unsigned np) {
+        y = rho & ((1u << ny_shift) - 1u);
+        const unsigned l = rho >> ny_shift;
+        lf = l / np;
+        lp = l - lf * np;
+    }
+    __device__ __forceinline__ void advance(const unsigned dy, const unsigned dlp, const unsigned dlf, const int ny_shift,
+                                            const unsigned np) {
+        y += dy;
+        lp += dlp + (y >> ny_shift);
+        y &= (1u << ny_shift) - 1u;
+        lf += dlf;
+        if (lp >= np) { lp -= np; ++lf; }
+        if (lp >= np) { lp -= np; ++lf; }                     // dlp + carry can reach np
+    }
+};
+
+// PAT510: the active columns are [0, col_lo) and [col_hi, NX) with 5T < col_lo <= 6T and 10T <= col_hi < 11T (every
+// grid whose band limit is set by the x direction: all five BASELINE configs).  Then the elements e = t + e T of a thread
+// are active for e < 5 and e > 10, inactive for 6 <= e <= 9 (compile-time zeros in, dead values out: the compiler prunes
+// the first and last butterflies accordingly), and only e = 5 and e = 10 carry a per-thread predicate.  The generic
+// variant tests one bit of a mask per element.
+template <int NX, bool FIRST, bool VAC /* vacuum shortcut (ps_set_vacuum_shortcut) */, bool PAT510>
 __global__ void __launch_bounds__(RowCfg<NX>::THREADS, RowCfg<NX>::MIN_BLOCKS)
-k_row_transmit(float2* __restrict__ W, const float2* __restrict__ psi0, const float* __restrict__ V,
-               const uint8_t* __restrict__ tile_active, const ChunkMap cm, const int ny, const int n_slices,
-               const int slice, const float sigma, const int n_items, const int col_lo, const int col_hi,
-               const int vacuum_shortcut) {
+k_row_transmit(float2* __restrict__ W, const float2* __restrict__ psi0, const float* __restrict__ V, const ChunkMap cm,
+               const int ny_shift, const int n_slices, const int slice, const float sigma, const int n_items,
+               const int col_lo, const int col_hi) {
     using Cfg = RowCfg<NX>;
     constexpr int T = Cfg::T;
+    using Slots = typename std::conditional<(T % 16 == 0), RowSlotsF<NX>, RowSlots>::type;
     extern __shared__ float2 smem[];
     const int t = threadIdx.x % T, r = threadIdx.x / T;
-    RowSlots slots{smem + (size_t)r * RowLine<NX>::LEN};
     Twiddles<NX> tw;
     tw.init(t);
-    unsigned amask = 0;                                  // bit e: column t+e*T lies in an active tile
+    // bit e: column t + e T lies in an active tile.  Active tiles are [0, col_lo) and [col_hi, NX) (FFT order).
+    unsigned amask = 0;
 #pragma unroll
-    for (int e = 0; e < 16; ++e) amask |= (tile_active[(t + e * T) / kColTile] ? 1u : 0u) << e;
-    // 32-bit index arithmetic (ps_multislice checks n_probes * n_frames * ny < 2^31; ny is a power of two):
-    // 64-bit divisions here cost about a tenth of the kernel's instructions
-    const unsigned n_rows = (unsigned)cm.np * (unsigned)cm.nf * (unsigned)ny;
-    const int ny_shift = __ffs(ny) - 1;
-    const unsigned np_u = (unsigned)cm.np;
+    for (int e = 0; e < 16; ++e) amask |= ((t + e * T < col_lo || t + e * T >= col_hi) ? 1u : 0u) << e;
+    const bool a_lo = t + 5 * T < col_lo, a_hi = t + 10 * T >= col_hi;          // PAT510: the two boundary elements
+    // 32-bit row indices (ps_multislice checks n_probes * n_frames * ny < 2^31 and n_frames * n_slices * ny < 2^31)
+    const unsigned np = (unsigned)cm.np;
+    const unsigned n_rows = np * (unsigned)cm.nf << ny_shift;
+    const unsigned stride = gridDim.x * Cfg::RPB;
+    const unsigned dy = stride & ((1u << ny_shift) - 1u), dl = stride >> ny_shift;
+    const unsigned dlf = dl / np, dlp = dl - dlf * np;
+    unsigned rho = blockIdx.x * Cfg::RPB + r;
+    RowCursor cur;
+    cur.init(rho, ny_shift, np);
+    // L2 prefetch of this group's NEXT row while the current one is transformed (measured: +3 % at 512^2, +4 % at
+    // 2048^2, -4 % at 256^2): one 128-byte line per thread, the T threads of a row cover the NX * 8 bytes of the wave
+    // row (lines wholly inside the inactive column range are skipped) and the first T/2 the NX * 4 bytes of V
+    const bool pf_wave = (16 * t < col_lo) || (16 * t + 16 > col_hi);
+    // rows per block divide ny for NX >= 128 (RPB <= 32 <= ny): every item is a full set of rows
+    constexpr bool ALWAYS_VALID = Cfg::RPB <= kMinGrid;
 
-    for (int item = blockIdx.x; item < n_items; item += gridDim.x) {
-        const unsigned rho = (unsigned)item * Cfg::RPB + r;
-        const bool valid = rho < n_rows;
-        int y = 0, p = 0, f = 0;
-        if (valid) {
-            const unsigned l = rho >> ny_shift;
-            y = (int)(rho & (unsigned)(ny - 1));
-            const unsigned lf = (np_u == 1u) ? l : l / np_u;
-            p = cm.p0 + (int)(l - lf * np_u);
-            f = cm.f0 + (int)lf;
+    for (int item = blockIdx.x; item < n_items; item += gridDim.x, rho += stride) {
+        const bool valid = ALWAYS_VALID || rho < n_rows;
+        const unsigned p = cm.p0 + cur.lp, f = cm.f0 + cur.lf, y = cur.y;
+        const unsigned wrow_i = ((p * (unsigned)cm.F + f) << ny_shift) + y;
+        const unsigned vrow_i = ((f * (unsigned)n_slices + (unsigned)slice) << ny_shift) + y;
+        cur.advance(dy, dlp, dlf, ny_shift, np);
+        if (NX >= 512 && rho + stride < n_rows) {
+            const unsigned pn = cm.p0 + cur.lp, fn = cm.f0 + cur.lf;
+            const unsigned wn_i = ((pn * (unsigned)cm.F + fn) << ny_shift) + cur.y;
+            const unsigned vn_i = ((fn * (unsigned)n_slices + (unsigned)slice) << ny_shift) + cur.y;
+            if (2 * t < T) tma::prefetch_l2(V + (size_t)vn_i * NX + 32 * t);
+            if (!FIRST && pf_wave) tma::prefetch_l2(W + (size_t)wn_i * NX + 16 * t);
         }
-        if (NX >= 512 && t == 0) {                           // this block's next row: HBM -> L2 while this one is transformed
-                                                             // (measured: +3 % at 512^2, +4 % at 2048^2, -4 % at 256^2)
-            const unsigned rn = rho + gridDim.x * Cfg::RPB;
-            if (rn < n_rows) {
-                const unsigned ln = rn >> ny_shift;
-                const int yn = (int)(rn & (unsigned)(ny - 1));
-                const unsigned lfn = (np_u == 1u) ? ln : ln / np_u;
-                const int pn = cm.p0 + (int)(ln - lfn * np_u), fn = cm.f0 + (int)lfn;
-                tma::bulk_prefetch_l2(V + (((size_t)fn * n_slices + slice) * ny + yn) * NX, NX * sizeof(float));
-                if (!FIRST) {
-                    const float2* wn = W + (((size_t)pn * cm.F + fn) * ny + yn) * NX;
-                    if (col_lo > 0) tma::bulk_prefetch_l2(wn, col_lo * sizeof(float2));
-                    if (col_hi < NX) tma::bulk_prefetch_l2(wn + col_hi, (NX - col_hi) * sizeof(float2));
-                }
-            }
-        }
-        float2* wrow = W + (((size_t)p * cm.F + f) * ny + y) * NX;
+        float2* wrow = W + (size_t)wrow_i * NX + t;
+        const float* vrow = V + (size_t)vrow_i * NX + t;
+        const Slots slots = [&]() {
+            if constexpr (T % 16 == 0) return RowSlotsF<NX>(smem + (size_t)r * RowLine<NX>::LEN, t);
+            else return RowSlots{smem + (size_t)r * RowLine<NX>::LEN};
+        }();
+        unsigned am = valid ? amask : 0u;
+        asm volatile("" : "+r"(am));                     // keep the mask in ONE register: bit tests, not 16 hoisted flags
+        auto active = [&](const int e) -> bool {
+            if constexpr (PAT510) return e < 5 || e > 10 || (e == 5 && a_lo) || (e == 10 && a_hi);
+            else return (am & (1u << e)) != 0u;
+        };
         float2 v[16];
-        float sv[16];                                    // sigma * V of this row, fetched with the wave
-        {
-            const float* vrow = V + (((size_t)f * n_slices + slice) * ny + y) * NX;
+        float sv[16];                                    // V of this row
+        // Where V is fetched: with the wave (NX <= 256: everything fits in registers) or after the inverse transform
+        // (NX >= 512: sixteen more live registers across the inverse transform would be spilled to local memory; the
+        // row was pulled into L2 by the previous item's prefetch, so the load is an L2 hit the other warps cover)
+        constexpr bool V_LATE = (PSB_ROW_VLATE != 0) && !FIRST && !VAC && NX >= 512;
+        if (!V_LATE) {
 #pragma unroll
-            for (int e = 0; e < 16; ++e) sv[e] = valid ? __ldg(vrow + t + e * T) : 0.f;
+            for (int e = 0; e < 16; ++e) sv[e] = valid ? __ldg(vrow + e * T) : 0.f;
         }
         if (FIRST) {
-            const float2* src = psi0 + ((size_t)p * ny + y) * NX;
+            const float2* src = psi0 + (((size_t)p << ny_shift) + y) * NX + t;
 #pragma unroll
-            for (int e = 0; e < 16; ++e) v[e] = valid ? __ldg(src + t + e * T) : make_float2(0.f, 0.f);
+            for (int e = 0; e < 16; ++e) v[e] = valid ? __ldg(src + e * T) : make_float2(0.f, 0.f);
         } else {
 #pragma unroll
-            for (int e = 0; e < 16; ++e)
-                v[e] = (valid && ((amask >> e) & 1u)) ? wrow[t + e * T] : make_float2(0.f, 0.f);
-            if (vacuum_shortcut) {
+            for (int e = 0; e < 16; ++e) v[e] = active(e) ? wrow[e * T] : make_float2(0.f, 0.f);
+            if (VAC) {
                 // V == 0 on the whole row (vacuum): exp(i sigma V) = 1 and FFT_x[IFFT_x[M]] = NX * M exactly, so the
                 // row is only rescaled (NX is a power of two: no rounding).  Decided per warp (T <= 32: the rows this
                 // warp carries) or per block, from the potential itself: any input with vacuum rows benefits.
@@ -109,24 +151,25 @@ k_row_transmit(float2* __restrict__ W, const float2* __restrict__ psi0, const fl
                 for (int e = 0; e < 16; ++e) z = z && (sv[e] == 0.f);
                 const bool all_z = (T <= 32) ? (bool)__all_sync(0xffffffffu, z) : (bool)__syncthreads_and(z);
                 if (all_z) {
-                    if (valid) {
 #pragma unroll
-                        for (int e = 0; e < 16; ++e)
-                            if ((amask >> e) & 1u) wrow[t + e * T] = make_float2(v[e].x * (float)NX, v[e].y * (float)NX);
-                    }
+                    for (int e = 0; e < 16; ++e)
+                        if (active(e)) wrow[e * T] = make_float2(v[e].x * (float)NX, v[e].y * (float)NX);
                     continue;
                 }
             }
-            fft_inverse<NX, RowSlots, typename Cfg::Sync>(v, t, tw, slots);
+            fft_inverse<NX, Slots, typename Cfg::Sync>(v, t, tw, slots);
+            if (V_LATE) {
+#pragma unroll
+                for (int e = 0; e < 16; ++e) sv[e] = __ldg(vrow + e * T);
+            }
         }
 #pragma unroll
         for (int e = 0; e < 16; ++e) v[e] = cmul(v[e], cis_fast(sigma * sv[e]));
-        fft_forward<NX, RowSlots, typename Cfg::Sync>(v, t, tw, slots);
-        if (valid) {
+        fft_forward<NX, Slots, typename Cfg::Sync>(v, t, tw, slots);
+        asm volatile("" : "+r"(am));                     // test the bits again rather than keep 16 flags alive (spills)
 #pragma unroll
-            for (int e = 0; e < 16; ++e)
-                if ((amask >> e) & 1u) wrow[t + e * T] = v[e];
-        }
+        for (int e = 0; e < 16; ++e)
+            if (active(e)) wrow[e * T] = v[e];
     }
 }
 
@@ -260,15 +303,22 @@ template <int NX, bool FIRST>
 static cudaError_t launch_row(ps_ctx* c, float2* W, const float2* psi0, const float* V, const ChunkMap& cm,
                               int slice, float sigma, int col_lo, int col_hi) {
     using Cfg = RowCfg<NX>;
-    auto kern = k_row_transmit<NX, FIRST>;
+    constexpr int T = Cfg::T;
+    const bool pat510 = !FIRST && !c->vacuum_shortcut && NX >= 256 && col_lo > 5 * T && col_lo <= 6 * T && col_hi >= 10 * T &&
+                        col_hi < 11 * T;
+    auto kern = (c->vacuum_shortcut && !FIRST) ? k_row_transmit<NX, FIRST, true, false>
+                : pat510                       ? k_row_transmit<NX, FIRST, false, (!FIRST && NX >= 256)>
+                                               : k_row_transmit<NX, FIRST, false, false>;
     int per_sm_grid = 0;
     cudaError_t ce = kernel_cap(c, kern, Cfg::THREADS, Cfg::SMEM, &per_sm_grid);
     if (ce != cudaSuccess) return ce;
     const long long n_rows = (long long)cm.np * cm.nf * c->ny;
     const int n_items = (int)((n_rows + Cfg::RPB - 1) / Cfg::RPB);
     const int grid = n_items < per_sm_grid ? n_items : per_sm_grid;
-    kern<<<grid, Cfg::THREADS, Cfg::SMEM, c->stream>>>(W, psi0, V, c->d_tile_active, cm, c->ny, c->n_slices, slice,
-                                                      sigma, n_items, col_lo, col_hi, c->vacuum_shortcut);
+    int ny_shift = 0;
+    while ((1 << ny_shift) < c->ny) ++ny_shift;
+    kern<<<grid, Cfg::THREADS, Cfg::SMEM, c->stream>>>(W, psi0, V, cm, ny_shift, c->n_slices, slice, sigma, n_items, col_lo,
+                                                      col_hi);
     return cudaGetLastError();
 }
 
@@ -342,6 +392,8 @@ extern "C" ps_status ps_multislice(ps_ctx* c, double kV, const void* d_psi0, int
     // TMA view of the wave array: float32 [P*F*ny][2 nx]; box = C columns x up to 256 rows
     const long long wave_rows = (long long)n_probes * n_frames * c->ny;
     if (wave_rows > 0x7fffffffLL) return fail(c, PS_EUNSUPPORTED, "ps_multislice: n_probes*n_frames*ny exceeds 2^31");
+    if ((long long)n_frames * c->n_slices * c->ny > 0x7fffffffLL)
+        return fail(c, PS_EUNSUPPORTED, "ps_multislice: n_frames*n_slices*ny exceeds 2^31 (propagate the frames in chunks)");
     CUtensorMap wmap;
     bool map_ok = false;
     PSB_DISPATCH_N(c->ny, (map_ok = make_wave_map<N_>(&wmap, d_exit, c->nx, wave_rows)));

@@ -33,6 +33,11 @@ template <int LEN> struct PitchSlots {
     __device__ __forceinline__ float2& at(const int idx) const { return base[idx * LEN]; }
     __device__ __forceinline__ float2& x1w(const int t, const int r) const { return at(16 * t + r); }
     template <int T> __device__ __forceinline__ float2& x1r(const int t, const int e) const { return at(t + e * T); }
+    template <int N> __device__ __forceinline__ float2& x2w(const int t, const int b, const int r) const {
+        const int j = t + b * Plan<N>::T;
+        return at((j >> 4) * (16 * Plan<N>::R2) + (j & 15) + 16 * r);
+    }
+    template <int T> __device__ __forceinline__ float2& x2r(const int t, const int e) const { return at(t + e * T); }
 };
 
 struct ResWaves {            // waves of this launch: probes [p0, p0+np) x frames [f0, f0+nf); F = frames of the exit layout
