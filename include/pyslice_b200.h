@@ -136,6 +136,10 @@ PS_API ps_status ps_set_wave_chunk(ps_ctx* ctx, int n_waves);
  *   "resident"  chip-resident slice loop for square grids nx = ny <= 128 (one launch per ps_multislice, the wave kept
  *               in shared memory through all slices; resident.cu): 0 = auto (batches of at most 2 x 148 waves, which
  *               cannot fill the GPU with streaming launches), 1 = always, -1 = never
+ *   "row32"     the row pass of ps_multislice at nx = 512 and 1024 (slices after the first) with 32 values per thread:
+ *               0 = auto (off: measured slower than the 16-value pass), 1 = on, -1 = off
+ *   "col32"     the column pass of ps_multislice at ny = 512 and 1024 with 32 values per thread (one shared-memory exchange
+ *               per transform instead of two): 0 = auto (on), 1 = on, -1 = off (the 16-value pass used at every other size)
  * Unknown keys and values are PS_EINVAL. */
 PS_API ps_status ps_set_tuning(ps_ctx* ctx, const char* key, int value);
 

@@ -341,6 +341,12 @@ extern "C" ps_status ps_set_tuning(ps_ctx* c, const char* key, int value) {
     if (k == "resident") {
         if (value < -1 || value > 1) return fail(c, PS_EINVAL, "ps_set_tuning: resident must be -1 (never), 0 (auto) or 1 (always)");
         c->tune_resident = value;
+    } else if (k == "row32") {
+        if (value < -1 || value > 1) return fail(c, PS_EINVAL, "ps_set_tuning: row32 must be -1 (off), 0 (auto) or 1 (on)");
+        c->tune_row32 = value;
+    } else if (k == "col32") {
+        if (value < -1 || value > 1) return fail(c, PS_EINVAL, "ps_set_tuning: col32 must be -1 (off), 0 (auto) or 1 (on)");
+        c->tune_col32 = value;
     } else {
         return fail(c, PS_EINVAL, "ps_set_tuning: unknown key '" + k + "'");
     }

@@ -113,6 +113,39 @@ template <> struct Dft<16> {
     }
 };
 
+template <> struct Dft<32> {
+    // decimation in time over two 16-point transforms: X[k] = E[k] + W32^k O[k], X[k + 16] = E[k] - W32^k O[k]
+    static __device__ __forceinline__ void run(float2 (&w)[32]) {
+        float2 a[16], b[16];
+#pragma unroll
+        for (int s = 0; s < 16; ++s) { a[s] = w[2 * s]; b[s] = w[2 * s + 1]; }
+        Dft<16>::run(a);
+        Dft<16>::run(b);
+        constexpr float h = 0.70710678118654752440f;
+        constexpr float c[16] = {1.f, 0.98078528040323044913f, 0.92387953251128675613f, 0.83146961230254523708f,
+                                 0.70710678118654752440f, 0.55557023301960222474f, 0.38268343236508977173f,
+                                 0.19509032201612826785f, 0.f, -0.19509032201612826785f, -0.38268343236508977173f,
+                                 -0.55557023301960222474f, -0.70710678118654752440f, -0.83146961230254523708f,
+                                 -0.92387953251128675613f, -0.98078528040323044913f};
+        constexpr float sn[16] = {0.f, 0.19509032201612826785f, 0.38268343236508977173f, 0.55557023301960222474f,
+                                  0.70710678118654752440f, 0.83146961230254523708f, 0.92387953251128675613f,
+                                  0.98078528040323044913f, 1.f, 0.98078528040323044913f, 0.92387953251128675613f,
+                                  0.83146961230254523708f, 0.70710678118654752440f, 0.55557023301960222474f,
+                                  0.38268343236508977173f, 0.19509032201612826785f};
+#pragma unroll
+        for (int k = 0; k < 16; ++k) {
+            float2 o;
+            if (k == 0) o = b[0];
+            else if (k == 4) o = make_float2((b[4].x + b[4].y) * h, (b[4].y - b[4].x) * h);            // (1 - i)/sqrt2
+            else if (k == 8) o = make_float2(b[8].y, -b[8].x);                                         // -i
+            else if (k == 12) o = make_float2((b[12].y - b[12].x) * h, -(b[12].x + b[12].y) * h);      // (-1 - i)/sqrt2
+            else o = cmul(b[k], make_float2(c[k], -sn[k]));                                             // W32^k
+            w[k] = make_float2(a[k].x + o.x, a[k].y + o.y);
+            w[k + 16] = make_float2(a[k].x - o.x, a[k].y - o.y);
+        }
+    }
+};
+
 // ---------------------------------------------------------------- plan
 template <int N> struct Plan {
     static_assert(N >= 32 && N <= 4096 && (N & (N - 1)) == 0, "N must be a power of two in [32, 4096]");
@@ -338,6 +371,101 @@ __device__ __forceinline__ void fft_inverse(float2 (&v)[16], const int t, const 
     fft_forward<N, Slots, Sync, TW>(v, t, tw, sm);
 #pragma unroll
     for (int e = 0; e < 16; ++e) v[e] = cswap(v[e]);
+}
+
+// ================================================================ 32 values per thread (N = 512, 1024)
+// The same Stockham scheme with E = 32 values per thread: T = N/32 threads per transform, canonical layout
+// v[e] = x[t + e T], first stage radix 32, second stage radix R2 = N/32 (16 or 32) and ONE shared-memory exchange
+// instead of the two the 16-value plan needs at these lengths.  The column-type kernels move every element through
+// shared memory 6 instead of 10 times per transform pair, which is what bounds them (ncu: LSU data pipe 64 % busy at
+// 57 % issue utilisation with the 16-value plan).  Costs registers: 64 for the data and 2 (R2 - 1) B2 for the twiddles.
+template <int N> struct Plan32 {
+    static_assert(N == 512 || N == 1024, "the 32-value plan covers N = 512 and 1024");
+    static constexpr int T = N / 32;
+    static constexpr int R2 = N / 32;                         // 16 or 32
+    static constexpr int B2 = 32 / R2;                        // butterflies per thread in stage 2
+    static constexpr int NTW2 = B2 * (R2 - 1);
+};
+
+template <int N> struct Twiddles32 {
+    using P = Plan32<N>;
+    float2 w2[P::NTW2];                                      // W_N^{((t + b T) mod 32) r}, r = 1..R2-1
+    __device__ __forceinline__ void init(const int t) {
+#pragma unroll
+        for (int b = 0; b < P::B2; ++b) {
+            const int q = (t + b * P::T) & 31;
+#pragma unroll
+            for (int r = 1; r < P::R2; ++r) w2[b * (P::R2 - 1) + r - 1] = root_of_unity(q * r, N);
+        }
+    }
+    __device__ __forceinline__ float2 tw2(const int b, const int r) const { return w2[b * (P::R2 - 1) + r - 1]; }
+};
+
+// C transforms interleaved as in ColSlots (a warp = 32/C consecutive t x C columns, linear [row][C] so that a TMA box
+// lands in it).  The exchange writes rows 32 t + r and reads rows t + e T; XOR-ing the row with (row >> 5) & M,
+// M = 16/C - 1, spreads the 32/C writes of a warp over the whole 128-byte bank window.  Both XOR terms are constants of
+// the thread (t & M) or of the unrolled index ((e T / 32) & M), folded into M + 1 base pointers on each side.
+template <int C, int T> struct ColSlots32 {
+    static constexpr int M = (C < 16) ? 16 / C - 1 : 0;
+    static_assert(T == 16 || T == 32, "ColSlots32: N = 512 or 1024");
+    float2* base;
+    float2* wb[M + 1];
+    float2* rb[M + 1];
+    __device__ __forceinline__ ColSlots32(float2* b, const int t) : base(b) {
+        const int sw = t & M;
+#pragma unroll
+        for (int k = 0; k <= M; ++k) {
+            wb[k] = b + (32 * t + ((k ^ sw) - k)) * C;
+            rb[k] = b + (t ^ k) * C;
+        }
+    }
+    __device__ __forceinline__ float2& at(const int idx) const { return base[idx * C]; }
+    __device__ __forceinline__ float2& x1w(const int r) const { return wb[r & M][r * C]; }
+    __device__ __forceinline__ float2& x1r(const int e) const { return rb[((e * T) >> 5) & M][e * T * C]; }
+};
+
+// One transform per contiguous line padded by one element per 32 (the 32 t + r writes of consecutive t land 33 elements
+// apart: conflict-free); every access is a per-thread base pointer plus a compile-time offset.
+template <int N> struct RowLine32 { static constexpr int LEN = N + N / 32; };
+template <int N> struct RowSlots32 {
+    static constexpr int T = Plan32<N>::T;
+    float2 *w1, *rd;
+    __device__ __forceinline__ RowSlots32(float2* line, const int t) : w1(line + 33 * t), rd(line + t) {}
+    __device__ __forceinline__ float2& x1w(const int r) const { return w1[r]; }
+    __device__ __forceinline__ float2& x1r(const int e) const { return rd[e * T + ((e * T) >> 5)]; }
+};
+
+template <int N, class Slots, class Sync>
+__device__ __forceinline__ void fft32_forward(float2 (&v)[32], const Twiddles32<N>& tw, const Slots& sm) {
+    using P = Plan32<N>;
+    Dft<32>::run(v);                                          // stage 1: radix 32, Ns = 1
+    Sync::sync();                                             // earlier readers of the buffer are done
+#pragma unroll
+    for (int r = 0; r < 32; ++r) sm.x1w(r) = v[r];
+    Sync::sync();
+#pragma unroll
+    for (int e = 0; e < 32; ++e) v[e] = sm.x1r(e);
+    constexpr int R2 = P::R2, B2 = P::B2;                     // stage 2: radix R2, Ns = 32 (last stage: output canonical)
+#pragma unroll
+    for (int b = 0; b < B2; ++b) {
+        float2 w[R2];
+#pragma unroll
+        for (int r = 0; r < R2; ++r) w[r] = v[b + r * B2];
+#pragma unroll
+        for (int r = 1; r < R2; ++r) w[r] = cmul(w[r], tw.tw2(b, r));
+        Dft<R2>::run(w);
+#pragma unroll
+        for (int r = 0; r < R2; ++r) v[b + r * B2] = w[r];
+    }
+}
+
+template <int N, class Slots, class Sync>
+__device__ __forceinline__ void fft32_inverse(float2 (&v)[32], const Twiddles32<N>& tw, const Slots& sm) {
+#pragma unroll
+    for (int e = 0; e < 32; ++e) v[e] = cswap(v[e]);
+    fft32_forward<N, Slots, Sync>(v, tw, sm);
+#pragma unroll
+    for (int e = 0; e < 32; ++e) v[e] = cswap(v[e]);
 }
 
 }  // namespace psb

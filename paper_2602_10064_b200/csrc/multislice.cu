@@ -173,6 +173,85 @@ k_row_transmit(float2* __restrict__ W, const float2* __restrict__ psi0, const fl
     }
 }
 
+// ------------------------------------------------------------------------------------ row pass, 32 values per thread
+// NX = 512 and 1024 with the 32-value transform plan: T = NX/32 threads per row (half a warp / one warp: no block
+// barrier at all), one shared-memory exchange per transform.  Used for the slices after the first when the active
+// columns [0, col_lo) and [col_hi, NX) satisfy 10T <= col_lo <= 12T and 20T <= col_hi <= 22T (band limit set by the
+// x direction): elements e <= 9 and e >= 22 are then always active, 12 <= e <= 19 never (compile-time zeros in, dead
+// values out), and e = 10, 11, 20, 21 carry a per-thread predicate.
+template <int NX> struct RowCfg32 {
+    static constexpr int T = Plan32<NX>::T;
+    static constexpr int THREADS = 128;
+    static constexpr int RPB = THREADS / T;
+#ifndef PSB_ROW32_BLOCKS
+#define PSB_ROW32_BLOCKS 3
+#endif
+    static constexpr int MIN_BLOCKS = PSB_ROW32_BLOCKS;
+    static constexpr size_t SMEM = (size_t)RPB * RowLine32<NX>::LEN * sizeof(float2);
+};
+
+template <int NX>
+__global__ void __launch_bounds__(RowCfg32<NX>::THREADS, RowCfg32<NX>::MIN_BLOCKS)
+k_row_transmit32(float2* __restrict__ W, const float* __restrict__ V, const ChunkMap cm, const int ny_shift,
+                 const int n_slices, const int slice, const float sigma, const int n_items, const int col_lo,
+                 const int col_hi) {
+    using Cfg = RowCfg32<NX>;
+    constexpr int T = Cfg::T;
+    using Slots = RowSlots32<NX>;
+    extern __shared__ float2 smem[];
+    const int t = threadIdx.x % T, r = threadIdx.x / T;
+    Twiddles32<NX> tw;
+    tw.init(t);
+    const Slots slots(smem + (size_t)r * RowLine32<NX>::LEN, t);
+    const bool a10 = t + 10 * T < col_lo, a11 = t + 11 * T < col_lo, a20 = t + 20 * T >= col_hi, a21 = t + 21 * T >= col_hi;
+    auto active = [&](const int e) -> bool {
+        return e <= 9 || e >= 22 || (e == 10 && a10) || (e == 11 && a11) || (e == 20 && a20) || (e == 21 && a21);
+    };
+    const unsigned np = (unsigned)cm.np;
+    const unsigned n_rows = np * (unsigned)cm.nf << ny_shift;
+    const unsigned stride = gridDim.x * Cfg::RPB;
+    const unsigned dy = stride & ((1u << ny_shift) - 1u), dl = stride >> ny_shift;
+    const unsigned dlf = dl / np, dlp = dl - dlf * np;
+    unsigned rho = blockIdx.x * Cfg::RPB + r;
+    RowCursor cur;
+    cur.init(rho, ny_shift, np);
+    // next-row L2 prefetch: the wave row is 2T lines of 128 bytes (two per thread), the V row T lines
+    const bool pf0 = (16 * t < col_lo) || (16 * t + 16 > col_hi);
+    const bool pf1 = (16 * (t + T) < col_lo) || (16 * (t + T) + 16 > col_hi);
+
+    for (int item = blockIdx.x; item < n_items; item += gridDim.x, rho += stride) {
+        const unsigned p = cm.p0 + cur.lp, f = cm.f0 + cur.lf, y = cur.y;
+        const unsigned wrow_i = ((p * (unsigned)cm.F + f) << ny_shift) + y;
+        const unsigned vrow_i = ((f * (unsigned)n_slices + (unsigned)slice) << ny_shift) + y;
+        cur.advance(dy, dlp, dlf, ny_shift, np);
+        if (rho + stride < n_rows) {
+            const unsigned pn = cm.p0 + cur.lp, fn = cm.f0 + cur.lf;
+            const unsigned wn_i = ((pn * (unsigned)cm.F + fn) << ny_shift) + cur.y;
+            const unsigned vn_i = ((fn * (unsigned)n_slices + (unsigned)slice) << ny_shift) + cur.y;
+            tma::prefetch_l2(V + (size_t)vn_i * NX + 32 * t);
+            if (pf0) tma::prefetch_l2(W + (size_t)wn_i * NX + 16 * t);
+            if (pf1) tma::prefetch_l2(W + (size_t)wn_i * NX + 16 * (t + T));
+        }
+        float2* wrow = W + (size_t)wrow_i * NX + t;
+        const float* vrow = V + (size_t)vrow_i * NX + t;
+        float2 v[32];
+#pragma unroll
+        for (int e = 0; e < 32; ++e) v[e] = active(e) ? wrow[e * T] : make_float2(0.f, 0.f);
+        fft32_inverse<NX, Slots, WarpSync>(v, tw, slots);
+        {
+            float sv[32];                                  // V of this row: an L2 hit (prefetched with the previous item)
+#pragma unroll
+            for (int e = 0; e < 32; ++e) sv[e] = __ldg(vrow + e * T);
+#pragma unroll
+            for (int e = 0; e < 32; ++e) v[e] = cmul(v[e], cis_fast(sigma * sv[e]));
+        }
+        fft32_forward<NX, Slots, WarpSync>(v, tw, slots);
+#pragma unroll
+        for (int e = 0; e < 32; ++e)
+            if (active(e)) wrow[e * T] = v[e];
+    }
+}
+
 // ------------------------------------------------------------------------------------ column pass
 // A block owns C adjacent k-columns x all NY rows of one wave per item.  The tile travels
 // global -> shared -> global through the TMA engine (2-D tensor map over the wave array viewed as
@@ -284,6 +363,152 @@ k_col_propagate(const __grid_constant__ CUtensorMap wmap, const int tiles_lo, co
     if (threadIdx.x == 0) tma::bulk_wait_all<0>();
 }
 
+// ------------------------------------------------------------------------------------ column pass, 32 values per thread
+// The same pass for NY = 512 and 1024 with the 32-value transform plan (fft_core.cuh): T = NY/32 threads per column,
+// one shared-memory exchange per transform instead of two.  Blocks are half as large (C columns x NY/32 threads), so
+// the same number of stages and resident blocks holds half as many warps, each with twice the independent work.
+template <int NY> struct ColCfg32 {
+    static constexpr int T = Plan32<NY>::T;
+#ifndef PSB_COL32_C512
+#define PSB_COL32_C512 8
+#endif
+    static constexpr int C = (NY <= 512) ? PSB_COL32_C512 : 4;
+    static constexpr int THREADS = C * T;                                  // 128
+#ifndef PSB_COL32_NS
+#define PSB_COL32_NS 2
+#endif
+#ifndef PSB_COL32_BLOCKS
+#define PSB_COL32_BLOCKS 3
+#endif
+    static constexpr int NS = PSB_COL32_NS;
+    static constexpr int BOX_R = 256;
+    static constexpr int NBOX = NY / BOX_R;
+    static constexpr int MIN_BLOCKS = PSB_COL32_BLOCKS;
+    static constexpr uint32_t STAGE_BYTES = (uint32_t)NY * C * sizeof(float2);
+    static constexpr size_t SMEM = (size_t)NS * STAGE_BYTES + (size_t)NY * sizeof(float2) + NS * sizeof(uint64_t) + 128;
+};
+
+template <int NY, bool LAST>
+__global__ void __launch_bounds__(ColCfg32<NY>::THREADS, ColCfg32<NY>::MIN_BLOCKS)
+k_col_propagate32(const __grid_constant__ CUtensorMap wmap, const int tiles_lo, const int tile_gap, const int n_tiles,
+                  const int32_t* __restrict__ nmax, const float2* __restrict__ px, const float2* __restrict__ py,
+                  const ChunkMap cm, const int n_items) {
+    using Cfg = ColCfg32<NY>;
+    constexpr int T = Cfg::T, C = Cfg::C, SUB = kColTile / C, NS = Cfg::NS, PF = 1;
+    using Slots = ColSlots32<C, T>;
+    extern __shared__ __align__(1024) float2 smem_col[];
+    float2* stage0 = smem_col;
+    float2* py_s = smem_col + (size_t)NS * NY * C;
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem_col + (size_t)NS * NY * C + NY);
+    const int c = threadIdx.x % C, t = threadIdx.x / C;
+    const int per_wave = n_tiles * SUB;
+
+    auto issue_load = [&](const int item, const int s) {
+        const int l = item / per_wave, rem = item % per_wave;
+        const int tj = rem / SUB;
+        const int kx0 = (tj < tiles_lo ? tj : tj + tile_gap) * kColTile + (rem % SUB) * C;
+        const int p = cm.p0 + l % cm.np, f = cm.f0 + l / cm.np;
+        const int row0 = (p * cm.F + f) * NY;
+        tma::mbar_arrive_expect_tx(&full[s], Cfg::STAGE_BYTES);
+#pragma unroll
+        for (int b = 0; b < Cfg::NBOX; ++b)
+            tma::tensor_load_2d(stage0 + (size_t)s * NY * C + (size_t)b * Cfg::BOX_R * C, &wmap, 2 * kx0,
+                                row0 + b * Cfg::BOX_R, &full[s]);
+    };
+
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int s = 0; s < NS; ++s) tma::mbar_init(&full[s], 1);
+        tma::fence_mbar_init();
+    }
+    for (int i = threadIdx.x; i < NY; i += Cfg::THREADS) py_s[i] = py[i];
+    Twiddles32<NY> tw;
+    tw.init(t);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int k = 0; k < PF; ++k)
+            if (blockIdx.x + k * gridDim.x < n_items) issue_load(blockIdx.x + k * gridDim.x, k);
+    }
+
+    int it = 0;
+    int rem = blockIdx.x % per_wave;
+    const int rem_step = gridDim.x % per_wave;
+    for (int item = blockIdx.x; item < n_items; item += gridDim.x, ++it) {
+        const int s = it % NS;
+        if (threadIdx.x == 0) {
+            const int nxt = item + PF * gridDim.x;
+            if (nxt < n_items) {
+                tma::bulk_wait_read<NS - 2>();                // the store that last used stage (it+1)%NS has drained
+                issue_load(nxt, (it + PF) % NS);
+            }
+        }
+        const int tj = rem / SUB;
+        const int kx0 = (tj < tiles_lo ? tj : tj + tile_gap) * kColTile + (rem % SUB) * C;
+        const int kx = kx0 + c;
+        const int nm = nmax[kx];
+        const float2 pxv = px[kx];
+        float2* st = stage0 + (size_t)s * NY * C;
+        const Slots slots(st + c, t);
+        tma::mbar_wait(&full[s], (it / NS) & 1);
+        float2 v[32];
+#pragma unroll
+        for (int e = 0; e < 32; ++e) v[e] = slots.at(t + e * T);
+        auto propagate = [&]() {
+#pragma unroll
+            for (int e = 0; e < 32; ++e) {
+                const int iy = t + e * T;
+                const int n = iy < NY / 2 ? iy : NY - iy;
+                v[e] = (n <= nm) ? cmul(v[e], cmul(pxv, py_s[iy])) : make_float2(0.f, 0.f);
+            }
+        };
+        // NY = 1024: both transforms run the SAME forward code in a two-trip loop, so that the loop body of the kernel
+        // fits the instruction cache (two unrolled copies of the 32-value transform do not; ncu: 10 % of the stall
+        // samples were "no instruction"; measured +5 % at 1024, -8 % at 512, hence per size).  The inverse is the
+        // forward transform read backwards: sum_k X[k] e^{+2 pi i n k / N} is element (-n) mod N of the forward
+        // transform of X, so after the second trip canonical position j holds row (-j) mod NY, and the tile is written
+        // back with reversed row addressing.
+        constexpr bool LOOPED = (NY == 1024) && !LAST;
+        if constexpr (LOOPED) {
+#pragma unroll 1
+            for (int pass = 0; pass < 2; ++pass) {
+                fft32_forward<NY, Slots, BlockSync>(v, tw, slots);
+                if (pass == 0) propagate();
+            }
+        } else {
+            fft32_forward<NY, Slots, BlockSync>(v, tw, slots);
+            propagate();
+            if (!LAST) fft32_inverse<NY, Slots, BlockSync>(v, tw, slots);
+        }
+        __syncthreads();
+        if constexpr (!LOOPED) {
+#pragma unroll
+            for (int e = 0; e < 32; ++e) slots.at(t + e * T) = v[e];
+        } else {
+            // row (NY - t - e T) mod NY = (T - t) + (31 - e) T, except (t, e) = (0, 0), which is row 0
+            float2* const pr = st + c + (size_t)(T - t) * C;
+            float2* const p0 = (t == 0) ? st + c : pr + 31 * T * C;
+            *p0 = v[0];
+#pragma unroll
+            for (int e = 1; e < 32; ++e) pr[(31 - e) * T * C] = v[e];
+        }
+        tma::fence_proxy_async();
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            const int l = item / per_wave;
+            const int p = cm.p0 + l % cm.np, f = cm.f0 + l / cm.np;
+            const int row0 = (p * cm.F + f) * NY;
+#pragma unroll
+            for (int b = 0; b < Cfg::NBOX; ++b)
+                tma::tensor_store_2d(&wmap, 2 * kx0, row0 + b * Cfg::BOX_R, st + (size_t)b * Cfg::BOX_R * C);
+            tma::bulk_commit();
+        }
+        rem += rem_step;
+        if (rem >= per_wave) rem -= per_wave;
+    }
+    if (threadIdx.x == 0) tma::bulk_wait_all<0>();
+}
+
 // last slice: column tiles outside the band limit of the k-space exit wave are exact zeros
 __global__ void k_zero_cols(float2* __restrict__ W, const int nx, const int ny, const int col_lo, const int col_hi,
                             const ChunkMap cm) {
@@ -322,6 +547,31 @@ static cudaError_t launch_row(ps_ctx* c, float2* W, const float2* psi0, const fl
     return cudaGetLastError();
 }
 
+template <int NX>
+static cudaError_t launch_row32(ps_ctx* c, float2* W, const float* V, const ChunkMap& cm, int slice, float sigma, int col_lo,
+                                int col_hi) {
+    using Cfg = RowCfg32<NX>;
+    auto kern = k_row_transmit32<NX>;
+    int per_sm_grid = 0;
+    cudaError_t ce = kernel_cap(c, kern, Cfg::THREADS, Cfg::SMEM, &per_sm_grid);
+    if (ce != cudaSuccess) return ce;
+    const long long n_rows = (long long)cm.np * cm.nf * c->ny;
+    const int n_items = (int)(n_rows / Cfg::RPB);                       // RPB <= 8 divides ny
+    const int grid = n_items < per_sm_grid ? n_items : per_sm_grid;
+    int ny_shift = 0;
+    while ((1 << ny_shift) < c->ny) ++ny_shift;
+    kern<<<grid, Cfg::THREADS, Cfg::SMEM, c->stream>>>(W, V, cm, ny_shift, c->n_slices, slice, sigma, n_items, col_lo, col_hi);
+    return cudaGetLastError();
+}
+
+// the row pass of slices s > 0 with the 32-value plan (ps_set_tuning "row32": 1 on where available; 0 auto = off:
+// measured 10 % slower than the 16-value pass at 512^2 and 1024^2, its 12 warps per SM do not cover the load latency)
+static bool use_row32(const ps_ctx* c, int col_lo, int col_hi) {
+    if (!(c->nx == 512 || c->nx == 1024) || c->tune_row32 < 1 || c->vacuum_shortcut) return false;
+    const int T = c->nx / 32;
+    return col_lo >= 10 * T && col_lo <= 12 * T && col_hi >= 20 * T && col_hi <= 22 * T;
+}
+
 template <int NY, bool LAST>
 static cudaError_t launch_col(ps_ctx* c, const CUtensorMap& wmap, const ChunkMap& cm, int zero_lo, int zero_hi) {
     using Cfg = ColCfg<NY>;
@@ -337,8 +587,29 @@ static cudaError_t launch_col(ps_ctx* c, const CUtensorMap& wmap, const ChunkMap
     return cudaGetLastError();
 }
 
+template <int NY, bool LAST>
+static cudaError_t launch_col32(ps_ctx* c, const CUtensorMap& wmap, const ChunkMap& cm, int zero_lo, int zero_hi) {
+    using Cfg = ColCfg32<NY>;
+    auto kern = k_col_propagate32<NY, LAST>;
+    int per_sm_grid = 0;
+    cudaError_t ce = kernel_cap(c, kern, Cfg::THREADS, Cfg::SMEM, &per_sm_grid);
+    if (ce != cudaSuccess) return ce;
+    const int n_tiles = c->n_tiles_active;
+    const int n_items = cm.np * cm.nf * n_tiles * (kColTile / Cfg::C);
+    const int grid = n_items < per_sm_grid ? n_items : per_sm_grid;
+    kern<<<grid, Cfg::THREADS, Cfg::SMEM, c->stream>>>(wmap, zero_lo / kColTile, (zero_hi - zero_lo) / kColTile, n_tiles, c->d_nmax,
+                                                      LAST ? c->kv.d_px_last : c->kv.d_px_mid, c->kv.d_py, cm, n_items);
+    return cudaGetLastError();
+}
+
+// the column pass of this grid uses the 32-value plan (ps_set_tuning "col32": 0 auto, 1 on where available, -1 off)
+static bool use_col32(const ps_ctx* c) { return (c->ny == 512 || c->ny == 1024) && c->tune_col32 >= 0; }
+
 template <int NY>
-static bool make_wave_map(CUtensorMap* map, void* W, int nx, long long rows) {
+static bool make_wave_map(CUtensorMap* map, void* W, int nx, long long rows, bool col32) {
+    if constexpr (NY == 512 || NY == 1024) {
+        if (col32) return tma::make_map_2d_f32(map, W, 2ull * nx, (uint64_t)rows, 2 * ColCfg32<NY>::C, ColCfg32<NY>::BOX_R);
+    }
     using Cfg = ColCfg<NY>;
     return tma::make_map_2d_f32(map, W, 2ull * nx, (uint64_t)rows, 2 * Cfg::C, Cfg::BOX_R);
 }
@@ -396,7 +667,8 @@ extern "C" ps_status ps_multislice(ps_ctx* c, double kV, const void* d_psi0, int
         return fail(c, PS_EUNSUPPORTED, "ps_multislice: n_frames*n_slices*ny exceeds 2^31 (propagate the frames in chunks)");
     CUtensorMap wmap;
     bool map_ok = false;
-    PSB_DISPATCH_N(c->ny, (map_ok = make_wave_map<N_>(&wmap, d_exit, c->nx, wave_rows)));
+    const bool col32 = use_col32(c);
+    PSB_DISPATCH_N(c->ny, (map_ok = make_wave_map<N_>(&wmap, d_exit, c->nx, wave_rows, col32)));
     if (!map_ok) return fail(c, PS_ECUDA, "ps_multislice: cuTensorMapEncodeTiled failed (exit-wave array must be 16-byte aligned)");
     // contiguous range of columns outside the band limit (zero in the k-space exit wave)
     int zero_lo = 0, zero_hi = 0;
@@ -421,6 +693,7 @@ extern "C" ps_status ps_multislice(ps_ctx* c, double kV, const void* d_psi0, int
         return PS_OK;
     }
 
+    const bool row32 = use_row32(c, zero_lo, zero_hi);
     for (int p0 = 0; p0 < n_probes; p0 += np) {
         for (int f0 = 0; f0 < n_frames; f0 += nf) {
             ChunkMap cm;
@@ -432,6 +705,8 @@ extern "C" ps_status ps_multislice(ps_ctx* c, double kV, const void* d_psi0, int
                 {
                 ProfScope ps_(c, K_ROW_TRANSMIT);
                 if (s == 0) { PSB_DISPATCH_N(c->nx, (e = launch_row<N_, true>(c, W, psi0, d_V, cm, s, sigma, zero_lo, zero_hi))); }
+                else if (row32 && c->nx == 512) e = launch_row32<512>(c, W, d_V, cm, s, sigma, zero_lo, zero_hi);
+                else if (row32 && c->nx == 1024) e = launch_row32<1024>(c, W, d_V, cm, s, sigma, zero_lo, zero_hi);
                 else        { PSB_DISPATCH_N(c->nx, (e = launch_row<N_, false>(c, W, psi0, d_V, cm, s, sigma, zero_lo, zero_hi))); }
                 }
                 if (e != cudaSuccess) return fail(c, PS_ECUDA, std::string("k_row_transmit: ") + cudaGetErrorString(e));
@@ -446,9 +721,13 @@ extern "C" ps_status ps_multislice(ps_ctx* c, double kV, const void* d_psi0, int
                         k_zero_cols<<<zb, 256, 0, c->stream>>>(W, c->nx, c->ny, zero_lo, zero_hi, cm);
                         c->launches++;
                     }
-                    PSB_DISPATCH_N(c->ny, (e = launch_col<N_, true>(c, wmap, cm, zero_lo, zero_hi)));
+                    if (col32 && c->ny == 512) e = launch_col32<512, true>(c, wmap, cm, zero_lo, zero_hi);
+                    else if (col32 && c->ny == 1024) e = launch_col32<1024, true>(c, wmap, cm, zero_lo, zero_hi);
+                    else { PSB_DISPATCH_N(c->ny, (e = launch_col<N_, true>(c, wmap, cm, zero_lo, zero_hi))); }
                 } else {
-                    PSB_DISPATCH_N(c->ny, (e = launch_col<N_, false>(c, wmap, cm, zero_lo, zero_hi)));
+                    if (col32 && c->ny == 512) e = launch_col32<512, false>(c, wmap, cm, zero_lo, zero_hi);
+                    else if (col32 && c->ny == 1024) e = launch_col32<1024, false>(c, wmap, cm, zero_lo, zero_hi);
+                    else { PSB_DISPATCH_N(c->ny, (e = launch_col<N_, false>(c, wmap, cm, zero_lo, zero_hi))); }
                 }
                 }
                 if (e != cudaSuccess) return fail(c, PS_ECUDA, std::string("k_col_propagate: ") + cudaGetErrorString(e));

@@ -137,6 +137,31 @@ def test_multislice_grid_sizes(torch, nx, ny):
         assert rel_l2(ex[0, i], eo) < TOL_EXIT
 
 
+@pytest.mark.parametrize("n,row32,col32", [(512, 1, 1), (512, 0, -1), (1024, 1, 1), (1024, 0, -1), (512, 1, -1)])
+def test_multislice_value_plans(torch, n, row32, col32):
+    """ps_set_tuning row32 / col32: the 32-values-per-thread row and column passes (one shared-memory exchange per
+    transform; the column pass of 1024 runs its inverse as a reversed forward transform) and the 16-value passes give
+    the oracle's exit wave on square 512 / 1024 grids, 3 probes x 2 frames so that several waves share a launch."""
+    import paper_2602_10064_b200 as ps
+    rng = np.random.default_rng(n + 10 * row32 + col32)
+    w = make_workload("c1_si_128", mini=True)
+    w.nx, w.ny, w.n_slices = n, n, 3
+    w.cell = np.array([n * 0.09, n * 0.09, 6.0])
+    ctx = make_ctx(w)
+    ctx.set_tuning("row32", row32)
+    ctx.set_tuning("col32", col32)
+    F, P = 2, 3
+    Vk = (rng.normal(size=(F, 3, n, n)) + 1j * rng.normal(size=(F, 3, n, n)))
+    ky = np.fft.fftfreq(n)[:, None]; kx = np.fft.fftfreq(n)[None, :]
+    V32 = (400.0 * np.real(np.fft.ifft2(Vk * np.exp(-200.0 * (kx ** 2 + ky ** 2)))) * n).astype(np.float32)
+    psi0 = np.stack([O.tilted_plane_wave(n, n, m, -m).astype(np.complex64) for m in range(P)])
+    ex = ps.ps_multislice(ctx, 80.0, _t(torch, psi0), _t(torch, V32)).cpu().numpy()
+    for p_ in (0, P - 1):
+        for i in range(F):
+            eo = O.multislice(psi0[p_].astype(np.complex128), V32[i].astype(np.float64), w.cell, 80.0)
+            assert rel_l2(ex[p_, i], eo) < TOL_EXIT
+
+
 def test_multislice_free_space_plane_wave_is_exact(torch):
     """P5: V = 0 leaves the plane wave untouched: exit = sqrt(nx ny) at k = 0, zero elsewhere."""
     import paper_2602_10064_b200 as ps
