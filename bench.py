@@ -255,15 +255,18 @@ def tacaw_micro(shapes_a=None, shapes_b=None):
                     (1, 2048, 512, 2048), (1, 4096, 256, 256), (8, 256, 512, 256), (16, 128, 512, 128),
                     (1, 256, 1024, 256), (1, 64, 128, 64)]
         shapes_b = [(1024, 64, 256), (512, 64, 256), (1024, 64, 64)]
-    for P, F, n, nb in shapes_a or []:
+    for shp in shapes_a or []:
+        P, F, n, nb = shp[:4]
+        tiled = len(shp) > 4 and shp[4] == 1
         ctx = ctx_for(n)
-        ex = torch.view_as_complex(torch.randn((P, F, n, n, 2), device="cuda"))
+        eshape = ps.exit_shape(ctx, P, F, ps.PS_LAYOUT_TILED_APERTURE if tiled else ps.PS_LAYOUT_DENSE)
+        ex = torch.view_as_complex(torch.randn(tuple(eshape) + (2,), device="cuda"))
         bins = None if nb == F else np.arange(nb, dtype=np.int32)
         I = torch.empty((P, nb, n, n), dtype=torch.float32, device="cuda")
         ms = _event_time(torch, lambda: ps.ps_tacaw(ctx, ex, 2.0, bins, d_I=I), flush)
         nk = ctx.n_k_aperture
         byts = (8.0 * F + 4.0 * nb) * nk * P + 4.0 * nb * (n * n - nk) * P
-        print(json.dumps({"micro": "ps_tacaw", "P": P, "frames": F, "grid": n, "bins": nb, "ms": ms,
+        print(json.dumps({"micro": "ps_tacaw", "layout": "tiled" if tiled else "dense", "P": P, "frames": F, "grid": n, "bins": nb, "ms": ms,
                           "algorithmic_GB": byts / 1e9, "GBps": byts / ms / 1e6, "frac_of_hbm_peak": byts / ms / 1e6 / peak}))
         del ex, I, ctx
     # path B: one 64-frame chunk of a 4096-frame stream, 256 bins (config 4's shape) and a 1024^2 grid
@@ -398,7 +401,7 @@ def main():
                          "and print one JSON line")
     ap.add_argument("--tacaw-micro", action="store_true",
                     help="time ps_tacaw / ps_tacaw_add alone on synthetic stacks of several shapes and exit")
-    ap.add_argument("--micro-a", action="append", default=None, metavar="P,FRAMES,GRID,BINS",
+    ap.add_argument("--micro-a", action="append", default=None, metavar="P,FRAMES,GRID,BINS[,TILED]",
                     help="--tacaw-micro: this path-A shape instead of the default list (repeatable)")
     ap.add_argument("--micro-b", action="append", default=None, metavar="GRID,CHUNK_FRAMES,BINS",
                     help="--tacaw-micro: this path-B shape instead of the default list (repeatable)")

@@ -78,14 +78,17 @@ typedef enum {
     PS_ESTATE = -5         /* call order violated (geometry / form factors not set, ...)       */
 } ps_status;
 
-/* exit-wave layouts accepted by ps_multislice / ps_tacaw / ps_haadf */
-#define PS_LAYOUT_DENSE 0  /* complex64 [P][F][ny][nx], k-space, FFT index order (A13)        */
-/* SURVEY.md 8(b) also sketched PS_LAYOUT_TILED_APERTURE (only the in-aperture k points, tiled for the
- * time transform: same values, 0.35x the bytes).  It is NOT offered: pixels outside the band limit
- * are written as exact zeros in the dense layout and are skipped (never read) by ps_tacaw, ps_haadf
- * and the streaming path, so the compact layout would save capacity only (config 3: 12 instead of
- * 34 GB per 16-probe chunk), not traffic; the time-major tiling measured no faster
- * (profiles/r1_tacaw_kernels.md).  Any other value of `exit_layout` returns PS_EUNSUPPORTED. */
+/* exit-wave layouts (PAPER.md:89 WFData "indexed by probe position, time, and reciprocal space
+ * coordinates").  Values are identical in both; ps_exit_bytes gives the size of an array, ps_exit_to_dense converts. */
+#define PS_LAYOUT_DENSE 0           /* complex64 [P][F][ny][nx], k-space, FFT index order (A13); accepted everywhere */
+#define PS_LAYOUT_TILED_APERTURE 1  /* complex64 [P][ny][n_tiles][F][8]: only the column tiles (8 adjacent kx, FFT order,
+                                     * ascending) that hold at least one in-band point, and the F frames of a (row, tile)
+                                     * contiguous: the time transform streams F*64-byte runs instead of gathering 64-byte
+                                     * pieces 8*nx*ny bytes apart.  n_tiles/(nx/8) = 0.69 of the dense size at the 2/3
+                                     * band limit.  Written by ps_multislice (the wave is then propagated chunk by chunk in
+                                     * a work array in scratch / the installed workspace), read by ps_tacaw and
+                                     * ps_exit_to_dense; every other consumer takes PS_LAYOUT_DENSE only and answers
+                                     * PS_EUNSUPPORTED otherwise. */
 
 /* ---------------------------------------------------------------- life cycle */
 
@@ -190,10 +193,19 @@ PS_API ps_status ps_make_incident(ps_ctx* ctx, double kV, double semi_angle_mrad
  *   exit = fft2(psi)/sqrt(nx ny)   (k-space, unitary, A9, A13)
  *   d_psi0  complex64 [n_probes][ny][nx]
  *   d_V     float32   [n_frames][n_slices][ny][nx]
- *   d_exit  complex64 [n_probes][n_frames][ny][nx]                              (written)
- * The wave is propagated in place inside d_exit (no other wave storage). */
+ *   d_exit  exit waves in `exit_layout` (ps_exit_bytes bytes)                   (written)
+ * PS_LAYOUT_DENSE: the wave is propagated in place inside d_exit (no other wave storage).  PS_LAYOUT_TILED_APERTURE: it is
+ * propagated in a dense work array of as many waves as the scratch holds (installed workspace, else a library-owned
+ * buffer of an eighth of the free device memory, 768 MB ... 16 GB), chunk by chunk, and the last column pass of every
+ * chunk writes the k-space exit waves straight into the tiled array. */
 PS_API ps_status ps_multislice(ps_ctx* ctx, double kV, const void* d_psi0, int n_probes, const float* d_V,
                         int n_frames, void* d_exit, int exit_layout);
+
+/* Bytes of an exit-wave array of n_probes x n_frames waves in `exit_layout` (0 for an unknown layout or before
+ * ps_set_geometry).  ps_exit_to_dense expands a PS_LAYOUT_TILED_APERTURE array into the dense one (exact zeros in the
+ * column tiles the tiled layout does not store); both arrays caller-owned device memory, asynchronous on the ctx stream. */
+PS_API size_t    ps_exit_bytes(const ps_ctx* ctx, int n_probes, int n_frames, int exit_layout);
+PS_API ps_status ps_exit_to_dense(ps_ctx* ctx, const void* d_tiled, int n_probes, int n_frames, void* d_dense);
 
 /* a7: TACAW transform (A14): for every probe and k,
  *   Psi~_n = sum_j (Psi_j - <Psi>_t) exp(-2 pi i n j / F),  I = |Psi~_n|^2,  f_n = n/(F dt).

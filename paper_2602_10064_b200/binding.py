@@ -17,6 +17,7 @@ _lib = None
 
 PS_OK, PS_EINVAL, PS_EUNSUPPORTED, PS_EWORKSPACE, PS_ECUDA, PS_ESTATE = 0, -1, -2, -3, -4, -5
 PS_LAYOUT_DENSE = 0
+PS_LAYOUT_TILED_APERTURE = 1
 
 _PROTOTYPES = {
     # name: (restype, argtypes)
@@ -39,6 +40,8 @@ _PROTOTYPES = {
     "ps_make_incident": (C.c_int, [C.c_void_p, C.c_double, C.c_double, C.c_int, C.c_void_p, C.c_int, C.c_void_p]),
     "ps_multislice": (C.c_int, [C.c_void_p, C.c_double, C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_void_p, C.c_int]),
     "ps_tacaw": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_double, C.c_int, C.c_void_p, C.c_void_p]),
+    "ps_exit_bytes": (C.c_size_t, [C.c_void_p, C.c_int, C.c_int, C.c_int]),
+    "ps_exit_to_dense": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_void_p]),
     "ps_tacaw_begin": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_double, C.c_int, C.c_void_p, C.c_void_p]),
     "ps_tacaw_set_reference": (C.c_int, [C.c_void_p, C.c_void_p]),
     "ps_tacaw_add": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_int]),
@@ -252,23 +255,52 @@ def ps_make_incident(ctx: Context, kV: float, semi_angle_mrad: float = 0.0, xy_o
     return d_psi0
 
 
-def ps_multislice(ctx: Context, kV: float, d_psi0, d_V, d_exit=None):
-    """psi0 complex64 [P][ny][nx], V float32 [F][S][ny][nx] -> exit waves complex64 [P][F][ny][nx] (k-space)."""
+def exit_shape(ctx: Context, n_probes: int, n_frames: int, layout: int = PS_LAYOUT_DENSE):
+    """Shape of a complex64 exit-wave array: dense [P][F][ny][nx], tiled [P][ny][n_tiles][F][8] (size from ps_exit_bytes)."""
+    if layout == PS_LAYOUT_DENSE:
+        return (n_probes, n_frames, ctx.ny, ctx.nx)
+    nbytes = int(ctx._lib.ps_exit_bytes(ctx._h, int(n_probes), int(n_frames), int(layout)))
+    if nbytes == 0:
+        raise ValueError("unknown exit layout")
+    return (n_probes, ctx.ny, nbytes // (n_probes * ctx.ny * n_frames * 64), n_frames, 8)
+
+
+def _exit_layout(d_exit):
+    return PS_LAYOUT_TILED_APERTURE if d_exit.dim() == 5 else PS_LAYOUT_DENSE
+
+
+def ps_multislice(ctx: Context, kV: float, d_psi0, d_V, d_exit=None, layout: int = PS_LAYOUT_DENSE):
+    """psi0 complex64 [P][ny][nx], V float32 [F][S][ny][nx] -> k-space exit waves complex64, dense [P][F][ny][nx] or
+    (layout = PS_LAYOUT_TILED_APERTURE, or a 5-D d_exit) tiled [P][ny][n_tiles][F][8]."""
     import torch
     _need(d_psi0, torch.complex64, "d_psi0"); _need(d_V, torch.float32, "d_V")
     P, F = int(d_psi0.shape[0]), int(d_V.shape[0])
     if d_exit is None:
-        d_exit = torch.empty((P, F, ctx.ny, ctx.nx), dtype=torch.complex64, device=ctx.device)
+        d_exit = torch.empty(exit_shape(ctx, P, F, layout), dtype=torch.complex64, device=ctx.device)
     _need(d_exit, torch.complex64, "d_exit")
-    ctx._check(ctx._lib.ps_multislice(ctx._h, float(kV), _ptr(d_psi0), P, _ptr(d_V), F, _ptr(d_exit), PS_LAYOUT_DENSE))
+    ctx._check(ctx._lib.ps_multislice(ctx._h, float(kV), _ptr(d_psi0), P, _ptr(d_V), F, _ptr(d_exit), _exit_layout(d_exit)))
     return d_exit
 
 
+def ps_exit_to_dense(ctx: Context, d_tiled, d_dense=None):
+    """Tiled exit waves [P][ny][n_tiles][F][8] -> dense [P][F][ny][nx] (zeros in the tiles the tiled layout omits)."""
+    import torch
+    _need(d_tiled, torch.complex64, "d_tiled")
+    P, F = int(d_tiled.shape[0]), int(d_tiled.shape[3])
+    if d_dense is None:
+        d_dense = torch.empty((P, F, ctx.ny, ctx.nx), dtype=torch.complex64, device=ctx.device)
+    _need(d_dense, torch.complex64, "d_dense")
+    ctx._check(ctx._lib.ps_exit_to_dense(ctx._h, _ptr(d_tiled), P, F, _ptr(d_dense)))
+    return d_dense
+
+
 def ps_tacaw(ctx: Context, d_exit, dt_fs: float, bins=None, d_I=None):
-    """exit waves complex64 [P][F][ny][nx] -> I float32 [P][n_bins][ny][nx]; bins = signed FFT bins or None (all)."""
+    """exit waves complex64 (dense [P][F][ny][nx] or tiled [P][ny][n_tiles][F][8]) -> I float32 [P][n_bins][ny][nx];
+    bins = signed FFT bins or None (all)."""
     import torch
     _need(d_exit, torch.complex64, "d_exit")
-    P, F = int(d_exit.shape[0]), int(d_exit.shape[1])
+    layout = _exit_layout(d_exit)
+    P, F = int(d_exit.shape[0]), int(d_exit.shape[1] if layout == PS_LAYOUT_DENSE else d_exit.shape[3])
     if bins is None:
         nb, bp, bh = F, C.c_void_p(0), None
     else:
@@ -277,7 +309,7 @@ def ps_tacaw(ctx: Context, d_exit, dt_fs: float, bins=None, d_I=None):
     if d_I is None:
         d_I = torch.empty((P, nb, ctx.ny, ctx.nx), dtype=torch.float32, device=ctx.device)
     _need(d_I, torch.float32, "d_I")
-    ctx._check(ctx._lib.ps_tacaw(ctx._h, _ptr(d_exit), PS_LAYOUT_DENSE, P, F, float(dt_fs), nb, bp, _ptr(d_I)))
+    ctx._check(ctx._lib.ps_tacaw(ctx._h, _ptr(d_exit), layout, P, F, float(dt_fs), nb, bp, _ptr(d_I)))
     return d_I
 
 

@@ -211,7 +211,7 @@ extern "C" void ps_destroy(ps_ctx* c) {
     if (!c) return;
     cudaSetDevice(c->device);
     cudaStreamSynchronize(c->stream);
-    cudaFree(c->d_nmax); cudaFree(c->d_tiles); cudaFree(c->d_tile_active);
+    cudaFree(c->d_nmax); cudaFree(c->d_tiles); cudaFree(c->d_tile_active); cudaFree(c->d_tile_slot);
     cudaFree(c->d_ftab); cudaFree(c->d_elem_of_Z);
     cudaFree(c->kv.d_px_mid); cudaFree(c->kv.d_px_last); cudaFree(c->kv.d_py);
     cudaFree(c->scratch.p); cudaFree(c->misc.p); cudaFree(c->qorder.p); cudaFree(c->ts.d_bins.p); cudaFree(c->ts.d_ref.p); cudaFree(c->ts.d_tw.p);
@@ -296,6 +296,9 @@ extern "C" ps_status ps_set_geometry(ps_ctx* c, const double cell[3], int nx, in
     if ((s = upload(c, &c->d_nmax, c->h_nmax)) != PS_OK) return s;
     if ((s = upload(c, &c->d_tiles, c->h_tiles)) != PS_OK) return s;
     if ((s = upload(c, &c->d_tile_active, act)) != PS_OK) return s;
+    c->h_tile_slot.assign(nt, -1);                               // tile -> position among the active tiles (tiled exit layout)
+    for (int j = 0; j < c->n_tiles_active; ++j) c->h_tile_slot[c->h_tiles[j]] = j;
+    if ((s = upload(c, &c->d_tile_slot, c->h_tile_slot)) != PS_OK) return s;
     c->kv.kV = -1.0;
     c->ftab_valid = false;
     c->qorder_valid = false;

@@ -90,6 +90,8 @@ struct ps_ctx {
     std::vector<int32_t> h_tiles;           // active column tiles (kColTile columns) in the aperture
     int32_t* d_tiles = nullptr;
     uint8_t* d_tile_active = nullptr;       // [nx/kColTile]
+    std::vector<int32_t> h_tile_slot;       // [nx/kColTile] position of a tile among the active ones, -1 if inactive
+    int32_t* d_tile_slot = nullptr;
     int n_tiles_active = 0;
     int wave_chunk = 0;
     int vacuum_shortcut = 0;                // ps_set_vacuum_shortcut: rows with V == 0 skip the transmit + FFT pair (exact)

@@ -36,7 +36,11 @@ template <int NX> struct RowCfg {
 };
 
 struct ChunkMap {           // chunk of waves: probes [p0,p0+np) x frames [f0,f0+nf); local l = lf*np + lp
-    int p0, np, f0, nf, F;  // F = total frames (exit layout [P][F][ny][nx])
+    int p0, np, f0, nf, F;  // F = total frames of the call (tiled exit layout, V and psi0 use p0 + lp, f0 + lf)
+    // the array the wave is propagated in, [.][wF][ny][nx]: wave (lp, lf) lives at ((wp0 + lp) * wF + wf0 + lf).
+    // Dense layout: the caller's exit array itself (wp0 = p0, wf0 = f0, wF = F); tiled layout: a chunk-local work
+    // array in scratch (wp0 = wf0 = 0, wF = nf).
+    int wp0, wf0, wF;
 };
 
 // Row coordinates of a persistent thread group: rho = (lf * np + lp) * ny + y, advanced by a constant stride per item.
@@ -102,13 +106,14 @@ k_row_transmit(float2* __restrict__ W, const float2* __restrict__ psi0, const fl
 
     for (int item = blockIdx.x; item < n_items; item += gridDim.x, rho += stride) {
         const bool valid = ALWAYS_VALID || rho < n_rows;
-        const unsigned p = cm.p0 + cur.lp, f = cm.f0 + cur.lf, y = cur.y;
-        const unsigned wrow_i = ((p * (unsigned)cm.F + f) << ny_shift) + y;
+        const unsigned cur_lp = cur.lp, cur_lf = cur.lf;
+        const unsigned p = cm.p0 + cur_lp, f = cm.f0 + cur_lf, y = cur.y;
+        const unsigned wrow_i = ((((unsigned)cm.wp0 + cur_lp) * (unsigned)cm.wF + (unsigned)cm.wf0 + cur_lf) << ny_shift) + y;
         const unsigned vrow_i = ((f * (unsigned)n_slices + (unsigned)slice) << ny_shift) + y;
         cur.advance(dy, dlp, dlf, ny_shift, np);
         if (NX >= 512 && rho + stride < n_rows) {
             const unsigned pn = cm.p0 + cur.lp, fn = cm.f0 + cur.lf;
-            const unsigned wn_i = ((pn * (unsigned)cm.F + fn) << ny_shift) + cur.y;
+            const unsigned wn_i = ((((unsigned)cm.wp0 + cur.lp) * (unsigned)cm.wF + (unsigned)cm.wf0 + cur.lf) << ny_shift) + cur.y;
             const unsigned vn_i = ((fn * (unsigned)n_slices + (unsigned)slice) << ny_shift) + cur.y;
             if (2 * t < T) tma::prefetch_l2(V + (size_t)vn_i * NX + 32 * t);
             if (!FIRST && pf_wave) tma::prefetch_l2(W + (size_t)wn_i * NX + 16 * t);
@@ -220,13 +225,14 @@ k_row_transmit32(float2* __restrict__ W, const float* __restrict__ V, const Chun
     const bool pf1 = (16 * (t + T) < col_lo) || (16 * (t + T) + 16 > col_hi);
 
     for (int item = blockIdx.x; item < n_items; item += gridDim.x, rho += stride) {
-        const unsigned p = cm.p0 + cur.lp, f = cm.f0 + cur.lf, y = cur.y;
-        const unsigned wrow_i = ((p * (unsigned)cm.F + f) << ny_shift) + y;
+        const unsigned cur_lp = cur.lp, cur_lf = cur.lf;
+        const unsigned p = cm.p0 + cur_lp, f = cm.f0 + cur_lf, y = cur.y;
+        const unsigned wrow_i = ((((unsigned)cm.wp0 + cur_lp) * (unsigned)cm.wF + (unsigned)cm.wf0 + cur_lf) << ny_shift) + y;
         const unsigned vrow_i = ((f * (unsigned)n_slices + (unsigned)slice) << ny_shift) + y;
         cur.advance(dy, dlp, dlf, ny_shift, np);
         if (rho + stride < n_rows) {
             const unsigned pn = cm.p0 + cur.lp, fn = cm.f0 + cur.lf;
-            const unsigned wn_i = ((pn * (unsigned)cm.F + fn) << ny_shift) + cur.y;
+            const unsigned wn_i = ((((unsigned)cm.wp0 + cur.lp) * (unsigned)cm.wF + (unsigned)cm.wf0 + cur.lf) << ny_shift) + cur.y;
             const unsigned vn_i = ((fn * (unsigned)n_slices + (unsigned)slice) << ny_shift) + cur.y;
             tma::prefetch_l2(V + (size_t)vn_i * NX + 32 * t);
             if (pf0) tma::prefetch_l2(W + (size_t)wn_i * NX + 16 * t);
@@ -270,9 +276,11 @@ template <int NY> struct ColCfg {
     static constexpr size_t SMEM = (size_t)NS * STAGE_BYTES + (size_t)NY * sizeof(float2) + NS * sizeof(uint64_t) + 128;
 };
 
-template <int NY, bool LAST>
+// TILED (last pass only): the k-space exit wave goes to the time-tiled layout [P][ny][active tile][F][8 kx] through a
+// second, 5-D tensor map instead of back into the array it was propagated in.
+template <int NY, bool LAST, bool TILED>
 __global__ void __launch_bounds__(ColCfg<NY>::THREADS, ColCfg<NY>::MIN_BLOCKS)
-k_col_propagate(const __grid_constant__ CUtensorMap wmap, const int tiles_lo, const int tile_gap, const int n_tiles,
+k_col_propagate(const __grid_constant__ CUtensorMap wmap, const __grid_constant__ CUtensorMap tmap, const int tiles_lo, const int tile_gap, const int n_tiles,
                 const int32_t* __restrict__ nmax, const float2* __restrict__ px, const float2* __restrict__ py,
                 const ChunkMap cm, const int n_items) {
     using Cfg = ColCfg<NY>;
@@ -288,8 +296,7 @@ k_col_propagate(const __grid_constant__ CUtensorMap wmap, const int tiles_lo, co
         const int l = item / per_wave, rem = item % per_wave;
         const int tj = rem / SUB;                             // active tiles: [0, tiles_lo) and [tiles_lo + gap, ..)
         const int kx0 = (tj < tiles_lo ? tj : tj + tile_gap) * kColTile + (rem % SUB) * C;
-        const int p = cm.p0 + l % cm.np, f = cm.f0 + l / cm.np;
-        const int row0 = (p * cm.F + f) * NY;
+        const int row0 = ((cm.wp0 + l % cm.np) * cm.wF + cm.wf0 + l / cm.np) * NY;
         tma::mbar_arrive_expect_tx(&full[s], Cfg::STAGE_BYTES);
 #pragma unroll
         for (int b = 0; b < Cfg::NBOX; ++b)
@@ -350,11 +357,18 @@ k_col_propagate(const __grid_constant__ CUtensorMap wmap, const int tiles_lo, co
         __syncthreads();
         if (threadIdx.x == 0) {
             const int l = item / per_wave;
-            const int p = cm.p0 + l % cm.np, f = cm.f0 + l / cm.np;
-            const int row0 = (p * cm.F + f) * NY;
+            if (TILED) {
+                const int p = cm.p0 + l % cm.np, f = cm.f0 + l / cm.np;
 #pragma unroll
-            for (int b = 0; b < Cfg::NBOX; ++b)
-                tma::tensor_store_2d(&wmap, 2 * kx0, row0 + b * Cfg::BOX_R, st + (size_t)b * Cfg::BOX_R * C);
+                for (int b = 0; b < Cfg::NBOX; ++b)
+                    tma::tensor_store_5d(&tmap, 2 * (rem % SUB) * C, f, rem / SUB, b * Cfg::BOX_R, p,
+                                         st + (size_t)b * Cfg::BOX_R * C);
+            } else {
+                const int row0 = ((cm.wp0 + l % cm.np) * cm.wF + cm.wf0 + l / cm.np) * NY;
+#pragma unroll
+                for (int b = 0; b < Cfg::NBOX; ++b)
+                    tma::tensor_store_2d(&wmap, 2 * kx0, row0 + b * Cfg::BOX_R, st + (size_t)b * Cfg::BOX_R * C);
+            }
             tma::bulk_commit();
         }
         rem += rem_step;
@@ -388,9 +402,9 @@ template <int NY> struct ColCfg32 {
     static constexpr size_t SMEM = (size_t)NS * STAGE_BYTES + (size_t)NY * sizeof(float2) + NS * sizeof(uint64_t) + 128;
 };
 
-template <int NY, bool LAST>
+template <int NY, bool LAST, bool TILED>
 __global__ void __launch_bounds__(ColCfg32<NY>::THREADS, ColCfg32<NY>::MIN_BLOCKS)
-k_col_propagate32(const __grid_constant__ CUtensorMap wmap, const int tiles_lo, const int tile_gap, const int n_tiles,
+k_col_propagate32(const __grid_constant__ CUtensorMap wmap, const __grid_constant__ CUtensorMap tmap, const int tiles_lo, const int tile_gap, const int n_tiles,
                   const int32_t* __restrict__ nmax, const float2* __restrict__ px, const float2* __restrict__ py,
                   const ChunkMap cm, const int n_items) {
     using Cfg = ColCfg32<NY>;
@@ -407,8 +421,7 @@ k_col_propagate32(const __grid_constant__ CUtensorMap wmap, const int tiles_lo, 
         const int l = item / per_wave, rem = item % per_wave;
         const int tj = rem / SUB;
         const int kx0 = (tj < tiles_lo ? tj : tj + tile_gap) * kColTile + (rem % SUB) * C;
-        const int p = cm.p0 + l % cm.np, f = cm.f0 + l / cm.np;
-        const int row0 = (p * cm.F + f) * NY;
+        const int row0 = ((cm.wp0 + l % cm.np) * cm.wF + cm.wf0 + l / cm.np) * NY;
         tma::mbar_arrive_expect_tx(&full[s], Cfg::STAGE_BYTES);
 #pragma unroll
         for (int b = 0; b < Cfg::NBOX; ++b)
@@ -496,11 +509,18 @@ k_col_propagate32(const __grid_constant__ CUtensorMap wmap, const int tiles_lo, 
         __syncthreads();
         if (threadIdx.x == 0) {
             const int l = item / per_wave;
-            const int p = cm.p0 + l % cm.np, f = cm.f0 + l / cm.np;
-            const int row0 = (p * cm.F + f) * NY;
+            if (TILED) {
+                const int p = cm.p0 + l % cm.np, f = cm.f0 + l / cm.np;
 #pragma unroll
-            for (int b = 0; b < Cfg::NBOX; ++b)
-                tma::tensor_store_2d(&wmap, 2 * kx0, row0 + b * Cfg::BOX_R, st + (size_t)b * Cfg::BOX_R * C);
+                for (int b = 0; b < Cfg::NBOX; ++b)
+                    tma::tensor_store_5d(&tmap, 2 * (rem % SUB) * C, f, rem / SUB, b * Cfg::BOX_R, p,
+                                         st + (size_t)b * Cfg::BOX_R * C);
+            } else {
+                const int row0 = ((cm.wp0 + l % cm.np) * cm.wF + cm.wf0 + l / cm.np) * NY;
+#pragma unroll
+                for (int b = 0; b < Cfg::NBOX; ++b)
+                    tma::tensor_store_2d(&wmap, 2 * kx0, row0 + b * Cfg::BOX_R, st + (size_t)b * Cfg::BOX_R * C);
+            }
             tma::bulk_commit();
         }
         rem += rem_step;
@@ -518,8 +538,8 @@ __global__ void k_zero_cols(float2* __restrict__ W, const int nx, const int ny, 
         const int x = (int)(i % width);
         const long long row = i / width;
         const int y = (int)(row % ny), l = (int)(row / ny);
-        const int p = cm.p0 + l % cm.np, f = cm.f0 + l / cm.np;
-        W[(((size_t)p * cm.F + f) * ny + y) * nx + col_lo + x] = make_float2(0.f, 0.f);
+        const int p = cm.wp0 + l % cm.np, f = cm.wf0 + l / cm.np;
+        W[(((size_t)p * cm.wF + f) * ny + y) * nx + col_lo + x] = make_float2(0.f, 0.f);
     }
 }
 
@@ -572,32 +592,34 @@ static bool use_row32(const ps_ctx* c, int col_lo, int col_hi) {
     return col_lo >= 10 * T && col_lo <= 12 * T && col_hi >= 20 * T && col_hi <= 22 * T;
 }
 
-template <int NY, bool LAST>
-static cudaError_t launch_col(ps_ctx* c, const CUtensorMap& wmap, const ChunkMap& cm, int zero_lo, int zero_hi) {
+template <int NY, bool LAST, bool TILED = false>
+static cudaError_t launch_col(ps_ctx* c, const CUtensorMap& wmap, const CUtensorMap& tmap, const ChunkMap& cm, int zero_lo,
+                              int zero_hi) {
     using Cfg = ColCfg<NY>;
-    auto kern = k_col_propagate<NY, LAST>;
+    auto kern = k_col_propagate<NY, LAST, TILED>;
     int per_sm_grid = 0;
     cudaError_t ce = kernel_cap(c, kern, Cfg::THREADS, Cfg::SMEM, &per_sm_grid);
     if (ce != cudaSuccess) return ce;
     const int n_tiles = c->n_tiles_active;
     const int n_items = cm.np * cm.nf * n_tiles * (kColTile / Cfg::C);
     const int grid = n_items < per_sm_grid ? n_items : per_sm_grid;
-    kern<<<grid, Cfg::THREADS, Cfg::SMEM, c->stream>>>(wmap, zero_lo / kColTile, (zero_hi - zero_lo) / kColTile, n_tiles, c->d_nmax,
+    kern<<<grid, Cfg::THREADS, Cfg::SMEM, c->stream>>>(wmap, tmap, zero_lo / kColTile, (zero_hi - zero_lo) / kColTile, n_tiles, c->d_nmax,
                                                       LAST ? c->kv.d_px_last : c->kv.d_px_mid, c->kv.d_py, cm, n_items);
     return cudaGetLastError();
 }
 
-template <int NY, bool LAST>
-static cudaError_t launch_col32(ps_ctx* c, const CUtensorMap& wmap, const ChunkMap& cm, int zero_lo, int zero_hi) {
+template <int NY, bool LAST, bool TILED = false>
+static cudaError_t launch_col32(ps_ctx* c, const CUtensorMap& wmap, const CUtensorMap& tmap, const ChunkMap& cm, int zero_lo,
+                                int zero_hi) {
     using Cfg = ColCfg32<NY>;
-    auto kern = k_col_propagate32<NY, LAST>;
+    auto kern = k_col_propagate32<NY, LAST, TILED>;
     int per_sm_grid = 0;
     cudaError_t ce = kernel_cap(c, kern, Cfg::THREADS, Cfg::SMEM, &per_sm_grid);
     if (ce != cudaSuccess) return ce;
     const int n_tiles = c->n_tiles_active;
     const int n_items = cm.np * cm.nf * n_tiles * (kColTile / Cfg::C);
     const int grid = n_items < per_sm_grid ? n_items : per_sm_grid;
-    kern<<<grid, Cfg::THREADS, Cfg::SMEM, c->stream>>>(wmap, zero_lo / kColTile, (zero_hi - zero_lo) / kColTile, n_tiles, c->d_nmax,
+    kern<<<grid, Cfg::THREADS, Cfg::SMEM, c->stream>>>(wmap, tmap, zero_lo / kColTile, (zero_hi - zero_lo) / kColTile, n_tiles, c->d_nmax,
                                                       LAST ? c->kv.d_px_last : c->kv.d_px_mid, c->kv.d_py, cm, n_items);
     return cudaGetLastError();
 }
@@ -626,11 +648,80 @@ static bool make_wave_map(CUtensorMap* map, void* W, int nx, long long rows, boo
         default: break;                                                            \
     }
 
-}  // namespace psb
+static constexpr long long kResidentMaxWaves = 2 * kNumSM;   // auto rule of the chip-resident path
 
+// scratch for the chunk-local work array of the tiled exit layout: the installed workspace, else the library-owned
+// buffer under the same budget rule as ps_build_slices (an eighth of the free device memory, 768 MB ... 16 GB, decided
+// once per context); returns the number of waves it holds
+static ps_status tiled_work_buffer(ps_ctx* c, long long n_waves_wanted, float2** W, long long* n_waves) {
+    const size_t per_wave = (size_t)c->nx * c->ny * sizeof(float2);
+    if (c->user_ws) {
+        *n_waves = (long long)(c->user_ws_bytes / per_wave);
+        if (*n_waves < 1) return fail(c, PS_EWORKSPACE, "ps_multislice: workspace smaller than one wave (tiled exit layout)");
+        *W = (float2*)c->user_ws;
+    } else {
+        if (c->scratch_budget == 0) {
+            size_t free_b = 0, total_b = 0;
+            c->scratch_budget = (size_t)768 << 20;
+            if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess) {
+                size_t want = (free_b + c->scratch.bytes) / 8;
+                if (want > ((size_t)16 << 30)) want = (size_t)16 << 30;
+                if (want > c->scratch_budget) c->scratch_budget = want;
+            }
+        }
+        size_t avail = c->scratch_budget > c->scratch.bytes ? c->scratch_budget : c->scratch.bytes;
+        long long nw = (long long)(avail / per_wave);
+        if (nw < 1) nw = 1;
+        if (nw > n_waves_wanted) nw = n_waves_wanted;
+        ps_status st = ensure_buf(c, c->scratch, (size_t)nw * per_wave);
+        if (st != PS_OK) return st;
+        *n_waves = nw;
+        *W = (float2*)c->scratch.p;
+    }
+    if (*n_waves > n_waves_wanted) *n_waves = n_waves_wanted;
+    return PS_OK;
+}
+
+// tiled exit layout -> dense [P][F][ny][nx] (zeros outside the stored tiles): for consumers that take the dense
+// layout only, and for parity tests.  One thread per complex value of the dense array.
+__global__ void k_exit_to_dense(const float2* __restrict__ Tl, float2* __restrict__ D, const int32_t* __restrict__ tile_slot,
+                                const int nx, const int ny, const int n_tiles, const int F, const long long total) {
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x) {
+        const int x = (int)(i % nx);
+        long long r = i / nx;
+        const int y = (int)(r % ny); r /= ny;
+        const int f = (int)(r % F);
+        const long long p = r / F;
+        const int tj = tile_slot[x / kColTile];
+        D[i] = tj < 0 ? make_float2(0.f, 0.f)
+                      : Tl[((((size_t)p * ny + y) * n_tiles + tj) * F + f) * kColTile + (x % kColTile)];
+    }
+}
+
+}  // namespace psb
 using namespace psb;
 
-static constexpr long long kResidentMaxWaves = 2 * kNumSM;   // auto rule of the chip-resident path
+extern "C" size_t ps_exit_bytes(const ps_ctx* c, int n_probes, int n_frames, int exit_layout) {
+    if (!c || !c->have_geom || n_probes < 1 || n_frames < 1) return 0;
+    if (exit_layout == PS_LAYOUT_DENSE) return (size_t)n_probes * n_frames * c->nx * c->ny * sizeof(float2);
+    if (exit_layout == PS_LAYOUT_TILED_APERTURE)
+        return (size_t)n_probes * c->ny * c->n_tiles_active * n_frames * kColTile * sizeof(float2);
+    return 0;
+}
+
+extern "C" ps_status ps_exit_to_dense(ps_ctx* c, const void* d_tiled, int n_probes, int n_frames, void* d_dense) {
+    if (!c) return PS_EINVAL;
+    if (!c->have_geom) return fail(c, PS_ESTATE, "ps_exit_to_dense: ps_set_geometry has not been called");
+    if (!d_tiled || !d_dense || n_probes < 1 || n_frames < 1) return fail(c, PS_EINVAL, "ps_exit_to_dense: null pointer or non-positive size");
+    ps_status st = enter(c, "ps_exit_to_dense");
+    if (st != PS_OK) return st;
+    const long long total = (long long)n_probes * n_frames * c->nx * c->ny;
+    const long long nb = (total + 255) / 256;
+    k_exit_to_dense<<<(unsigned)(nb < 148 * 64 ? nb : 148 * 64), 256, 0, c->stream>>>(
+        (const float2*)d_tiled, (float2*)d_dense, c->d_tile_slot, c->nx, c->ny, c->n_tiles_active, n_frames, total);
+    PSB_LAUNCH_CHECK(c, "k_exit_to_dense");
+    return PS_OK;
+}
 
 extern "C" ps_status ps_multislice(ps_ctx* c, double kV, const void* d_psi0, int n_probes, const float* d_V,
                                    int n_frames, void* d_exit, int exit_layout) {
@@ -638,16 +729,31 @@ extern "C" ps_status ps_multislice(ps_ctx* c, double kV, const void* d_psi0, int
     if (!c->have_geom) return fail(c, PS_ESTATE, "ps_multislice: ps_set_geometry has not been called");
     if (!d_psi0 || !d_V || !d_exit || n_probes < 1 || n_frames < 1 || !(kV > 0.0))
         return fail(c, PS_EINVAL, "ps_multislice: null pointer or non-positive size / voltage");
-    if (exit_layout != PS_LAYOUT_DENSE) return fail(c, PS_EUNSUPPORTED, "ps_multislice: unknown exit layout");
+    if (exit_layout != PS_LAYOUT_DENSE && exit_layout != PS_LAYOUT_TILED_APERTURE)
+        return fail(c, PS_EUNSUPPORTED, "ps_multislice: unknown exit layout");
+    const bool tiled = exit_layout == PS_LAYOUT_TILED_APERTURE;
     ps_status st = enter(c, "ps_multislice");
     if (st != PS_OK) return st;
     if ((st = ensure_kv(c, kV)) != PS_OK) return st;
 
+    const long long wave_rows = (long long)n_probes * n_frames * c->ny;
+    if (wave_rows > 0x7fffffffLL) return fail(c, PS_EUNSUPPORTED, "ps_multislice: n_probes*n_frames*ny exceeds 2^31");
+    if ((long long)n_frames * c->n_slices * c->ny > 0x7fffffffLL)
+        return fail(c, PS_EUNSUPPORTED, "ps_multislice: n_frames*n_slices*ny exceeds 2^31 (propagate the frames in chunks)");
+
     // Waves per launch.  Measured on B200 (c2, 256^2, 512 waves; profiles/r1_chunk_sweep.md): streaming the whole
     // batch from HBM in one launch per pass beats L2-resident chunks of 40-80 MB, whose launches are too short
-    // to amortise launch latency, twiddle set-up and the last partial wave of blocks.  Default: no chunking.
+    // to amortise launch latency, twiddle set-up and the last partial wave of blocks.  Default: no chunking in the
+    // dense layout (the wave is propagated inside the caller's array); the tiled layout propagates chunk by chunk in a
+    // work array that lives in scratch, as many waves at a time as it holds.
+    float2* W = (float2*)d_exit;
     long long chunk = c->wave_chunk;
     if (chunk <= 0) chunk = (long long)n_probes * n_frames;
+    if (tiled) {
+        long long held = 0;
+        if ((st = tiled_work_buffer(c, chunk, &W, &held)) != PS_OK) return st;
+        if (held < chunk) chunk = held;
+    }
     const int np = (int)(n_probes < chunk ? n_probes : chunk);
     int nf = (int)(chunk / np);
     if (nf < 1) nf = 1;
@@ -655,21 +761,30 @@ extern "C" ps_status ps_multislice(ps_ctx* c, double kV, const void* d_psi0, int
         const int n_chunks = (n_frames + nf - 1) / nf;
         nf = (n_frames + n_chunks - 1) / n_chunks;
     }
-    float2* W = (float2*)d_exit;
     const float2* psi0 = (const float2*)d_psi0;
     const float sigma = (float)c->kv.sigma;
     const int S = c->n_slices;
 
-    // TMA view of the wave array: float32 [P*F*ny][2 nx]; box = C columns x up to 256 rows
-    const long long wave_rows = (long long)n_probes * n_frames * c->ny;
-    if (wave_rows > 0x7fffffffLL) return fail(c, PS_EUNSUPPORTED, "ps_multislice: n_probes*n_frames*ny exceeds 2^31");
-    if ((long long)n_frames * c->n_slices * c->ny > 0x7fffffffLL)
-        return fail(c, PS_EUNSUPPORTED, "ps_multislice: n_frames*n_slices*ny exceeds 2^31 (propagate the frames in chunks)");
-    CUtensorMap wmap;
+    // TMA view of the array the wave is propagated in: float32 [waves*ny][2 nx]; box = C columns x up to 256 rows
+    CUtensorMap wmap, tmap;
+    memset(&tmap, 0, sizeof(tmap));
     bool map_ok = false;
     const bool col32 = use_col32(c);
-    PSB_DISPATCH_N(c->ny, (map_ok = make_wave_map<N_>(&wmap, d_exit, c->nx, wave_rows, col32)));
+    const long long w_rows = tiled ? (long long)np * nf * c->ny : wave_rows;
+    PSB_DISPATCH_N(c->ny, (map_ok = make_wave_map<N_>(&wmap, W, c->nx, w_rows, col32)));
     if (!map_ok) return fail(c, PS_ECUDA, "ps_multislice: cuTensorMapEncodeTiled failed (exit-wave array must be 16-byte aligned)");
+    if (tiled) {
+        // [P][ny][active tile][F][8 kx] as float32, innermost first: (16, F, n_tiles, ny, P); box = one column (sub)tile x
+        // up to 256 rows of one frame
+        const int Cc = (c->ny == 2048) ? 4 : 8;              // columns per block of the column pass (ColCfg / ColCfg32)
+        const uint64_t dims[5] = {2ull * kColTile, (uint64_t)n_frames, (uint64_t)c->n_tiles_active, (uint64_t)c->ny, (uint64_t)n_probes};
+        const uint64_t row_b = 2ull * kColTile * sizeof(float);
+        const uint64_t strides[4] = {row_b, row_b * n_frames, row_b * n_frames * c->n_tiles_active,
+                                     row_b * n_frames * c->n_tiles_active * c->ny};
+        const uint32_t box[5] = {2u * Cc, 1u, 1u, (uint32_t)(c->ny < 256 ? c->ny : 256), 1u};
+        if (!tma::make_map_5d_f32(&tmap, d_exit, dims, strides, box))
+            return fail(c, PS_ECUDA, "ps_multislice: cuTensorMapEncodeTiled failed for the tiled exit layout (array must be 16-byte aligned)");
+    }
     // contiguous range of columns outside the band limit (zero in the k-space exit wave)
     int zero_lo = 0, zero_hi = 0;
     {
@@ -685,7 +800,7 @@ extern "C" ps_status ps_multislice(ps_ctx* c, double kV, const void* d_psi0, int
 
     // Small square grids, small batches: the whole slice loop in one launch with the wave resident in shared memory
     // (resident.cu).  Batches that fill the GPU stay on the streaming passes (measured cross-over: profiles/r2_resident.md).
-    if (resident_supported(c) && !c->vacuum_shortcut && c->wave_chunk == 0 &&
+    if (!tiled && resident_supported(c) && !c->vacuum_shortcut && c->wave_chunk == 0 &&
         (c->tune_resident == 1 || (c->tune_resident == 0 && (long long)n_probes * n_frames <= kResidentMaxWaves))) {
         cudaError_t e = launch_slice_resident(c, W, psi0, d_V, n_probes, n_frames, sigma, zero_lo, zero_hi);
         if (e != cudaSuccess) return fail(c, PS_ECUDA, std::string("k_slice_resident: ") + cudaGetErrorString(e));
@@ -700,6 +815,8 @@ extern "C" ps_status ps_multislice(ps_ctx* c, double kV, const void* d_psi0, int
             cm.p0 = p0; cm.np = (n_probes - p0 < np) ? n_probes - p0 : np;
             cm.f0 = f0; cm.nf = (n_frames - f0 < nf) ? n_frames - f0 : nf;
             cm.F = n_frames;
+            if (tiled) { cm.wp0 = 0; cm.wf0 = 0; cm.wF = cm.nf; }
+            else       { cm.wp0 = cm.p0; cm.wf0 = cm.f0; cm.wF = n_frames; }
             for (int s = 0; s < S; ++s) {
                 cudaError_t e = cudaErrorInvalidValue;
                 {
@@ -714,20 +831,24 @@ extern "C" ps_status ps_multislice(ps_ctx* c, double kV, const void* d_psi0, int
                 e = cudaErrorInvalidValue;
                 {
                 ProfScope ps_(c, K_COL_PROPAGATE);
-                if (s == S - 1) {
+                if (s == S - 1 && tiled) {
+                    if (col32 && c->ny == 512) e = launch_col32<512, true, true>(c, wmap, tmap, cm, zero_lo, zero_hi);
+                    else if (col32 && c->ny == 1024) e = launch_col32<1024, true, true>(c, wmap, tmap, cm, zero_lo, zero_hi);
+                    else { PSB_DISPATCH_N(c->ny, (e = launch_col<N_, true, true>(c, wmap, tmap, cm, zero_lo, zero_hi))); }
+                } else if (s == S - 1) {
                     if (zero_hi > zero_lo) {
                         const long long tot = (long long)cm.np * cm.nf * c->ny * (zero_hi - zero_lo);
                         const int zb = (int)((tot + 255) / 256 < 148 * 16 ? (tot + 255) / 256 : 148 * 16);
                         k_zero_cols<<<zb, 256, 0, c->stream>>>(W, c->nx, c->ny, zero_lo, zero_hi, cm);
                         c->launches++;
                     }
-                    if (col32 && c->ny == 512) e = launch_col32<512, true>(c, wmap, cm, zero_lo, zero_hi);
-                    else if (col32 && c->ny == 1024) e = launch_col32<1024, true>(c, wmap, cm, zero_lo, zero_hi);
-                    else { PSB_DISPATCH_N(c->ny, (e = launch_col<N_, true>(c, wmap, cm, zero_lo, zero_hi))); }
+                    if (col32 && c->ny == 512) e = launch_col32<512, true>(c, wmap, tmap, cm, zero_lo, zero_hi);
+                    else if (col32 && c->ny == 1024) e = launch_col32<1024, true>(c, wmap, tmap, cm, zero_lo, zero_hi);
+                    else { PSB_DISPATCH_N(c->ny, (e = launch_col<N_, true>(c, wmap, tmap, cm, zero_lo, zero_hi))); }
                 } else {
-                    if (col32 && c->ny == 512) e = launch_col32<512, false>(c, wmap, cm, zero_lo, zero_hi);
-                    else if (col32 && c->ny == 1024) e = launch_col32<1024, false>(c, wmap, cm, zero_lo, zero_hi);
-                    else { PSB_DISPATCH_N(c->ny, (e = launch_col<N_, false>(c, wmap, cm, zero_lo, zero_hi))); }
+                    if (col32 && c->ny == 512) e = launch_col32<512, false>(c, wmap, tmap, cm, zero_lo, zero_hi);
+                    else if (col32 && c->ny == 1024) e = launch_col32<1024, false>(c, wmap, tmap, cm, zero_lo, zero_hi);
+                    else { PSB_DISPATCH_N(c->ny, (e = launch_col<N_, false>(c, wmap, tmap, cm, zero_lo, zero_hi))); }
                 }
                 }
                 if (e != cudaSuccess) return fail(c, PS_ECUDA, std::string("k_col_propagate: ") + cudaGetErrorString(e));

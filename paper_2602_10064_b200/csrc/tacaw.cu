@@ -14,19 +14,31 @@
 
 namespace psb {
 
-template <int NF> struct TacawCfg {
+#ifndef PSB_TACAW_TILED_RING
+#define PSB_TACAW_TILED_RING 1
+#endif
+#ifndef PSB_TACAW_C512
+#define PSB_TACAW_C512 16
+#endif
+#ifndef PSB_TACAW_C1024
+#define PSB_TACAW_C1024 8
+#endif
+// TILED: the exit waves come in PS_LAYOUT_TILED_APERTURE, [P][ny][tile][F][8 kx]: a pixel group must lie inside one
+// 8-column tile (C <= 8), and its F frames are one contiguous run of F * 64 bytes.
+template <int NF, bool TILED = false> struct TacawCfg {
     static constexpr int T = Plan<NF>::T;
-    static constexpr int C = (NF <= 512) ? 16 : ((NF == 1024) ? 8 : 4);
+    static constexpr int C0 = (NF < 512) ? 16 : (NF == 512) ? PSB_TACAW_C512 : ((NF == 1024) ? PSB_TACAW_C1024 : 4);
+    static constexpr int C = (TILED && C0 > kColTile) ? kColTile : C0;
     static constexpr int THREADS = C * T;
     static constexpr size_t SMEM = (size_t)NF * C * sizeof(float2);
 };
 
-template <int NF>
-__global__ void __launch_bounds__(TacawCfg<NF>::THREADS)
+template <int NF, bool TILED>
+__global__ void __launch_bounds__(TacawCfg<NF, TILED>::THREADS)
 k_tacaw_fft(const float2* __restrict__ exitw, float* __restrict__ I, const int32_t* __restrict__ slot_of_bin,
             const int n_out, const int nx, const int ny, const int32_t* __restrict__ nmax, const int n_items,
-            const int prefetch) {
-    using Cfg = TacawCfg<NF>;
+            const int prefetch, const int32_t* __restrict__ tile_slot, const int n_tiles) {
+    using Cfg = TacawCfg<NF, TILED>;
     constexpr int T = Cfg::T, C = Cfg::C;
     extern __shared__ float2 smem[];
     const int c = threadIdx.x % C, t = threadIdx.x / C;
@@ -53,7 +65,7 @@ k_tacaw_fft(const float2* __restrict__ exitw, float* __restrict__ I, const int32
             // beyond (an item then touches more 2 MB pages than the TLB holds, and the prefetch doubles the misses):
             // the host switches it per shape.
             const int nxt = item + gridDim.x;
-            if (prefetch && nxt < n_items) {
+            if (!TILED && prefetch && nxt < n_items) {
                 const int pn = nxt >> gpp_shift, gn = nxt & (groups_per_probe - 1);
                 const int iyn = gn >> gpr_shift, ixn = (gn & (groups_per_row - 1)) * C;
                 const int ayn = iyn < ny / 2 ? iyn : ny - iyn;
@@ -71,19 +83,23 @@ k_tacaw_fft(const float2* __restrict__ exitw, float* __restrict__ I, const int32
                 if (slot[e] >= 0) out[(size_t)slot[e] * npix] = 0.f;
             continue;
         }
-        const float2* src = exitw + (size_t)p * NF * npix + pix;
+        // frame j of this thread's pixel: dense [P][F][ny][nx], or tiled [P][ny][tile][F][8]
+        const float2* src = TILED ? exitw + ((((size_t)p * ny + iy) * n_tiles + tile_slot[ix0 / kColTile]) * NF) * kColTile +
+                                        (ix0 % kColTile) + c
+                                  : exitw + (size_t)p * NF * npix + pix;
+        const size_t fstride = TILED ? (size_t)kColTile : npix;
         const float2 ref = __ldg(src);                       // frame 0 (A14: mean removal, see header)
         float2 v[16];
 #pragma unroll
         for (int e = 0; e < 16; ++e) {
-            const float2 x = src[(size_t)(t + e * T) * npix];
+            const float2 x = src[(size_t)(t + e * T) * fstride];
             v[e] = make_float2(x.x - ref.x, x.y - ref.y);
         }
         fft_forward<NF, ColSlots<C>, BlockSync>(v, t, tw, slots);
 #pragma unroll
         for (int e = 0; e < 16; ++e) {
             if (slot[e] >= 0) {
-                const bool dc = (t + e * T) == 0;
+                const bool dc = (t + e * T) == 0 || !mine;   // out-of-band pixels of a group that straddles the edge
                 out[(size_t)slot[e] * npix] = dc ? 0.f : fmaf(v[e].x, v[e].x, v[e].y * v[e].y);
             }
         }
@@ -97,9 +113,10 @@ k_tacaw_fft(const float2* __restrict__ exitw, float* __restrict__ I, const int32
 // keeps the loads of the next items in flight while the current one is transformed, so one 512-thread block per SM
 // streams from HBM without exposing the load latency.  Only groups with at least one in-band pixel are visited (list
 // built once per geometry); the other pixels of I are zero-filled by k_tacaw_zero.
-template <int NF> struct TacawTmaCfg {
+template <int NF, bool TILED = false> struct TacawTmaCfg {
     static constexpr int T = Plan<NF>::T;
-    static constexpr int C = (NF <= 512) ? 16 : ((NF == 1024) ? 8 : 4);
+    static constexpr int C0 = (NF <= 512) ? 16 : ((NF == 1024) ? 8 : 4);
+    static constexpr int C = (TILED && C0 > kColTile) ? kColTile : C0;
     static constexpr int THREADS = C * T;
     static constexpr int NS = 3;
     static constexpr int BOX_R = (NF < 256) ? NF : 256;
@@ -109,12 +126,15 @@ template <int NF> struct TacawTmaCfg {
     static constexpr int MIN_BLOCKS = (THREADS <= 256) ? 2 : 1;
 };
 
-template <int NF>
-__global__ void __launch_bounds__(TacawTmaCfg<NF>::THREADS, TacawTmaCfg<NF>::MIN_BLOCKS)
+// TILED: emap views the tiled array as float32 [P*ny*n_tiles*F rows][16]; the F frames of a (row, tile) are consecutive
+// rows, so an item is NBOX boxes of up to 256 consecutive 64-byte rows: contiguous runs for the copy engine.
+template <int NF, bool TILED>
+__global__ void __launch_bounds__(TacawTmaCfg<NF, TILED>::THREADS, TacawTmaCfg<NF, TILED>::MIN_BLOCKS)
 k_tacaw_tma(const __grid_constant__ CUtensorMap emap, float* __restrict__ I, const int32_t* __restrict__ slot_of_bin,
             const int n_out, const int nx, const int ny, const int32_t* __restrict__ nmax,
-            const int32_t* __restrict__ groups, const int n_groups, const int n_items) {
-    using Cfg = TacawTmaCfg<NF>;
+            const int32_t* __restrict__ groups, const int n_groups, const int n_items,
+            const int32_t* __restrict__ tile_slot, const int n_tiles) {
+    using Cfg = TacawTmaCfg<NF, TILED>;
     constexpr int T = Cfg::T, C = Cfg::C, NS = Cfg::NS, PF = NS - 1;
     extern __shared__ __align__(1024) float2 smem_t[];
     float2* stage0 = smem_t;
@@ -124,7 +144,13 @@ k_tacaw_tma(const __grid_constant__ CUtensorMap emap, float* __restrict__ I, con
 
     auto issue_load = [&](const int item, const int s) {
         const int p = item / n_groups;
-        const int c0 = 2 * groups[item % n_groups], c1 = p * NF;
+        int c0 = 2 * groups[item % n_groups], c1 = p * NF;
+        if (TILED) {
+            const int pix0 = groups[item % n_groups];
+            const int gx = pix0 & (nx - 1), gy = pix0 / nx;
+            c0 = 2 * (gx % kColTile);
+            c1 = ((p * ny + gy) * n_tiles + tile_slot[gx / kColTile]) * NF;
+        }
         tma::mbar_arrive_expect_tx(&full[s], Cfg::STAGE_BYTES);
 #pragma unroll
         for (int b = 0; b < Cfg::NBOX; ++b)
@@ -310,10 +336,10 @@ __global__ void k_tacaw_finish(const float2* __restrict__ acc, float* __restrict
     I[i] = (bins[b] == 0) ? 0.f : fmaf(a.x, a.x, a.y * a.y);
 }
 
-template <int NF>
+template <int NF, bool TILED>
 static cudaError_t launch_tacaw(ps_ctx* c, const float2* exitw, float* I, const int32_t* slot, int n_out, int P) {
-    using Cfg = TacawCfg<NF>;
-    auto kern = k_tacaw_fft<NF>;
+    using Cfg = TacawCfg<NF, TILED>;
+    auto kern = k_tacaw_fft<NF, TILED>;
     int cap = 0;
     cudaError_t ce = kernel_cap(c, kern, Cfg::THREADS, Cfg::SMEM, &cap);
     if (ce != cudaSuccess) return ce;
@@ -321,7 +347,8 @@ static cudaError_t launch_tacaw(ps_ctx* c, const float2* exitw, float* I, const 
     if (n_items > 0x7fffffffLL) return cudaErrorInvalidValue;
     const int prefetch = (NF <= 512 && (long long)c->nx * c->ny <= 512LL * 512LL) ? 1 : 0;
     kern<<<(int)(n_items < cap ? n_items : cap), Cfg::THREADS, Cfg::SMEM, c->stream>>>(exitw, I, slot, n_out, c->nx, c->ny,
-                                                                                      c->d_nmax, (int)n_items, prefetch);
+                                                                                      c->d_nmax, (int)n_items, prefetch,
+                                                                                      c->d_tile_slot, c->n_tiles_active);
     return cudaGetLastError();
 }
 
@@ -346,19 +373,22 @@ static ps_status ensure_tacaw_groups(ps_ctx* c, int C) {
     return PS_OK;
 }
 
-template <int NF>
+template <int NF, bool TILED>
 static ps_status launch_tacaw_tma(ps_ctx* c, const float2* exitw, float* I, const int32_t* slot, int n_out, int P) {
-    using Cfg = TacawTmaCfg<NF>;
-    auto kern = k_tacaw_tma<NF>;
+    using Cfg = TacawTmaCfg<NF, TILED>;
+    auto kern = k_tacaw_tma<NF, TILED>;
     int cap = 0;
     PSB_CUDA(c, kernel_cap(c, kern, Cfg::THREADS, Cfg::SMEM, &cap));
     ps_status st = ensure_tacaw_groups(c, Cfg::C);
     if (st != PS_OK) return st;
     const size_t npix = (size_t)c->nx * c->ny;
-    if ((long long)P * NF > 0x7fffffffLL || 2 * npix > 0xffffffffULL)
+    const long long tiled_rows = (long long)P * c->ny * c->n_tiles_active * NF;
+    if ((long long)P * NF > 0x7fffffffLL || 2 * npix > 0xffffffffULL || (TILED && tiled_rows > 0x7fffffffLL))
         return fail(c, PS_EUNSUPPORTED, "ps_tacaw: exit-wave stack has more than 2^31 rows");
     CUtensorMap emap;
-    if (!tma::make_map_2d_f32(&emap, (void*)exitw, 2ull * npix, (uint64_t)P * NF, 2 * Cfg::C, Cfg::BOX_R))
+    const bool map_ok = TILED ? tma::make_map_2d_f32(&emap, (void*)exitw, 2ull * kColTile, (uint64_t)tiled_rows, 2 * Cfg::C, Cfg::BOX_R)
+                              : tma::make_map_2d_f32(&emap, (void*)exitw, 2ull * npix, (uint64_t)P * NF, 2 * Cfg::C, Cfg::BOX_R);
+    if (!map_ok)
         return fail(c, PS_ECUDA, "ps_tacaw: cuTensorMapEncodeTiled failed (exit-wave array must be 16-byte aligned)");
     const int32_t* groups = (const int32_t*)c->tacaw_groups.p;
     const long long n_items = (long long)P * c->tacaw_n_active;
@@ -372,7 +402,8 @@ static ps_status launch_tacaw_tma(ps_ctx* c, const float2* exitw, float* I, cons
     }
     if (n_items > 0) {
         kern<<<(int)(n_items < cap ? n_items : cap), Cfg::THREADS, Cfg::SMEM, c->stream>>>(
-            emap, I, slot, n_out, c->nx, c->ny, c->d_nmax, groups, c->tacaw_n_active, (int)n_items);
+            emap, I, slot, n_out, c->nx, c->ny, c->d_nmax, groups, c->tacaw_n_active, (int)n_items, c->d_tile_slot,
+            c->n_tiles_active);
         PSB_LAUNCH_CHECK(c, "k_tacaw_tma");
     }
     return PS_OK;
@@ -388,7 +419,9 @@ extern "C" ps_status ps_tacaw(ps_ctx* c, const void* d_exit, int exit_layout, in
     if (!c->have_geom) return fail(c, PS_ESTATE, "ps_tacaw: ps_set_geometry has not been called");
     if (!d_exit || !d_I || n_probes < 1 || n_frames < 1 || n_bins < 1 || !(dt_fs > 0.0))
         return fail(c, PS_EINVAL, "ps_tacaw: null pointer or non-positive size / dt");
-    if (exit_layout != PS_LAYOUT_DENSE) return fail(c, PS_EUNSUPPORTED, "ps_tacaw: unknown exit layout");
+    if (exit_layout != PS_LAYOUT_DENSE && exit_layout != PS_LAYOUT_TILED_APERTURE)
+        return fail(c, PS_EUNSUPPORTED, "ps_tacaw: unknown exit layout");
+    const bool tiled = exit_layout == PS_LAYOUT_TILED_APERTURE;
     if (!is_pow2(n_frames) || n_frames < 32 || n_frames > 4096)
         return fail(c, PS_EUNSUPPORTED, "ps_tacaw: n_frames must be a power of two in [32, 4096] (use ps_tacaw_begin/add/finish otherwise)");
     if (!bins && n_bins != n_frames) return fail(c, PS_EINVAL, "ps_tacaw: bins == NULL requires n_bins == n_frames");
@@ -415,35 +448,33 @@ extern "C" ps_status ps_tacaw(ps_ctx* c, const void* d_exit, int exit_layout, in
     // Kernel choice measured on B200 (profiles/r1_tacaw_kernels.md): the TMA-staged ring wins where one block per
     // SM is all that fits anyway (2048 frames) and where few bins are written (reads dominate, 512-1024 frames);
     // the register-staged kernel with several resident blocks wins for short stacks and when every bin is written.
-    const bool use_ring = n_frames == 2048 ||
-                          ((n_frames == 512 || n_frames == 1024) && 4 * n_bins <= n_frames);
-    if (!use_ring) {
-        cudaError_t e = cudaErrorInvalidValue;
-        switch (n_frames) {
-            case 32: e = launch_tacaw<32>(c, ex, d_I, d_slot, n_bins, n_probes); break;
-            case 64: e = launch_tacaw<64>(c, ex, d_I, d_slot, n_bins, n_probes); break;
-            case 128: e = launch_tacaw<128>(c, ex, d_I, d_slot, n_bins, n_probes); break;
-            case 256: e = launch_tacaw<256>(c, ex, d_I, d_slot, n_bins, n_probes); break;
-            case 512: e = launch_tacaw<512>(c, ex, d_I, d_slot, n_bins, n_probes); break;
-            case 1024: e = launch_tacaw<1024>(c, ex, d_I, d_slot, n_bins, n_probes); break;
-            case 4096: e = launch_tacaw<4096>(c, ex, d_I, d_slot, n_bins, n_probes); break;
-            default: break;
-        }
-        if (e != cudaSuccess) return fail(c, PS_ECUDA, std::string("k_tacaw_fft: ") + cudaGetErrorString(e));
-        c->launches++;
-        return PS_OK;
-    }
-    switch (n_frames) {                                       // TMA-staged ring up to 2048 frames (64 KB stages)
-        case 32: return launch_tacaw_tma<32>(c, ex, d_I, d_slot, n_bins, n_probes);
-        case 64: return launch_tacaw_tma<64>(c, ex, d_I, d_slot, n_bins, n_probes);
-        case 128: return launch_tacaw_tma<128>(c, ex, d_I, d_slot, n_bins, n_probes);
-        case 256: return launch_tacaw_tma<256>(c, ex, d_I, d_slot, n_bins, n_probes);
-        case 512: return launch_tacaw_tma<512>(c, ex, d_I, d_slot, n_bins, n_probes);
-        case 1024: return launch_tacaw_tma<1024>(c, ex, d_I, d_slot, n_bins, n_probes);
-        case 2048: return launch_tacaw_tma<2048>(c, ex, d_I, d_slot, n_bins, n_probes);
+    const bool use_ring = tiled ? (PSB_TACAW_TILED_RING != 0 && n_frames <= 2048)
+                                : (n_frames == 2048 || ((n_frames == 512 || n_frames == 1024) && 4 * n_bins <= n_frames));
+#define PSB_TACAW_CASE(NFV)                                                                                         \
+    case NFV:                                                                                                       \
+        if (use_ring) return tiled ? launch_tacaw_tma<NFV, true>(c, ex, d_I, d_slot, n_bins, n_probes)             \
+                                   : launch_tacaw_tma<NFV, false>(c, ex, d_I, d_slot, n_bins, n_probes);           \
+        e = tiled ? launch_tacaw<NFV, true>(c, ex, d_I, d_slot, n_bins, n_probes)                                   \
+                  : launch_tacaw<NFV, false>(c, ex, d_I, d_slot, n_bins, n_probes);                                 \
+        break;
+    cudaError_t e = cudaErrorInvalidValue;
+    switch (n_frames) {
+        PSB_TACAW_CASE(32) PSB_TACAW_CASE(64) PSB_TACAW_CASE(128) PSB_TACAW_CASE(256) PSB_TACAW_CASE(512)
+        PSB_TACAW_CASE(1024)
+        case 2048:
+            if (use_ring) return tiled ? launch_tacaw_tma<2048, true>(c, ex, d_I, d_slot, n_bins, n_probes)
+                                       : launch_tacaw_tma<2048, false>(c, ex, d_I, d_slot, n_bins, n_probes);
+            break;
+        case 4096:
+            e = tiled ? launch_tacaw<4096, true>(c, ex, d_I, d_slot, n_bins, n_probes)
+                      : launch_tacaw<4096, false>(c, ex, d_I, d_slot, n_bins, n_probes);
+            break;
         default: break;
     }
-    return fail(c, PS_EUNSUPPORTED, "ps_tacaw: unsupported n_frames for this layout");
+#undef PSB_TACAW_CASE
+    if (e != cudaSuccess) return fail(c, PS_ECUDA, std::string("k_tacaw_fft: ") + cudaGetErrorString(e));
+    c->launches++;
+    return PS_OK;
 }
 
 extern "C" ps_status ps_tacaw_begin(ps_ctx* c, int n_probes, int n_frames_total, double dt_fs, int n_bins,

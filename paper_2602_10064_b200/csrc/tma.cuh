@@ -68,6 +68,13 @@ __device__ __forceinline__ void tensor_store_2d(const CUtensorMap* map, const in
                  "r"(c1), "r"(smem_u32(smem_src))
                  : "memory");
 }
+// 5-D tiled tensor copy shared -> global (the time-tiled exit-wave layout: coordinates innermost first)
+__device__ __forceinline__ void tensor_store_5d(const CUtensorMap* map, const int c0, const int c1, const int c2, const int c3,
+                                                const int c4, const void* smem_src) {
+    asm volatile("cp.async.bulk.tensor.5d.global.shared::cta.tile.bulk_group [%0, {%1, %2, %3, %4, %5}], [%6];" ::"l"(map),
+                 "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4), "r"(smem_u32(smem_src))
+                 : "memory");
+}
 // asks the copy engine to bring [g, g + bytes) into L2 (16-byte aligned, size % 16 == 0); no completion to wait for
 __device__ __forceinline__ void bulk_prefetch_l2(const void* g, const uint32_t bytes) {
     asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(g), "r"(bytes) : "memory");
@@ -113,6 +120,20 @@ inline bool make_map_2d_f32(CUtensorMap* map, void* base, uint64_t row_floats, u
     const cuuint32_t box[2] = {box_floats, box_rows};
     const cuuint32_t estr[2] = {1, 1};
     return fn(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, base, gdim, gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+              CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) ==
+           CUDA_SUCCESS;
+}
+
+// float32 5-D tensor, dims innermost first, byte strides of dims 1..4 (multiples of 16), box extents per dim
+inline bool make_map_5d_f32(CUtensorMap* map, void* base, const uint64_t dims[5], const uint64_t strides_bytes[4],
+                            const uint32_t box[5]) {
+    EncodeTiledFn fn = encode_fn();
+    if (!fn) return false;
+    cuuint64_t gdim[5], gstride[4];
+    cuuint32_t b[5], estr[5] = {1, 1, 1, 1, 1};
+    for (int i = 0; i < 5; ++i) { gdim[i] = dims[i]; b[i] = box[i]; }
+    for (int i = 0; i < 4; ++i) gstride[i] = strides_bytes[i];
+    return fn(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 5, base, gdim, gstride, b, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) ==
            CUDA_SUCCESS;
 }

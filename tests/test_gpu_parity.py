@@ -685,3 +685,75 @@ def test_resident_slice_loop_matches_oracle_and_streaming_path(torch, n, beam):
             assert rel_l2(outs[1][p, i], eo) < TOL_EXIT
     A = O.aperture_mask(w.cell, n, n)
     assert float(np.abs(outs[1][:, :, ~A]).max()) == 0.0                 # exact zeros outside the band limit
+
+
+@pytest.mark.parametrize("name", ["c1_si_128", "c3_si_probe_512", "c5_al_sweep"])
+def test_tiled_exit_layout_matches_dense_and_oracle(torch, name):
+    """PS_LAYOUT_TILED_APERTURE ([P][ny][n_tiles][F][8]): ps_multislice writes the same exit values as in
+    the dense layout (bit for bit: the same kernels, another store), the omitted column tiles are exact zeros in the
+    dense array, and ps_tacaw of the tiled array gives the oracle's |Psi(k,w)|^2 of those exit waves."""
+    import paper_2602_10064_b200 as ps
+    w = make_workload(name, mini=True)
+    ctx = make_ctx(w)
+    F = 32
+    pos = w.positions(0, F)
+    V = ps.ps_build_slices(ctx, _t(torch, pos), _t(torch, w.Z))
+    psi0 = gpu_incident(ctx, w)
+    ctx.set_tuning("resident", -1)                      # the chip-resident path writes the dense layout only
+    dense = ps.ps_multislice(ctx, w.kV, psi0, V)
+    tiled = ps.ps_multislice(ctx, w.kV, psi0, V, layout=ps.PS_LAYOUT_TILED_APERTURE)
+    assert tiled.dim() == 5 and tiled.shape[2] * 8 < w.nx          # fewer columns than the dense array
+    back = ps.ps_exit_to_dense(ctx, tiled)
+    assert torch.equal(back, dense)
+    I_d = ps.ps_tacaw(ctx, dense, w.dt_fs).cpu().numpy()
+    I_t = ps.ps_tacaw(ctx, tiled, w.dt_fs).cpu().numpy()
+    dn = dense.cpu().numpy().astype(np.complex128)
+    Io = np.stack([O.tacaw_intensity(dn[p_]) for p_ in range(dn.shape[0])])
+    assert rel_l2(I_t, Io) < TOL_I and rel_l2(I_d, Io) < TOL_I
+    bins = np.array([1, 5, -3, 9], dtype=np.int32)
+    I_tb = ps.ps_tacaw(ctx, tiled, w.dt_fs, bins).cpu().numpy()
+    assert rel_l2(I_tb, Io[:, bins % F]) < TOL_I
+
+
+def test_tiled_exit_layout_work_array_chunks(torch):
+    """The tiled layout propagates in a scratch work array: a workspace that holds only 5 waves forces ragged chunks
+    (7 frames x 3 probes = 21 waves) and must give the same exit waves; consumers of dense arrays reject the layout."""
+    import paper_2602_10064_b200 as ps
+    w = make_workload("c3_si_probe_512", mini=True)
+    ctx = make_ctx(w)
+    pos = w.positions(0, 7)
+    V = ps.ps_build_slices(ctx, _t(torch, pos), _t(torch, w.Z))
+    psi0 = gpu_incident(ctx, w)[:3].contiguous()
+    dense = ps.ps_multislice(ctx, w.kV, psi0, V)
+    ws = torch.empty(5 * w.nx * w.ny * 8 + 4096, dtype=torch.uint8, device="cuda")
+    ctx.set_workspace(ws)
+    tiled = ps.ps_multislice(ctx, w.kV, psi0, V, layout=ps.PS_LAYOUT_TILED_APERTURE)
+    assert torch.equal(ps.ps_exit_to_dense(ctx, tiled), dense)
+    ctx.set_workspace(None)
+    with pytest.raises(ps.PSError):
+        ctx._check(ctx._lib.ps_haadf(ctx._h, tiled.data_ptr(), ps.PS_LAYOUT_TILED_APERTURE, 3, 7, 0.5, 1.0,
+                                     torch.empty(3, device="cuda").data_ptr()))
+
+
+@pytest.mark.parametrize("F,n,P", [(512, 64, 2), (1024, 128, 3), (2048, 64, 1), (4096, 32, 1)])
+def test_tacaw_tiled_lengths(torch, F, n, P):
+    """Every time-transform length through the tiled layout (ring kernel up to 2048 frames, register-staged at 4096),
+    on synthetic stacks with a large constant term, against the oracle transform."""
+    import paper_2602_10064_b200 as ps
+    rng = np.random.default_rng(F + n)
+    w = make_workload("c1_si_128", mini=True)
+    w.nx, w.ny = n, n
+    w.cell = np.array([n * 0.1, n * 0.1, w.cell[2]])
+    ctx = make_ctx(w)
+    shape = ps.exit_shape(ctx, P, F, ps.PS_LAYOUT_TILED_APERTURE)
+    x = (rng.normal(size=shape) + 1j * rng.normal(size=shape)).astype(np.complex64) + np.complex64(30 - 20j)
+    tiled = _t(torch, x)
+    dense = ps.ps_exit_to_dense(ctx, tiled)
+    I_t = ps.ps_tacaw(ctx, tiled, 2.0).cpu().numpy()
+    dn = dense.cpu().numpy().astype(np.complex128)
+    mask = np.zeros((n, n), bool)                       # the library reads in-aperture pixels only (others: zeros)
+    kx = np.fft.fftfreq(n, d=w.cell[0] / n)[None, :]; ky = np.fft.fftfreq(n, d=w.cell[1] / n)[:, None]
+    kc = (2.0 / 3.0) * min(n / (2 * w.cell[0]), n / (2 * w.cell[1]))
+    mask[(kx ** 2 + ky ** 2) <= kc ** 2] = True
+    Io = np.stack([O.tacaw_intensity(dn[p_] * mask[None]) for p_ in range(P)])
+    assert rel_l2(I_t, Io) < TOL_I
