@@ -341,7 +341,7 @@ def full_config(which, quiet=False):
         V = ps.ps_build_slices(ctx, pos_d[:8], Z_d)                      # warm-up
         del V
         torch.cuda.synchronize()
-        ex = torch.empty((pc, F, ny, nx), dtype=torch.complex64, device="cuda")
+        ex = torch.empty(ps.exit_shape(ctx, pc, F, ps.PS_LAYOUT_TILED_APERTURE), dtype=torch.complex64, device="cuda")
         I = torch.empty((pc, F, ny, nx), dtype=torch.float32, device="cuda")
         simg = torch.empty((P, F), dtype=torch.float32, device="cuda")
         sdp = torch.zeros((ny, nx), dtype=torch.float32, device="cuda")
@@ -359,7 +359,8 @@ def full_config(which, quiet=False):
         b.record()
         torch.cuda.synchronize()
         check = float(simg.sum())
-        plan = f"V of all {F} frames resident (86 GB); {P // pc} chunks of {pc} probes: incident -> multislice (34 GB) -> ps_tacaw -> reductions"
+        plan = (f"V of all {F} frames resident (86 GB); {P // pc} chunks of {pc} probes: incident -> multislice (tiled exit "
+                f"layout, {ex.numel() * 8 / 1e9:.0f} GB) -> ps_tacaw -> reductions")
     sec = a.elapsed_time(b) * 1e-3
     units = float(nx) * ny * S * F * P
     out = {"full_config": w.name, "grid": [nx, ny], "n_slices": S, "frames": F, "probes": P, "atoms": int(w.n_atoms),
@@ -387,6 +388,9 @@ def main():
     ap.add_argument("--grid", type=int, default=None, help="override the grid size (config 5 sweeps 256..2048)")
     ap.add_argument("--probes-side", type=int, default=None, help="override probes per scan side / number of tilts")
     ap.add_argument("--wave-chunk", type=int, default=0)
+    ap.add_argument("--exit-layout", default="auto", choices=["auto", "dense", "tiled"],
+                    help="exit-wave layout between ps_multislice and ps_tacaw: tiled = PS_LAYOUT_TILED_APERTURE (auto: tiled "
+                         "unless the batch takes the chip-resident small-grid path, which writes the dense layout)")
     ap.add_argument("--tune", action="append", default=[], metavar="KEY=VALUE",
                     help="ps_set_tuning knob (resident=-1|0|1); repeatable")
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
@@ -453,15 +457,18 @@ def main():
     bins = w.bins if w.bins is not None else None
     nb = F if bins is None else len(bins)
 
-    need = 4.0 * F * S * ny * nx + 8.0 * P * F * ny * nx + 4.0 * P * nb * ny * nx
-    free_b, _ = torch.cuda.mem_get_info()
-    if need > 0.97 * free_b:
-        raise SystemExit(f"workload needs {need / 1e9:.0f} GB of HBM (V + exit waves + I), {free_b / 1e9:.0f} GB free")
-
     ctx = ps.Context(local_rank)
     nl, ng, coef = form_factor_coefficients(w.elements, w.ff_kind)
     ctx.set_form_factors(w.elements, nl, ng, coef)
     ctx.set_geometry(w.cell, nx, ny, w.slice_dz)
+    small_resident = nx == ny and nx <= 128 and P * F <= 2 * N_SM          # ps_multislice's chip-resident path (dense only)
+    tiled = args.exit_layout == "tiled" or (args.exit_layout == "auto" and not small_resident)
+    exit_shape = ps.exit_shape(ctx, P, F, ps.PS_LAYOUT_TILED_APERTURE if tiled else ps.PS_LAYOUT_DENSE)
+    exit_bytes = 8.0 * float(np.prod(exit_shape))
+    need = 4.0 * F * S * ny * nx + exit_bytes + 4.0 * P * nb * ny * nx
+    free_b, _ = torch.cuda.mem_get_info()
+    if need > 0.97 * free_b:
+        raise SystemExit(f"workload needs {need / 1e9:.0f} GB of HBM (V + exit waves + I), {free_b / 1e9:.0f} GB free")
     if args.wave_chunk:
         ctx.set_wave_chunk(args.wave_chunk)
     for kv in args.tune:
@@ -472,7 +479,7 @@ def main():
     Z_d = Z_h.to(dev)
     V = torch.empty((F, S, ny, nx), dtype=torch.float32, device=dev)
     psi0 = torch.empty((P, ny, nx), dtype=torch.complex64, device=dev)
-    exitw = torch.empty((P, F, ny, nx), dtype=torch.complex64, device=dev)
+    exitw = torch.empty(exit_shape, dtype=torch.complex64, device=dev)
     I = torch.empty((P, nb, ny, nx), dtype=torch.float32, device=dev)
     sdp = torch.empty((ny, nx), dtype=torch.float32, device=dev)
     simg = torch.empty((P, nb), dtype=torch.float32, device=dev)
@@ -620,7 +627,8 @@ def main():
                 tr = st["dram_bytes_per_px"].get(str(P), st["dram_bytes_per_px"].get("any"))
                 tr = tr * px_launch if tr is not None else None
             ach = alg[kname] * px_launch / (k_ms / k_n * 1e-3) / 1e9
-            per[kname] = {"kernel": f"{kname}<{n_grid}>", "achieved": ach, "frac": ach / peak, "traffic": tr,
+            per[kname] = {"kernel": (st or {}).get("sass_kernel", f"{kname}<{n_grid}>"), "achieved": ach, "frac": ach / peak,
+                          "traffic": tr,
                           "bytes_per_launch": alg[kname] * px_launch, "avg_launch_ms": k_ms / k_n,
                           "algorithmic_bytes_per_px": alg[kname], "fp32_issue": issue}
         ms_pair = kern["k_row_transmit"][0] + kern["k_col_propagate"][0]
@@ -640,12 +648,14 @@ def main():
                                  "on its stream (ps_profile_*), not the pass `value` was timed on",
             "profiled_ms_per_step": ms_prof_total / K})
     if "k_tacaw_fft" in kern:
-        tb = (8.0 * F + 4.0 * nb) * ctx.n_k_aperture * P + 4.0 * nb * (nx * ny - ctx.n_k_aperture) * P
-        tms = kern["k_tacaw_fft"][0] / kern["k_tacaw_fft"][1]
+        tb_in = (8.0 * F + 4.0 * nb) * ctx.n_k_aperture * P              # transform kernel: exit values in, I out
+        tb_zero = 4.0 * nb * (nx * ny - ctx.n_k_aperture) * P              # zero fill of the out-of-band pixels of I
+        tb = tb_in + tb_zero
+        tms = kern["k_tacaw_fft"][0] / K
         tst = stats.get(f"k_tacaw<{F}>")
         roofline["tacaw"] = {"achieved": tb / (tms * 1e-3) / 1e9, "frac": tb / (tms * 1e-3) / 1e9 / peak,
-                             "bytes_per_launch": tb, "avg_launch_ms": tms,
-                             "traffic": (tst["dram_bytes_per_algorithmic_byte"] * tb) if tst else None}
+                             "bytes_per_step": tb, "ms_per_step": tms,
+                             "traffic": (tst["dram_bytes_per_inband_algorithmic_byte"] * tb_in + tb_zero) if tst else None}
     if "k_vk" in kern:
         # V(k) structure-factor sums: 4 real sums per quarter-plane point and atom, x3 for the 3xTF32 split (tensor path)
         flop = 24.0 * (ctx.n_k_aperture / 4.0) * float(w.n_atoms) * F
@@ -674,6 +684,7 @@ def main():
             "config": workload_config(w, omega_bins=nb,
                                       l2="256 MiB buffer written between timed steps (L2 flush); per-step CUDA events",
                                       hbm_resident_GB=need / 1e9,
+                                      exit_layout="tiled [P][ny][tile][F][8] (PS_LAYOUT_TILED_APERTURE)" if tiled else "dense [P][F][ny][nx]",
                                       parallelism=f"independent trajectory per GPU x{world}, one all-reduce of the reductions"),
             "tacaw_end_to_end_s": ms_total / K * 1e-3,
             "clocks": clocks,

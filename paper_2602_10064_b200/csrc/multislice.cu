@@ -28,7 +28,9 @@ template <int NX> struct RowCfg {
     static constexpr int T = Plan<NX>::T;
     static constexpr int THREADS = (T > 256) ? T : 256;
     static constexpr int RPB = THREADS / T;                               // rows per block
-    static constexpr int MIN_BLOCKS = (THREADS <= 256) ? 2 : 1;           // cap registers at 128
+    // two blocks of eight warps per SM at up to 128 registers; measured at 512^2 (config 3): four blocks of 128
+    // threads the same (69.7 vs 69.2 ms per 80 slices), five blocks at 96 registers slower (75.9), six at 80 slower (82.3)
+    static constexpr int MIN_BLOCKS = (THREADS <= 256) ? 2 : 1;
     static constexpr size_t SMEM = (size_t)RPB * RowLine<NX>::LEN * sizeof(float2);
     // rows are independent: only the T threads of a row synchronise (a warp, or a named barrier per row)
     using Sync = typename std::conditional<(T <= 32), WarpSync,
