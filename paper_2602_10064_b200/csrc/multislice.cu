@@ -114,7 +114,7 @@ k_row_transmit(float2* __restrict__ W, const float2* __restrict__ psi0, const fl
         const unsigned vrow_i = ((f * (unsigned)n_slices + (unsigned)slice) << ny_shift) + y;
         cur.advance(dy, dlp, dlf, ny_shift, np);
         if (NX >= 512 && rho + stride < n_rows) {
-            const unsigned pn = cm.p0 + cur.lp, fn = cm.f0 + cur.lf;
+            const unsigned fn = cm.f0 + cur.lf;
             const unsigned wn_i = ((((unsigned)cm.wp0 + cur.lp) * (unsigned)cm.wF + (unsigned)cm.wf0 + cur.lf) << ny_shift) + cur.y;
             const unsigned vn_i = ((fn * (unsigned)n_slices + (unsigned)slice) << ny_shift) + cur.y;
             if (2 * t < T) tma::prefetch_l2(V + (size_t)vn_i * NX + 32 * t);
@@ -228,12 +228,12 @@ k_row_transmit32(float2* __restrict__ W, const float* __restrict__ V, const Chun
 
     for (int item = blockIdx.x; item < n_items; item += gridDim.x, rho += stride) {
         const unsigned cur_lp = cur.lp, cur_lf = cur.lf;
-        const unsigned p = cm.p0 + cur_lp, f = cm.f0 + cur_lf, y = cur.y;
+        const unsigned f = cm.f0 + cur_lf, y = cur.y;
         const unsigned wrow_i = ((((unsigned)cm.wp0 + cur_lp) * (unsigned)cm.wF + (unsigned)cm.wf0 + cur_lf) << ny_shift) + y;
         const unsigned vrow_i = ((f * (unsigned)n_slices + (unsigned)slice) << ny_shift) + y;
         cur.advance(dy, dlp, dlf, ny_shift, np);
         if (rho + stride < n_rows) {
-            const unsigned pn = cm.p0 + cur.lp, fn = cm.f0 + cur.lf;
+            const unsigned fn = cm.f0 + cur.lf;
             const unsigned wn_i = ((((unsigned)cm.wp0 + cur.lp) * (unsigned)cm.wF + (unsigned)cm.wf0 + cur.lf) << ny_shift) + cur.y;
             const unsigned vn_i = ((fn * (unsigned)n_slices + (unsigned)slice) << ny_shift) + cur.y;
             tma::prefetch_l2(V + (size_t)vn_i * NX + 32 * t);
@@ -266,27 +266,64 @@ k_row_transmit32(float2* __restrict__ W, const float* __restrict__ V, const Chun
 // float32 [P*F*ny][2 nx]); the ring of NS shared-memory stages is, in turn, TMA destination, FFT
 // exchange buffer and TMA store source, so the load of item i+1 and the store of item i-1 overlap the
 // transforms of item i and no register is spent on staging.
-template <int NY> struct ColCfg {
-    static constexpr int T = Plan<NY>::T;
-    static constexpr int C = (NY <= 1024) ? 8 : 4;   // columns per block
+//
+// E = values per thread of the transform plan (fft_core.cuh).  E = 16: NY/16 threads per column, two shared-memory
+// exchanges per transform at NY >= 512.  E = 32 (NY = 512, 1024): NY/32 threads per column, ONE exchange; blocks are
+// half as large (128 threads, 168 registers), three of them per SM with a 2-stage ring.  The pass is bound by the LSU
+// data pipe, which every element crosses 10 (E = 16) or 6 (E = 32) times per transform pair (profiles/r2_slice_step.md).
+#ifndef PSB_COL32_NS
+#define PSB_COL32_NS 2
+#endif
+#ifndef PSB_COL32_BLOCKS
+#define PSB_COL32_BLOCKS 3
+#endif
+template <int NY, int E> struct ColCfg {
+    static_assert(E == 16 || (E == 32 && (NY == 512 || NY == 1024)), "32 values per thread: NY = 512 or 1024");
+    static constexpr int T = NY / E;
+    static constexpr int C = (E == 32) ? ((NY <= 512) ? 8 : 4) : ((NY <= 1024) ? 8 : 4);   // columns per block
     static constexpr int THREADS = C * T;
-    static constexpr int NS = 3;                                          // pipeline stages
+    static constexpr int NS = (E == 32) ? PSB_COL32_NS : 3;               // pipeline stages
     static constexpr int BOX_R = (NY < 256) ? NY : 256;                   // TMA box rows (<= 256)
     static constexpr int NBOX = NY / BOX_R;
-    static constexpr int MIN_BLOCKS = (THREADS <= 256) ? 2 : 1;           // cap registers at 128
+    static constexpr int MIN_BLOCKS = (E == 32) ? PSB_COL32_BLOCKS : (THREADS <= 256) ? 2 : 1;   // E = 16: cap registers at 128
     static constexpr uint32_t STAGE_BYTES = (uint32_t)NY * C * sizeof(float2);
     static constexpr size_t SMEM = (size_t)NS * STAGE_BYTES + (size_t)NY * sizeof(float2) + NS * sizeof(uint64_t) + 128;
 };
 
+// the transform plan of a column pass: slots, twiddles, forward / inverse
+template <int NY, int E, int C> struct ColFft;
+template <int NY, int C> struct ColFft<NY, 16, C> {
+    using Slots = ColSlots<C>;
+    using TW = Twiddles<NY>;
+    static __device__ __forceinline__ void forward(float2 (&v)[16], const int t, const TW& tw, const Slots& sm) {
+        fft_forward<NY, Slots, BlockSync>(v, t, tw, sm);
+    }
+    static __device__ __forceinline__ void inverse(float2 (&v)[16], const int t, const TW& tw, const Slots& sm) {
+        fft_inverse<NY, Slots, BlockSync>(v, t, tw, sm);
+    }
+};
+template <int NY, int C> struct ColFft<NY, 32, C> {
+    using Slots = ColSlots32<C, NY / 32>;
+    using TW = Twiddles32<NY>;
+    static __device__ __forceinline__ void forward(float2 (&v)[32], const int, const TW& tw, const Slots& sm) {
+        fft32_forward<NY, Slots, BlockSync>(v, tw, sm);
+    }
+    static __device__ __forceinline__ void inverse(float2 (&v)[32], const int, const TW& tw, const Slots& sm) {
+        fft32_inverse<NY, Slots, BlockSync>(v, tw, sm);
+    }
+};
+
 // TILED (last pass only): the k-space exit wave goes to the time-tiled layout [P][ny][active tile][F][8 kx] through a
 // second, 5-D tensor map instead of back into the array it was propagated in.
-template <int NY, bool LAST, bool TILED>
-__global__ void __launch_bounds__(ColCfg<NY>::THREADS, ColCfg<NY>::MIN_BLOCKS)
-k_col_propagate(const __grid_constant__ CUtensorMap wmap, const __grid_constant__ CUtensorMap tmap, const int tiles_lo, const int tile_gap, const int n_tiles,
-                const int32_t* __restrict__ nmax, const float2* __restrict__ px, const float2* __restrict__ py,
-                const ChunkMap cm, const int n_items) {
-    using Cfg = ColCfg<NY>;
-    constexpr int T = Cfg::T, C = Cfg::C, SUB = kColTile / C, NS = Cfg::NS, PF = NS - 2;   // prefetch distance
+template <int NY, int E, bool LAST, bool TILED>
+__global__ void __launch_bounds__(ColCfg<NY, E>::THREADS, ColCfg<NY, E>::MIN_BLOCKS)
+k_col_propagate(const __grid_constant__ CUtensorMap wmap, const __grid_constant__ CUtensorMap tmap, const int tiles_lo,
+                const int tile_gap, const int n_tiles, const int32_t* __restrict__ nmax, const float2* __restrict__ px,
+                const float2* __restrict__ py, const ChunkMap cm, const int n_items) {
+    using Cfg = ColCfg<NY, E>;
+    constexpr int T = Cfg::T, C = Cfg::C, SUB = kColTile / C, NS = Cfg::NS;
+    using Fft = ColFft<NY, E, C>;
+    using Slots = typename Fft::Slots;
     extern __shared__ __align__(1024) float2 smem_col[];      // no static shared memory: the window starts aligned
     float2* stage0 = smem_col;
     float2* py_s = smem_col + (size_t)NS * NY * C;
@@ -312,14 +349,10 @@ k_col_propagate(const __grid_constant__ CUtensorMap wmap, const __grid_constant_
         tma::fence_mbar_init();
     }
     for (int i = threadIdx.x; i < NY; i += Cfg::THREADS) py_s[i] = py[i];
-    Twiddles<NY> tw;
+    typename Fft::TW tw;
     tw.init(t);
     __syncthreads();
-    if (threadIdx.x == 0) {
-#pragma unroll
-        for (int k = 0; k < PF; ++k)
-            if (blockIdx.x + k * gridDim.x < n_items) issue_load(blockIdx.x + k * gridDim.x, k);
-    }
+    if (threadIdx.x == 0 && blockIdx.x < n_items) issue_load(blockIdx.x, 0);   // the load runs one item ahead
 
     int it = 0;
     int rem = blockIdx.x % per_wave;                         // item % per_wave, kept incrementally (no division per item)
@@ -327,135 +360,10 @@ k_col_propagate(const __grid_constant__ CUtensorMap wmap, const __grid_constant_
     for (int item = blockIdx.x; item < n_items; item += gridDim.x, ++it) {
         const int s = it % NS;
         if (threadIdx.x == 0) {
-            const int nxt = item + PF * gridDim.x;
+            const int nxt = item + gridDim.x;
             if (nxt < n_items) {
-                tma::bulk_wait_read<1>();                     // stage (it+PF)%NS was stored NS-PF = 2 items ago: drained
-                issue_load(nxt, (it + PF) % NS);
-            }
-        }
-        const int tj = rem / SUB;
-        const int kx0 = (tj < tiles_lo ? tj : tj + tile_gap) * kColTile + (rem % SUB) * C;
-        const int kx = kx0 + c;
-        const int nm = nmax[kx];
-        const float2 pxv = px[kx];
-        float2* st = stage0 + (size_t)s * NY * C;
-        ColSlots<C> slots(st + c, t);
-        tma::mbar_wait(&full[s], (it / NS) & 1);
-        float2 v[16];
-#pragma unroll
-        for (int e = 0; e < 16; ++e) v[e] = slots.at(t + e * T);
-        fft_forward<NY, ColSlots<C>, BlockSync>(v, t, tw, slots);
-#pragma unroll
-        for (int e = 0; e < 16; ++e) {
-            const int iy = t + e * T;
-            const int n = iy < NY / 2 ? iy : NY - iy;         // |signed index|
-            v[e] = (n <= nm) ? cmul(v[e], cmul(pxv, py_s[iy])) : make_float2(0.f, 0.f);
-        }
-        if (!LAST) fft_inverse<NY, ColSlots<C>, BlockSync>(v, t, tw, slots);
-        __syncthreads();                                      // exchange reads of this stage are done
-#pragma unroll
-        for (int e = 0; e < 16; ++e) slots.at(t + e * T) = v[e];
-        tma::fence_proxy_async();
-        __syncthreads();
-        if (threadIdx.x == 0) {
-            const int l = item / per_wave;
-            if (TILED) {
-                const int p = cm.p0 + l % cm.np, f = cm.f0 + l / cm.np;
-#pragma unroll
-                for (int b = 0; b < Cfg::NBOX; ++b)
-                    tma::tensor_store_5d(&tmap, 2 * (rem % SUB) * C, f, rem / SUB, b * Cfg::BOX_R, p,
-                                         st + (size_t)b * Cfg::BOX_R * C);
-            } else {
-                const int row0 = ((cm.wp0 + l % cm.np) * cm.wF + cm.wf0 + l / cm.np) * NY;
-#pragma unroll
-                for (int b = 0; b < Cfg::NBOX; ++b)
-                    tma::tensor_store_2d(&wmap, 2 * kx0, row0 + b * Cfg::BOX_R, st + (size_t)b * Cfg::BOX_R * C);
-            }
-            tma::bulk_commit();
-        }
-        rem += rem_step;
-        if (rem >= per_wave) rem -= per_wave;
-    }
-    if (threadIdx.x == 0) tma::bulk_wait_all<0>();
-}
-
-// ------------------------------------------------------------------------------------ column pass, 32 values per thread
-// The same pass for NY = 512 and 1024 with the 32-value transform plan (fft_core.cuh): T = NY/32 threads per column,
-// one shared-memory exchange per transform instead of two.  Blocks are half as large (C columns x NY/32 threads), so
-// the same number of stages and resident blocks holds half as many warps, each with twice the independent work.
-template <int NY> struct ColCfg32 {
-    static constexpr int T = Plan32<NY>::T;
-#ifndef PSB_COL32_C512
-#define PSB_COL32_C512 8
-#endif
-    static constexpr int C = (NY <= 512) ? PSB_COL32_C512 : 4;
-    static constexpr int THREADS = C * T;                                  // 128
-#ifndef PSB_COL32_NS
-#define PSB_COL32_NS 2
-#endif
-#ifndef PSB_COL32_BLOCKS
-#define PSB_COL32_BLOCKS 3
-#endif
-    static constexpr int NS = PSB_COL32_NS;
-    static constexpr int BOX_R = 256;
-    static constexpr int NBOX = NY / BOX_R;
-    static constexpr int MIN_BLOCKS = PSB_COL32_BLOCKS;
-    static constexpr uint32_t STAGE_BYTES = (uint32_t)NY * C * sizeof(float2);
-    static constexpr size_t SMEM = (size_t)NS * STAGE_BYTES + (size_t)NY * sizeof(float2) + NS * sizeof(uint64_t) + 128;
-};
-
-template <int NY, bool LAST, bool TILED>
-__global__ void __launch_bounds__(ColCfg32<NY>::THREADS, ColCfg32<NY>::MIN_BLOCKS)
-k_col_propagate32(const __grid_constant__ CUtensorMap wmap, const __grid_constant__ CUtensorMap tmap, const int tiles_lo, const int tile_gap, const int n_tiles,
-                  const int32_t* __restrict__ nmax, const float2* __restrict__ px, const float2* __restrict__ py,
-                  const ChunkMap cm, const int n_items) {
-    using Cfg = ColCfg32<NY>;
-    constexpr int T = Cfg::T, C = Cfg::C, SUB = kColTile / C, NS = Cfg::NS, PF = 1;
-    using Slots = ColSlots32<C, T>;
-    extern __shared__ __align__(1024) float2 smem_col[];
-    float2* stage0 = smem_col;
-    float2* py_s = smem_col + (size_t)NS * NY * C;
-    uint64_t* full = reinterpret_cast<uint64_t*>(smem_col + (size_t)NS * NY * C + NY);
-    const int c = threadIdx.x % C, t = threadIdx.x / C;
-    const int per_wave = n_tiles * SUB;
-
-    auto issue_load = [&](const int item, const int s) {
-        const int l = item / per_wave, rem = item % per_wave;
-        const int tj = rem / SUB;
-        const int kx0 = (tj < tiles_lo ? tj : tj + tile_gap) * kColTile + (rem % SUB) * C;
-        const int row0 = ((cm.wp0 + l % cm.np) * cm.wF + cm.wf0 + l / cm.np) * NY;
-        tma::mbar_arrive_expect_tx(&full[s], Cfg::STAGE_BYTES);
-#pragma unroll
-        for (int b = 0; b < Cfg::NBOX; ++b)
-            tma::tensor_load_2d(stage0 + (size_t)s * NY * C + (size_t)b * Cfg::BOX_R * C, &wmap, 2 * kx0,
-                                row0 + b * Cfg::BOX_R, &full[s]);
-    };
-
-    if (threadIdx.x == 0) {
-#pragma unroll
-        for (int s = 0; s < NS; ++s) tma::mbar_init(&full[s], 1);
-        tma::fence_mbar_init();
-    }
-    for (int i = threadIdx.x; i < NY; i += Cfg::THREADS) py_s[i] = py[i];
-    Twiddles32<NY> tw;
-    tw.init(t);
-    __syncthreads();
-    if (threadIdx.x == 0) {
-#pragma unroll
-        for (int k = 0; k < PF; ++k)
-            if (blockIdx.x + k * gridDim.x < n_items) issue_load(blockIdx.x + k * gridDim.x, k);
-    }
-
-    int it = 0;
-    int rem = blockIdx.x % per_wave;
-    const int rem_step = gridDim.x % per_wave;
-    for (int item = blockIdx.x; item < n_items; item += gridDim.x, ++it) {
-        const int s = it % NS;
-        if (threadIdx.x == 0) {
-            const int nxt = item + PF * gridDim.x;
-            if (nxt < n_items) {
-                tma::bulk_wait_read<NS - 2>();                // the store that last used stage (it+1)%NS has drained
-                issue_load(nxt, (it + PF) % NS);
+                tma::bulk_wait_read<NS - 2>();                // the store that last used stage (it + 1) % NS has drained
+                issue_load(nxt, (it + 1) % NS);
             }
         }
         const int tj = rem / SUB;
@@ -466,46 +374,46 @@ k_col_propagate32(const __grid_constant__ CUtensorMap wmap, const __grid_constan
         float2* st = stage0 + (size_t)s * NY * C;
         const Slots slots(st + c, t);
         tma::mbar_wait(&full[s], (it / NS) & 1);
-        float2 v[32];
+        float2 v[E];
 #pragma unroll
-        for (int e = 0; e < 32; ++e) v[e] = slots.at(t + e * T);
+        for (int e = 0; e < E; ++e) v[e] = slots.at(t + e * T);
         auto propagate = [&]() {
 #pragma unroll
-            for (int e = 0; e < 32; ++e) {
+            for (int e = 0; e < E; ++e) {
                 const int iy = t + e * T;
-                const int n = iy < NY / 2 ? iy : NY - iy;
+                const int n = iy < NY / 2 ? iy : NY - iy;     // |signed index|
                 v[e] = (n <= nm) ? cmul(v[e], cmul(pxv, py_s[iy])) : make_float2(0.f, 0.f);
             }
         };
-        // NY = 1024: both transforms run the SAME forward code in a two-trip loop, so that the loop body of the kernel
-        // fits the instruction cache (two unrolled copies of the 32-value transform do not; ncu: 10 % of the stall
-        // samples were "no instruction"; measured +5 % at 1024, -8 % at 512, hence per size).  The inverse is the
-        // forward transform read backwards: sum_k X[k] e^{+2 pi i n k / N} is element (-n) mod N of the forward
-        // transform of X, so after the second trip canonical position j holds row (-j) mod NY, and the tile is written
-        // back with reversed row addressing.
-        constexpr bool LOOPED = (NY == 1024) && !LAST;
+        // E = 32, NY = 1024: both transforms run the SAME forward code in a two-trip loop, so that the loop body of the
+        // kernel fits the instruction cache (two unrolled copies of the 32-value transform do not; ncu: 10 % of the stall
+        // samples were "no instruction"; measured +5 % at 1024, -8 % at 512, hence per size).  The inverse is the forward
+        // transform read backwards: sum_k X[k] e^{+2 pi i n k / N} is element (-n) mod N of the forward transform of X,
+        // so after the second trip canonical position j holds row (-j) mod NY, and the tile is written back with
+        // reversed row addressing.
+        constexpr bool LOOPED = (E == 32) && (NY == 1024) && !LAST;
         if constexpr (LOOPED) {
 #pragma unroll 1
             for (int pass = 0; pass < 2; ++pass) {
-                fft32_forward<NY, Slots, BlockSync>(v, tw, slots);
+                Fft::forward(v, t, tw, slots);
                 if (pass == 0) propagate();
             }
         } else {
-            fft32_forward<NY, Slots, BlockSync>(v, tw, slots);
+            Fft::forward(v, t, tw, slots);
             propagate();
-            if (!LAST) fft32_inverse<NY, Slots, BlockSync>(v, tw, slots);
+            if (!LAST) Fft::inverse(v, t, tw, slots);
         }
-        __syncthreads();
+        __syncthreads();                                      // exchange reads of this stage are done
         if constexpr (!LOOPED) {
 #pragma unroll
-            for (int e = 0; e < 32; ++e) slots.at(t + e * T) = v[e];
+            for (int e = 0; e < E; ++e) slots.at(t + e * T) = v[e];
         } else {
-            // row (NY - t - e T) mod NY = (T - t) + (31 - e) T, except (t, e) = (0, 0), which is row 0
+            // row (NY - t - e T) mod NY = (T - t) + (E - 1 - e) T, except (t, e) = (0, 0), which is row 0
             float2* const pr = st + c + (size_t)(T - t) * C;
-            float2* const p0 = (t == 0) ? st + c : pr + 31 * T * C;
+            float2* const p0 = (t == 0) ? st + c : pr + (E - 1) * T * C;
             *p0 = v[0];
 #pragma unroll
-            for (int e = 1; e < 32; ++e) pr[(31 - e) * T * C] = v[e];
+            for (int e = 1; e < E; ++e) pr[(E - 1 - e) * T * C] = v[e];
         }
         tma::fence_proxy_async();
         __syncthreads();
@@ -546,6 +454,18 @@ __global__ void k_zero_cols(float2* __restrict__ W, const int nx, const int ny, 
 }
 
 // ------------------------------------------------------------------------------------ launch helpers
+#define PSB_DISPATCH_N(n, CALL)                                                    \
+    switch (n) {                                                                   \
+        case 32: { constexpr int N_ = 32; CALL; } break;                           \
+        case 64: { constexpr int N_ = 64; CALL; } break;                           \
+        case 128: { constexpr int N_ = 128; CALL; } break;                         \
+        case 256: { constexpr int N_ = 256; CALL; } break;                         \
+        case 512: { constexpr int N_ = 512; CALL; } break;                         \
+        case 1024: { constexpr int N_ = 1024; CALL; } break;                       \
+        case 2048: { constexpr int N_ = 2048; CALL; } break;                       \
+        default: break;                                                            \
+    }
+
 template <int NX, bool FIRST>
 static cudaError_t launch_row(ps_ctx* c, float2* W, const float2* psi0, const float* V, const ChunkMap& cm,
                               int slice, float sigma, int col_lo, int col_hi) {
@@ -594,11 +514,11 @@ static bool use_row32(const ps_ctx* c, int col_lo, int col_hi) {
     return col_lo >= 10 * T && col_lo <= 12 * T && col_hi >= 20 * T && col_hi <= 22 * T;
 }
 
-template <int NY, bool LAST, bool TILED = false>
+template <int NY, int E, bool LAST, bool TILED = false>
 static cudaError_t launch_col(ps_ctx* c, const CUtensorMap& wmap, const CUtensorMap& tmap, const ChunkMap& cm, int zero_lo,
                               int zero_hi) {
-    using Cfg = ColCfg<NY>;
-    auto kern = k_col_propagate<NY, LAST, TILED>;
+    using Cfg = ColCfg<NY, E>;
+    auto kern = k_col_propagate<NY, E, LAST, TILED>;
     int per_sm_grid = 0;
     cudaError_t ce = kernel_cap(c, kern, Cfg::THREADS, Cfg::SMEM, &per_sm_grid);
     if (ce != cudaSuccess) return ce;
@@ -610,20 +530,15 @@ static cudaError_t launch_col(ps_ctx* c, const CUtensorMap& wmap, const CUtensor
     return cudaGetLastError();
 }
 
-template <int NY, bool LAST, bool TILED = false>
-static cudaError_t launch_col32(ps_ctx* c, const CUtensorMap& wmap, const CUtensorMap& tmap, const ChunkMap& cm, int zero_lo,
-                                int zero_hi) {
-    using Cfg = ColCfg32<NY>;
-    auto kern = k_col_propagate32<NY, LAST, TILED>;
-    int per_sm_grid = 0;
-    cudaError_t ce = kernel_cap(c, kern, Cfg::THREADS, Cfg::SMEM, &per_sm_grid);
-    if (ce != cudaSuccess) return ce;
-    const int n_tiles = c->n_tiles_active;
-    const int n_items = cm.np * cm.nf * n_tiles * (kColTile / Cfg::C);
-    const int grid = n_items < per_sm_grid ? n_items : per_sm_grid;
-    kern<<<grid, Cfg::THREADS, Cfg::SMEM, c->stream>>>(wmap, tmap, zero_lo / kColTile, (zero_hi - zero_lo) / kColTile, n_tiles, c->d_nmax,
-                                                      LAST ? c->kv.d_px_last : c->kv.d_px_mid, c->kv.d_py, cm, n_items);
-    return cudaGetLastError();
+// column pass of size ny: 32 values per thread where available and wanted, 16 otherwise
+template <bool LAST, bool TILED>
+static cudaError_t launch_col_any(ps_ctx* c, bool col32, const CUtensorMap& wmap, const CUtensorMap& tmap, const ChunkMap& cm,
+                                  int zero_lo, int zero_hi) {
+    cudaError_t e = cudaErrorInvalidValue;
+    if (col32 && c->ny == 512) return launch_col<512, 32, LAST, TILED>(c, wmap, tmap, cm, zero_lo, zero_hi);
+    if (col32 && c->ny == 1024) return launch_col<1024, 32, LAST, TILED>(c, wmap, tmap, cm, zero_lo, zero_hi);
+    PSB_DISPATCH_N(c->ny, (e = launch_col<N_, 16, LAST, TILED>(c, wmap, tmap, cm, zero_lo, zero_hi)));
+    return e;
 }
 
 // the column pass of this grid uses the 32-value plan (ps_set_tuning "col32": 0 auto, 1 on where available, -1 off)
@@ -632,23 +547,12 @@ static bool use_col32(const ps_ctx* c) { return (c->ny == 512 || c->ny == 1024) 
 template <int NY>
 static bool make_wave_map(CUtensorMap* map, void* W, int nx, long long rows, bool col32) {
     if constexpr (NY == 512 || NY == 1024) {
-        if (col32) return tma::make_map_2d_f32(map, W, 2ull * nx, (uint64_t)rows, 2 * ColCfg32<NY>::C, ColCfg32<NY>::BOX_R);
+        if (col32) return tma::make_map_2d_f32(map, W, 2ull * nx, (uint64_t)rows, 2 * ColCfg<NY, 32>::C, ColCfg<NY, 32>::BOX_R);
     }
-    using Cfg = ColCfg<NY>;
+    using Cfg = ColCfg<NY, 16>;
     return tma::make_map_2d_f32(map, W, 2ull * nx, (uint64_t)rows, 2 * Cfg::C, Cfg::BOX_R);
 }
 
-#define PSB_DISPATCH_N(n, CALL)                                                    \
-    switch (n) {                                                                   \
-        case 32: { constexpr int N_ = 32; CALL; } break;                           \
-        case 64: { constexpr int N_ = 64; CALL; } break;                           \
-        case 128: { constexpr int N_ = 128; CALL; } break;                         \
-        case 256: { constexpr int N_ = 256; CALL; } break;                         \
-        case 512: { constexpr int N_ = 512; CALL; } break;                         \
-        case 1024: { constexpr int N_ = 1024; CALL; } break;                       \
-        case 2048: { constexpr int N_ = 2048; CALL; } break;                       \
-        default: break;                                                            \
-    }
 
 static constexpr long long kResidentMaxWaves = 2 * kNumSM;   // auto rule of the chip-resident path
 
@@ -834,9 +738,7 @@ extern "C" ps_status ps_multislice(ps_ctx* c, double kV, const void* d_psi0, int
                 {
                 ProfScope ps_(c, K_COL_PROPAGATE);
                 if (s == S - 1 && tiled) {
-                    if (col32 && c->ny == 512) e = launch_col32<512, true, true>(c, wmap, tmap, cm, zero_lo, zero_hi);
-                    else if (col32 && c->ny == 1024) e = launch_col32<1024, true, true>(c, wmap, tmap, cm, zero_lo, zero_hi);
-                    else { PSB_DISPATCH_N(c->ny, (e = launch_col<N_, true, true>(c, wmap, tmap, cm, zero_lo, zero_hi))); }
+                    e = launch_col_any<true, true>(c, col32, wmap, tmap, cm, zero_lo, zero_hi);
                 } else if (s == S - 1) {
                     if (zero_hi > zero_lo) {
                         const long long tot = (long long)cm.np * cm.nf * c->ny * (zero_hi - zero_lo);
@@ -844,13 +746,9 @@ extern "C" ps_status ps_multislice(ps_ctx* c, double kV, const void* d_psi0, int
                         k_zero_cols<<<zb, 256, 0, c->stream>>>(W, c->nx, c->ny, zero_lo, zero_hi, cm);
                         c->launches++;
                     }
-                    if (col32 && c->ny == 512) e = launch_col32<512, true>(c, wmap, tmap, cm, zero_lo, zero_hi);
-                    else if (col32 && c->ny == 1024) e = launch_col32<1024, true>(c, wmap, tmap, cm, zero_lo, zero_hi);
-                    else { PSB_DISPATCH_N(c->ny, (e = launch_col<N_, true>(c, wmap, tmap, cm, zero_lo, zero_hi))); }
+                    e = launch_col_any<true, false>(c, col32, wmap, tmap, cm, zero_lo, zero_hi);
                 } else {
-                    if (col32 && c->ny == 512) e = launch_col32<512, false>(c, wmap, tmap, cm, zero_lo, zero_hi);
-                    else if (col32 && c->ny == 1024) e = launch_col32<1024, false>(c, wmap, tmap, cm, zero_lo, zero_hi);
-                    else { PSB_DISPATCH_N(c->ny, (e = launch_col<N_, false>(c, wmap, tmap, cm, zero_lo, zero_hi))); }
+                    e = launch_col_any<false, false>(c, col32, wmap, tmap, cm, zero_lo, zero_hi);
                 }
                 }
                 if (e != cudaSuccess) return fail(c, PS_ECUDA, std::string("k_col_propagate: ") + cudaGetErrorString(e));

@@ -270,17 +270,22 @@ def test_end_to_end_mini(torch, name):
     assert rel_l2(qg.cpu().numpy(), qo) < TOL_RED
 
 
-def test_results_are_deterministic(torch):
+@pytest.mark.parametrize("vk_mode", [1, 2])
+def test_results_are_deterministic(torch, vk_mode):
+    """Repeated calls on one ctx (scratch holding the previous call's V(k) and mixed arrays) give identical bits:
+    nothing is accumulated onto stale scratch, no floating-point atomics."""
     import paper_2602_10064_b200 as ps
     w = make_workload("c2_hbn_256", mini=True)
     ctx = make_ctx(w)
+    ctx.set_vk_mode(vk_mode)
     pos = _t(torch, w.positions()); Z = _t(torch, w.Z)
-    outs = []
+    outs, Vs = [], []
     for _ in range(2):
         V = ps.ps_build_slices(ctx, pos, Z)
+        Vs.append(V.clone())
         ex = ps.ps_multislice(ctx, w.kV, gpu_incident(ctx, w), V)
         outs.append(ps.ps_tacaw(ctx, ex, w.dt_fs, w.bins).clone())
-    assert torch.equal(outs[0], outs[1])
+    assert torch.equal(Vs[0], Vs[1]) and torch.equal(outs[0], outs[1])
 
 
 # ----------------------------------------------------------------------------- SURVEY §8(f) 2 and 4
