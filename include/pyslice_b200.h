@@ -86,9 +86,9 @@ typedef enum {
                                      * contiguous: the time transform streams F*64-byte runs instead of gathering 64-byte
                                      * pieces 8*nx*ny bytes apart.  n_tiles/(nx/8) = 0.69 of the dense size at the 2/3
                                      * band limit.  Written by ps_multislice (the wave is then propagated chunk by chunk in
-                                     * a work array in scratch / the installed workspace), read by ps_tacaw and
-                                     * ps_exit_to_dense; every other consumer takes PS_LAYOUT_DENSE only and answers
-                                     * PS_EUNSUPPORTED otherwise. */
+                                     * a work array in scratch / the installed workspace), read by ps_tacaw, ps_haadf and
+                                     * ps_exit_to_dense; ps_tacaw_add (chunks of a stream) and ps_apply_aberrations take
+                                     * dense arrays. */
 
 /* ---------------------------------------------------------------- life cycle */
 
@@ -253,7 +253,7 @@ PS_API ps_status ps_spectrum_image(ps_ctx* ctx, const float* d_I, int P, int n_b
 /* ps_haadf: annular detector on the k-space exit waves,
  *   d_out[p] = (1/F) sum_f sum_{k_in <= |k| < k_out} |Psi_pf(k)|^2 / (nx ny)      (k_out <= 0: no outer limit)
  * = fraction of the incident intensity on the detector, averaged over frames -> float32 [n_probes].
- * d_exit complex64 [n_probes][n_frames][ny][nx] as written by ps_multislice. */
+ * d_exit: exit waves as written by ps_multislice, in either layout. */
 PS_API ps_status ps_haadf(ps_ctx* ctx, const void* d_exit, int exit_layout, int n_probes, int n_frames, double k_in,
                    double k_out, float* d_out);
 /* ps_accumulate_intensity: d_acc <- w_acc * d_acc + w_new * d_I over

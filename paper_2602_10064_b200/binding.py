@@ -375,13 +375,15 @@ def ps_spectrum_image(ctx: Context, d_I, k_in: float = 0.0, k_out: float = 0.0, 
 
 
 def ps_haadf(ctx: Context, d_exit, k_in: float, k_out: float = 0.0, d_out=None):
-    """exit waves complex64 [P][F][ny][nx] -> float32 [P]: frame-averaged fraction of the beam on the annulus."""
+    """exit waves complex64 (dense [P][F][ny][nx] or tiled [P][ny][n_tiles][F][8]) -> float32 [P]: frame-averaged
+    fraction of the beam on the annulus."""
     import torch
     _need(d_exit, torch.complex64, "d_exit")
-    P, F = int(d_exit.shape[0]), int(d_exit.shape[1])
+    layout = _exit_layout(d_exit)
+    P, F = int(d_exit.shape[0]), int(d_exit.shape[1] if layout == PS_LAYOUT_DENSE else d_exit.shape[3])
     if d_out is None:
         d_out = torch.empty((P,), dtype=torch.float32, device=ctx.device)
-    ctx._check(ctx._lib.ps_haadf(ctx._h, _ptr(d_exit), PS_LAYOUT_DENSE, P, F, float(k_in), float(k_out), _ptr(d_out)))
+    ctx._check(ctx._lib.ps_haadf(ctx._h, _ptr(d_exit), layout, P, F, float(k_in), float(k_out), _ptr(d_out)))
     return d_out
 
 

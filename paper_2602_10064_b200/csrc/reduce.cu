@@ -89,6 +89,38 @@ k_haadf_frame(const float2* __restrict__ exitw, const uint8_t* __restrict__ mask
     s = block_sum(s, sh);
     if (threadIdx.x == 0) tmp[blockIdx.x] = s;
 }
+// Tiled exit layout [P][ny][tile][F][8]: a block owns one (probe, row) and sums |Psi|^2 over the row's in-band tiles for
+// every frame (threads = frames: consecutive 64-byte chunks), part[(p * ny + iy) * F + f]; k_haadf_rows then adds the
+// rows in fixed order into the same tmp[p * F + f] the dense path produces.
+__global__ void __launch_bounds__(256)
+k_haadf_tiled(const float2* __restrict__ Tl, const uint8_t* __restrict__ mask, const int32_t* __restrict__ tiles,
+              float* __restrict__ part, const int nx, const int ny, const int n_tiles, const int F) {
+    const int iy = blockIdx.x, p = blockIdx.y;
+    const float2* row = Tl + ((size_t)p * ny + iy) * n_tiles * F * kColTile;
+    for (int f = threadIdx.x; f < F; f += blockDim.x) {
+        float s = 0.f;
+        for (int tj = 0; tj < n_tiles; ++tj) {
+            const float4* src = reinterpret_cast<const float4*>(row + ((size_t)tj * F + f) * kColTile);
+            const uint8_t* m = mask + (size_t)iy * nx + tiles[tj] * kColTile;
+#pragma unroll
+            for (int q = 0; q < kColTile / 2; ++q) {
+                const float4 x = src[q];
+                float v = m[2 * q] ? fmaf(x.x, x.x, x.y * x.y) : 0.f;
+                v += m[2 * q + 1] ? fmaf(x.z, x.z, x.w * x.w) : 0.f;
+                s += v;
+            }
+        }
+        part[((size_t)p * ny + iy) * F + f] = s;
+    }
+}
+__global__ void k_haadf_rows(const float* __restrict__ part, float* __restrict__ tmp, const int ny, const int F, const long long total) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;       // p * F + f
+    if (i >= total) return;
+    const long long p = i / F; const int f = (int)(i % F);
+    float s = 0.f;
+    for (int iy = 0; iy < ny; ++iy) s += part[((size_t)p * ny + iy) * F + f];
+    tmp[i] = s;
+}
 __global__ void k_haadf_mean(const float* __restrict__ tmp, float* __restrict__ out, const int P, const int F, const float scale) {
     const int p = blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= P) return;
@@ -247,13 +279,17 @@ extern "C" ps_status ps_haadf(ps_ctx* c, const void* d_exit, int exit_layout, in
     if (!c) return PS_EINVAL;
     if (!c->have_geom) return fail(c, PS_ESTATE, "ps_haadf: ps_set_geometry has not been called");
     if (!d_exit || !d_out || n_probes < 1 || n_frames < 1) return fail(c, PS_EINVAL, "ps_haadf: null pointer or non-positive size");
-    if (exit_layout != PS_LAYOUT_DENSE) return fail(c, PS_EUNSUPPORTED, "ps_haadf: unknown exit layout");
+    if (exit_layout != PS_LAYOUT_DENSE && exit_layout != PS_LAYOUT_TILED_APERTURE)
+        return fail(c, PS_EUNSUPPORTED, "ps_haadf: unknown exit layout");
+    const bool tiled = exit_layout == PS_LAYOUT_TILED_APERTURE;
     if (k_in < 0.0) return fail(c, PS_EINVAL, "ps_haadf: k_in must be >= 0");
     ps_status st_in = enter(c, "ps_haadf");
     if (st_in != PS_OK) return st_in;
     const size_t npix = (size_t)c->nx * c->ny;
     const size_t tmp_off = (4096 + npix + 255) & ~(size_t)255;
-    ps_status st = ensure_buf(c, c->misc, tmp_off + (size_t)n_probes * n_frames * sizeof(float));
+    const size_t tmp_bytes = ((size_t)n_probes * n_frames * sizeof(float) + 255) & ~(size_t)255;
+    const size_t part_bytes = tiled ? (size_t)n_probes * c->ny * n_frames * sizeof(float) : 0;   // per-row partial sums
+    ps_status st = ensure_buf(c, c->misc, tmp_off + tmp_bytes + part_bytes);
     if (st != PS_OK) return st;
     uint8_t* d_mask = (uint8_t*)c->misc.p + 4096;
     float* d_tmp = (float*)((char*)c->misc.p + tmp_off);
@@ -261,8 +297,19 @@ extern "C" ps_status ps_haadf(ps_ctx* c, const void* d_exit, int exit_layout, in
     k_detector_mask<<<(unsigned)((npix + 255) / 256), 256, 0, c->stream>>>(d_mask, c->nx, c->ny, c->cell[0], c->cell[1], k_in,
                                                                            k_out, k_out > 0.0 ? 1 : 0);
     PSB_LAUNCH_CHECK(c, "k_detector_mask");
-    k_haadf_frame<<<n_probes * n_frames, 1024, 0, c->stream>>>((const float2*)d_exit, d_mask, d_tmp, npix);
-    PSB_LAUNCH_CHECK(c, "k_haadf_frame");
+    if (tiled) {
+        if (n_probes > 65535) return fail(c, PS_EUNSUPPORTED, "ps_haadf: more than 65535 probes in the tiled layout");
+        float* d_part = (float*)((char*)c->misc.p + tmp_off + tmp_bytes);
+        k_haadf_tiled<<<dim3(c->ny, n_probes), 256, 0, c->stream>>>((const float2*)d_exit, d_mask, c->d_tiles, d_part, c->nx,
+                                                                    c->ny, c->n_tiles_active, n_frames);
+        PSB_LAUNCH_CHECK(c, "k_haadf_tiled");
+        const long long total = (long long)n_probes * n_frames;
+        k_haadf_rows<<<(unsigned)((total + 255) / 256), 256, 0, c->stream>>>(d_part, d_tmp, c->ny, n_frames, total);
+        PSB_LAUNCH_CHECK(c, "k_haadf_rows");
+    } else {
+        k_haadf_frame<<<n_probes * n_frames, 1024, 0, c->stream>>>((const float2*)d_exit, d_mask, d_tmp, npix);
+        PSB_LAUNCH_CHECK(c, "k_haadf_frame");
+    }
     k_haadf_mean<<<(n_probes + 127) / 128, 128, 0, c->stream>>>(d_tmp, d_out, n_probes, n_frames,
                                                                  (float)(1.0 / ((double)n_frames * (double)npix)));
     PSB_LAUNCH_CHECK(c, "k_haadf_mean");

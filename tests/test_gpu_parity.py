@@ -722,7 +722,8 @@ def test_tiled_exit_layout_matches_dense_and_oracle(torch, name):
 
 def test_tiled_exit_layout_work_array_chunks(torch):
     """The tiled layout propagates in a scratch work array: a workspace that holds only 5 waves forces ragged chunks
-    (7 frames x 3 probes = 21 waves) and must give the same exit waves; consumers of dense arrays reject the layout."""
+    (7 frames x 3 probes = 21 waves) and must give the same exit waves; ps_haadf reads the tiled array directly;
+    an unknown layout value is refused."""
     import paper_2602_10064_b200 as ps
     w = make_workload("c3_si_probe_512", mini=True)
     ctx = make_ctx(w)
@@ -735,9 +736,13 @@ def test_tiled_exit_layout_work_array_chunks(torch):
     tiled = ps.ps_multislice(ctx, w.kV, psi0, V, layout=ps.PS_LAYOUT_TILED_APERTURE)
     assert torch.equal(ps.ps_exit_to_dense(ctx, tiled), dense)
     ctx.set_workspace(None)
-    with pytest.raises(ps.PSError):
-        ctx._check(ctx._lib.ps_haadf(ctx._h, tiled.data_ptr(), ps.PS_LAYOUT_TILED_APERTURE, 3, 7, 0.5, 1.0,
-                                     torch.empty(3, device="cuda").data_ptr()))
+    # HAADF straight from the tiled array = from the dense one (another summation order) = the oracle
+    h_t = ps.ps_haadf(ctx, tiled, 0.5, 2.0).cpu().numpy()
+    h_d = ps.ps_haadf(ctx, dense, 0.5, 2.0).cpu().numpy()
+    h_o = O.haadf(dense.cpu().numpy().astype(np.complex128), w.cell, 0.5, 2.0)
+    assert np.allclose(h_t, h_d, rtol=TOL_RED) and np.allclose(h_t, h_o, rtol=1e-4)
+    with pytest.raises(ps.PSError):                          # the streaming path takes dense chunks only: 5-D tensor refused
+        ctx._check(ctx._lib.ps_multislice(ctx._h, w.kV, psi0.data_ptr(), 3, V.data_ptr(), 7, tiled.data_ptr(), 7))
 
 
 @pytest.mark.parametrize("F,n,P", [(512, 64, 2), (1024, 128, 3), (2048, 64, 1), (4096, 32, 1)])
