@@ -682,7 +682,9 @@ extern "C" ps_status ps_multislice(ps_ctx* c, double kV, const void* d_psi0, int
     if (tiled) {
         // [P][ny][active tile][F][8 kx] as float32, innermost first: (16, F, n_tiles, ny, P); box = one column (sub)tile x
         // up to 256 rows of one frame
-        const int Cc = (c->ny == 2048) ? 4 : 8;              // columns per block of the column pass (ColCfg / ColCfg32)
+        // columns per block of the column pass that will run (ColCfg<NY, E>::C)
+        const int Cc = (col32 && c->ny == 512) ? ColCfg<512, 32>::C : (col32 && c->ny == 1024) ? ColCfg<1024, 32>::C
+                       : (c->ny == 2048) ? ColCfg<2048, 16>::C : ColCfg<1024, 16>::C;
         const uint64_t dims[5] = {2ull * kColTile, (uint64_t)n_frames, (uint64_t)c->n_tiles_active, (uint64_t)c->ny, (uint64_t)n_probes};
         const uint64_t row_b = 2ull * kColTile * sizeof(float);
         const uint64_t strides[4] = {row_b, row_b * n_frames, row_b * n_frames * c->n_tiles_active,

@@ -131,10 +131,14 @@ def test_multislice_grid_sizes(torch, nx, ny):
     ky = np.fft.fftfreq(ny)[:, None]; kx = np.fft.fftfreq(nx)[None, :]
     V32 = (400.0 * np.real(np.fft.ifft2(Vk * np.exp(-200.0 * (kx ** 2 + ky ** 2)))) * np.sqrt(nx * ny)).astype(np.float32)
     psi0 = O.tilted_plane_wave(nx, ny, 1, -1).astype(np.complex64)[None]
-    ex = ps.ps_multislice(ctx, 80.0, _t(torch, psi0), _t(torch, V32)).cpu().numpy()
+    ex_d = ps.ps_multislice(ctx, 80.0, _t(torch, psi0), _t(torch, V32))
+    ex = ex_d.cpu().numpy()
     for i in range(F):
         eo = O.multislice(psi0[0].astype(np.complex128), V32[i].astype(np.float64), w.cell, 80.0)
         assert rel_l2(ex[0, i], eo) < TOL_EXIT
+    # tiled exit layout at this size (sub-tiles of 4 columns at ny = 2048): the same bits
+    tiled = ps.ps_multislice(ctx, 80.0, _t(torch, psi0), _t(torch, V32), layout=ps.PS_LAYOUT_TILED_APERTURE)
+    assert torch.equal(ps.ps_exit_to_dense(ctx, tiled), ex_d)
 
 
 @pytest.mark.parametrize("n,row32,col32", [(512, 1, 1), (512, 0, -1), (1024, 1, 1), (1024, 0, -1), (512, 1, -1)])
@@ -155,11 +159,15 @@ def test_multislice_value_plans(torch, n, row32, col32):
     ky = np.fft.fftfreq(n)[:, None]; kx = np.fft.fftfreq(n)[None, :]
     V32 = (400.0 * np.real(np.fft.ifft2(Vk * np.exp(-200.0 * (kx ** 2 + ky ** 2)))) * n).astype(np.float32)
     psi0 = np.stack([O.tilted_plane_wave(n, n, m, -m).astype(np.complex64) for m in range(P)])
-    ex = ps.ps_multislice(ctx, 80.0, _t(torch, psi0), _t(torch, V32)).cpu().numpy()
+    ex_d = ps.ps_multislice(ctx, 80.0, _t(torch, psi0), _t(torch, V32))
+    ex = ex_d.cpu().numpy()
     for p_ in (0, P - 1):
         for i in range(F):
             eo = O.multislice(psi0[p_].astype(np.complex128), V32[i].astype(np.float64), w.cell, 80.0)
             assert rel_l2(ex[p_, i], eo) < TOL_EXIT
+    # the same kernels with the tiled store of the last column pass (5-D tensor map) at this size: identical bits
+    tiled = ps.ps_multislice(ctx, 80.0, _t(torch, psi0), _t(torch, V32), layout=ps.PS_LAYOUT_TILED_APERTURE)
+    assert torch.equal(ps.ps_exit_to_dense(ctx, tiled), ex_d)
 
 
 def test_multislice_free_space_plane_wave_is_exact(torch):
