@@ -98,7 +98,10 @@ def test_c3_full_grid_probe_chunk(torch):
     V, sidx = ps.ps_build_slices(ctx, _t(torch, pos), _t(torch, w.Z), want_slice_idx=True)
     psi0 = gpu_incident(ctx, w)
     ex = ps.ps_multislice(ctx, w.kV, psi0, V)
-    I = ps.ps_tacaw(ctx, ex, w.dt_fs)
+    # bench.py's default step keeps the exit waves in the tiled layout: the same bits, and I(k, w) is taken from it
+    tiled = ps.ps_multislice(ctx, w.kV, psi0, V, layout=ps.PS_LAYOUT_TILED_APERTURE)
+    assert torch.equal(ps.ps_exit_to_dense(ctx, tiled), ex)
+    I = ps.ps_tacaw(ctx, tiled, w.dt_fs)
     f = 17
     Vo, so = oracle_potential(w, pos[f], slices=(0, 41, 79))
     assert np.array_equal(sidx[f].cpu().numpy(), so)
