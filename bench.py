@@ -292,7 +292,7 @@ def tacaw_micro(shapes_a=None, shapes_b=None):
 
 
 # --------------------------------------------------------------------------------------------- configs 3 / 4 at full size
-def full_config(which, quiet=False):
+def full_config(which, quiet=False, fused_v=False):
     """Config 4: 4096 frames x 1024^2 x 120 slices, V built and propagated 64 frames at a time, exit waves folded into the
     streaming per-bin DFT (path B, 256 bins) chunk by chunk (SURVEY.md 8(d) capacity plan).  Config 3: 1024 frames x
     256 probes x 512^2 x 80 slices: V of all frames resident (86 GB), probes 16 at a time (34 GB of exit waves),
@@ -327,15 +327,19 @@ def full_config(which, quiet=False):
         a.record()
         ts = TacawStream(ctx, 1, F, w.dt_fs, bins)
         for f0 in range(0, F, chunk):
-            ps.ps_build_slices(ctx, pos_d[f0:f0 + chunk], Z_d, d_V=V)
-            ps.ps_multislice(ctx, w.kV, psi0, V, d_exit=ex)
+            if fused_v:
+                ps.ps_multislice_fused(ctx, w.kV, psi0, pos_d[f0:f0 + chunk], Z_d, d_exit=ex)
+            else:
+                ps.ps_build_slices(ctx, pos_d[f0:f0 + chunk], Z_d, d_V=V)
+                ps.ps_multislice(ctx, w.kV, psi0, V, d_exit=ex)
             ts.add(ex, f0)
         I = ts.finish()
         simg = ps.ps_spectrum_image(ctx, I)
         b.record()
         torch.cuda.synchronize()
         check = float(simg.sum())
-        plan = f"{F // chunk} chunks of {chunk} frames: build V (30 GB) -> multislice -> ps_tacaw_add (path B, {len(bins)} bins)"
+        plan = (f"{F // chunk} chunks of {chunk} frames: " + ("ps_multislice_fused (no V array)" if fused_v else "build V (30 GB) -> multislice") +
+                f" -> ps_tacaw_add (path B, {len(bins)} bins)")
     else:
         pc = 16
         V = ps.ps_build_slices(ctx, pos_d[:8], Z_d)                      # warm-up
@@ -396,6 +400,9 @@ def main():
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
                     help="N > 1: weak = an independent trajectory per rank (reductions averaged); strong = ONE problem "
                          "sharded by sharding.plan() (probe shards, or frame shards + reduce-scatter of the accumulators)")
+    ap.add_argument("--fused-v", action="store_true",
+                    help="positions -> exit waves through ps_multislice_fused (the row pass builds V row by row from the "
+                         "y-transformed slice pairs; no V array; dense exit layout) instead of ps_build_slices + ps_multislice")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--with-full-configs", action="store_true",
                     help="also run configs 3 and 4 at their FULL size after the timed steps and carry their end-to-end "
@@ -427,7 +434,7 @@ def main():
             tacaw_micro(parse(args.micro_a) or [], parse(args.micro_b) or [])
         return
     if args.full_config:
-        full_config(args.full_config)
+        full_config(args.full_config, fused_v=args.fused_v)
         return
 
     import torch
@@ -462,7 +469,7 @@ def main():
     ctx.set_form_factors(w.elements, nl, ng, coef)
     ctx.set_geometry(w.cell, nx, ny, w.slice_dz)
     small_resident = nx == ny and nx <= 128 and P * F <= 2 * N_SM          # ps_multislice's chip-resident path (dense only)
-    tiled = args.exit_layout == "tiled" or (args.exit_layout == "auto" and not small_resident)
+    tiled = (args.exit_layout == "tiled" or (args.exit_layout == "auto" and not small_resident)) and not args.fused_v
     exit_shape = ps.exit_shape(ctx, P, F, ps.PS_LAYOUT_TILED_APERTURE if tiled else ps.PS_LAYOUT_DENSE)
     exit_bytes = 8.0 * float(np.prod(exit_shape))
     need = 4.0 * F * S * ny * nx + exit_bytes + 4.0 * P * nb * ny * nx
@@ -504,9 +511,12 @@ def main():
         inc = dict(n=1)
 
     def step(pos_dev):
-        ps.ps_build_slices(ctx, pos_dev, Z_d, d_V=V)
         ps.ps_make_incident(ctx, w.kV, d_psi0=psi0, **inc)
-        ps.ps_multislice(ctx, w.kV, psi0, V, d_exit=exitw)
+        if args.fused_v:
+            ps.ps_multislice_fused(ctx, w.kV, psi0, pos_dev, Z_d, d_exit=exitw)
+        else:
+            ps.ps_build_slices(ctx, pos_dev, Z_d, d_V=V)
+            ps.ps_multislice(ctx, w.kV, psi0, V, d_exit=exitw)
         ps.ps_tacaw(ctx, exitw, w.dt_fs, bins, d_I=I)
         ps.ps_sdp(ctx, I, 1, min(8, nb - 1), d_out=sdp)
         ps.ps_spectrum_image(ctx, I, 0.0, 0.0, d_out=simg)
@@ -685,6 +695,7 @@ def main():
                                       l2="256 MiB buffer written between timed steps (L2 flush); per-step CUDA events",
                                       hbm_resident_GB=need / 1e9,
                                       exit_layout="tiled [P][ny][tile][F][8] (PS_LAYOUT_TILED_APERTURE)" if tiled else "dense [P][F][ny][nx]",
+                                      potential="ps_multislice_fused (no V array)" if args.fused_v else "ps_build_slices -> V",
                                       parallelism=f"independent trajectory per GPU x{world}, one all-reduce of the reductions"),
             "tacaw_end_to_end_s": ms_total / K * 1e-3,
             "clocks": clocks,

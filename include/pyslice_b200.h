@@ -201,6 +201,19 @@ PS_API ps_status ps_make_incident(ps_ctx* ctx, double kV, double semi_angle_mrad
 PS_API ps_status ps_multislice(ps_ctx* ctx, double kV, const void* d_psi0, int n_probes, const float* d_V,
                         int n_frames, void* d_exit, int exit_layout);
 
+/* a0 ... a6 in one call, without the V array (second half; "An inverse FFT then yields
+ * the real-space projected potential"): positions -> exit waves.  Frame chunk by frame chunk (as many frames
+ * as the scratch holds) the library bins and sorts the atoms, forms V(k) and its y-inverse transform, and runs the slice
+ * loop of those frames with a row pass that performs the x-inverse transform of the slice pair itself: the projected
+ * potential exists only row by row in shared memory and never travels through HBM.  Same values as ps_build_slices
+ * followed by ps_multislice to FP32 rounding (the same transforms in the same order).  It costs a third 1-D transform per
+ * row and slice, so it pays only where V would be used once (a single probe per frame) and memory, not time, is short:
+ * measured numbers in DESIGN.md section 10.  d_exit: PS_LAYOUT_DENSE only (the wave is propagated in place).
+ *   d_pos float32 [n_frames][n_atoms][3], d_Z int32 [n_atoms], d_psi0 complex64 [n_probes][ny][nx],
+ *   d_exit complex64 [n_probes][n_frames][ny][nx]                                (written) */
+PS_API ps_status ps_multislice_fused(ps_ctx* ctx, double kV, const void* d_psi0, int n_probes, const float* d_pos,
+                              const int32_t* d_Z, int n_frames, int n_atoms, void* d_exit, int exit_layout);
+
 /* Bytes of an exit-wave array of n_probes x n_frames waves in `exit_layout` (0 for an unknown layout or before
  * ps_set_geometry).  ps_exit_to_dense expands a PS_LAYOUT_TILED_APERTURE array into the dense one (exact zeros in the
  * column tiles the tiled layout does not store); both arrays caller-owned device memory, asynchronous on the ctx stream. */

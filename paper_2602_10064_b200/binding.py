@@ -40,6 +40,8 @@ _PROTOTYPES = {
     "ps_make_incident": (C.c_int, [C.c_void_p, C.c_double, C.c_double, C.c_int, C.c_void_p, C.c_int, C.c_void_p]),
     "ps_multislice": (C.c_int, [C.c_void_p, C.c_double, C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_void_p, C.c_int]),
     "ps_tacaw": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_double, C.c_int, C.c_void_p, C.c_void_p]),
+    "ps_multislice_fused": (C.c_int, [C.c_void_p, C.c_double, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_int, C.c_int,
+                                      C.c_void_p, C.c_int]),
     "ps_exit_bytes": (C.c_size_t, [C.c_void_p, C.c_int, C.c_int, C.c_int]),
     "ps_exit_to_dense": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_void_p]),
     "ps_tacaw_begin": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_double, C.c_int, C.c_void_p, C.c_void_p]),
@@ -279,6 +281,20 @@ def ps_multislice(ctx: Context, kV: float, d_psi0, d_V, d_exit=None, layout: int
         d_exit = torch.empty(exit_shape(ctx, P, F, layout), dtype=torch.complex64, device=ctx.device)
     _need(d_exit, torch.complex64, "d_exit")
     ctx._check(ctx._lib.ps_multislice(ctx._h, float(kV), _ptr(d_psi0), P, _ptr(d_V), F, _ptr(d_exit), _exit_layout(d_exit)))
+    return d_exit
+
+
+def ps_multislice_fused(ctx: Context, kV: float, d_psi0, d_pos, d_Z, d_exit=None):
+    """positions float32 [F][Na][3] + Z int32 [Na] + psi0 complex64 [P][ny][nx] -> exit waves complex64 [P][F][ny][nx]
+    without the V array (the row pass builds each row of V from the y-transformed slice pair)."""
+    import torch
+    _need(d_psi0, torch.complex64, "d_psi0"); _need(d_pos, torch.float32, "d_pos"); _need(d_Z, torch.int32, "d_Z")
+    P, F, Na = int(d_psi0.shape[0]), int(d_pos.shape[0]), int(d_pos.shape[1])
+    if d_exit is None:
+        d_exit = torch.empty((P, F, ctx.ny, ctx.nx), dtype=torch.complex64, device=ctx.device)
+    _need(d_exit, torch.complex64, "d_exit")
+    ctx._check(ctx._lib.ps_multislice_fused(ctx._h, float(kV), _ptr(d_psi0), P, _ptr(d_pos), _ptr(d_Z), F, Na, _ptr(d_exit),
+                                            PS_LAYOUT_DENSE))
     return d_exit
 
 

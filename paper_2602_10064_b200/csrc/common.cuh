@@ -216,6 +216,19 @@ inline cudaError_t kernel_cap(ps_ctx* c, K kern, int threads, size_t smem, int* 
     c->kern_cap.emplace(key, *cap);
     return cudaSuccess;
 }
+// Where the slice loop takes the projected potential from: the V array of ps_build_slices, or (ps_multislice_fused) the
+// mixed array Zm[(f - zm_f0) * n_pairs + pair][y][kx] of a frame chunk — the y-transformed pair of slices, complex, in-band
+// column tiles only — whose x-inverse transform the row pass then runs itself; `off` = sorted-atom offsets of that chunk
+// ([frames][n_slices * n_elem + 1]), which say which slices of a pair are empty.
+struct VSrc {
+    const float* V = nullptr;
+    const float2* Zm = nullptr;
+    const int32_t* off = nullptr;
+    int zm_f0 = 0;
+};
+// the slice loop of frames [fr0, fr0 + fr_n) of an exit array of n_frames frames (multislice.cu)
+ps_status multislice_range(ps_ctx* c, double kV, const void* d_psi0, int n_probes, const VSrc& src, int n_frames, int fr0,
+                           int fr_n, void* d_exit, int exit_layout);
 ps_status ensure_kv(ps_ctx* c, double kV);
 ps_status ensure_ftab(ps_ctx* c);
 ps_status ensure_abtab(ps_ctx* c, double kV);                           // incident.cu

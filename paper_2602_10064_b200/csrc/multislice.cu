@@ -180,6 +180,97 @@ k_row_transmit(float2* __restrict__ W, const float2* __restrict__ psi0, const fl
     }
 }
 
+// ------------------------------------------------------------------------------------ row pass, potential from Zm
+// ps_multislice_fused (second half; "An inverse FFT then yields the real-space
+// projected potential"): the row pass takes row y of the y-transformed slice PAIR (s/2) from the mixed array Zm,
+// runs the x-inverse transform itself — real part = slice 2 pr, imaginary part = slice 2 pr + 1, exactly what k_v_row
+// would have written to V — parks the row of V it needs in shared memory and carries on as k_row_transmit does.  V is
+// never written to or read from HBM.  Costs a third transform per row and slice; meant for single-probe runs.
+template <int NX> struct RowZmCfg {
+    static constexpr int T = Plan<NX>::T;
+    static constexpr int THREADS = RowCfg<NX>::THREADS;
+    static constexpr int RPB = RowCfg<NX>::RPB;
+    static constexpr int MIN_BLOCKS = RowCfg<NX>::MIN_BLOCKS;
+    static constexpr size_t SMEM = (size_t)RPB * (RowLine<NX>::LEN * sizeof(float2) + NX * sizeof(float));
+    using Sync = typename RowCfg<NX>::Sync;
+};
+
+template <int NX, bool FIRST>
+__global__ void __launch_bounds__(RowZmCfg<NX>::THREADS, RowZmCfg<NX>::MIN_BLOCKS)
+k_row_transmit_zm(float2* __restrict__ W, const float2* __restrict__ psi0, const float2* __restrict__ Zm,
+                  const int32_t* __restrict__ offsets, const int zm_f0, const int n_pairs, const int n_elem,
+                  const ChunkMap cm, const int ny_shift, const int n_slices, const int slice, const float sigma,
+                  const int n_items, const int col_lo, const int col_hi) {
+    using Cfg = RowZmCfg<NX>;
+    constexpr int T = Cfg::T;
+    extern __shared__ float2 smem[];
+    const int t = threadIdx.x % T, r = threadIdx.x / T;
+    RowSlots slots{smem + (size_t)r * RowLine<NX>::LEN};
+    float* svline = reinterpret_cast<float*>(smem + (size_t)Cfg::RPB * RowLine<NX>::LEN) + (size_t)r * NX;
+    Twiddles<NX> tw;
+    tw.init(t);
+    unsigned amask = 0;
+#pragma unroll
+    for (int e = 0; e < 16; ++e) amask |= ((t + e * T < col_lo || t + e * T >= col_hi) ? 1u : 0u) << e;
+    const unsigned np = (unsigned)cm.np;
+    const unsigned n_rows = np * (unsigned)cm.nf << ny_shift;
+    const unsigned stride = gridDim.x * Cfg::RPB;
+    const unsigned dy = stride & ((1u << ny_shift) - 1u), dl = stride >> ny_shift;
+    const unsigned dlf = dl / np, dlp = dl - dlf * np;
+    unsigned rho = blockIdx.x * Cfg::RPB + r;
+    RowCursor cur;
+    cur.init(rho, ny_shift, np);
+    const int pr = slice >> 1, part = slice & 1, n_bins = n_slices * n_elem;
+    const int sa = 2 * pr, sb = 2 * pr + 1;
+
+    for (int item = blockIdx.x; item < n_items; item += gridDim.x, rho += stride) {
+        const bool valid = rho < n_rows;
+        const unsigned cur_lp = cur.lp, cur_lf = cur.lf;
+        const unsigned p = cm.p0 + cur_lp, f = cm.f0 + cur_lf, y = cur.y;
+        const unsigned wrow_i = ((((unsigned)cm.wp0 + cur_lp) * (unsigned)cm.wF + (unsigned)cm.wf0 + cur_lf) << ny_shift) + y;
+        cur.advance(dy, dlp, dlf, ny_shift, np);
+        float2* wrow = W + (size_t)wrow_i * NX + t;
+        unsigned am = valid ? amask : 0u;
+        asm volatile("" : "+r"(am));
+        // ---- V of this row: x-inverse transform of the pair's mixed row (skipped when both slices are vacuum)
+        const int fl = (int)f - zm_f0;                                       // frame inside the Zm chunk
+        bool any = false;
+        if (valid) {
+            const int32_t* off = offsets + (size_t)fl * (n_bins + 1);
+            const bool has_a = off[(sa + 1) * n_elem] > off[sa * n_elem];
+            const bool has_b = (sb < n_slices) && off[(sb + 1) * n_elem] > off[sb * n_elem];
+            any = has_a || has_b;
+        }
+        float2 v[16];
+        {
+            const float2* zrow = Zm + ((((size_t)fl * n_pairs + pr) << ny_shift) + y) * NX + t;
+#pragma unroll
+            for (int e = 0; e < 16; ++e) v[e] = (any && (am & (1u << e))) ? zrow[e * T] : make_float2(0.f, 0.f);
+        }
+        fft_inverse<NX, RowSlots, typename Cfg::Sync>(v, t, tw, slots);
+#pragma unroll
+        for (int e = 0; e < 16; ++e) svline[t + e * T] = any ? (part ? v[e].y : v[e].x) : 0.f;
+        // ---- the wave row (each thread re-reads the elements of V it wrote itself: no barrier needed)
+        asm volatile("" : "+r"(am));
+        if (FIRST) {
+            const float2* src = psi0 + (((size_t)p << ny_shift) + y) * NX + t;
+#pragma unroll
+            for (int e = 0; e < 16; ++e) v[e] = valid ? __ldg(src + e * T) : make_float2(0.f, 0.f);
+        } else {
+#pragma unroll
+            for (int e = 0; e < 16; ++e) v[e] = (am & (1u << e)) ? wrow[e * T] : make_float2(0.f, 0.f);
+            fft_inverse<NX, RowSlots, typename Cfg::Sync>(v, t, tw, slots);
+        }
+#pragma unroll
+        for (int e = 0; e < 16; ++e) v[e] = cmul(v[e], cis_fast(sigma * svline[t + e * T]));
+        fft_forward<NX, RowSlots, typename Cfg::Sync>(v, t, tw, slots);
+        asm volatile("" : "+r"(am));
+#pragma unroll
+        for (int e = 0; e < 16; ++e)
+            if (am & (1u << e)) wrow[e * T] = v[e];
+    }
+}
+
 // ------------------------------------------------------------------------------------ row pass, 32 values per thread
 // NX = 512 and 1024 with the 32-value transform plan: T = NX/32 threads per row (half a warp / one warp: no block
 // barrier at all), one shared-memory exchange per transform.  Used for the slices after the first when the active
@@ -489,6 +580,24 @@ static cudaError_t launch_row(ps_ctx* c, float2* W, const float2* psi0, const fl
     return cudaGetLastError();
 }
 
+template <int NX, bool FIRST>
+static cudaError_t launch_row_zm(ps_ctx* c, float2* W, const float2* psi0, const VSrc& src, const ChunkMap& cm, int slice,
+                                 float sigma, int col_lo, int col_hi) {
+    using Cfg = RowZmCfg<NX>;
+    auto kern = k_row_transmit_zm<NX, FIRST>;
+    int per_sm_grid = 0;
+    cudaError_t ce = kernel_cap(c, kern, Cfg::THREADS, Cfg::SMEM, &per_sm_grid);
+    if (ce != cudaSuccess) return ce;
+    const long long n_rows = (long long)cm.np * cm.nf * c->ny;
+    const int n_items = (int)((n_rows + Cfg::RPB - 1) / Cfg::RPB);
+    const int grid = n_items < per_sm_grid ? n_items : per_sm_grid;
+    int ny_shift = 0;
+    while ((1 << ny_shift) < c->ny) ++ny_shift;
+    kern<<<grid, Cfg::THREADS, Cfg::SMEM, c->stream>>>(W, psi0, src.Zm, src.off, src.zm_f0, (c->n_slices + 1) / 2, c->n_elem, cm,
+                                                      ny_shift, c->n_slices, slice, sigma, n_items, col_lo, col_hi);
+    return cudaGetLastError();
+}
+
 template <int NX>
 static cudaError_t launch_row32(ps_ctx* c, float2* W, const float* V, const ChunkMap& cm, int slice, float sigma, int col_lo,
                                 int col_hi) {
@@ -637,9 +746,20 @@ extern "C" ps_status ps_multislice(ps_ctx* c, double kV, const void* d_psi0, int
         return fail(c, PS_EINVAL, "ps_multislice: null pointer or non-positive size / voltage");
     if (exit_layout != PS_LAYOUT_DENSE && exit_layout != PS_LAYOUT_TILED_APERTURE)
         return fail(c, PS_EUNSUPPORTED, "ps_multislice: unknown exit layout");
-    const bool tiled = exit_layout == PS_LAYOUT_TILED_APERTURE;
     ps_status st = enter(c, "ps_multislice");
     if (st != PS_OK) return st;
+    VSrc src;
+    src.V = d_V;
+    return multislice_range(c, kV, d_psi0, n_probes, src, n_frames, 0, n_frames, d_exit, exit_layout);
+}
+
+// The slice loop of frames [fr0, fr0 + fr_n) of an exit array laid out for n_frames frames.  ps_multislice runs the whole
+// range with the potential taken from V; ps_multislice_fused calls it once per frame chunk with the chunk's mixed array.
+ps_status psb::multislice_range(ps_ctx* c, double kV, const void* d_psi0, int n_probes, const VSrc& src, int n_frames,
+                                int fr0, int fr_n, void* d_exit, int exit_layout) {
+    const bool tiled = exit_layout == PS_LAYOUT_TILED_APERTURE;
+    const float* d_V = src.V;
+    ps_status st;
     if ((st = ensure_kv(c, kV)) != PS_OK) return st;
 
     const long long wave_rows = (long long)n_probes * n_frames * c->ny;
@@ -654,7 +774,7 @@ extern "C" ps_status ps_multislice(ps_ctx* c, double kV, const void* d_psi0, int
     // work array that lives in scratch, as many waves at a time as it holds.
     float2* W = (float2*)d_exit;
     long long chunk = c->wave_chunk;
-    if (chunk <= 0) chunk = (long long)n_probes * n_frames;
+    if (chunk <= 0) chunk = (long long)n_probes * fr_n;
     if (tiled) {
         long long held = 0;
         if ((st = tiled_work_buffer(c, chunk, &W, &held)) != PS_OK) return st;
@@ -663,9 +783,10 @@ extern "C" ps_status ps_multislice(ps_ctx* c, double kV, const void* d_psi0, int
     const int np = (int)(n_probes < chunk ? n_probes : chunk);
     int nf = (int)(chunk / np);
     if (nf < 1) nf = 1;
-    if (nf < n_frames) {                                     // equal-sized frame chunks (no short tail chunk)
-        const int n_chunks = (n_frames + nf - 1) / nf;
-        nf = (n_frames + n_chunks - 1) / n_chunks;
+    if (nf > fr_n) nf = fr_n;
+    if (nf < fr_n) {                                         // equal-sized frame chunks (no short tail chunk)
+        const int n_chunks = (fr_n + nf - 1) / nf;
+        nf = (fr_n + n_chunks - 1) / n_chunks;
     }
     const float2* psi0 = (const float2*)d_psi0;
     const float sigma = (float)c->kv.sigma;
@@ -708,7 +829,7 @@ extern "C" ps_status ps_multislice(ps_ctx* c, double kV, const void* d_psi0, int
 
     // Small square grids, small batches: the whole slice loop in one launch with the wave resident in shared memory
     // (resident.cu).  Batches that fill the GPU stay on the streaming passes (measured cross-over: profiles/r2_resident.md).
-    if (!tiled && resident_supported(c) && !c->vacuum_shortcut && c->wave_chunk == 0 &&
+    if (!tiled && d_V && fr0 == 0 && fr_n == n_frames && resident_supported(c) && !c->vacuum_shortcut && c->wave_chunk == 0 &&
         (c->tune_resident == 1 || (c->tune_resident == 0 && (long long)n_probes * n_frames <= kResidentMaxWaves))) {
         cudaError_t e = launch_slice_resident(c, W, psi0, d_V, n_probes, n_frames, sigma, zero_lo, zero_hi);
         if (e != cudaSuccess) return fail(c, PS_ECUDA, std::string("k_slice_resident: ") + cudaGetErrorString(e));
@@ -716,12 +837,12 @@ extern "C" ps_status ps_multislice(ps_ctx* c, double kV, const void* d_psi0, int
         return PS_OK;
     }
 
-    const bool row32 = use_row32(c, zero_lo, zero_hi);
+    const bool row32 = d_V && use_row32(c, zero_lo, zero_hi);
     for (int p0 = 0; p0 < n_probes; p0 += np) {
-        for (int f0 = 0; f0 < n_frames; f0 += nf) {
+        for (int f0 = fr0; f0 < fr0 + fr_n; f0 += nf) {
             ChunkMap cm;
             cm.p0 = p0; cm.np = (n_probes - p0 < np) ? n_probes - p0 : np;
-            cm.f0 = f0; cm.nf = (n_frames - f0 < nf) ? n_frames - f0 : nf;
+            cm.f0 = f0; cm.nf = (fr0 + fr_n - f0 < nf) ? fr0 + fr_n - f0 : nf;
             cm.F = n_frames;
             if (tiled) { cm.wp0 = 0; cm.wf0 = 0; cm.wF = cm.nf; }
             else       { cm.wp0 = cm.p0; cm.wf0 = cm.f0; cm.wF = n_frames; }
@@ -729,7 +850,11 @@ extern "C" ps_status ps_multislice(ps_ctx* c, double kV, const void* d_psi0, int
                 cudaError_t e = cudaErrorInvalidValue;
                 {
                 ProfScope ps_(c, K_ROW_TRANSMIT);
-                if (s == 0) { PSB_DISPATCH_N(c->nx, (e = launch_row<N_, true>(c, W, psi0, d_V, cm, s, sigma, zero_lo, zero_hi))); }
+                if (!d_V) {                                          // potential from the mixed array (ps_multislice_fused)
+                    if (s == 0) { PSB_DISPATCH_N(c->nx, (e = launch_row_zm<N_, true>(c, W, psi0, src, cm, s, sigma, zero_lo, zero_hi))); }
+                    else        { PSB_DISPATCH_N(c->nx, (e = launch_row_zm<N_, false>(c, W, psi0, src, cm, s, sigma, zero_lo, zero_hi))); }
+                }
+                else if (s == 0) { PSB_DISPATCH_N(c->nx, (e = launch_row<N_, true>(c, W, psi0, d_V, cm, s, sigma, zero_lo, zero_hi))); }
                 else if (row32 && c->nx == 512) e = launch_row32<512>(c, W, d_V, cm, s, sigma, zero_lo, zero_hi);
                 else if (row32 && c->nx == 1024) e = launch_row32<1024>(c, W, d_V, cm, s, sigma, zero_lo, zero_hi);
                 else        { PSB_DISPATCH_N(c->nx, (e = launch_row<N_, false>(c, W, psi0, d_V, cm, s, sigma, zero_lo, zero_hi))); }

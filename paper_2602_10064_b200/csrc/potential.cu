@@ -8,6 +8,7 @@
 //   k_v_col    Hermitian completion + two slices packed as re/im + inverse column FFT                (a3)
 //   k_v_row    inverse row FFT, unpack -> V[f][s][ny][nx] float32 (V*Angstrom)
 // Phases are formed as (m * U) mod 2^32 in integer arithmetic, so their error does not grow with |m|.
+#include <functional>
 #include <type_traits>
 
 #include "common.cuh"
@@ -471,15 +472,14 @@ extern "C" size_t ps_workspace_bytes(const ps_ctx* c, int n_frames_chunk, int n_
     return scratch_layout(c, n_frames_chunk, n_atoms).total;
 }
 
-extern "C" ps_status ps_build_slices(ps_ctx* c, const float* d_pos, const int32_t* d_Z, int n_frames, int n_atoms,
-                                     float* d_V, int32_t* d_slice_idx) {
-    if (!c) return PS_EINVAL;
-    if (!c->have_geom || !c->have_ff)
-        return fail(c, PS_ESTATE, "ps_build_slices: ps_set_geometry and ps_set_form_factors must be called first");
-    if (!d_pos || !d_Z || !d_V || n_frames < 1 || n_atoms < 1)
-        return fail(c, PS_EINVAL, "ps_build_slices: null pointer or non-positive size");
-    ps_status st = enter(c, "ps_build_slices");
-    if (st != PS_OK) return st;
+// Frame chunk by frame chunk: ingest, sort, V(k), y-inverse transform into the mixed array Zm.  Then either the
+// x-inverse transform into the caller's V (ps_build_slices) or `consume(f0, nf, Zm, offsets)` (ps_multislice_fused: the
+// slice loop of these frames takes the potential from Zm directly).
+typedef std::function<ps_status(int f0, int nf, const float2* Zm, const int32_t* off)> ZmConsumer;
+
+static ps_status build_chunks(ps_ctx* c, const float* d_pos, const int32_t* d_Z, int n_frames, int n_atoms, float* d_V,
+                              int32_t* d_slice_idx, const ZmConsumer* consume) {
+    ps_status st;
     if ((st = ensure_ftab(c)) != PS_OK) return st;
     const long long n_bins = (long long)c->n_slices * c->n_elem;
     if ((2 * n_bins + 2) * 4 > 200 * 1024)
@@ -600,11 +600,45 @@ extern "C" ps_status ps_build_slices(ps_ctx* c, const float* d_pos, const int32_
         PSB_DISPATCH_N(c->ny, (e = launch_v_col<N_>(c, Vk, off, Zm, nf))); }
         if (e != cudaSuccess) return fail(c, PS_ECUDA, std::string("k_v_col: ") + cudaGetErrorString(e));
         c->launches++;
-        e = cudaErrorInvalidValue;
-        { ProfScope ps_(c, K_V_ROW);
-        PSB_DISPATCH_N(c->nx, (e = launch_v_row<N_>(c, Zm, off, d_V + (size_t)f0 * c->n_slices * img, nf))); }
-        if (e != cudaSuccess) return fail(c, PS_ECUDA, std::string("k_v_row: ") + cudaGetErrorString(e));
-        c->launches++;
+        if (d_V) {
+            e = cudaErrorInvalidValue;
+            { ProfScope ps_(c, K_V_ROW);
+            PSB_DISPATCH_N(c->nx, (e = launch_v_row<N_>(c, Zm, off, d_V + (size_t)f0 * c->n_slices * img, nf))); }
+            if (e != cudaSuccess) return fail(c, PS_ECUDA, std::string("k_v_row: ") + cudaGetErrorString(e));
+            c->launches++;
+        }
+        if (consume && (st = (*consume)(f0, nf, Zm, off)) != PS_OK) return st;
     }
     return PS_OK;
+}
+
+extern "C" ps_status ps_build_slices(ps_ctx* c, const float* d_pos, const int32_t* d_Z, int n_frames, int n_atoms,
+                                     float* d_V, int32_t* d_slice_idx) {
+    if (!c) return PS_EINVAL;
+    if (!c->have_geom || !c->have_ff)
+        return fail(c, PS_ESTATE, "ps_build_slices: ps_set_geometry and ps_set_form_factors must be called first");
+    if (!d_pos || !d_Z || !d_V || n_frames < 1 || n_atoms < 1)
+        return fail(c, PS_EINVAL, "ps_build_slices: null pointer or non-positive size");
+    ps_status st = enter(c, "ps_build_slices");
+    if (st != PS_OK) return st;
+    return build_chunks(c, d_pos, d_Z, n_frames, n_atoms, d_V, d_slice_idx, nullptr);
+}
+
+extern "C" ps_status ps_multislice_fused(ps_ctx* c, double kV, const void* d_psi0, int n_probes, const float* d_pos,
+                                         const int32_t* d_Z, int n_frames, int n_atoms, void* d_exit, int exit_layout) {
+    if (!c) return PS_EINVAL;
+    if (!c->have_geom || !c->have_ff)
+        return fail(c, PS_ESTATE, "ps_multislice_fused: ps_set_geometry and ps_set_form_factors must be called first");
+    if (!d_psi0 || !d_pos || !d_Z || !d_exit || n_probes < 1 || n_frames < 1 || n_atoms < 1 || !(kV > 0.0))
+        return fail(c, PS_EINVAL, "ps_multislice_fused: null pointer or non-positive size / voltage");
+    if (exit_layout != PS_LAYOUT_DENSE)
+        return fail(c, PS_EUNSUPPORTED, "ps_multislice_fused: the wave is propagated in place inside d_exit: dense layout only");
+    ps_status st = enter(c, "ps_multislice_fused");
+    if (st != PS_OK) return st;
+    const ZmConsumer slice_loop = [&](int f0, int nf, const float2* Zm, const int32_t* off) -> ps_status {
+        VSrc src;
+        src.Zm = Zm; src.off = off; src.zm_f0 = f0;
+        return multislice_range(c, kV, d_psi0, n_probes, src, n_frames, f0, nf, d_exit, exit_layout);
+    };
+    return build_chunks(c, d_pos, d_Z, n_frames, n_atoms, nullptr, nullptr, &slice_loop);
 }

@@ -775,3 +775,45 @@ def test_tacaw_tiled_lengths(torch, F, n, P):
     mask[(kx ** 2 + ky ** 2) <= kc ** 2] = True
     Io = np.stack([O.tacaw_intensity(dn[p_] * mask[None]) for p_ in range(P)])
     assert rel_l2(I_t, Io) < TOL_I
+
+
+@pytest.mark.parametrize("name", ["c1_si_128", "c2_hbn_256", "c4_interface_1024", "c3_si_probe_512"])
+def test_multislice_fused_matches_build_then_multislice(torch, name):
+    """ps_multislice_fused (second half): positions -> exit waves with V built row by row inside the row
+    pass, against ps_build_slices + ps_multislice (same transforms: agreement far below the parity tolerance) and against
+    the oracle end to end; vacuum slices (config 2), several elements (config 4) and several probes (config 3) included;
+    a small workspace forces several frame chunks."""
+    import paper_2602_10064_b200 as ps
+    w = make_workload(name, mini=True)
+    ctx = make_ctx(w)
+    ctx.set_tuning("resident", -1)
+    F = 7
+    pos = w.positions(0, F)
+    pos_d, Z_d = _t(torch, pos), _t(torch, w.Z)
+    psi0 = gpu_incident(ctx, w)
+    V = ps.ps_build_slices(ctx, pos_d, Z_d)
+    ref = ps.ps_multislice(ctx, w.kV, psi0, V)
+    ws = torch.empty(ctx.workspace_bytes(3, pos.shape[1]) + 4096, dtype=torch.uint8, device="cuda")   # 3 frames per chunk
+    ctx.set_workspace(ws)
+    fused = ps.ps_multislice_fused(ctx, w.kV, psi0, pos_d, Z_d)
+    ctx.set_workspace(None)
+    assert rel_l2(fused.cpu().numpy(), ref.cpu().numpy()) < 2e-6
+    po = oracle_incident(w)
+    for f in (0, F - 1):
+        Vo, _ = oracle_potential(w, pos[f])
+        eo = O.multislice(po[-1], Vo, w.cell, w.kV)
+        assert rel_l2(fused[-1, f].cpu().numpy(), eo) < TOL_EXIT
+
+
+@pytest.mark.parametrize("grid", [512, 1024])
+def test_multislice_fused_large_grids(torch, grid):
+    """The fused row pass at the grid sizes of configs 3-5 (two shared-memory exchanges per transform), config 5 geometry
+    with 2 frames x 8 tilts: equal to ps_build_slices + ps_multislice (which test_gpu_full_size.py ties to the oracle)."""
+    import paper_2602_10064_b200 as ps
+    w = make_workload("c5_al_sweep", n_frames=32, grid=grid)
+    ctx = make_ctx(w)
+    pos_d, Z_d = _t(torch, w.positions(0, 2)), _t(torch, w.Z)
+    psi0 = gpu_incident(ctx, w)
+    ref = ps.ps_multislice(ctx, w.kV, psi0, ps.ps_build_slices(ctx, pos_d, Z_d))
+    fused = ps.ps_multislice_fused(ctx, w.kV, psi0, pos_d, Z_d)
+    assert rel_l2(fused.cpu().numpy(), ref.cpu().numpy()) < 2e-6
