@@ -118,12 +118,14 @@ PS_API ps_status ps_set_geometry(ps_ctx* ctx, const double cell[3], int nx, int 
 /* n_k_aperture = number of grid points with A(k) = 1.  Any out pointer may be NULL. */
 PS_API ps_status ps_get_geometry(const ps_ctx* ctx, int* n_slices, double* dz_eff, int* n_k_aperture);
 
-/* Scratch needed by ps_build_slices on `n_frames_chunk` frames of `n_atoms` atoms at a time (the
- * only call that needs scratch: fixed-point coordinates and sort keys, 5 x 4 B per atom-frame,
- * plus V(k) and the mixed array of the inverse transform, which depend on the geometry alone).
+/* Scratch needed by ps_build_slices / ps_multislice_fused on `n_frames_chunk` frames of `n_atoms` atoms at
+ * a time (fixed-point coordinates and sort keys, 5 x 4 B per atom-frame, plus V(k) and the mixed
+ * array of the inverse transform, which depend on the geometry alone).  The only other user of
+ * scratch is ps_multislice with PS_LAYOUT_TILED_APERTURE, whose dense work array takes nx*ny*8
+ * bytes per wave of a chunk (it uses whatever the workspace or the library-owned buffer holds).
  * NOTE: SURVEY.md 8(b) sketched the second argument as `n_probes_chunk`; the probe count does not
- * enter any scratch size here (ps_multislice propagates in place inside d_exit and needs none),
- * while the atom count does, so the argument is `n_atoms`.  Returns 0 before geometry and form
+ * enter the scratch of the potential build (and ps_multislice with the dense layout propagates in
+ * place inside d_exit and needs none), while the atom count does, so the argument is `n_atoms`.  Returns 0 before geometry and form
  * factors are set.  ps_set_workspace installs caller-owned device memory (d_ws == NULL removes
  * it and returns the ctx to self-allocation).  ps_build_slices processes frames in chunks that
  * fit whatever scratch is available. */
