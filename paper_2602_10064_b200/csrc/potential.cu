@@ -242,13 +242,18 @@ template <int NY> struct VColCfg {
     static constexpr int T = Plan<NY>::T;
     static constexpr int C = (NY <= 1024) ? 8 : 4;
     static constexpr int THREADS = C * T;
+    // up to 1024: 1024 threads per SM at 64 registers — the gather is latency-bound, and twice the warps of the
+    // 128-register build cover more of it (measured per 64 frames: 512^2 2.07 -> 1.96 ms, 1024^2 12.1 -> 9.8 ms; at
+    // 2048^2 the 64-register build spills 144 bytes and loses, 19.3 -> 21.6 ms, so it keeps 512 threads per SM)
+    static constexpr int PER_SM = (NY <= 1024) ? 1024 : 512;
+    static constexpr int MIN_BLOCKS = (THREADS >= PER_SM) ? 1 : (PER_SM / THREADS > 4 ? 4 : PER_SM / THREADS);
     static constexpr size_t SMEM = (size_t)NY * C * sizeof(float2);
 };
 
 // reads the half-plane box of Va (slice 2*pr) and Vb (slice 2*pr+1), forms z = Va + i Vb on the full
 // plane by Hermitian symmetry, inverse-transforms along y, writes the mixed array Zm[f][pr][y][kx].
 template <int NY>
-__global__ void __launch_bounds__(VColCfg<NY>::THREADS)
+__global__ void __launch_bounds__(VColCfg<NY>::THREADS, VColCfg<NY>::MIN_BLOCKS)
 k_v_col(const float2* __restrict__ Vk, const int32_t* __restrict__ offsets, float2* __restrict__ Zm, const int nx,
         const int32_t* __restrict__ tiles, const int n_tiles, const int32_t* __restrict__ nmax, const int n_slices,
         const int n_elem, const int mcut, const int ncut, const int n_pairs, const int n_items) {
