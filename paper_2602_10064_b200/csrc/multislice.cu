@@ -17,10 +17,6 @@
 #include "tma.cuh"
 #include <type_traits>
 
-#ifndef PSB_ROW_VLATE
-#define PSB_ROW_VLATE 1
-#endif
-
 namespace psb {
 
 // ------------------------------------------------------------------------------------ row pass
@@ -137,7 +133,7 @@ k_row_transmit(float2* __restrict__ W, const float2* __restrict__ psi0, const fl
         // Where V is fetched: with the wave (NX <= 256: everything fits in registers) or after the inverse transform
         // (NX >= 512: sixteen more live registers across the inverse transform would be spilled to local memory; the
         // row was pulled into L2 by the previous item's prefetch, so the load is an L2 hit the other warps cover)
-        constexpr bool V_LATE = (PSB_ROW_VLATE != 0) && !FIRST && !VAC && NX >= 512;
+        constexpr bool V_LATE = !FIRST && !VAC && NX >= 512;
         if (!V_LATE) {
 #pragma unroll
             for (int e = 0; e < 16; ++e) sv[e] = valid ? __ldg(vrow + e * T) : 0.f;
@@ -281,10 +277,7 @@ template <int NX> struct RowCfg32 {
     static constexpr int T = Plan32<NX>::T;
     static constexpr int THREADS = 128;
     static constexpr int RPB = THREADS / T;
-#ifndef PSB_ROW32_BLOCKS
-#define PSB_ROW32_BLOCKS 3
-#endif
-    static constexpr int MIN_BLOCKS = PSB_ROW32_BLOCKS;
+    static constexpr int MIN_BLOCKS = 3;                                  // 168 registers; 2 and 4 blocks measured slower
     static constexpr size_t SMEM = (size_t)RPB * RowLine32<NX>::LEN * sizeof(float2);
 };
 
@@ -362,21 +355,17 @@ k_row_transmit32(float2* __restrict__ W, const float* __restrict__ V, const Chun
 // exchanges per transform at NY >= 512.  E = 32 (NY = 512, 1024): NY/32 threads per column, ONE exchange; blocks are
 // half as large (128 threads, 168 registers), three of them per SM with a 2-stage ring.  The pass is bound by the LSU
 // data pipe, which every element crosses 10 (E = 16) or 6 (E = 32) times per transform pair (profiles/r2_slice_step.md).
-#ifndef PSB_COL32_NS
-#define PSB_COL32_NS 2
-#endif
-#ifndef PSB_COL32_BLOCKS
-#define PSB_COL32_BLOCKS 3
-#endif
 template <int NY, int E> struct ColCfg {
     static_assert(E == 16 || (E == 32 && (NY == 512 || NY == 1024)), "32 values per thread: NY = 512 or 1024");
     static constexpr int T = NY / E;
     static constexpr int C = (E == 32) ? ((NY <= 512) ? 8 : 4) : ((NY <= 1024) ? 8 : 4);   // columns per block
     static constexpr int THREADS = C * T;
-    static constexpr int NS = (E == 32) ? PSB_COL32_NS : 3;               // pipeline stages
+    static constexpr int NS = (E == 32) ? 2 : 3;                          // pipeline stages
     static constexpr int BOX_R = (NY < 256) ? NY : 256;                   // TMA box rows (<= 256)
     static constexpr int NBOX = NY / BOX_R;
-    static constexpr int MIN_BLOCKS = (E == 32) ? PSB_COL32_BLOCKS : (THREADS <= 256) ? 2 : 1;   // E = 16: cap registers at 128
+    // E = 32: three blocks at 168 registers (two blocks x three stages at 218 registers measured 8 % slower);
+    // E = 16: cap registers at 128
+    static constexpr int MIN_BLOCKS = (E == 32) ? 3 : (THREADS <= 256) ? 2 : 1;
     static constexpr uint32_t STAGE_BYTES = (uint32_t)NY * C * sizeof(float2);
     static constexpr size_t SMEM = (size_t)NS * STAGE_BYTES + (size_t)NY * sizeof(float2) + NS * sizeof(uint64_t) + 128;
 };

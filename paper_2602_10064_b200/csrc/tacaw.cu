@@ -14,20 +14,13 @@
 
 namespace psb {
 
-#ifndef PSB_TACAW_TILED_RING
-#define PSB_TACAW_TILED_RING 1
-#endif
-#ifndef PSB_TACAW_C512
-#define PSB_TACAW_C512 16
-#endif
-#ifndef PSB_TACAW_C1024
-#define PSB_TACAW_C1024 8
-#endif
 // TILED: the exit waves come in PS_LAYOUT_TILED_APERTURE, [P][ny][tile][F][8 kx]: a pixel group must lie inside one
 // 8-column tile (C <= 8), and its F frames are one contiguous run of F * 64 bytes.
 template <int NF, bool TILED = false> struct TacawCfg {
     static constexpr int T = Plan<NF>::T;
-    static constexpr int C0 = (NF < 512) ? 16 : (NF == 512) ? PSB_TACAW_C512 : ((NF == 1024) ? PSB_TACAW_C1024 : 4);
+    // pixels per group: narrower groups would allow two resident blocks at 512 / 1024 frames but read 32-byte pieces:
+    // measured 0.39 -> 0.16 of the HBM roofline at 1024 frames (profiles/r2_tacaw.md)
+    static constexpr int C0 = (NF <= 512) ? 16 : ((NF == 1024) ? 8 : 4);
     static constexpr int C = (TILED && C0 > kColTile) ? kColTile : C0;
     static constexpr int THREADS = C * T;
     static constexpr size_t SMEM = (size_t)NF * C * sizeof(float2);
@@ -448,7 +441,9 @@ extern "C" ps_status ps_tacaw(ps_ctx* c, const void* d_exit, int exit_layout, in
     // Kernel choice measured on B200 (profiles/r1_tacaw_kernels.md): the TMA-staged ring wins where one block per
     // SM is all that fits anyway (2048 frames) and where few bins are written (reads dominate, 512-1024 frames);
     // the register-staged kernel with several resident blocks wins for short stacks and when every bin is written.
-    const bool use_ring = tiled ? (PSB_TACAW_TILED_RING != 0 && n_frames <= 2048)
+    // tiled layout: the ring kernel at every length it covers (register-staged on the tiled layout measured 0.44 against
+    // 0.65 at 1024 frames); dense layout: measured choice per shape (profiles/r1_tacaw_kernels.md)
+    const bool use_ring = tiled ? (n_frames <= 2048)
                                 : (n_frames == 2048 || ((n_frames == 512 || n_frames == 1024) && 4 * n_bins <= n_frames));
 #define PSB_TACAW_CASE(NFV)                                                                                         \
     case NFV:                                                                                                       \
