@@ -400,6 +400,8 @@ def main():
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
                     help="N > 1: weak = an independent trajectory per rank (reductions averaged); strong = ONE problem "
                          "sharded by sharding.plan() (probe shards, or frame shards + reduce-scatter of the accumulators)")
+    ap.add_argument("--vk-mode", type=int, default=0, choices=[0, 1, 2],
+                    help="ps_set_vk_mode: 0 library default, 1 FP32 SIMT structure-factor sums, 2 tcgen05 3xTF32")
     ap.add_argument("--fused-v", action="store_true",
                     help="positions -> exit waves through ps_multislice_fused (the row pass builds V row by row from the "
                          "y-transformed slice pairs; no V array; dense exit layout) instead of ps_build_slices + ps_multislice")
@@ -478,6 +480,8 @@ def main():
         raise SystemExit(f"workload needs {need / 1e9:.0f} GB of HBM (V + exit waves + I), {free_b / 1e9:.0f} GB free")
     if args.wave_chunk:
         ctx.set_wave_chunk(args.wave_chunk)
+    if args.vk_mode:
+        ctx.set_vk_mode(args.vk_mode)
     for kv in args.tune:
         k, v = kv.split("=")
         ctx.set_tuning(k, int(v))
