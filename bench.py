@@ -291,6 +291,43 @@ def tacaw_micro(shapes_a=None, shapes_b=None):
         del ex, ts, ctx
 
 
+# --------------------------------------------------------------------------------------------- cuFFT reference point
+def cufft_reference(w, n_waves, n_slices=8):
+    """The slice step written with library calls (north_star: "cuFFT timed only as a reference point"): torch.exp for
+    the transmission function, torch.fft.fft2 / ifft2 (cuFFT) and elementwise products, on `n_waves` random waves of the
+    workload's grid.  Not part of the library and never linked into it: a yardstick for the fused passes."""
+    import torch
+    nx, ny = w.nx, w.ny
+    dev = torch.device("cuda")
+    psi = torch.view_as_complex(torch.randn((n_waves, ny, nx, 2), device=dev))
+    V = torch.randn((n_slices, ny, nx), device=dev)
+    kx = torch.fft.fftfreq(nx, d=w.cell[0] / nx, device=dev)[None, :]
+    ky = torch.fft.fftfreq(ny, d=w.cell[1] / ny, device=dev)[:, None]
+    k2 = kx * kx + ky * ky
+    kc = (2.0 / 3.0) * min(nx / (2 * w.cell[0]), ny / (2 * w.cell[1]))
+    prop = (torch.polar(torch.ones_like(k2), -3.14159265 * 0.037 * 1.36 * k2) * (k2 <= kc * kc)).to(torch.complex64)
+
+    def one_slice(s):
+        nonlocal psi
+        t = torch.polar(torch.ones_like(V[s]), 9.24e-4 * V[s])
+        psi = torch.fft.ifft2(torch.fft.fft2(psi * t) * prop)
+
+    for s in range(3):
+        one_slice(s % n_slices)
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    a.record()
+    for s in range(n_slices):
+        one_slice(s)
+    b.record()
+    torch.cuda.synchronize()
+    ms = a.elapsed_time(b) / n_slices
+    out = {"reference": "cuFFT slice step (torch.fft.fft2/ifft2 + elementwise kernels; no band-limit pruning, no fusion)",
+           "grid": [nx, ny], "waves": n_waves, "ms_per_slice": ms, "gpx_slice_s": nx * ny * n_waves / ms / 1e6}
+    print(json.dumps(out))
+    return out
+
+
 # --------------------------------------------------------------------------------------------- configs 3 / 4 at full size
 def full_config(which, quiet=False, fused_v=False):
     """Config 4: 4096 frames x 1024^2 x 120 slices, V built and propagated 64 frames at a time, exit waves folded into the
@@ -412,6 +449,9 @@ def main():
     ap.add_argument("--full-config", choices=["c3", "c4"], default=None,
                     help="run config 3 or 4 at its FULL size (all frames, all probes) in chunks that fit 180 GB, one step, "
                          "and print one JSON line")
+    ap.add_argument("--cufft-reference", action="store_true",
+                    help="time the slice step written with torch.fft (cuFFT) + elementwise kernels on 1024 waves (or as many "
+                         "as fit 2 GB) of the workload's grid and exit: a reference point, not part of the library")
     ap.add_argument("--tacaw-micro", action="store_true",
                     help="time ps_tacaw / ps_tacaw_add alone on synthetic stacks of several shapes and exit")
     ap.add_argument("--micro-a", action="append", default=None, metavar="P,FRAMES,GRID,BINS[,TILED]",
@@ -427,6 +467,9 @@ def main():
 
     if args.impl == "reference":
         run_reference(args, w, rank)
+        return
+    if args.cufft_reference:
+        cufft_reference(w, max(1, min(1024, (2 << 30) // (w.nx * w.ny * 8))))
         return
     if args.tacaw_micro:
         parse = lambda xs: None if xs is None else [tuple(int(v) for v in x.split(",")) for x in xs]
