@@ -325,6 +325,24 @@ def cufft_reference(w, n_waves, n_slices=8):
     out = {"reference": "cuFFT slice step (torch.fft.fft2/ifft2 + elementwise kernels; no band-limit pruning, no fusion)",
            "grid": [nx, ny], "waves": n_waves, "ms_per_slice": ms, "gpx_slice_s": nx * ny * n_waves / ms / 1e6}
     print(json.dumps(out))
+    # the time transform with cuFFT: fft along the frame axis of a dense [P][F][ny][nx] stack, then |.|^2
+    P, F = 4, min(w.n_frames, 1024)
+    while P > 1 and P * F * ny * nx * 8 > (10 << 30):
+        P //= 2
+    ex = torch.view_as_complex(torch.randn((P, F, ny, nx, 2), device=dev))
+    for _ in range(2):
+        I = torch.fft.fft(ex - ex.mean(dim=1, keepdim=True), dim=1).abs().square()
+    torch.cuda.synchronize()
+    a.record()
+    I = torch.fft.fft(ex - ex.mean(dim=1, keepdim=True), dim=1).abs().square()
+    b.record()
+    torch.cuda.synchronize()
+    ms_t = a.elapsed_time(b)
+    byts = (8.0 * F + 4.0 * F) * P * nx * ny
+    peak, _, _ = measured_peaks()
+    out_t = {"reference": "cuFFT time transform (mean removal, torch.fft.fft over the frame axis of the dense stack, |.|^2; all pixels)",
+             "P": P, "frames": F, "grid": [nx, ny], "ms": ms_t, "frac_of_hbm_peak_on_its_own_bytes": byts / ms_t / 1e6 / peak}
+    print(json.dumps(out_t))
     return out
 
 
