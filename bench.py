@@ -463,7 +463,9 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--with-full-configs", action="store_true",
                     help="also run configs 3 and 4 at their FULL size after the timed steps and carry their end-to-end "
-                         "seconds in the same JSON line (adds about two minutes)")
+                         "seconds in the same JSON line (adds about two minutes); on by default for the default workload "
+                         "on one GPU")
+    ap.add_argument("--no-full-configs", action="store_true", help="skip the full-size runs of configs 3 and 4")
     ap.add_argument("--full-config", choices=["c3", "c4"], default=None,
                     help="run config 3 or 4 at its FULL size (all frames, all probes) in chunks that fit 180 GB, one step, "
                          "and print one JSON line")
@@ -746,10 +748,18 @@ def main():
 
     cube_gb = I.numel() * 4 / 1e9
     full = None
-    if rank == 0 and world == 1 and args.with_full_configs:
+    is_default = (args.workload == "c3_si_probe_512" and not (args.frames or args.grid or args.probes_side) and
+                  args.probe_chunk == 16 and not args.fused_v and not args.tune and not args.wave_chunk)
+    if rank == 0 and world == 1 and (args.with_full_configs or (is_default and not args.no_full_configs)):
         del V, exitw, I, psi0
         torch.cuda.empty_cache()
-        full = {k: full_config(k, quiet=True) for k in ("c3", "c4")}
+        full = {}
+        for k in ("c3", "c4"):                                   # never lose the main line to a failure here
+            try:
+                full[k] = full_config(k, quiet=True)
+            except Exception as exc:                             # noqa: BLE001
+                full[k] = {"error": f"{type(exc).__name__}: {exc}"[:300]}
+                torch.cuda.empty_cache()
 
     if rank == 0:
         line = {
