@@ -753,13 +753,19 @@ def main():
     if rank == 0 and world == 1 and (args.with_full_configs or (is_default and not args.no_full_configs)):
         del V, exitw, I, psi0
         torch.cuda.empty_cache()
+        ctx = None                                               # this process keeps only its CUDA context
+        torch.cuda.empty_cache()
         full = {}
-        for k in ("c3", "c4"):                                   # never lose the main line to a failure here
+        import subprocess
+        for k in ("c3", "c4"):                                   # a child process each: a failure there cannot take the main line along
             try:
-                full[k] = full_config(k, quiet=True)
+                res = subprocess.run([sys.executable, os.path.abspath(__file__), "--full-config", k], capture_output=True,
+                                     text=True, timeout=1500)
+                last = [ln for ln in res.stdout.strip().splitlines() if ln.startswith("{")]
+                full[k] = json.loads(last[-1]) if (res.returncode == 0 and last) else {
+                    "error": f"exit code {res.returncode}: {res.stderr.strip()[-300:]}"}
             except Exception as exc:                             # noqa: BLE001
                 full[k] = {"error": f"{type(exc).__name__}: {exc}"[:300]}
-                torch.cuda.empty_cache()
 
     if rank == 0:
         line = {
