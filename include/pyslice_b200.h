@@ -265,6 +265,24 @@ PS_API ps_status ps_sdp(ps_ctx* ctx, const float* d_I, int P, int n_bins, int bi
  * no outer limit) of I[p][b][k] -> float32 [P][n_bins]. */
 PS_API ps_status ps_spectrum_image(ps_ctx* ctx, const float* d_I, int P, int n_bins, double k_in, double k_out,
                             float* d_out);
+/* ps_spectrum_image_static: same arguments, same result as ps_spectrum_image (A16), for callers that
+ * cannot let the library allocate: a process that has handed all free HBM to its own pool at start-up (a cudaMalloc
+ * made by the library then fails), or a latency-bound loop that cannot take the device-wide stall of cudaMalloc /
+ * cudaFree.  ps_spectrum_image keeps its one-byte-per-pixel detector mask in a ctx buffer from cudaMalloc; this
+ * variant keeps it in a fixed 1 MiB array inside the library image and calls no allocator, ever.
+ *   - Cost: every GPU that loads the library holds those ps_static_scratch_bytes() bytes until the process exits.
+ *   - Limit: nx * ny <= ps_static_scratch_bytes() (1024 x 1024 pixels); larger grids return PS_EUNSUPPORTED with a
+ *     message and launch nothing.
+ *   - One array per device, shared by all ctxs and streams: calls that can overlap on the GPU race on it (wrong
+ *     results, no error).  Keep them in one stream or order them yourself.  The array keeps the previous call's
+ *     bytes; each call rewrites every byte it later reads, so no clearing is needed or done.
+ *   - The first call on a device looks up the array's device address (cudaGetSymbolAddress, once per device, with
+ *     that device current) and may trigger module loading: make that first call before any stream capture begins.
+ * d_I and d_out are caller-owned device memory as for ps_spectrum_image; asynchronous on the ctx stream. */
+PS_API ps_status ps_spectrum_image_static(ps_ctx* ctx, const float* d_I, int P, int n_bins, double k_in, double k_out,
+                                   float* d_out);
+/* size in bytes (= pixels) of the built-in scratch array used by ps_spectrum_image_static */
+PS_API size_t ps_static_scratch_bytes(void);
 /* ps_haadf: annular detector on the k-space exit waves,
  *   d_out[p] = (1/F) sum_f sum_{k_in <= |k| < k_out} |Psi_pf(k)|^2 / (nx ny)      (k_out <= 0: no outer limit)
  * = fraction of the incident intensity on the detector, averaged over frames -> float32 [n_probes].

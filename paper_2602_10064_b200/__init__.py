@@ -8,5 +8,5 @@ without the built library or without a CUDA device raises.
 """
 from .binding import (Context, PSError, library_path, load_library, exported_symbols,  # noqa: F401
                       ps_build_slices, ps_make_incident, ps_multislice, ps_tacaw, ps_sdp,
-                      ps_spectrum_image, ps_dispersion, ps_qbin, ps_haadf, ps_accumulate_intensity,
+                      ps_spectrum_image, ps_spectrum_image_static, static_scratch_bytes, ps_dispersion, ps_qbin, ps_haadf, ps_accumulate_intensity,
                       ps_exit_to_dense, ps_multislice_fused, exit_shape, PS_LAYOUT_DENSE, PS_LAYOUT_TILED_APERTURE)

@@ -51,6 +51,8 @@ _PROTOTYPES = {
     "ps_tacaw_finish_shard": (C.c_int, [C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]),
     "ps_sdp": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_void_p]),
     "ps_spectrum_image": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_double, C.c_double, C.c_void_p]),
+    "ps_spectrum_image_static": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_double, C.c_double, C.c_void_p]),
+    "ps_static_scratch_bytes": (C.c_size_t, []),
     "ps_haadf": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_void_p]),
     "ps_accumulate_intensity": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t, C.c_double, C.c_double]),
     "ps_dispersion": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
@@ -388,6 +390,27 @@ def ps_spectrum_image(ctx: Context, d_I, k_in: float = 0.0, k_out: float = 0.0, 
         d_out = torch.empty((P, nb), dtype=torch.float32, device=ctx.device)
     ctx._check(ctx._lib.ps_spectrum_image(ctx._h, _ptr(d_I), P, nb, float(k_in), float(k_out), _ptr(d_out)))
     return d_out
+
+
+def ps_spectrum_image_static(ctx: Context, d_I, d_out, k_in: float = 0.0, k_out: float = 0.0):
+    """`ps_spectrum_image` for callers that must not allocate device memory: a process whose pool already owns all of
+    HBM, or a loop that cannot take the device-wide stall of cudaMalloc.  The detector mask sits in a 1 MiB array built
+    into the library (grids up to 1024 x 1024; larger ones raise PSError with PS_EUNSUPPORTED), so neither the library
+    nor this wrapper allocates: `d_out` (float32 [P][n_bins]) is therefore a required argument, not an optional one.
+    The array is shared by every context on the device: do not let two of these calls overlap on the GPU.  Make the
+    first call on a device outside any stream capture (it looks up the array's address)."""
+    import torch
+    _need(d_I, torch.float32, "d_I"); _need(d_out, torch.float32, "d_out")
+    P, nb = int(d_I.shape[0]), int(d_I.shape[1])
+    if tuple(d_out.shape) != (P, nb):
+        raise ValueError(f"d_out must have shape ({P}, {nb})")
+    ctx._check(ctx._lib.ps_spectrum_image_static(ctx._h, _ptr(d_I), P, nb, float(k_in), float(k_out), _ptr(d_out)))
+    return d_out
+
+
+def static_scratch_bytes() -> int:
+    """Bytes (= pixels) of the built-in scratch array behind `ps_spectrum_image_static`."""
+    return int(load_library().ps_static_scratch_bytes())
 
 
 def ps_haadf(ctx: Context, d_exit, k_in: float, k_out: float = 0.0, d_out=None):

@@ -18,7 +18,8 @@ CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 BUILD = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libpyslice_b200.so")
-SOURCES = ("api.cu", "potential.cu", "vk_tc.cu", "incident.cu", "multislice.cu", "resident.cu", "tacaw.cu", "reduce.cu")
+SOURCES = ("api.cu", "potential.cu", "vk_tc.cu", "incident.cu", "multislice.cu", "resident.cu", "tacaw.cu", "reduce.cu",
+           "static_scratch.cu")
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "-I", INCLUDE]
 
