@@ -511,6 +511,28 @@ def test_aberration_function_against_propagator_and_textbook():
     assert np.allclose(np.abs(O.apply_aberrations(W, cell, kV, full)), np.abs(W), rtol=1e-12)
 
 
+def test_apply_aberrations_sign_tied_to_propagator_and_probe_formation():
+    """PAPER.md:143 (§4 "applied either during probe formation or post-hoc to stored wavefunctions"): the post-hoc route
+    must carry the same sign as the other two pinned objects.  (i) pure C10 = 37.5 A applied post-hoc to the k-space of
+    the focused probe equals that probe sent through 37.5 A of vacuum by the propagator (pinned by P5/P7: exp(-i pi
+    lambda dz k^2)) — the probe is band-limited, so the propagator's aperture changes nothing; (ii) for a full set of
+    coefficients, post-hoc application to the unaberrated probe's k-space equals the k-space of the probe formed with
+    those aberrations.  exp(+i chi) in apply_aberrations fails both."""
+    cell = np.array([14.0, 11.0, 5.0]); nx, ny = 64, 48; kV = 100.0
+    p0 = O.probe_wave(cell, nx, ny, kV, 25.0, 3.0, 4.0)
+    c = np.zeros(8); c[0] = 37.5
+    post_hoc = np.fft.ifft2(O.apply_aberrations(np.fft.fft2(p0), cell, kV, c))
+    via_prop = O.multislice(p0, np.zeros((1, ny, nx)), np.array([cell[0], cell[1], 37.5]), kV, return_real_space=True)
+    assert rel_l2(post_hoc, via_prop) < 1e-12
+    wrong_sign = np.fft.ifft2(np.fft.fft2(p0) * np.exp(+1j * O.aberration_function(cell, nx, ny, kV, c)))
+    assert rel_l2(wrong_sign, via_prop) > 0.1                         # the check can tell the two signs apart
+    full = np.array([30.0, 20.0, 0.4, 500.0, 1.0, 300.0, -0.7, 2.0e5])
+    formed = O.probe_wave(cell, nx, ny, kV, 25.0, 3.0, 4.0, aberrations=full)
+    assert rel_l2(O.apply_aberrations(np.fft.fft2(p0), cell, kV, full), np.fft.fft2(formed)) < 1e-12
+    stack = np.stack([np.fft.fft2(p0), 2.0 * np.fft.fft2(p0)])        # leading axes are carried along
+    assert rel_l2(O.apply_aberrations(stack, cell, kV, full)[1], 2.0 * np.fft.fft2(formed)) < 1e-12
+
+
 def test_aberration_function_hand_evaluated_C12_C21_C23():
     """Pins the 1/2, 1/3 prefactors and the cos 2(phi-phi12), cos(phi-phi21), cos 3(phi-phi23) factors of reading A24
     (PAPER.md:143 "standard aberration function supporting defocus, astigmatism, coma, spherical aberration"): chi is
