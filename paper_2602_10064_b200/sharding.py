@@ -77,8 +77,9 @@ def max_over_ranks(x: float, device=None, group=None) -> float:
 # collectives below are exactly what `bench.py --scaling strong` runs.
 def reduce_scatter_sum(t, group=None):
     """t: [world][...] on every rank -> the sum over ranks of slice [rank] (complex goes through its real view).
-    NCCL: one reduce_scatter_tensor.  Backends without reduce-scatter (gloo, used by the CPU test) fall back to an
-    all-reduce followed by the slice: same result, more traffic."""
+    NCCL: one reduce_scatter_tensor.  Other backends (gloo, used by the CPU test, has no reduce-scatter) use an
+    all-reduce followed by the slice: same result, more traffic.  The choice is made by backend name, never by catching
+    an error, so a real NCCL failure is not turned into world x the traffic."""
     import torch
     import torch.distributed as dist
     world, rank = dist.get_world_size(group), dist.get_rank(group)
@@ -86,9 +87,9 @@ def reduce_scatter_sum(t, group=None):
     v = torch.view_as_real(t) if t.is_complex() else t
     v = v.contiguous()
     out = torch.empty(v.shape[1:], dtype=v.dtype, device=v.device)
-    try:
-        dist.reduce_scatter_tensor(out, v, op=dist.ReduceOp.SUM, group=group)
-    except (RuntimeError, NotImplementedError):
+    if dist.get_backend(group) == "nccl":
+        dist.reduce_scatter_tensor(out, v, op=dist.ReduceOp.SUM, group=group)   # a failure here is a failure: it propagates
+    else:
         dist.all_reduce(v, op=dist.ReduceOp.SUM, group=group)
         out.copy_(v[rank])
     return torch.view_as_complex(out) if t.is_complex() else out
