@@ -116,6 +116,84 @@ def test_c3_full_grid_probe_chunk(torch):
     _check_tacaw_sample(torch, ps, ctx, w, ex, I, None, 1024, 31)
 
 
+def test_c3_bench_shape(torch):
+    """The step bench.py times by default, unchanged: config 3's own 10 240 atoms, 512^2, 80 slices, ALL 1024 frames x one
+    16-probe scan row, exit waves in PS_LAYOUT_TILED_APERTURE (several work-array chunks per call, library-default
+    chunking), k_tacaw_tma<1024, tiled> over all 1024 bins, then the spectrum image.  127 GB resident, ~2 s of GPU time.
+      (a) V from positions on 2 frames x 3 slices; slice binning of those frames bit-exact;
+      (b) exit waves of 4 (probe, frame) pairs spread over the work-array chunks against the oracle's slice loop;
+      (c) I(k, w) at 1024 seeded in-band pixels x all 1024 bins against the oracle transform of the same exit-wave
+          columns, as a whole and bin by bin (weak bins get the fp32 floor of a length-F transform, eps log2(F) times
+          the strongest line's amplitude, the elastic one included: DESIGN.md §7); out-of-band pixels exactly zero;
+      (d) Parseval over the whole cube (pin P11, holds at any size): sum_{k, n} I = F sum_{k, t} |Psi - <Psi>_t|^2 per
+          probe, the left side taken from ps_spectrum_image over all k — the number bench.py --full-config c3 prints as
+          its checksum is the sum of exactly these."""
+    import paper_2602_10064_b200 as ps
+    w = make_workload("c3_si_probe_512")
+    w.probe_xy = w.probe_xy[:16]
+    F, S, nx, ny = w.n_frames, w.n_slices, w.nx, w.ny
+    assert (F, S, nx, ny, w.n_atoms) == (1024, 80, 512, 512, 10240)
+    ctx = make_ctx(w)
+    pos = w.positions()
+    V = torch.empty((F, S, ny, nx), dtype=torch.float32, device="cuda")
+    sidx = torch.empty((F, w.n_atoms), dtype=torch.int32, device="cuda")
+    ps.ps_build_slices(ctx, _t(torch, pos), _t(torch, w.Z), d_V=V, d_slice_idx=sidx)
+    psi0 = gpu_incident(ctx, w)
+    ex = ps.ps_multislice(ctx, w.kV, psi0, V, layout=ps.PS_LAYOUT_TILED_APERTURE)
+    I = ps.ps_tacaw(ctx, ex, w.dt_fs)
+    simg = ps.ps_spectrum_image(ctx, I)
+    ctx.check_async()
+    assert tuple(I.shape) == (16, F, ny, nx)
+
+    # (a)
+    for f in (205, 1023):
+        Vo, so = oracle_potential(w, pos[f], slices=(0, 41, 79))
+        assert np.array_equal(sidx[f].cpu().numpy(), so), "slice binning must be bit-exact"
+        Vg = V[f].cpu().numpy()
+        for s in (0, 41, 79):
+            assert rel_l2(Vg[s], Vo[s]) < TOL_V
+
+    # (b), (d): one probe at a time through the dense view (2.1 GB)
+    po = oracle_incident(w)
+    pairs = {0: (0,), 5: (205,), 10: (613,), 15: (1023,)}
+    A = O.aperture_mask(w.cell, nx, ny)
+    iy, ix = np.nonzero(A)
+    sel = np.random.default_rng(1024).choice(iy.size, size=1024, replace=False)
+    sy, sx = torch.as_tensor(iy[sel]).cuda(), torch.as_tensor(ix[sel]).cuda()
+    eps32 = float(np.finfo(np.float32).eps)
+    dense = torch.empty((1, F, ny, nx), dtype=torch.complex64, device="cuda")
+    for p in range(16):
+        ps.ps_exit_to_dense(ctx, ex[p:p + 1], d_dense=dense)
+        for fr in pairs.get(p, ()):
+            eo = O.multislice(po[p], V[fr].cpu().numpy().astype(np.float64), w.cell, w.kV)
+            assert rel_l2(dense[0, fr].cpu().numpy(), eo) < TOL_EXIT, (p, fr)
+        # (c)
+        cols = dense[0][:, sy, sx].cpu().numpy().astype(np.complex128)            # [F][1024]
+        Io = O.tacaw_intensity(cols, None)
+        Ig = I[p][:, sy, sx].cpu().numpy().astype(np.float64)
+        assert rel_l2(Ig, Io) < TOL_I, p
+        # amplitude floor of the fp32 transform: eps log2(F) x the strongest line it carries, the elastic one (F <Psi>_t,
+        # removed by the mean subtraction only up to rounding) included
+        strongest = max(Io.mean(axis=1).max(), float(np.mean(np.abs(cols.sum(axis=0)) ** 2)))
+        floor = eps32 * np.log2(F) * np.sqrt(strongest)
+        for b in range(F):
+            allowed = TOL_I * np.linalg.norm(Io[b]) + np.linalg.norm(2.0 * np.sqrt(Io[b]) * floor + floor ** 2)
+            assert np.linalg.norm(Ig[b] - Io[b]) <= allowed, (p, b)
+        # (d)
+        if p in pairs:
+            tot = 0.0
+            for y0 in range(0, ny, 64):
+                blk = dense[0, :, y0:y0 + 64].to(torch.complex128)
+                blk = blk - blk.mean(dim=0, keepdim=True)
+                tot += float((blk.real ** 2 + blk.imag ** 2).sum())
+            assert abs(float(simg[p].double().sum()) - F * tot) < TOL_I * F * tot, p
+    out = torch.as_tensor(~A).cuda()
+    for p in range(16):
+        assert float(I[p][:, out].abs().max()) == 0.0, "I outside the band limit must be exactly zero"
+    del V, ex, I, dense
+    torch.cuda.empty_cache()
+
+
 def test_c4_full_grid_streaming_bins(torch):
     """Config 4 geometry (48 600 atoms, 1024^2, 120 slices, 200 kV), 32 frames; path B (streaming per-bin DFT, two
     chunks) against the oracle and against path A."""
