@@ -402,6 +402,15 @@ static ps_status launch_tacaw_tma(ps_ctx* c, const float2* exitw, float* I, cons
     return PS_OK;
 }
 
+// ref[p][q] = chunk[p][frame 0][q]: the default reference wave of a stream (first frame of every probe)
+__global__ void k_tacaw_first_frame(const float4* __restrict__ chunk, float4* __restrict__ ref, const size_t q_per_probe,
+                                    const size_t probe_stride, const size_t total) {
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+        const size_t p = i / q_per_probe, q = i - p * q_per_probe;
+        ref[i] = chunk[p * probe_stride + q];
+    }
+}
+
 }  // namespace psb
 
 using namespace psb;
@@ -528,8 +537,15 @@ extern "C" ps_status ps_tacaw_add(ps_ctx* c, const void* d_exit_chunk, int frame
     if ((long long)ts.n_probes * n_frames_chunk > 0x7fffffffLL || 2 * npix > 0xffffffffULL)
         return fail(c, PS_EUNSUPPORTED, "ps_tacaw_add: chunk has more than 2^31 rows");
     if (!ts.have_ref) {                                                 // reference = the first frame this stream sees
-        PSB_CUDA(c, cudaMemcpy2DAsync(ts.d_ref.p, npix * sizeof(float2), d_exit_chunk, (size_t)n_frames_chunk * npix * sizeof(float2),
-                                      npix * sizeof(float2), ts.n_probes, cudaMemcpyDeviceToDevice, c->stream));
+        // a strided gather of our own: cudaMemcpy2D refuses source pitches above 2^31-1 bytes, i.e. any chunk of 2 GiB
+        // or more per probe (1024^2 x 256 frames, 512^2 x 1024 frames)
+        const size_t q_per_probe = npix / 2;                            // float4 = two complex64
+        const size_t total = q_per_probe * ts.n_probes;
+        const size_t nb = (total + 255) / 256;
+        k_tacaw_first_frame<<<(unsigned)(nb < (size_t)kNumSM * 16 ? nb : (size_t)kNumSM * 16), 256, 0, c->stream>>>(
+            reinterpret_cast<const float4*>(d_exit_chunk), reinterpret_cast<float4*>(ts.d_ref.p), q_per_probe,
+            q_per_probe * (size_t)n_frames_chunk, total);
+        PSB_LAUNCH_CHECK(c, "k_tacaw_first_frame");
         ts.have_ref = true;
     }
     if ((st = ensure_buf(c, ts.d_tw, (size_t)n_frames_chunk * ts.n_bins * sizeof(float2))) != PS_OK) return st;
