@@ -32,9 +32,15 @@
  *     copied into a page-locked staging ring owned by the ctx and sent with cudaMemcpyAsync,
  *     so host arrays are never retained past the call.
  *   - Asynchronous errors: ps_build_slices re-checks every atomic number on the device in
- *     every call; an unknown Z met by a call that did not validate synchronously (case c) is
- *     raised through a page-locked word and reported as PS_EUNSUPPORTED by the next ps_* call
- *     on the ctx that observes it.
+ *     every call; an unknown Z met by a call that did not validate synchronously (case c: the
+ *     same (d_Z, n_atoms) pair as a validated call, e.g. Z edited in place, or a new tensor the
+ *     allocator placed at the old address) is raised through a page-locked word and reported as
+ *     PS_EUNSUPPORTED by the next ps_* call on the ctx that observes it.  What that call produced
+ *     is not left looking valid: its V (ps_build_slices) or its potential chunk and with it the
+ *     exit waves (ps_multislice_fused) are filled with NaN on the device.  ps_check_async() waits
+ *     for the stream and reports the word; call it after the last call of a run, before results
+ *     are read.  ps_profile_read reports it too, and ps_destroy prints a warning to stderr if it
+ *     was never read.
  *   - Scratch memory the library needs is allocated by the ctx itself (cudaMalloc, grown
  *     on demand, freed by ps_destroy) unless the caller installs a workspace with
  *     ps_set_workspace().
@@ -302,6 +308,11 @@ PS_API ps_status ps_dispersion(ps_ctx* ctx, const float* d_I, int P, int n_bins,
  * d_qidx int32 [ny][nx] (bit-exact), d_out[b][q] = sum_p sum_{k in q} I[p][b][k]. */
 PS_API ps_status ps_qbin(ps_ctx* ctx, const float* d_I, int P, int n_bins, double dq, int n_q, int32_t* d_qidx,
                   float* d_out);
+
+/* Waits for the ctx stream, then reports (once) an error that a kernel of an earlier asynchronous call raised
+ * (today: an atomic number without coefficients met by ps_build_slices / ps_multislice_fused after their one-time
+ * synchronous validation) as PS_EUNSUPPORTED with a message; PS_OK if there is none.  Blocks the host. */
+PS_API ps_status ps_check_async(ps_ctx* ctx);
 
 /* Optional per-kernel timing.  While enabled, every launch group of the hot path is bracketed by a CUDA
  * event pair on the ctx stream.  ps_profile_read synchronises the stream, folds the pending pairs into

@@ -58,6 +58,7 @@ _PROTOTYPES = {
     "ps_dispersion": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
     "ps_qbin": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_double, C.c_int, C.c_void_p, C.c_void_p]),
     "ps_launch_count": (C.c_longlong, [C.c_void_p]),
+    "ps_check_async": (C.c_int, [C.c_void_p]),
     "ps_profile_enable": (C.c_int, [C.c_void_p, C.c_int]),
     "ps_profile_read": (C.c_int, [C.c_void_p, C.c_int, C.POINTER(C.c_int), C.c_void_p, C.c_void_p, C.c_void_p]),
 }
@@ -152,6 +153,13 @@ class Context:
     @property
     def launches(self) -> int:
         return int(self._lib.ps_launch_count(self._h))
+
+    def check_async(self):
+        """Wait for the ctx stream and raise the error an earlier asynchronous call flagged on the device, if any
+        (`ps_check_async`): call it after the last call of a run, before reading results."""
+        self._check(self._lib.ps_check_async(self._h))
+
+    synchronize = check_async
 
     def profile_enable(self, on: bool = True):
         self._check(self._lib.ps_profile_enable(self._h, int(bool(on))))

@@ -54,10 +54,18 @@ ps_status upload_async(ps_ctx* c, void* d_dst, const void* h_src, size_t bytes) 
     }
     if (r.head + need > r.cap) r.head = 0;                   // wrap
     const size_t lo = r.head, hi = r.head + need;
-    while (!r.live.empty() && r.live.front().off < hi && r.live.front().end > lo) {  // oldest copies still own the range
-        PSB_CUDA(c, cudaEventSynchronize(r.live.front().ev));
-        r.pool.push_back(r.live.front().ev);
-        r.live.pop_front();
+    // Any in-flight copy whose source overlaps [lo, hi) must finish first.  After a wrap the oldest segment may sit in
+    // the skipped tail while younger ones occupy the start of the ring, so every live segment is examined, not only the
+    // front.  Copies complete in stream order: waiting for the youngest overlapping one retires all that precede it.
+    int last = -1;
+    for (int i = 0; i < (int)r.live.size(); ++i)
+        if (r.live[i].off < hi && r.live[i].end > lo) last = i;
+    if (last >= 0) {
+        PSB_CUDA(c, cudaEventSynchronize(r.live[last].ev));
+        for (int i = 0; i <= last; ++i) {
+            r.pool.push_back(r.live.front().ev);
+            r.live.pop_front();
+        }
     }
     memcpy(r.base + lo, h_src, bytes);
     PSB_CUDA(c, cudaMemcpyAsync(d_dst, r.base + lo, bytes, cudaMemcpyHostToDevice, c->stream));
@@ -76,6 +84,7 @@ ps_status enter(ps_ctx* c, const char* who) {
         const int z = *(volatile int*)c->h_async_err;        // written by k_bin of an earlier asynchronous call
         if (z != 0) {
             *(volatile int*)c->h_async_err = 0;
+            if (c->d_bad_z) cudaMemsetAsync(c->d_bad_z, 0, sizeof(int), c->stream);   // builds queued from here on are clean
             return fail(c, PS_EUNSUPPORTED, std::string(who) + ": an earlier ps_build_slices met atomic number " +
                                                 std::to_string(z == -1 ? 0 : z) + " without form-factor coefficients "
                                                 "(its potentials are invalid)");
@@ -203,6 +212,12 @@ extern "C" ps_status ps_create(ps_ctx** out, int device, void* cuda_stream) {
         delete c;
         return PS_ECUDA;
     }
+    if (cudaMalloc((void**)&c->d_bad_z, 256) != cudaSuccess || cudaMemset(c->d_bad_z, 0, 256) != cudaSuccess) {
+        g_create_err = "ps_create: device allocation of the error word failed";
+        cudaFree(c->d_bad_z); cudaFreeHost(c->h_async_err);
+        delete c;
+        return PS_ECUDA;
+    }
     *out = c;
     return PS_OK;
 }
@@ -211,6 +226,11 @@ extern "C" void ps_destroy(ps_ctx* c) {
     if (!c) return;
     cudaSetDevice(c->device);
     cudaStreamSynchronize(c->stream);
+    if (c->h_async_err && *(volatile int*)c->h_async_err != 0)         // nobody called ps_check_async: do not lose it silently
+        fprintf(stderr, "pyslice_b200: ps_destroy: an earlier ps_build_slices met an atomic number without form-factor "
+                        "coefficients (%d) and its potentials were NaN-filled; the error was never read (ps_check_async)\n",
+                *(volatile int*)c->h_async_err == -1 ? 0 : *(volatile int*)c->h_async_err);
+    cudaFree(c->d_bad_z);
     cudaFree(c->d_nmax); cudaFree(c->d_tiles); cudaFree(c->d_tile_active); cudaFree(c->d_tile_slot);
     cudaFree(c->d_ftab); cudaFree(c->d_elem_of_Z);
     cudaFree(c->kv.d_px_mid); cudaFree(c->kv.d_px_last); cudaFree(c->kv.d_py);
@@ -365,6 +385,13 @@ extern "C" ps_status ps_set_workspace(ps_ctx* c, void* d_ws, size_t bytes) {
     return PS_OK;
 }
 
+extern "C" ps_status ps_check_async(ps_ctx* c) {
+    if (!c) return PS_EINVAL;
+    PSB_CUDA(c, cudaSetDevice(c->device));
+    PSB_CUDA(c, cudaStreamSynchronize(c->stream));
+    return enter(c, "ps_check_async");
+}
+
 extern "C" ps_status ps_profile_enable(ps_ctx* c, int on) {
     if (!c) return PS_EINVAL;
     c->prof_on = on != 0;
@@ -390,5 +417,5 @@ extern "C" ps_status ps_profile_read(ps_ctx* c, int reset, int* n_kernels, const
         if (launches) launches[i] = c->prof_n[i];
         if (reset) { c->prof_ms[i] = 0.0; c->prof_n[i] = 0; }
     }
-    return PS_OK;
+    return enter(c, "ps_profile_read");                           // the outputs above are filled either way
 }

@@ -77,6 +77,7 @@ struct ps_ctx {
     std::unordered_map<const void*, int> kern_cap;   // per kernel: resident blocks on this device (attributes set once)
     int* h_async_err = nullptr;             // mapped pinned word written by kernels (bad atomic number, ...)
     int* d_async_err = nullptr;             // its device alias
+    int* d_bad_z = nullptr;                 // device-memory twin of the word: set by k_bin, read by k_poison (in stream order)
 
     // geometry
     bool have_geom = false;
@@ -97,7 +98,7 @@ struct ps_ctx {
     int vacuum_shortcut = 0;                // ps_set_vacuum_shortcut: rows with V == 0 skip the transmit + FFT pair (exact)
     int vk_mode = 0;                        // ps_set_vk_mode: 0 auto, 1 FP32 SIMT sums, 2 tcgen05 3xTF32 sums
     int tune_resident = 0;                  // ps_set_tuning("resident"): chip-resident slice loop, 0 auto, 1 always, -1 never
-    int tune_row32 = 0;                     // ps_set_tuning("row32"): 32-value row pass at nx = 512/1024, 0 auto (on), -1 off
+    int tune_row32 = 0;                     // ps_set_tuning("row32"): 32-value row pass at nx = 512/1024, 0 auto (off), 1 on, -1 off
     int tune_col32 = 0;                     // ps_set_tuning("col32"): 32-value column pass at ny = 512/1024, 0 auto (on), -1 off
 
     // form factors

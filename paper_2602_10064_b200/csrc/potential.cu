@@ -37,7 +37,7 @@ __global__ void k_bin(const float* __restrict__ pos, const int32_t* __restrict__
                       const int32_t* __restrict__ elem_of_Z, const long long n_total, const int n_atoms,
                       const double Lx, const double Ly, const double Lz, const int n_slices, const int n_elem,
                       uint32_t* __restrict__ Ux, uint32_t* __restrict__ Uy, int32_t* __restrict__ key,
-                      int32_t* __restrict__ slice_idx, int* __restrict__ async_err) {
+                      int32_t* __restrict__ slice_idx, int* __restrict__ async_err, int* __restrict__ bad_dev) {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n_total) return;
     const int j = (int)(i % n_atoms);
@@ -49,8 +49,20 @@ __global__ void k_bin(const float* __restrict__ pos, const int32_t* __restrict__
     const int zz = Z[j];
     const int e = (zz >= 1 && zz <= 127) ? elem_of_Z[zz] : -1;
     key[i] = (e >= 0) ? s * n_elem + e : -1;
-    if (e < 0) { *(volatile int*)async_err = (zz == 0) ? -1 : zz; __threadfence_system(); }   // mapped host word (ps_ctx)
+    if (e < 0) {
+        *(volatile int*)bad_dev = 1;                                       // device word: k_poison of this chunk reads it
+        *(volatile int*)async_err = (zz == 0) ? -1 : zz; __threadfence_system();   // mapped host word (ps_ctx)
+    }
     if (slice_idx) slice_idx[i] = s;
+}
+
+// NaN-fills `dst` when the device error word is set (unknown atomic number in this or an earlier, still unreported
+// ps_build_slices); returns at once otherwise.
+__global__ void k_poison(float4* __restrict__ dst, const size_t n4, const int* __restrict__ bad_dev) {
+    if (*(volatile const int*)bad_dev == 0) return;
+    const float q = __int_as_float(0x7fc00000);
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += (size_t)gridDim.x * blockDim.x)
+        dst[i] = make_float4(q, q, q, q);
 }
 
 // One block per frame, W warps: warp w owns the contiguous atom segment [w*seg, (w+1)*seg).  Per-warp histograms,
@@ -570,7 +582,7 @@ static ps_status build_chunks(ps_ctx* c, const float* d_pos, const int32_t* d_Z,
         k_bin<<<(unsigned)((n_total + 255) / 256), 256, 0, c->stream>>>(
             d_pos + (size_t)f0 * n_atoms * 3, d_Z, c->d_elem_of_Z, n_total, n_atoms, c->cell[0], c->cell[1], c->cell[2],
             c->n_slices, c->n_elem, Ux, Uy, key, d_slice_idx ? d_slice_idx + (size_t)f0 * n_atoms : nullptr,
-            c->d_async_err);
+            c->d_async_err, c->d_bad_z);
         }
         PSB_LAUNCH_CHECK(c, "k_bin");
         { ProfScope ps_(c, K_SORT);
@@ -611,6 +623,14 @@ static ps_status build_chunks(ps_ctx* c, const float* d_pos, const int32_t* d_Z,
             PSB_DISPATCH_N(c->nx, (e = launch_v_row<N_>(c, Zm, off, d_V + (size_t)f0 * c->n_slices * img, nf))); }
             if (e != cudaSuccess) return fail(c, PS_ECUDA, std::string("k_v_row: ") + cudaGetErrorString(e));
             c->launches++;
+        }
+        // An atom k_bin could not place (no coefficients for its Z) was dropped from the sums: what this chunk produced
+        // must not be consumed as if it were a potential.  NaN-fill it (no-op launch unless k_bin raised the word).
+        {
+            float* dst = d_V ? d_V + (size_t)f0 * c->n_slices * img : (float*)Zm;
+            const size_t n4 = d_V ? (size_t)nf * c->n_slices * img / 4 : (L.total - L.zm) / 16;
+            k_poison<<<kNumSM * 4, 256, 0, c->stream>>>(reinterpret_cast<float4*>(dst), n4, c->d_bad_z);
+            PSB_LAUNCH_CHECK(c, "k_poison");
         }
         if (consume && (st = (*consume)(f0, nf, Zm, off)) != PS_OK) return st;
     }

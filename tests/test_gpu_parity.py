@@ -533,6 +533,47 @@ def test_tacaw_streaming_full_length_with_large_elastic_term(torch):
     assert rel_l2(Ig, Io) < TOL_I
 
 
+def test_tacaw_streaming_first_chunk_of_2_GiB_per_probe(torch):
+    """A first chunk whose probes lie 2 GiB apart (1024^2 x 256 frames x 8 B): the default reference wave (first frame
+    of every probe) must still be picked up — cudaMemcpy2D cannot express that pitch — and the result must match the
+    oracle's mean-subtracted FFT on sampled in-band pixels, and a run fed the same frames in small chunks everywhere."""
+    import paper_2602_10064_b200 as ps
+    from paper_2602_10064_b200.binding import TacawStream
+    P, F, n = 2, 256, 1024
+    cell = np.array([40.0, 40.0, 4.0])
+    ctx = ps.Context(0)
+    ctx.set_geometry(cell, n, n, 4.0)
+    g = torch.Generator(device="cuda").manual_seed(2048)
+    x = torch.empty((P, F, n, n), dtype=torch.complex64, device="cuda")
+    assert x[0].numel() * 8 >= 2**31
+    xr = torch.view_as_real(x)
+    xr.normal_(0.0, 0.1, generator=g)
+    xr[..., 0] += 1.5                                                   # elastic part, different per probe below
+    xr[1] *= 0.5
+    bins = np.array([0, 1, 5, -7, 100], dtype=np.int32)
+    ts = TacawStream(ctx, P, F, 2.0, bins)
+    ts.add(x, 0)
+    I_big = ts.finish()
+    ts = TacawStream(ctx, P, F, 2.0, bins)
+    for f0 in range(0, F, 64):
+        ts.add(x[:, f0:f0 + 64].contiguous(), f0)
+    I_small = ts.finish()
+    assert rel_l2(I_big.cpu().numpy(), I_small.cpu().numpy()) < 1e-5
+    rng = np.random.default_rng(3)
+    A = O.aperture_mask(cell, n, n)
+    iy, ix = np.nonzero(A)
+    pick = rng.choice(iy.size, 256, replace=False)
+    iy, ix = iy[pick], ix[pick]
+    for p in range(P):
+        cols = x[p][:, torch.as_tensor(iy, device="cuda"), torch.as_tensor(ix, device="cuda")].cpu().numpy()   # [F][256]
+        Io = O.tacaw_intensity(cols.astype(np.complex128), bins)
+        Ig = I_big[p][:, torch.as_tensor(iy, device="cuda"), torch.as_tensor(ix, device="cuda")].cpu().numpy()
+        ok = np.asarray(bins) != 0                                      # bin 0 is the mean term: zero up to rounding
+        assert rel_l2(Ig[ok], Io[ok]) < TOL_I
+        assert np.abs(Ig[~ok]).max() <= 1e-6 * Io[ok].max() * F
+    ctx.close()
+
+
 def test_tacaw_streaming_rejects_out_of_order_chunks(torch):
     import paper_2602_10064_b200 as ps
     from paper_2602_10064_b200.binding import TacawStream
@@ -653,14 +694,38 @@ def test_unknown_Z_after_validation_is_reported_by_the_next_call(torch):
     pos = _t(torch, w.positions(0, 2)); Z = _t(torch, w.Z)
     ps.ps_build_slices(ctx, pos, Z)
     Z[5] = 79                                                            # in place: same pointer, same count
-    ps.ps_build_slices(ctx, pos, Z)                                      # queued without a host wait
+    Vbad = ps.ps_build_slices(ctx, pos, Z)                               # queued without a host wait
     torch.cuda.synchronize()
+    assert torch.isnan(Vbad).all(), "a potential built without one of its atoms must not look valid"
     with pytest.raises(ps.PSError) as ei:
         ps.ps_make_incident(ctx, w.kV)
     assert ei.value.status == -2 and "79" in str(ei.value)
     Z[5] = int(w.Z[5])
     V = ps.ps_build_slices(ctx, pos, Z)                                  # the ctx stays usable
     assert torch.isfinite(V).all()
+    ctx.check_async()                                                    # nothing pending any more
+
+    # the last call of a run: no later ps_* call would see the word; ps_check_async waits and reports it
+    Z[7] = 0
+    Vbad = ps.ps_build_slices(ctx, pos, Z)
+    with pytest.raises(ps.PSError) as ei:
+        ctx.check_async()
+    assert ei.value.status == -2 and "atomic number 0" in str(ei.value)
+    assert torch.isnan(Vbad).all()
+    # the fused path: its exit waves carry the NaN
+    Z[7] = int(w.Z[7])
+    psi0 = ps.ps_make_incident(ctx, w.kV)
+    ex = ps.ps_multislice_fused(ctx, w.kV, psi0, pos, Z)
+    ctx.check_async()
+    assert torch.isfinite(torch.view_as_real(ex)).all()
+    Z[3] = 92
+    ex = ps.ps_multislice_fused(ctx, w.kV, psi0, pos, Z)
+    with pytest.raises(ps.PSError):
+        ctx.check_async()
+    assert torch.isnan(torch.view_as_real(ex)).any(dim=-1).any(dim=-1).any(dim=-1).all(), "every (probe, frame) wave is poisoned"
+    Z[3] = int(w.Z[3])
+    assert torch.isfinite(ps.ps_build_slices(ctx, pos, Z)).all()
+    ctx.check_async()
 
 
 @pytest.mark.parametrize("n,beam", [(32, "plane"), (64, "probe"), (128, "plane"), (128, "probe")])
