@@ -591,7 +591,7 @@ def test_tacaw_streaming_rejects_out_of_order_chunks(torch):
 
 
 @pytest.mark.parametrize("F", [1024, 2048])
-def test_tacaw_ring_many_probes_large_grid(torch, F):
+def test_tacaw_ring_many_probes_group_carry(torch, F):
     """The TMA-ring kernels with more blocks than pixel groups per probe and P = 5 (the per-probe carry of the group
     list), few bins (the shape for which the ring is chosen)."""
     import paper_2602_10064_b200 as ps
