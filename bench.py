@@ -49,13 +49,32 @@ def measured_peaks():
     return 6650.0, 1590.0, "fallback (B200_PROFILING.md: 6.65 TB/s, 1.59 PFLOP/s)"
 
 
+STATS_SOURCES = ("multislice.cu", "resident.cu", "tacaw.cu", "fft_core.cuh", "tma.cuh")
+
+
+def library_source_sha16():
+    """sha256[:16] over the CUDA sources the slice-step, resident and time-transform kernels are built from."""
+    import hashlib
+    h = hashlib.sha256()
+    for f in STATS_SOURCES:
+        with open(os.path.join(ROOT, "paper_2602_10064_b200", "csrc", f), "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()[:16]
+
+
 def kernel_stats():
-    """ncu-derived per-kernel constants (profiles/r2_kernel_stats.json, written from the --set full captures named in
-    profiles/r2_slice_step.md): DRAM bytes and thread instructions per pixel of one wave, keyed by kernel<N>."""
-    path = os.path.join(ROOT, "profiles", "r2_kernel_stats.json")
-    if os.path.exists(path):
-        with open(path) as fh:
-            return json.load(fh)
+    """ncu-derived per-kernel constants (DRAM bytes and thread instructions per pixel of one wave, keyed by kernel<N>),
+    taken from --set full captures named in the profile notes.  They describe the kernels of ONE source state: the file
+    carries `_source_sha16` (library_source_sha16() when it was captured) and is ignored — `traffic` and `fp32_issue`
+    print as null — when the sources have changed since, instead of silently quoting figures of older kernels."""
+    for name in ("r3_kernel_stats.json", "r2_kernel_stats.json"):
+        path = os.path.join(ROOT, "profiles", name)
+        if os.path.exists(path):
+            with open(path) as fh:
+                d = json.load(fh)
+            if d.get("_source_sha16") == library_source_sha16():
+                d["_file"] = name
+                return d
     return {}
 
 
@@ -265,9 +284,11 @@ def tacaw_micro(shapes_a=None, shapes_b=None):
         I = torch.empty((P, nb, n, n), dtype=torch.float32, device="cuda")
         ms = _event_time(torch, lambda: ps.ps_tacaw(ctx, ex, 2.0, bins, d_I=I), flush)
         nk = ctx.n_k_aperture
-        byts = (8.0 * F + 4.0 * nb) * nk * P + 4.0 * nb * (n * n - nk) * P
+        byts = (8.0 * F + 4.0 * nb) * nk * P                        # in-aperture reads + in-aperture writes
+        zero = 4.0 * nb * (n * n - nk) * P                          # zero fill of the dense I cube: traffic, not algorithm
         print(json.dumps({"micro": "ps_tacaw", "layout": "tiled" if tiled else "dense", "P": P, "frames": F, "grid": n, "bins": nb, "ms": ms,
-                          "algorithmic_GB": byts / 1e9, "GBps": byts / ms / 1e6, "frac_of_hbm_peak": byts / ms / 1e6 / peak}))
+                          "algorithmic_GB": byts / 1e9, "GBps": byts / ms / 1e6, "frac_of_hbm_peak": byts / ms / 1e6 / peak,
+                          "zero_fill_GB": zero / 1e9, "frac_with_zero_fill": (byts + zero) / ms / 1e6 / peak}))
         del ex, I, ctx
     # path B: one 64-frame chunk of a 4096-frame stream, 256 bins (config 4's shape) and a 1024^2 grid
     for n, Fc, nb in shapes_b or []:
@@ -347,6 +368,27 @@ def cufft_reference(w, n_waves, n_slices=8):
 
 
 # --------------------------------------------------------------------------------------------- configs 3 / 4 at full size
+def slice_step_roofline(prof, px, f_col, P):
+    """HBM roofline of the two slice-step passes from the library's per-launch events: `px` pixel-slices of one wave
+    batch, algorithmic bytes per pixel 16 f_col + 4/P (row pass: wave in + out on the in-band columns, V once per frame)
+    and 16 f_col (column pass), against the measured copy rate."""
+    peak, _, src = measured_peaks()
+    alg = {"k_row_transmit": 16.0 * f_col + 4.0 / P, "k_col_propagate": 16.0 * f_col}
+    out = {"bound": "hbm", "unit": "GB/s", "peak": peak, "peak_source": src}
+    ms_pair = 0.0
+    for k, b in alg.items():
+        if k not in prof or prof[k][1] == 0:
+            return None
+        ms = prof[k][0]
+        ms_pair += ms
+        out[k] = {"ms": ms, "algorithmic_bytes_per_px": b, "achieved": b * px / (ms * 1e-3) / 1e9,
+                  "frac": b * px / (ms * 1e-3) / 1e9 / peak}
+    tot = sum(alg.values())
+    out["slice_step_pair"] = {"achieved": tot * px / (ms_pair * 1e-3) / 1e9, "frac": tot * px / (ms_pair * 1e-3) / 1e9 / peak,
+                              "gpx_slice_s": px / (ms_pair * 1e-3) / 1e9}
+    return out
+
+
 def full_config(which, quiet=False, fused_v=False):
     """Config 4: 4096 frames x 1024^2 x 120 slices, V built and propagated 64 frames at a time, exit waves folded into the
     streaming per-bin DFT (path B, 256 bins) chunk by chunk (SURVEY.md 8(d) capacity plan).  Config 3: 1024 frames x
@@ -393,6 +435,16 @@ def full_config(which, quiet=False, fused_v=False):
         b.record()
         torch.cuda.synchronize()
         check = float(simg.sum())
+        # untimed: one more chunk with the library's per-launch events -> kernel split and slice-step roofline of config 4
+        ctx.profile_read(reset=True)
+        ctx.profile_enable(True)
+        ts1 = TacawStream(ctx, 1, F, w.dt_fs, bins)
+        ps.ps_build_slices(ctx, pos_d[:chunk], Z_d, d_V=V); ps.ps_multislice(ctx, w.kV, psi0, V, d_exit=ex); ts1.add(ex, 0)
+        prof = ctx.profile_read(reset=True)
+        ctx.profile_enable(False)
+        del ts1
+        extra = {"kernel_ms_per_chunk": {k: v[0] for k, v in prof.items() if v[1] > 0},
+                 "roofline": slice_step_roofline(prof, float(nx) * ny * S * chunk, band_columns(w.cell, nx, ny) / nx, 1)}
         plan = (f"{F // chunk} chunks of {chunk} frames: " + ("ps_multislice_fused (no V array)" if fused_v else "build V (30 GB) -> multislice") +
                 f" -> ps_tacaw_add (path B, {len(bins)} bins)")
     else:
@@ -418,6 +470,17 @@ def full_config(which, quiet=False, fused_v=False):
         b.record()
         torch.cuda.synchronize()
         check = float(simg.sum())
+        # untimed: Parseval on the last probe chunk (pin P11; tests/test_gpu_full_size.py::test_c3_bench_shape checks the same
+        # identity against the oracle-verified exit waves): sum_{k,n} I = F sum_{k,t} |Psi - <Psi>_t|^2, left side from simg
+        worst = 0.0
+        for p in range(pc):
+            tot = 0.0
+            for y0 in range(0, ny, 64):
+                blk = ex[p, y0:y0 + 64].to(torch.complex128)              # tiled layout [rows][tiles][F][8]
+                blk = blk - blk.mean(dim=2, keepdim=True)
+                tot += float((blk.real ** 2 + blk.imag ** 2).sum())
+            worst = max(worst, abs(float(simg[P - pc + p].double().sum()) - F * tot) / (F * tot))
+        extra = {"parseval_rel_err_last_probe_chunk": worst}
         plan = (f"V of all {F} frames resident (86 GB); {P // pc} chunks of {pc} probes: incident -> multislice (tiled exit "
                 f"layout, {ex.numel() * 8 / 1e9:.0f} GB) -> ps_tacaw -> reductions")
     sec = a.elapsed_time(b) * 1e-3
@@ -426,6 +489,7 @@ def full_config(which, quiet=False, fused_v=False):
            "tacaw_end_to_end_s": sec, "value": units / sec / 1e9, "unit": UNIT, "plan": plan,
            "gpu_launches": int(ctx.launches - l0), "host_setup_s": t_host, "checksum_spectrum_image": check,
            "hbm_peak_allocated_GB": torch.cuda.max_memory_allocated() / 1e9}
+    out.update(extra)
     del V, ex, I, ctx, pos_d
     torch.cuda.empty_cache()
     if not quiet:
@@ -514,9 +578,10 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     dev = torch.device("cuda", local_rank)
 
-    if world > 1 and args.scaling == "strong":
+    if args.scaling == "strong":                                  # world = 1 too: the same loop on one rank
         sharding.run_strong_bench(args, w, rank, world, dev, ps, METRIC, UNIT)
-        dist.destroy_process_group()
+        if world > 1:
+            dist.destroy_process_group()
         return
 
     # ---- inputs: an independent seeded trajectory per rank (rank 0 = the workload's own seed)
@@ -666,7 +731,7 @@ def main():
             return None, None
         return st, {"thread_inst_per_px": st["thread_inst_per_px"], "peak_thread_inst_per_s": issue_peak,
                     "frac": st["thread_inst_per_px"] * px_per_s / issue_peak,
-                    "note": "thread instructions per pixel (ncu, profiles/r2_kernel_stats.json) x pixels/s / (148 SMs x 128 "
+                    "note": "thread instructions per pixel (ncu, profiles/" + stats.get("_file", "?") + ") x pixels/s / (148 SMs x 128 "
                             "lanes x SM clock sampled in this run): the FP32-issue co-limit of the FFT passes"}
 
     if "k_slice_resident" in kern:
@@ -725,22 +790,36 @@ def main():
                                  "on its stream (ps_profile_*), not the pass `value` was timed on",
             "profiled_ms_per_step": ms_prof_total / K})
     if "k_tacaw_fft" in kern:
-        tb_in = (8.0 * F + 4.0 * nb) * ctx.n_k_aperture * P              # transform kernel: exit values in, I out
-        tb_zero = 4.0 * nb * (nx * ny - ctx.n_k_aperture) * P              # zero fill of the out-of-band pixels of I
-        tb = tb_in + tb_zero
+        # the method's own bytes are the in-aperture exit values read once (8 B k F P) and the in-aperture
+        # intensities written once (4 B k n_w P).  The dense I[P][n_w][ny][nx] cube also makes the stage write zeros to the
+        # out-of-band pixels: that is traffic, not algorithm, and is reported as such.
+        tb_in = (8.0 * F + 4.0 * nb) * ctx.n_k_aperture * P
+        tb_zero = 4.0 * nb * (nx * ny - ctx.n_k_aperture) * P
         tms = kern["k_tacaw_fft"][0] / K
         tst = stats.get(f"k_tacaw<{F}>")
-        roofline["tacaw"] = {"achieved": tb / (tms * 1e-3) / 1e9, "frac": tb / (tms * 1e-3) / 1e9 / peak,
-                             "bytes_per_step": tb, "ms_per_step": tms,
-                             "traffic": (tst["dram_bytes_per_inband_algorithmic_byte"] * tb_in + tb_zero) if tst else None}
+        roofline["tacaw"] = {"achieved": tb_in / (tms * 1e-3) / 1e9, "frac": tb_in / (tms * 1e-3) / 1e9 / peak,
+                             "bytes_per_step": tb_in, "ms_per_step": tms,
+                             "zero_fill_bytes_per_step": tb_zero,
+                             "frac_with_zero_fill": (tb_in + tb_zero) / (tms * 1e-3) / 1e9 / peak,
+                             "traffic": (tst["dram_bytes_per_inband_algorithmic_byte"] * tb_in + tb_zero) if tst else None,
+                             "note": "frac counts the method's bytes only (in-aperture reads + in-aperture writes); the dense "
+                                     "I cube adds zero_fill_bytes_per_step of writes the method does not need"}
     if "k_vk" in kern:
-        # V(k) structure-factor sums: 4 real sums per quarter-plane point and atom, x3 for the 3xTF32 split (tensor path)
-        flop = 24.0 * (ctx.n_k_aperture / 4.0) * float(w.n_atoms) * F
+        # V(k) structure-factor sums over the in-aperture quarter plane: 4 real sums = 8 flops per (point, atom) in the
+        # method; the tensor path issues each product three times (3xTF32 split) to stay at fp32 accuracy
+        flop8 = 8.0 * (ctx.n_k_aperture / 4.0) * float(w.n_atoms) * F
         tms = kern["k_vk"][0] / K
-        roofline["vk"] = {"bound": "tensor", "unit": "TFLOP/s", "achieved": flop / (tms * 1e-3) / 1e12,
-                          "peak": 0.5 * bf16_peak, "frac": flop / (tms * 1e-3) / 1e12 / (0.5 * bf16_peak),
-                          "note": "algorithmic 3xTF32 flops over the in-aperture quarter plane; peak = measured bf16 x 0.5 "
-                                  "(guide's nominal tf32:bf16 ratio); FP32 path when ps_set_vk_mode(1) or few atoms per slice"}
+        tf32_peak = 0.5 * bf16_peak
+        fp32_alu_peak = 2.0 * N_SM * LANES_PER_SM * sm_clock / 1e12
+        roofline["vk"] = {"bound": "tensor", "unit": "TFLOP/s", "achieved": flop8 / (tms * 1e-3) / 1e12,
+                          "peak": tf32_peak, "frac": flop8 / (tms * 1e-3) / 1e12 / tf32_peak,
+                          "issued_3xtf32": {"achieved": 3.0 * flop8 / (tms * 1e-3) / 1e12,
+                                            "frac": 3.0 * flop8 / (tms * 1e-3) / 1e12 / tf32_peak},
+                          "vs_fp32_alu_peak": flop8 / (tms * 1e-3) / 1e12 / fp32_alu_peak,
+                          "note": "frac = the method's 8 flops per (k point, atom) against measured bf16 x 0.5 (guide's nominal "
+                                  "tf32:bf16 ratio); issued_3xtf32 counts the three TF32 products per fp32-accurate product; "
+                                  "vs_fp32_alu_peak = the same 8 flops against 2 x 148 x 128 lanes x sampled clock; FP32 SIMT "
+                                  "path when ps_set_vk_mode(1) or few atoms per slice"}
 
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -764,6 +843,28 @@ def main():
                 last = [ln for ln in res.stdout.strip().splitlines() if ln.startswith("{")]
                 full[k] = json.loads(last[-1]) if (res.returncode == 0 and last) else {
                     "error": f"exit code {res.returncode}: {res.stderr.strip()[-300:]}"}
+            except Exception as exc:                             # noqa: BLE001
+                full[k] = {"error": f"{type(exc).__name__}: {exc}"[:300]}
+
+        # the other shapes the bar is held on, small samples through this same script: config 5's largest grid (2 tilts x 32
+        # frames of 2048^2) and the time transform alone at config 2's (50 of 512 bins) and config 5's (2048 frames) shapes
+        me = [sys.executable, os.path.abspath(__file__)]
+        for k, cmd in (("c5_2048_sample", me + ["--workload", "c5_al_sweep", "--grid", "2048", "--frames", "32", "--probes-side", "2",
+                                                 "--steps", "2", "--no-cpu-baseline", "--no-full-configs"]),
+                       ("tacaw_micro", me + ["--tacaw-micro", "--micro-a", "1,512,256,50", "--micro-a", "8,2048,512,2048,1",
+                                             "--micro-a", "16,1024,512,1024,1"])):
+            try:
+                res = subprocess.run(cmd, capture_output=True, text=True, timeout=600)
+                rows = [json.loads(ln) for ln in res.stdout.strip().splitlines() if ln.startswith("{")]
+                if res.returncode != 0 or not rows:
+                    full[k] = {"error": f"exit code {res.returncode}: {res.stderr.strip()[-300:]}"}
+                elif k == "tacaw_micro":
+                    full[k] = rows
+                else:
+                    r = rows[-1]
+                    full[k] = {"config": r["config"], "value": r["value"], "unit": r["unit"], "ms_per_step": r["ms_per_step"],
+                               "roofline": {kk: r["roofline"].get(kk) for kk in ("kernel", "achieved", "frac", "peak", "avg_launch_ms",
+                                                                               "other_pass", "slice_step_pair", "tacaw")}}
             except Exception as exc:                             # noqa: BLE001
                 full[k] = {"error": f"{type(exc).__name__}: {exc}"[:300]}
 

@@ -37,11 +37,16 @@ class ShardPlan:
     exchange: str        # which collective finishes the job
 
 
-def plan(n_probes: int, n_frames: int, rank: int, world: int) -> ShardPlan:
-    """Pick the sharding axis for this rank (see module docstring)."""
-    if world == 1:
+def plan(n_probes: int, n_frames: int, rank: int, world: int, axis: str | None = None) -> ShardPlan:
+    """Pick the sharding axis for this rank (see module docstring); `axis` ("probe" | "frame") overrides the choice
+    (used to drive the frame branch at world = 1, and to shard frames although there are enough probes)."""
+    if axis not in (None, "probe", "frame"):
+        raise ValueError("axis must be None, 'probe' or 'frame'")
+    if axis is None and world == 1:
         return ShardPlan("probe", (0, n_probes), (0, n_frames), "none")
-    if n_probes >= world:
+    if axis == "probe" and n_probes < world:
+        raise ValueError("fewer probes than ranks: cannot shard probes")
+    if axis == "probe" or (axis is None and n_probes >= world):
         return ShardPlan("probe", shard_range(n_probes, rank, world), (0, n_frames),
                          "all_reduce(sdp image); spectrum image rank-local")
     return ShardPlan("frame", (0, n_probes), shard_range(n_frames, rank, world),
@@ -82,6 +87,9 @@ def reduce_scatter_sum(t, group=None):
     an error, so a real NCCL failure is not turned into world x the traffic."""
     import torch
     import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()):
+        assert t.shape[0] == 1
+        return t[0]
     world, rank = dist.get_world_size(group), dist.get_rank(group)
     assert t.shape[0] == world
     v = torch.view_as_real(t) if t.is_complex() else t
@@ -99,6 +107,8 @@ def all_gather_cat(t, group=None):
     """[n, ...] on every rank (same shape) -> [world * n, ...] in rank order."""
     import torch
     import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()):
+        return t
     world = dist.get_world_size(group)
     v = (torch.view_as_real(t) if t.is_complex() else t).contiguous()
     parts = [torch.empty_like(v) for _ in range(world)]
@@ -107,29 +117,63 @@ def all_gather_cat(t, group=None):
     return torch.view_as_complex(out) if t.is_complex() else out
 
 
-def run_sharded(ops, n_probes: int, n_frames: int, bins, rank: int, world: int, frame_chunk: int = 64, sdp_bins=(1, 4)):
+def tiled_exit_fraction(cell, nx: int, ny: int) -> float:
+    """Share of the nx/8 column tiles that PS_LAYOUT_TILED_APERTURE stores: tiles holding a column m with
+    |m| / Lx <= kc, kc = (2/3) min(nx / 2Lx, ny / 2Ly) (reading A10) — 44 of 64 at 512^2 on a square cell."""
+    kc = (2.0 / 3.0) * min(nx / (2.0 * cell[0]), ny / (2.0 * cell[1]))
+    tiles = set()
+    for ix in range(nx):
+        m = ix if ix < (nx + 1) // 2 else ix - nx
+        if abs(m) / cell[0] <= kc:
+            tiles.add(ix // 8)
+    return len(tiles) / (nx // 8)
+
+
+def probe_branch_bytes(cell, nx: int, ny: int, n_slices: int, n_frames: int, n_bins: int, probe_chunk: int,
+                       work_bytes: int = 16 << 30) -> int:
+    """Device bytes the probe branch of run_sharded holds on ONE rank, whatever the number of ranks: V of all frames,
+    one probe chunk of tiled exit waves, its I cube, plus the library's work array (at most `work_bytes`)."""
+    npix = nx * ny
+    V = 4 * n_frames * n_slices * npix
+    ex = int(8 * probe_chunk * n_frames * npix * tiled_exit_fraction(cell, nx, ny))
+    I = 4 * probe_chunk * n_bins * npix
+    return V + ex + I + work_bytes
+
+
+def run_sharded(ops, n_probes: int, n_frames: int, bins, rank: int, world: int, frame_chunk: int = 64, sdp_bins=(1, 4),
+                probe_chunk: int = 16, axis: str | None = None):
     """positions -> I(k, w) reductions for ONE trajectory, sharded per plan():
 
-    probe axis: this rank's probes x all frames: ps_build_slices (all frames) -> ps_multislice -> ps_tacaw ->
-        rank-local spectrum-image rows; ONE all-reduce of the [ny][nx] spectral diffraction pattern and one of the
-        zero-padded [P][n_bins] spectrum image.  No wave ever leaves its GPU.
+    probe axis: this rank's probes x all frames.  ps_build_slices (all frames) once, then `probe_chunk` probes at a time
+        through ONE reused pair of buffers: ps_multislice into the tiled in-band exit layout -> ps_tacaw -> spectrum-image
+        rows of the chunk, spectral diffraction pattern added up with ps_accumulate_intensity (the loop bench.py's
+        full_config("c3") runs; config 3 per rank: 86 + 24 + 17 GB whatever the number of ranks, see
+        probe_branch_bytes).  Then ONE all-reduce of the [ny][nx] spectral diffraction pattern and one of the zero-padded
+        [P][n_bins] spectrum image.  No wave ever leaves its GPU.
     frame axis: this rank's frames x all probes, chunk by chunk: build V -> multislice -> ps_tacaw_add with the GLOBAL
         frame index (every rank subtracts the SAME reference wave: the exit wave of global frame 0, which each rank
         computes for itself); then ONE reduce-scatter of the complex accumulators over k (rank r keeps k-slice r),
         ps_tacaw_finish_shard on the owned slice, an all-gather of the I slices and the usual reductions.
 
-    Returns {"sdp": [ny][nx], "spectrum_image": [P][n_bins], "I_local": this rank's part of I, "plan": ShardPlan}."""
+    Returns {"sdp": [ny][nx], "spectrum_image": [P][n_bins], "I_local": this rank's part of I (probe axis: the cube of
+    the LAST probe chunk only — earlier chunks' cubes are reduced and overwritten), "plan": ShardPlan}."""
     import torch
-    pl = plan(n_probes, n_frames, rank, world)
+    pl = plan(n_probes, n_frames, rank, world, axis)
     nb = n_frames if bins is None else len(bins)
     if pl.axis == "probe":
         p0, p1 = pl.probes
         V = ops.build_slices(0, n_frames)
-        ex = ops.multislice(ops.incident(p0, p1), V)
-        I = ops.tacaw(ex, bins)                                           # [p1-p0][nb][ny][nx]
-        sdp = ops.sdp(I, *sdp_bins)
-        simg = torch.zeros((n_probes, nb), dtype=torch.float32, device=I.device)
-        simg[p0:p1] = ops.spectrum_image(I)
+        sdp = simg = I = None
+        for c0 in range(p0, p1, max(1, probe_chunk)):
+            c1 = min(p1, c0 + max(1, probe_chunk))
+            ex = ops.multislice(ops.incident(c0, c1), V, tiled=True)
+            I = ops.tacaw(ex, bins)                                       # [c1-c0][nb][ny][nx], buffer reused per chunk
+            rows = ops.spectrum_image(I)
+            if simg is None:
+                simg = torch.zeros((n_probes, nb), dtype=torch.float32, device=rows.device)
+            simg[c0:c1] = rows
+            part = ops.sdp(I, *sdp_bins)
+            sdp = part.clone() if sdp is None else ops.accumulate(sdp, part)
         all_reduce_sum_(sdp)
         all_reduce_sum_(simg)
         return {"sdp": sdp, "spectrum_image": simg, "I_local": I, "plan": pl}
@@ -162,9 +206,12 @@ class LibraryOps:
     def __init__(self, ps, ctx, w, pos_d, Z_d):
         self.ps, self.ctx, self.w, self.pos_d, self.Z_d = ps, ctx, w, pos_d, Z_d
         self.stream = None
+        self._bufs = {}
 
     def build_slices(self, f0, f1):
-        return self.ps.ps_build_slices(self.ctx, self.pos_d[f0:f1], self.Z_d)
+        import torch
+        d_V = self._buf("V", (f1 - f0, self.ctx.n_slices, self.ctx.ny, self.ctx.nx), torch.float32)
+        return self.ps.ps_build_slices(self.ctx, self.pos_d[f0:f1], self.Z_d, d_V=d_V)
 
     def incident(self, p0, p1):
         import numpy as np
@@ -175,14 +222,38 @@ class LibraryOps:
             return self.ps.ps_make_incident(self.ctx, w.kV, 0.0, w.tilts[p0:p1].astype(np.float64), is_tilt=True)
         return self.ps.ps_make_incident(self.ctx, w.kV)
 
-    def multislice(self, psi0, V):
-        return self.ps.ps_multislice(self.ctx, self.w.kV, psi0, V)
+    def _buf(self, key, shape, dtype):
+        """one device buffer per role, re-used while the shape stays the same (probe chunks, timed steps)"""
+        import torch
+        b = self._bufs.get(key)
+        if b is None or tuple(b.shape) != tuple(shape) or b.dtype != dtype:
+            self._bufs.pop(key, None)
+            b = self._bufs[key] = torch.empty(tuple(shape), dtype=dtype, device=self.ctx.device)
+        return b
+
+    def multislice(self, psi0, V, tiled=False):
+        import torch
+        ps = self.ps
+        if not tiled:
+            return ps.ps_multislice(self.ctx, self.w.kV, psi0, V)
+        shape = ps.exit_shape(self.ctx, int(psi0.shape[0]), int(V.shape[0]), ps.PS_LAYOUT_TILED_APERTURE)
+        return ps.ps_multislice(self.ctx, self.w.kV, psi0, V, d_exit=self._buf("exit_tiled", shape, torch.complex64))
 
     def tacaw(self, ex, bins):
-        return self.ps.ps_tacaw(self.ctx, ex, self.w.dt_fs, bins)
+        import torch
+        P = int(ex.shape[0])
+        F = int(ex.shape[1] if ex.dim() == 4 else ex.shape[3])
+        nb = F if bins is None else len(bins)
+        d_I = self._buf("I", (P, nb, self.ctx.ny, self.ctx.nx), torch.float32)
+        return self.ps.ps_tacaw(self.ctx, ex, self.w.dt_fs, bins, d_I=d_I)
 
     def sdp(self, I, lo, hi):
-        return self.ps.ps_sdp(self.ctx, I, lo, min(hi, I.shape[1] - 1))
+        import torch
+        d_out = self._buf("sdp_part", (self.ctx.ny, self.ctx.nx), torch.float32)
+        return self.ps.ps_sdp(self.ctx, I, lo, min(hi, I.shape[1] - 1), d_out=d_out)
+
+    def accumulate(self, acc, part):
+        return self.ps.ps_accumulate_intensity(self.ctx, acc, part, 1.0, 1.0)
 
     def spectrum_image(self, I):
         return self.ps.ps_spectrum_image(self.ctx, I)
@@ -229,10 +300,11 @@ def run_strong_bench(args, w, rank, world, dev, ps, metric, unit):
         bins = np.arange(min(256, w.n_frames), dtype=np.int32)
 
     def step():
-        return run_sharded(ops, w.n_probes, w.n_frames, bins, rank, world)
+        return run_sharded(ops, w.n_probes, w.n_frames, bins, rank, world, probe_chunk=getattr(args, "probe_chunk", 16) or 16)
 
     def barrier():
-        dist.barrier()
+        if dist.is_available() and dist.is_initialized():
+            dist.barrier()
         torch.cuda.synchronize()
 
     W, K = max(3, args.warmup), max(1, args.steps)

@@ -54,7 +54,11 @@ class OracleOps:
             return [O.probe_wave(w.cell, w.nx, w.ny, w.kV, w.semi_angle_mrad, x, y) for x, y in w.probe_xy[p0:p1]]
         return [O.plane_wave(w.nx, w.ny)]
 
-    def multislice(self, psi0, V):
+    def accumulate(self, acc, part):
+        acc += part
+        return acc
+
+    def multislice(self, psi0, V, tiled=False):                          # the layout is the library's business: same values
         return torch.from_numpy(np.stack([[O.multislice(p, v, self.w.cell, self.w.kV) for v in V] for p in psi0]))
 
     def tacaw(self, ex, bins):
@@ -104,7 +108,7 @@ def _sharded_case(case, rank, world):
         w.n_slices = 2
         bins = np.array([0, 1, 2, -1, 5, -6], dtype=np.int64)
     ops = OracleOps(w)
-    out = sharding.run_sharded(ops, w.n_probes, w.n_frames, bins, rank, world, frame_chunk=3)
+    out = sharding.run_sharded(ops, w.n_probes, w.n_frames, bins, rank, world, frame_chunk=3, probe_chunk=1)   # 2 chunks per rank
     assert out["plan"].axis == ("probe" if case == "sharded_probe" else "frame")
     I_all, _ = O.run_path(ops.pos, ops.elem, ops.coef, ops.nl, ops.ng, w.cell, w.nx, w.ny, w.n_slices, w.kV,
                           ops.incident(0, w.n_probes), bins)
@@ -202,3 +206,29 @@ def test_plan_axes():
     assert sharding.plan(256, 1024, 3, 8).axis == "probe"
     assert sharding.plan(1, 4096, 3, 8).axis == "frame"
     assert sharding.plan(1, 4096, 0, 1).exchange == "none"
+
+
+def test_probe_branch_fits_config_3_on_every_rank_count():
+    """the probe branch of run_sharded holds V of all frames plus ONE 16-probe chunk of
+    tiled exit waves and its I cube, whatever the number of ranks: config 3 (1024 frames x 512^2 x 80 slices, all 1024
+    bins) must stay under 170 GB of a 180 GB B200, work array of the library included."""
+    from workloads import make_workload
+    w = make_workload("c3_si_probe_512")
+    assert abs(sharding.tiled_exit_fraction(w.cell, w.nx, w.ny) - 44 / 64) < 1e-12
+    need = sharding.probe_branch_bytes(w.cell, w.nx, w.ny, w.n_slices, w.n_frames, w.n_frames, probe_chunk=16)
+    assert need < 170e9, need
+    dense_all = 8 * 32 * w.n_frames * w.nx * w.ny + 4 * 32 * w.n_frames * w.nx * w.ny + 4 * w.n_frames * w.n_slices * w.nx * w.ny
+    assert dense_all > 180e9                                            # what the unchunked dense plan needed at 8 ranks
+    for world in (1, 2, 4, 8):
+        for rank in range(world):
+            pl = sharding.plan(w.n_probes, w.n_frames, rank, world)
+            assert pl.axis == "probe" and (pl.probes[1] - pl.probes[0]) * world == w.n_probes
+
+
+def test_plan_forced_axis():
+    pl = sharding.plan(4, 10, 0, 1, axis="frame")
+    assert pl.axis == "frame" and pl.frames == (0, 10) and pl.probes == (0, 4)
+    with pytest.raises(ValueError):
+        sharding.plan(1, 10, 0, 2, axis="probe")
+    with pytest.raises(ValueError):
+        sharding.plan(1, 10, 0, 2, axis="time")

@@ -728,6 +728,34 @@ def test_unknown_Z_after_validation_is_reported_by_the_next_call(torch):
     ctx.check_async()
 
 
+@pytest.mark.parametrize("axis", ["probe", "frame"])
+def test_run_sharded_through_the_library_on_one_rank(torch, axis):
+    """sharding.run_sharded with LibraryOps (what bench.py --scaling strong runs) on ONE rank, both branches: the probe
+    branch in chunks of 3 probes through the tiled exit layout and the reused buffers, the frame branch (forced) through
+    ps_tacaw_begin/add/finish_shard; both against the oracle's run_path on the whole problem."""
+    import paper_2602_10064_b200 as ps
+    from paper_2602_10064_b200 import sharding
+    from workloads import form_factor_coefficients
+    w = make_workload("c3_si_probe_512", mini=True)
+    ctx = make_ctx(w)
+    pos = w.positions()
+    ops = sharding.LibraryOps(ps, ctx, w, _t(torch, pos), _t(torch, w.Z))
+    bins = None if axis == "probe" else np.array([0, 1, 2, -1, 5, -6], dtype=np.int32)
+    out = sharding.run_sharded(ops, w.n_probes, w.n_frames, bins, 0, 1, frame_chunk=5, probe_chunk=3, axis=axis)
+    ctx.check_async()
+    assert out["plan"].axis == axis
+    nl, ng, coef = form_factor_coefficients(w.elements, w.ff_kind)
+    Io, _ = O.run_path(pos, np.searchsorted(w.elements, w.Z), coef, nl, ng, w.cell, w.nx, w.ny, w.n_slices, w.kV,
+                       oracle_incident(w), bins)
+    assert rel_l2(out["sdp"].cpu().numpy(), O.sdp(Io, 1, min(4, Io.shape[1] - 1))) < TOL_I
+    assert rel_l2(out["spectrum_image"].cpu().numpy(), Io.sum(axis=(2, 3))) < TOL_I
+    if axis == "frame":
+        assert rel_l2(out["I_local"].cpu().numpy().reshape(Io.shape), Io) < TOL_I
+    else:
+        n_last = w.n_probes - 3 * ((w.n_probes - 1) // 3)
+        assert rel_l2(out["I_local"].cpu().numpy(), Io[-n_last:]) < TOL_I
+
+
 @pytest.mark.parametrize("n,beam", [(32, "plane"), (64, "probe"), (128, "plane"), (128, "probe")])
 def test_resident_slice_loop_matches_oracle_and_streaming_path(torch, n, beam):
     """The chip-resident slice loop (one launch, wave kept in shared memory; square grids <= 128) against the oracle
