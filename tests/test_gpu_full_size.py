@@ -205,13 +205,15 @@ def test_c4_full_grid_streaming_bins(torch):
     pos = w.positions()
     V, sidx = ps.ps_build_slices(ctx, _t(torch, pos), _t(torch, w.Z), want_slice_idx=True)
     ex = ps.ps_multislice(ctx, w.kV, gpu_incident(ctx, w), V)
-    f = 5
-    Vo, so = oracle_potential(w, pos[f], slices=(3, 118))
-    assert np.array_equal(sidx[f].cpu().numpy(), so)
-    for s in (3, 118):
-        assert rel_l2(V[f, s].cpu().numpy(), Vo[s]) < TOL_V
-    eo = O.multislice(oracle_incident(w)[0], V[f].cpu().numpy().astype(np.float64), w.cell, w.kV)
-    assert rel_l2(ex[0, f].cpu().numpy(), eo) < TOL_EXIT
+    for f in (5, 27):                                                     # V on 2 frames, from positions
+        Vo, so = oracle_potential(w, pos[f], slices=(3, 60, 118))
+        assert np.array_equal(sidx[f].cpu().numpy(), so)
+        for s in (3, 60, 118):
+            assert rel_l2(V[f, s].cpu().numpy(), Vo[s]) < TOL_V
+    psi0_o = oracle_incident(w)[0]
+    for f in (0, 5, 19, 31):                                              # ... exit waves on 4 (frame, probe) pairs
+        eo = O.multislice(psi0_o, V[f].cpu().numpy().astype(np.float64), w.cell, w.kV)
+        assert rel_l2(ex[0, f].cpu().numpy(), eo) < TOL_EXIT, f
     del V
     bins = np.arange(-8, 16, dtype=np.int32)
     ts = TacawStream(ctx, 1, F, w.dt_fs, bins)
@@ -223,6 +225,50 @@ def test_c4_full_grid_streaming_bins(torch):
     _check_tacaw_sample(torch, ps, ctx, w, ex, IB, bins, 2048, 41)
     _check_tacaw_sample(torch, ps, ctx, w, ex, IA, bins, 2048, 42)
     assert rel_l2(IB.cpu().numpy(), IA.cpu().numpy()) < TOL_I
+
+
+def test_c4_streaming_loop_four_chunks(torch):
+    """The loop bench.py --full-config c4 runs (build V of 64 frames -> multislice -> ps_tacaw_add, buffers reused), on
+    256 frames = 4 chunks at config 4's own grid, slices, atoms and its 256 bins.  The exit-wave columns of 2048 seeded
+    in-band pixels are kept from every chunk; path B's I at those pixels must equal the oracle's mean-subtracted FFT of
+    the columns, as a whole and bin by bin (same floor as test_c3_bench_shape); out-of-band pixels exactly zero."""
+    import paper_2602_10064_b200 as ps
+    from paper_2602_10064_b200.binding import TacawStream
+    F, chunk = 256, 64
+    w = make_workload("c4_interface_1024", n_frames=F)
+    ctx = make_ctx(w)
+    nx, ny, S = w.nx, w.ny, w.n_slices
+    bins = np.arange(256, dtype=np.int32)
+    A = O.aperture_mask(w.cell, nx, ny)
+    iy, ix = np.nonzero(A)
+    sel = np.random.default_rng(404).choice(iy.size, size=2048, replace=False)
+    sy, sx = torch.as_tensor(iy[sel]).cuda(), torch.as_tensor(ix[sel]).cuda()
+    Z_d = _t(torch, w.Z)
+    V = torch.empty((chunk, S, ny, nx), dtype=torch.float32, device="cuda")
+    ex = torch.empty((1, chunk, ny, nx), dtype=torch.complex64, device="cuda")
+    psi0 = ps.ps_make_incident(ctx, w.kV)
+    ts = TacawStream(ctx, 1, F, w.dt_fs, bins)
+    cols = []
+    for f0 in range(0, F, chunk):
+        ps.ps_build_slices(ctx, _t(torch, w.positions(f0, f0 + chunk)), Z_d, d_V=V)
+        ps.ps_multislice(ctx, w.kV, psi0, V, d_exit=ex)
+        ts.add(ex, f0)
+        cols.append(ex[0][:, sy, sx].cpu().numpy())
+    I = ts.finish()
+    ctx.check_async()
+    cols = np.concatenate(cols).astype(np.complex128)                       # [256][2048]
+    Io = O.tacaw_intensity(cols, bins)
+    Ig = I[0][:, sy, sx].cpu().numpy().astype(np.float64)
+    nz = np.asarray(bins) != 0                                              # bin 0 (the mean term) is defined as zero
+    assert rel_l2(Ig[nz], Io[nz]) < TOL_I
+    assert not Ig[~nz].any()
+    eps32 = float(np.finfo(np.float32).eps)
+    floor = eps32 * np.log2(F) * np.sqrt(max(Io[nz].mean(axis=1).max(), float(np.mean(np.abs(cols.sum(axis=0)) ** 2))))
+    for b in np.nonzero(nz)[0]:
+        allowed = TOL_I * np.linalg.norm(Io[b]) + np.linalg.norm(2.0 * np.sqrt(Io[b]) * floor + floor ** 2)
+        assert np.linalg.norm(Ig[b] - Io[b]) <= allowed, b
+    out = torch.as_tensor(~A).cuda()
+    assert float(I[0][:, out].abs().max()) == 0.0
 
 
 @pytest.mark.parametrize("grid", [1024, 2048])
@@ -237,12 +283,16 @@ def test_c5_large_grids_tilts(torch, grid):
     pos = w.positions(0, nf)
     V, sidx = ps.ps_build_slices(ctx, _t(torch, pos), _t(torch, w.Z), want_slice_idx=True)
     ex = ps.ps_multislice(ctx, w.kV, gpu_incident(ctx, w), V)
-    f = nf - 1
-    Vo, so = oracle_potential(w, pos[f], slices=(40,))
-    assert np.array_equal(sidx[f].cpu().numpy(), so)
-    assert rel_l2(V[f, 40].cpu().numpy(), Vo[40]) < TOL_V
+    v_slices = (0, 40) if grid == 1024 else (40,)                         # the 2048^2 oracle potential is ~15 s per slice
+    for f in (0, nf - 1):                                                 # V on 2 frames, from positions
+        Vo, so = oracle_potential(w, pos[f], slices=v_slices)
+        assert np.array_equal(sidx[f].cpu().numpy(), so)
+        for s in v_slices:
+            assert rel_l2(V[f, s].cpu().numpy(), Vo[s]) < TOL_V
     po = oracle_incident(w)
-    p = 7 if grid == 1024 else 3
-    eo = O.multislice(po[p], V[f].cpu().numpy().astype(np.float64), w.cell, w.kV)
-    assert rel_l2(ex[p, f].cpu().numpy(), eo) < TOL_EXIT
+    # exit waves of 4 (tilt, frame) pairs at 1024^2; 1 at 2048^2, where one oracle slice loop is half a minute of host FFTs
+    pairs = ((7, nf - 1), (0, 0), (3, 4), (5, 2)) if grid == 1024 else ((3, 1),)
+    for p, f in pairs:
+        eo = O.multislice(po[p], V[f].cpu().numpy().astype(np.float64), w.cell, w.kV)
+        assert rel_l2(ex[p, f].cpu().numpy(), eo) < TOL_EXIT, (p, f)
     _check_norm(torch, ex, w)
